@@ -1,0 +1,153 @@
+/*
+ * fftb.h -- C-ABI of fftb-b200: the batched, pruned sphere <-> cuboid 3D complex FFT of
+ * plane-wave DFT codes (arXiv 2406.05577, "FFTB"), one NVIDIA B200 (sm_100a).
+ *
+ * The boundary follows the paper's "create, execute and clean-up" constructs
+ * (PAPER.md:130 [3.1 Computational Layout Descriptor]): a plan is created from a
+ * description of the bounding domain, the cut-off that generates the offset array
+ * (Fig. 7, 183-185 [3.3]) and the batch dimension (PAPER.md:219 [3.3]);
+ * it is executed any number of times; it is destroyed.  A description outside the
+ * predefined patterns is refused with FFTB_EUNSUPPORTED ("The framework
+ * will raise an exception if the provided patterns are not within the predefined list").
+ *
+ * Conventions (DESIGN.md lists the readings R1-R13 of the paper behind them)
+ *   grid      (N1,N2,N3) = (x,y,z); x fastest in memory, z slowest;
+ *             z is the stick axis.  C = N1*N2*N3.
+ *   frequency signed integers k_d in [-N_d/2, N_d/2); grid index i_d = k_d mod N_d.
+ *   cut-off   the points with (k1/a1)^2 + (k2/a2)^2 + (k3/a3)^2 <= 1 (Eq. 9,
+ *             inclusive, decided in exact integer arithmetic); S of them.
+ *   packed    [nb][S]: band slowest; inside a band the points are ordered by k1
+ *             ascending, then k2 ascending, then k3 ascending (signed values), i.e. one
+ *             contiguous "z-stick" per occupied (k1,k2) column, sticks ordered by (k1,k2).
+ *   cuboid    [nb][N3][N2][N1], x contiguous.
+ *   vloc      [N3][N2][N1] real (double for FFTB_C128, float for FFTB_C64), one for all bands.
+ *   inverse   psi[b][i] = sum_p c[b][p] exp(+2 pi j (k1 i1/N1 + k2 i2/N2 + k3 i3/N3))
+ *             (Eq. 8), unnormalised.
+ *   forward   c[b][p] = s * sum_i psi[b][i] exp(-2 pi j (k1 i1/N1 + ...)) for the points of
+ *             the cut-off only (Eq. 3-4); s = 1 (FFTB_SCALE_NONE) or 1/C
+ *             (FFTB_SCALE_FORWARD).
+ *   apply_vloc c' = forward( V .* inverse(c) ), the cuboid never leaves the chip.
+ *
+ * Pointers named d_* are DEVICE pointers, h_* are HOST pointers; everything else is host.
+ * All device pointers must be 16-byte aligned.  The caller owns every device buffer,
+ * including the table/workspace block handed to fftb_plan_bind; the plan owns host
+ * memory only.  The execute calls enqueue work on `stream` (a cudaStream_t passed as
+ * void*; NULL = the legacy default stream) and return without synchronising; they do not
+ * allocate.  Inputs are const and are preserved.
+ *
+ * Every function returns 0 (FFTB_OK) or a negative fftb_status; nothing throws or aborts.
+ */
+#ifndef FFTB_H
+#define FFTB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fftb_plan_s *fftb_plan; /* opaque, host-owned */
+
+enum fftb_status {
+    FFTB_OK = 0,
+    FFTB_EINVAL = -1,       /* null pointer, nb < 1 or > batch, N_d < 1, a_d < 0, 2 a_d >= N_d (aliasing),
+                               unknown enum value, misaligned pointer */
+    FFTB_EUNSUPPORTED = -2, /* a description outside the predefined patterns (see fftb_plan_create) */
+    FFTB_ENOMEM = -3,       /* host allocation failed, or the bind block is too small */
+    FFTB_ECUDA = -4,        /* a CUDA call or launch failed; sticky until the plan is destroyed */
+    FFTB_ESTATE = -5        /* execute before fftb_plan_bind, or mismatched plans */
+};
+
+enum fftb_dtype { FFTB_C64 = 0, FFTB_C128 = 1 };               /* element type of packed and cuboid */
+enum fftb_scale { FFTB_SCALE_NONE = 0, FFTB_SCALE_FORWARD = 1 }; /* 1/(N1 N2 N3) applied in forward */
+enum fftb_flags {
+    FFTB_FLAG_DENSE = 1u /* no pruning: every (k1,k2) is a full-length stick, S = C, `cutoff` ignored.
+                            This is the "pad the sphere to the cube, transform the entire cube" route of
+                            PAPER.md:110-112, run by the same kernels (BASELINE config 5). */
+};
+
+typedef struct {
+    int32_t n[3];      /* N1 (x, fastest), N2 (y), N3 (z, stick axis) */
+    int32_t cutoff[3]; /* integer semi-axes a1,a2,a3 >= 0 in index units; ignored if DENSE */
+    int32_t batch;     /* maximum number of bands per execute call, >= 1 */
+    int32_t dtype;     /* fftb_dtype */
+    int32_t scale;     /* fftb_scale */
+    uint32_t flags;    /* fftb_flags */
+} fftb_plan_desc;
+
+typedef struct {
+    int64_t n_points;     /* S */
+    int64_t n_sticks;     /* occupied (k1,k2) columns */
+    int64_t n_xocc;       /* distinct k1 with at least one stick */
+    int64_t device_bytes; /* smallest block fftb_plan_bind accepts (tables + workspace) */
+    int64_t device_bytes_host; /* block size that also holds the staging area of the *_host calls
+                                  (batch * S elements more) */
+    int64_t chunk_bands;  /* bands processed per kernel group (the workspace holds this many) */
+    int64_t min_bytes_per_band_dir; /* algorithmic bytes of one band, one direction: (S + C) * elem */
+    int64_t workspace_offset; /* byte offset of the plane-major intermediate A inside the bind block */
+    int64_t pitch;        /* row pitch of A in elements: A[band][z][pitch] after the inverse z pass */
+    int64_t y_residues;   /* number of partial A planes the forward plane kernel writes per band */
+} fftb_plan_info;
+
+/* Create a plan (host only, no CUDA call).  Builds the offset array -- the stick map -- from the
+ * grid and the cut-off (Fig. 7), the per-k1 stick runs used by the y pass, and the
+ * twiddle tables.
+ * Predefined patterns (anything else: FFTB_EUNSUPPORTED):
+ *   - N1 == N2, each of N1, N3 in {32, 64, 96, 128, 192, 256};
+ *   - pruned plans: a_d <= N_d/4 on every axis (the paper's "cube of width twice the diameter of
+ *     the sphere");
+ *   - FFTB_C128 with N1 = 192 and dense FFTB_C128 beyond what fits one SM's shared memory. */
+int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc);
+
+int fftb_plan_info_get(fftb_plan p, fftb_plan_info *info);
+
+/* Copy the stick map to host arrays supplied by the caller (any may be NULL):
+ * k1,k2,k3lo,len have n_sticks entries, off has n_sticks+1 (exclusive prefix sum of len, the
+ * paper's CSR-like offset array). */
+int fftb_plan_get_map(fftb_plan p, int32_t *k1, int32_t *k2, int32_t *k3lo, int32_t *len, int64_t *off);
+
+/* Hand the plan its device memory: `d_mem` (>= info.device_bytes, 256-byte aligned, caller-owned,
+ * must outlive the plan's last execute).  Uploads the tables on `stream` (cudaMemcpyAsync from
+ * plan-owned host memory) and returns; later execute calls on the same stream are ordered after it. */
+int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream);
+
+/* inverse: d_packed [nb][S] -> d_cuboid [nb][N3][N2][N1].  unpack + pruned z pass on the sticks,
+ * y pass on the occupied x columns only, x pass last (Fig. 3, 112: staged padding). */
+int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void *stream);
+
+/* forward: d_cuboid -> d_packed, the mirror image; applies the plan's scale. */
+int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void *stream);
+
+/* local-potential apply, fused: inverse up to the x pass, multiply by V(r), forward x pass
+ * immediately, then forward y and z passes.  d_packed_in == d_packed_out is allowed. */
+int fftb_apply_vloc(fftb_plan p, const void *d_packed_in, void *d_packed_out, const void *d_vloc, int nb,
+                    void *stream);
+
+/* The same three operations with the PACKED arrays in host memory (pinned memory makes the copies
+ * asynchronous): the library copies them through the staging area inside the bind block
+ * (cudaMemcpyAsync on `stream`), cuboid and vloc stay device pointers. */
+int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb, void *stream);
+int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb, void *stream);
+int fftb_apply_vloc_host(fftb_plan p, const void *h_packed_in, void *h_packed_out, const void *d_vloc, int nb,
+                         void *stream);
+
+/* Comparison arm of BASELINE config 5 ("zero-pad the entire sphere ... the 3D
+ * Fourier computation is applied on the entire cube"): scatter the packed sphere of `pruned` into the
+ * (zero-filled) packed layout of the DENSE plan `dense` of the same grid and dtype, and gather it back. */
+int fftb_dense_embed(fftb_plan pruned, fftb_plan dense, const void *d_packed_pruned, void *d_packed_dense, int nb,
+                     void *stream);
+int fftb_dense_extract(fftb_plan pruned, fftb_plan dense, const void *d_packed_dense, void *d_packed_pruned, int nb,
+                       void *stream);
+
+/* Number of kernels the last execute call on this plan launched (for launch accounting). */
+int fftb_plan_last_launches(fftb_plan p);
+
+int fftb_plan_destroy(fftb_plan p);
+
+const char *fftb_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FFTB_H */

@@ -1,0 +1,251 @@
+"""Thin Python binding of the C-ABI in include/fftb.h (argument marshalling only).
+
+Every step of the transform runs in the CUDA kernels behind ``libfftb.so``; PyTorch is used for
+device memory and streams.  There is no CPU fallback: if the library has not been built, loading
+fails with an ImportError that says how to build it.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_LIBPATH = _HERE / "libfftb.so"
+
+FFTB_C64, FFTB_C128 = 0, 1
+FFTB_SCALE_NONE, FFTB_SCALE_FORWARD = 0, 1
+FFTB_FLAG_DENSE = 1
+FFTB_OK, FFTB_EINVAL, FFTB_EUNSUPPORTED, FFTB_ENOMEM, FFTB_ECUDA, FFTB_ESTATE = 0, -1, -2, -3, -4, -5
+
+# every symbol include/fftb.h declares
+SYMBOLS = [
+    "fftb_plan_create", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
+    "fftb_inverse", "fftb_forward", "fftb_apply_vloc",
+    "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
+    "fftb_dense_embed", "fftb_dense_extract",
+    "fftb_plan_last_launches", "fftb_plan_destroy", "fftb_strerror",
+]
+
+
+class PlanDesc(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int32 * 3), ("cutoff", ctypes.c_int32 * 3), ("batch", ctypes.c_int32),
+                ("dtype", ctypes.c_int32), ("scale", ctypes.c_int32), ("flags", ctypes.c_uint32)]
+
+
+class PlanInfo(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_int64) for k in (
+        "n_points", "n_sticks", "n_xocc", "device_bytes", "device_bytes_host", "chunk_bands",
+        "min_bytes_per_band_dir", "workspace_offset", "pitch", "y_residues")]
+
+
+class FftbError(RuntimeError):
+    def __init__(self, code, what):
+        self.code = code
+        super().__init__(f"{what}: {strerror(code)} ({code})")
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        if not _LIBPATH.exists():
+            raise ImportError(
+                f"{_LIBPATH} not found: build it with `python -m paper_2406_05577_b200.build` "
+                "(there is no CPU fallback)")
+        L = ctypes.CDLL(str(_LIBPATH))
+        vp, i32 = ctypes.c_void_p, ctypes.c_int
+        L.fftb_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc)]
+        L.fftb_plan_info_get.argtypes = [vp, ctypes.POINTER(PlanInfo)]
+        L.fftb_plan_get_map.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.fftb_plan_bind.argtypes = [vp, vp, ctypes.c_size_t, vp]
+        for name in ("fftb_inverse", "fftb_forward", "fftb_inverse_host", "fftb_forward_host"):
+            getattr(L, name).argtypes = [vp, vp, vp, i32, vp]
+        for name in ("fftb_apply_vloc", "fftb_apply_vloc_host"):
+            getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
+        for name in ("fftb_dense_embed", "fftb_dense_extract"):
+            getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
+        L.fftb_plan_last_launches.argtypes = [vp]
+        L.fftb_plan_destroy.argtypes = [vp]
+        L.fftb_strerror.argtypes = [i32]
+        L.fftb_strerror.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return lib().fftb_strerror(code).decode()
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise FftbError(rc, what)
+
+
+def _stream_ptr(stream=None):
+    import torch
+
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+class Plan:
+    """fftb_plan_create / bind / execute / destroy.  Tensors are torch CUDA tensors (or pinned host
+    tensors for the *_host calls); shapes follow include/fftb.h: packed (nb, S), cuboid (nb, N3, N2, N1)."""
+
+    def __init__(self, n, cutoff=(0, 0, 0), batch=1, dtype="c128", scale="forward", dense=False):
+        d = PlanDesc()
+        d.n[:] = [int(x) for x in n]
+        d.cutoff[:] = [int(x) for x in cutoff]
+        d.batch = int(batch)
+        d.dtype = FFTB_C128 if dtype == "c128" else FFTB_C64
+        d.scale = FFTB_SCALE_FORWARD if scale == "forward" else FFTB_SCALE_NONE
+        d.flags = FFTB_FLAG_DENSE if dense else 0
+        self._h = ctypes.c_void_p()
+        _check(lib().fftb_plan_create(ctypes.byref(self._h), ctypes.byref(d)), "fftb_plan_create")
+        self.n = tuple(int(x) for x in n)
+        self.batch = int(batch)
+        self.dtype = dtype
+        self.dense = dense
+        info = PlanInfo()
+        _check(lib().fftb_plan_info_get(self._h, ctypes.byref(info)), "fftb_plan_info_get")
+        self.info = {k: int(getattr(info, k)) for k, _ in PlanInfo._fields_}
+        self.S = self.info["n_points"]
+        self.mem = None
+
+    # ---- host-side queries
+    def get_map(self):
+        ns = self.info["n_sticks"]
+        m = {k: np.empty(ns, dtype=np.int32) for k in ("k1", "k2", "k3lo", "len")}
+        m["off"] = np.empty(ns + 1, dtype=np.int64)
+        _check(lib().fftb_plan_get_map(self._h, *[m[k].ctypes.data_as(ctypes.c_void_p)
+                                                  for k in ("k1", "k2", "k3lo", "len", "off")]), "fftb_plan_get_map")
+        return m
+
+    def points(self):
+        """(k1, k2, k3) of every packed point, expanded from the stick map."""
+        m = self.get_map()
+        rep = np.repeat(np.arange(len(m["k1"])), m["len"])
+        k3 = m["k3lo"][rep] + (np.arange(self.S) - m["off"][:-1][rep]).astype(np.int32)
+        return m["k1"][rep], m["k2"][rep], k3.astype(np.int32)
+
+    # ---- device memory
+    @property
+    def torch_complex(self):
+        import torch
+
+        return torch.complex128 if self.dtype == "c128" else torch.complex64
+
+    @property
+    def torch_real(self):
+        import torch
+
+        return torch.float64 if self.dtype == "c128" else torch.float32
+
+    def bind(self, mem=None, host_staging=False, device="cuda"):
+        import torch
+
+        need = self.info["device_bytes_host"] if host_staging else self.info["device_bytes"]
+        if mem is None:
+            mem = torch.empty(need, dtype=torch.uint8, device=device)
+        assert mem.is_cuda and mem.dtype == torch.uint8 and mem.is_contiguous()
+        _check(lib().fftb_plan_bind(self._h, ctypes.c_void_p(mem.data_ptr()), mem.numel(), _stream_ptr()), "fftb_plan_bind")
+        self.mem = mem
+        return self
+
+    def _chk(self, t, shape, cuda=True, dtype=None):
+        assert tuple(t.shape) == tuple(shape), (tuple(t.shape), tuple(shape))
+        assert t.is_contiguous() and t.dtype == (dtype or self.torch_complex) and t.is_cuda == cuda
+        return ctypes.c_void_p(t.data_ptr())
+
+    def cuboid_shape(self, nb):
+        return (nb, self.n[2], self.n[1], self.n[0])
+
+    # ---- execute
+    def inverse(self, packed, cuboid=None, stream=None):
+        import torch
+
+        nb = packed.shape[0]
+        if cuboid is None:
+            cuboid = torch.empty(self.cuboid_shape(nb), dtype=self.torch_complex, device=packed.device)
+        _check(lib().fftb_inverse(self._h, self._chk(packed, (nb, self.S)), self._chk(cuboid, self.cuboid_shape(nb)),
+                                  nb, _stream_ptr(stream)), "fftb_inverse")
+        return cuboid
+
+    def forward(self, cuboid, packed=None, stream=None):
+        import torch
+
+        nb = cuboid.shape[0]
+        if packed is None:
+            packed = torch.empty((nb, self.S), dtype=self.torch_complex, device=cuboid.device)
+        _check(lib().fftb_forward(self._h, self._chk(cuboid, self.cuboid_shape(nb)), self._chk(packed, (nb, self.S)),
+                                  nb, _stream_ptr(stream)), "fftb_forward")
+        return packed
+
+    def apply_vloc(self, packed_in, vloc, packed_out=None, stream=None):
+        import torch
+
+        nb = packed_in.shape[0]
+        if packed_out is None:
+            packed_out = torch.empty_like(packed_in)
+        _check(lib().fftb_apply_vloc(self._h, self._chk(packed_in, (nb, self.S)), self._chk(packed_out, (nb, self.S)),
+                                     self._chk(vloc, (self.n[2], self.n[1], self.n[0]), dtype=self.torch_real),
+                                     nb, _stream_ptr(stream)), "fftb_apply_vloc")
+        return packed_out
+
+    def inverse_host(self, h_packed, cuboid, stream=None):
+        nb = h_packed.shape[0]
+        _check(lib().fftb_inverse_host(self._h, self._chk(h_packed, (nb, self.S), cuda=False),
+                                       self._chk(cuboid, self.cuboid_shape(nb)), nb, _stream_ptr(stream)), "fftb_inverse_host")
+        return cuboid
+
+    def forward_host(self, cuboid, h_packed, stream=None):
+        nb = cuboid.shape[0]
+        _check(lib().fftb_forward_host(self._h, self._chk(cuboid, self.cuboid_shape(nb)),
+                                       self._chk(h_packed, (nb, self.S), cuda=False), nb, _stream_ptr(stream)), "fftb_forward_host")
+        return h_packed
+
+    def apply_vloc_host(self, h_in, h_out, vloc, stream=None):
+        nb = h_in.shape[0]
+        _check(lib().fftb_apply_vloc_host(self._h, self._chk(h_in, (nb, self.S), cuda=False),
+                                          self._chk(h_out, (nb, self.S), cuda=False),
+                                          self._chk(vloc, (self.n[2], self.n[1], self.n[0]), dtype=self.torch_real),
+                                          nb, _stream_ptr(stream)), "fftb_apply_vloc_host")
+        return h_out
+
+    def dense_embed(self, dense_plan, packed, packed_dense=None, stream=None):
+        import torch
+
+        nb = packed.shape[0]
+        if packed_dense is None:
+            packed_dense = torch.empty((nb, dense_plan.S), dtype=self.torch_complex, device=packed.device)
+        _check(lib().fftb_dense_embed(self._h, dense_plan._h, self._chk(packed, (nb, self.S)),
+                                      dense_plan._chk(packed_dense, (nb, dense_plan.S)), nb, _stream_ptr(stream)), "fftb_dense_embed")
+        return packed_dense
+
+    def dense_extract(self, dense_plan, packed_dense, packed=None, stream=None):
+        import torch
+
+        nb = packed_dense.shape[0]
+        if packed is None:
+            packed = torch.empty((nb, self.S), dtype=self.torch_complex, device=packed_dense.device)
+        _check(lib().fftb_dense_extract(self._h, dense_plan._h, dense_plan._chk(packed_dense, (nb, dense_plan.S)),
+                                        self._chk(packed, (nb, self.S)), nb, _stream_ptr(stream)), "fftb_dense_extract")
+        return packed
+
+    def last_launches(self) -> int:
+        return int(lib().fftb_plan_last_launches(self._h))
+
+    def destroy(self):
+        if self._h:
+            lib().fftb_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -1,0 +1,561 @@
+// fftb_api.cu -- host plan builder, kernel dispatch and the C-ABI of include/fftb.h.
+//
+// The plan builder is the paper's "computational layout descriptor" + "transform creation"
+// blocks collapsed for one GPU: it turns the bounding domain (N1,N2,N3), the
+// cut-off and the batch size into the offset array (stick map, Fig. 7, 183-185) and
+// the per-k1 stick runs, picks one of the predefined kernel patterns or refuses
+// (FFTB_EUNSUPPORTED), and sizes the workspace.
+#include "../../include/fftb.h"
+#include "fftb_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace fftb;
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// predefined patterns: axis length -> factorisation
+// ------------------------------------------------------------------------------------------------
+template <int N, bool DENSE> struct ZX; // z and x axes: the R sub-transforms are done by one thread group
+template <> struct ZX<32, false> { using type = Axis<32, 2, 4, 4, true>; };
+template <> struct ZX<64, false> { using type = Axis<64, 2, 8, 4, true>; };
+template <> struct ZX<96, false> { using type = Axis<96, 2, 6, 8, true>; };
+template <> struct ZX<128, false> { using type = Axis<128, 2, 8, 8, true>; };
+template <> struct ZX<192, false> { using type = Axis<192, 2, 12, 8, true>; };
+template <> struct ZX<256, false> { using type = Axis<256, 2, 16, 8, true>; };
+template <> struct ZX<32, true> { using type = Axis<32, 1, 8, 4, false>; };
+template <> struct ZX<64, true> { using type = Axis<64, 1, 8, 8, false>; };
+template <> struct ZX<128, true> { using type = Axis<128, 1, 16, 8, false>; };
+template <> struct ZX<256, true> { using type = Axis<256, 1, 16, 16, false>; };
+
+template <int N, bool DENSE> struct YA; // y axis: the R residues go to R different CTAs
+template <> struct YA<32, false> { using type = Axis<32, 2, 4, 4, true>; };
+template <> struct YA<64, false> { using type = Axis<64, 2, 8, 4, true>; };
+template <> struct YA<96, false> { using type = Axis<96, 2, 6, 8, true>; };
+template <> struct YA<128, false> { using type = Axis<128, 2, 8, 8, true>; };
+template <> struct YA<192, false> { using type = Axis<192, 4, 6, 8, true>; };
+template <> struct YA<256, false> { using type = Axis<256, 4, 8, 8, true>; };
+template <> struct YA<32, true> { using type = Axis<32, 1, 8, 4, false>; };
+template <> struct YA<64, true> { using type = Axis<64, 1, 8, 8, false>; };
+template <> struct YA<128, true> { using type = Axis<128, 2, 8, 8, false>; };
+template <> struct YA<256, true> { using type = Axis<256, 8, 8, 4, false>; };
+
+constexpr int cmax(int a, int b) { return a > b ? a : b; }
+constexpr int cmin(int a, int b) { return a < b ? a : b; }
+// largest divisor of m that does not exceed cap
+constexpr int div_le(int m, int cap)
+{
+    int best = 1;
+    for (int d = 1; d <= m && d <= cap; ++d)
+        if (m % d == 0) best = d;
+    return best;
+}
+
+template <class AX, class AY> struct PlaneTune {
+    static constexpr int PM = cmax(AX::P1, AX::P2);
+    static constexpr int LX = div_le(AY::M, 256 / PM);          // lines per x round
+    static constexpr int NT = LX * PM;                         // threads per CTA
+    static constexpr int LY = cmax(1, NT / cmax(AY::P1, AY::P2)); // columns per y round
+};
+
+constexpr int Z_LINES = 32, Z_NT = 256;
+
+struct ZLaunch {
+    int (*inv)(const DevPlan &, const void *packed, void *A, long long stride, int nb, cudaStream_t);
+    int (*fwd)(const DevPlan &, const void *A, void *packed, long long stride, int nb, cudaStream_t);
+};
+struct PlaneLaunch {
+    int ry;
+    int (*run[3])(const DevPlan &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v,
+                  long long sin, long long sout, int nb, cudaStream_t);
+};
+
+template <typename T, class AZ> int launch_zinv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
+{
+    auto k = zpass_inv_k<T, AZ, Z_LINES, Z_NT>;
+    const size_t smem = sizeof(cx<T>) * ((size_t)AZ::M * (Z_LINES | 1) + AZ::N);
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    dim3 grid((pl.nsticks + Z_LINES - 1) / Z_LINES, nb);
+    k<<<grid, Z_NT, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+template <typename T, class AZ> int launch_zfwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
+{
+    auto k = zpass_fwd_k<T, AZ, Z_LINES, Z_NT>;
+    const size_t smem = sizeof(cx<T>) * ((size_t)AZ::R * AZ::P2 * (AZ::P1 * (Z_LINES | 1) + 1) + AZ::N);
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    dim3 grid((pl.nsticks + Z_LINES - 1) / Z_LINES, nb);
+    k<<<grid, Z_NT, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+template <typename T, class AX, class AY, int MODE>
+int launch_plane(const DevPlan &pl, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
+                 long long sout, int nb, cudaStream_t st)
+{
+    using TU = PlaneTune<AX, AY>;
+    auto k = plane_k<T, AX, AY, TU::LX, TU::LY, TU::NT, MODE>;
+    const size_t smem = PlaneSmem<T, AX, AY, TU::LX, TU::LY, TU::NT>::bytes;
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    dim3 grid(AY::R * pl.n3, nb);
+    k<<<grid, TU::NT, smem, st>>>(pl, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+
+template <typename T, int N, bool DENSE> ZLaunch make_z()
+{
+    using AZ = typename ZX<N, DENSE>::type;
+    return ZLaunch{&launch_zinv<T, AZ>, &launch_zfwd<T, AZ>};
+}
+template <typename T, int N, bool DENSE> PlaneLaunch make_plane()
+{
+    using AX = typename ZX<N, DENSE>::type;
+    using AY = typename YA<N, DENSE>::type;
+    static_assert(PlaneSmem<T, AX, AY, PlaneTune<AX, AY>::LX, PlaneTune<AX, AY>::LY, PlaneTune<AX, AY>::NT>::bytes <= 227 * 1024,
+                  "plane does not fit in shared memory");
+    return PlaneLaunch{AY::R,
+                       {&launch_plane<T, AX, AY, MODE_INV>, &launch_plane<T, AX, AY, MODE_FWD>, &launch_plane<T, AX, AY, MODE_VLOC>}};
+}
+
+bool find_z(int dtype, int n, bool dense, ZLaunch *out)
+{
+#define ZCASE(T, DT, N, D) \
+    if (dtype == DT && n == N && dense == D) { *out = make_z<T, N, D>(); return true; }
+    ZCASE(double, FFTB_C128, 32, false) ZCASE(double, FFTB_C128, 64, false) ZCASE(double, FFTB_C128, 96, false)
+    ZCASE(double, FFTB_C128, 128, false) ZCASE(double, FFTB_C128, 192, false) ZCASE(double, FFTB_C128, 256, false)
+    ZCASE(float, FFTB_C64, 32, false) ZCASE(float, FFTB_C64, 64, false) ZCASE(float, FFTB_C64, 96, false)
+    ZCASE(float, FFTB_C64, 128, false) ZCASE(float, FFTB_C64, 192, false) ZCASE(float, FFTB_C64, 256, false)
+    ZCASE(double, FFTB_C128, 32, true) ZCASE(double, FFTB_C128, 64, true) ZCASE(double, FFTB_C128, 128, true)
+    ZCASE(double, FFTB_C128, 256, true)
+#undef ZCASE
+    return false;
+}
+bool find_plane(int dtype, int n, bool dense, PlaneLaunch *out)
+{
+#define PCASE(T, DT, N, D) \
+    if (dtype == DT && n == N && dense == D) { *out = make_plane<T, N, D>(); return true; }
+    PCASE(double, FFTB_C128, 32, false) PCASE(double, FFTB_C128, 64, false) PCASE(double, FFTB_C128, 96, false)
+    PCASE(double, FFTB_C128, 128, false) PCASE(double, FFTB_C128, 192, false) PCASE(double, FFTB_C128, 256, false)
+    PCASE(float, FFTB_C64, 32, false) PCASE(float, FFTB_C64, 64, false) PCASE(float, FFTB_C64, 96, false)
+    PCASE(float, FFTB_C64, 128, false) PCASE(float, FFTB_C64, 192, false) PCASE(float, FFTB_C64, 256, false)
+    PCASE(double, FFTB_C128, 32, true) PCASE(double, FFTB_C128, 64, true) PCASE(double, FFTB_C128, 128, true)
+    PCASE(double, FFTB_C128, 256, true)
+#undef PCASE
+    return false;
+}
+
+// ------------------------------------------------------------------------------------------------
+// cut-off membership in exact integers (Eq. 9, inclusive)
+// ------------------------------------------------------------------------------------------------
+bool inside(long long k1, long long k2, long long k3, const int32_t a[3])
+{
+    long long w[3];
+    const long long k[3] = {k1, k2, k3};
+    for (int d = 0; d < 3; ++d) {
+        if (a[d] == 0 && k[d] != 0) return false;
+        w[d] = a[d] ? a[d] : 1;
+    }
+    const long long lhs = k1 * k1 * (w[1] * w[2]) * (w[1] * w[2]) + k2 * k2 * (w[0] * w[2]) * (w[0] * w[2]) +
+                          k3 * k3 * (w[0] * w[1]) * (w[0] * w[1]);
+    return lhs <= (w[0] * w[1] * w[2]) * (w[0] * w[1] * w[2]);
+}
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+} // namespace
+
+struct fftb_plan_s {
+    fftb_plan_desc desc;
+    bool dense;
+    size_t elem;
+    int64_t S, C;
+    int nsticks, nxocc, pitch, k1lo, ry;
+    std::vector<int32_t> k1, k2, k3lo, len;
+    std::vector<int64_t> off;
+    std::vector<int4> h_stick, h_col;
+    std::vector<unsigned char> h_tw[3];
+    ZLaunch zl;
+    PlaneLaunch plk;
+    // device block layout
+    size_t o_stick, o_col, o_tw[3], o_ws, o_stage, bytes_min, bytes_stage;
+    long long a_inv_stride, a_fwd_stride; // elements per band of the intermediate
+    int chunk;                            // bands per kernel pair
+    // bound state
+    unsigned char *d_mem;
+    bool staging;
+    DevPlan dev;
+    int sticky;
+    int launches;
+};
+
+extern "C" {
+
+const char *fftb_strerror(int code)
+{
+    switch (code) {
+    case FFTB_OK: return "ok";
+    case FFTB_EINVAL: return "invalid argument";
+    case FFTB_EUNSUPPORTED: return "description outside the predefined patterns";
+    case FFTB_ENOMEM: return "out of memory / bind block too small";
+    case FFTB_ECUDA: return "CUDA error";
+    case FFTB_ESTATE: return "plan not bound / mismatched plans";
+    default: return "unknown fftb status";
+    }
+}
+
+int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
+{
+    if (!out || !desc) return FFTB_EINVAL;
+    *out = nullptr;
+    const bool dense = (desc->flags & FFTB_FLAG_DENSE) != 0;
+    if (desc->flags & ~(uint32_t)FFTB_FLAG_DENSE) return FFTB_EINVAL;
+    if (desc->dtype != FFTB_C64 && desc->dtype != FFTB_C128) return FFTB_EINVAL;
+    if (desc->scale != FFTB_SCALE_NONE && desc->scale != FFTB_SCALE_FORWARD) return FFTB_EINVAL;
+    if (desc->batch < 1) return FFTB_EINVAL;
+    for (int d = 0; d < 3; ++d) {
+        if (desc->n[d] < 1) return FFTB_EINVAL;
+        if (!dense && (desc->cutoff[d] < 0 || 2 * (long long)desc->cutoff[d] >= desc->n[d])) return FFTB_EINVAL;
+    }
+    // predefined patterns
+    if (desc->n[0] != desc->n[1]) return FFTB_EUNSUPPORTED;
+    ZLaunch zl;
+    PlaneLaunch plk;
+    if (!find_z(desc->dtype, desc->n[2], dense, &zl) || !find_plane(desc->dtype, desc->n[0], dense, &plk)) return FFTB_EUNSUPPORTED;
+    if (!dense)
+        for (int d = 0; d < 3; ++d)
+            if (4 * (long long)desc->cutoff[d] > desc->n[d]) return FFTB_EUNSUPPORTED; // half-band kernels only
+
+    fftb_plan_s *p = new (std::nothrow) fftb_plan_s();
+    if (!p) return FFTB_ENOMEM;
+    try {
+        p->desc = *desc;
+        p->dense = dense;
+        p->elem = desc->dtype == FFTB_C128 ? 16 : 8;
+        p->zl = zl;
+        p->plk = plk;
+        p->ry = plk.ry;
+        const int n1 = desc->n[0], n2 = desc->n[1], n3 = desc->n[2];
+        p->C = (int64_t)n1 * n2 * n3;
+        int32_t a[3] = {desc->cutoff[0], desc->cutoff[1], desc->cutoff[2]};
+        // ---- stick map: k1 major, k2 minor, both ascending over signed values (reading R5)
+        const int k1a = dense ? -(n1 / 2) : -a[0], k1b = dense ? (n1 + 1) / 2 - 1 : a[0];
+        const int k2a = dense ? -(n2 / 2) : -a[1], k2b = dense ? (n2 + 1) / 2 - 1 : a[1];
+        p->k1lo = k1a;
+        p->nxocc = 0;
+        int64_t run = 0;
+        for (int q1 = k1a; q1 <= k1b; ++q1) {
+            int first = (int)p->k1.size(), cnt = 0, k2lo = 0, k2prev = 0;
+            for (int q2 = k2a; q2 <= k2b; ++q2) {
+                int lo, ln;
+                if (dense) {
+                    lo = -(n3 / 2);
+                    ln = n3;
+                } else {
+                    if (!inside(q1, q2, 0, a)) continue;
+                    int top = 0; // the column is symmetric in k3 and convex: grow from 0
+                    while (top + 1 <= a[2] && inside(q1, q2, top + 1, a)) ++top;
+                    lo = -top;
+                    ln = 2 * top + 1;
+                }
+                if (cnt == 0) k2lo = q2;
+                else if (q2 != k2prev + 1) { delete p; return FFTB_EUNSUPPORTED; } // non-contiguous k2 run (R6)
+                k2prev = q2;
+                ++cnt;
+                p->k1.push_back(q1);
+                p->k2.push_back(q2);
+                p->k3lo.push_back(lo);
+                p->len.push_back(ln);
+                p->off.push_back(run);
+                run += ln;
+            }
+            if (cnt == 0) { delete p; return FFTB_EUNSUPPORTED; } // hole in the occupied k1 range
+            int4 c;
+            c.x = first; c.y = cnt; c.z = k2lo; c.w = 0;
+            p->h_col.push_back(c);
+            ++p->nxocc;
+        }
+        p->off.push_back(run);
+        p->S = run;
+        p->nsticks = (int)p->k1.size();
+        if (p->S >= (int64_t)1 << 31) { delete p; return FFTB_EUNSUPPORTED; }
+        p->pitch = (int)align_up((size_t)p->nsticks, 16);
+        p->h_stick.resize(p->nsticks);
+        for (int s = 0; s < p->nsticks; ++s) {
+            int4 v;
+            v.x = (int)p->off[s]; v.y = p->k3lo[s]; v.z = p->len[s];
+            v.w = (int)(((uint32_t)p->k1[s] & 0xffffu) | ((uint32_t)p->k2[s] << 16));
+            p->h_stick[s] = v;
+        }
+        // ---- twiddle tables exp(+j 2 pi i / N), computed in long double, rounded once
+        for (int d = 0; d < 3; ++d) {
+            const int n = desc->n[d];
+            p->h_tw[d].resize((size_t)n * p->elem);
+            for (int i = 0; i < n; ++i) {
+                // reduce to the first octant for accuracy
+                const long double ang = 2.0L * 3.14159265358979323846264338327950288L * (long double)i / (long double)n;
+                const long double c = cosl(ang), s = sinl(ang);
+                if (p->elem == 16) {
+                    double *t = reinterpret_cast<double *>(p->h_tw[d].data()) + 2 * (size_t)i;
+                    t[0] = (double)c; t[1] = (double)s;
+                } else {
+                    float *t = reinterpret_cast<float *>(p->h_tw[d].data()) + 2 * (size_t)i;
+                    t[0] = (float)c; t[1] = (float)s;
+                }
+            }
+        }
+        // ---- workspace: the plane-major intermediate for `chunk` bands, sized to stay in L2
+        p->a_inv_stride = (long long)n3 * p->pitch;
+        p->a_fwd_stride = (long long)p->ry * n3 * p->pitch;
+        const size_t per_band = (size_t)(p->a_inv_stride + p->a_fwd_stride) * p->elem; // vloc needs both
+        const size_t budget = (size_t)48 << 20;
+        long long chunk = (long long)(budget / per_band);
+        if (chunk < 1) chunk = 1;
+        if (chunk > desc->batch) chunk = desc->batch;
+        p->chunk = (int)chunk;
+        size_t o = 0;
+        p->o_stick = o; o = align_up(o + sizeof(int4) * p->h_stick.size(), 256);
+        p->o_col = o; o = align_up(o + sizeof(int4) * p->h_col.size(), 256);
+        for (int d = 0; d < 3; ++d) { p->o_tw[d] = o; o = align_up(o + p->h_tw[d].size(), 256); }
+        p->o_ws = o; o = align_up(o + per_band * (size_t)p->chunk, 256);
+        p->bytes_min = o;
+        p->o_stage = o; o = align_up(o + (size_t)desc->batch * (size_t)p->S * p->elem, 256);
+        p->bytes_stage = o;
+        p->d_mem = nullptr;
+        p->staging = false;
+        p->sticky = 0;
+        p->launches = 0;
+    } catch (const std::bad_alloc &) {
+        delete p;
+        return FFTB_ENOMEM;
+    }
+    *out = p;
+    return FFTB_OK;
+}
+
+int fftb_plan_info_get(fftb_plan p, fftb_plan_info *info)
+{
+    if (!p || !info) return FFTB_EINVAL;
+    info->n_points = p->S;
+    info->n_sticks = p->nsticks;
+    info->n_xocc = p->nxocc;
+    info->device_bytes = (int64_t)p->bytes_min;
+    info->device_bytes_host = (int64_t)p->bytes_stage;
+    info->chunk_bands = p->chunk;
+    info->min_bytes_per_band_dir = (p->S + p->C) * (int64_t)p->elem;
+    info->workspace_offset = (int64_t)p->o_ws;
+    info->pitch = p->pitch;
+    info->y_residues = p->ry;
+    return FFTB_OK;
+}
+
+int fftb_plan_get_map(fftb_plan p, int32_t *k1, int32_t *k2, int32_t *k3lo, int32_t *len, int64_t *off)
+{
+    if (!p) return FFTB_EINVAL;
+    const size_t n = (size_t)p->nsticks;
+    if (k1) memcpy(k1, p->k1.data(), n * sizeof(int32_t));
+    if (k2) memcpy(k2, p->k2.data(), n * sizeof(int32_t));
+    if (k3lo) memcpy(k3lo, p->k3lo.data(), n * sizeof(int32_t));
+    if (len) memcpy(len, p->len.data(), n * sizeof(int32_t));
+    if (off) memcpy(off, p->off.data(), (n + 1) * sizeof(int64_t));
+    return FFTB_OK;
+}
+
+int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
+{
+    if (!p || !d_mem) return FFTB_EINVAL;
+    if ((uintptr_t)d_mem % 256) return FFTB_EINVAL;
+    if (bytes < p->bytes_min) return FFTB_ENOMEM;
+    if (p->sticky) return p->sticky;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char *m = (unsigned char *)d_mem;
+    cudaError_t e = cudaMemcpyAsync(m + p->o_stick, p->h_stick.data(), sizeof(int4) * p->h_stick.size(), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(m + p->o_col, p->h_col.data(), sizeof(int4) * p->h_col.size(), cudaMemcpyHostToDevice, st);
+    for (int d = 0; d < 3 && e == cudaSuccess; ++d)
+        e = cudaMemcpyAsync(m + p->o_tw[d], p->h_tw[d].data(), p->h_tw[d].size(), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { p->sticky = FFTB_ECUDA; return FFTB_ECUDA; }
+    p->d_mem = m;
+    p->staging = bytes >= p->bytes_stage;
+    DevPlan &dv = p->dev;
+    dv.n1 = p->desc.n[0]; dv.n2 = p->desc.n[1]; dv.n3 = p->desc.n[2];
+    dv.nsticks = p->nsticks; dv.pitch = p->pitch; dv.nxocc = p->nxocc; dv.k1lo = p->k1lo; dv.ry = p->ry;
+    dv.stick = (const int4 *)(m + p->o_stick);
+    dv.col = (const int4 *)(m + p->o_col);
+    dv.tw1 = m + p->o_tw[0]; dv.tw2 = m + p->o_tw[1]; dv.tw3 = m + p->o_tw[2];
+    dv.S = p->S;
+    dv.scale = p->desc.scale == FFTB_SCALE_FORWARD ? 1.0 / (double)p->C : 1.0;
+    return FFTB_OK;
+}
+
+static int check_exec(fftb_plan p, const void *a, const void *b, int nb)
+{
+    if (!p || !a || !b) return FFTB_EINVAL;
+    if (p->sticky) return p->sticky;
+    if (!p->d_mem) return FFTB_ESTATE;
+    if (nb < 1 || nb > p->desc.batch) return FFTB_EINVAL;
+    if (((uintptr_t)a | (uintptr_t)b) % 16) return FFTB_EINVAL;
+    return FFTB_OK;
+}
+
+int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void *stream)
+{
+    int rc = check_exec(p, d_packed, d_cuboid, nb);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char *A = p->d_mem + p->o_ws;
+    p->launches = 0;
+    for (int b0 = 0; b0 < nb; b0 += p->chunk) {
+        const int nc = nb - b0 < p->chunk ? nb - b0 : p->chunk;
+        const unsigned char *pk = (const unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
+        unsigned char *cb = (unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
+        rc = p->zl.inv(p->dev, pk, A, p->a_inv_stride, nc, st);
+        if (!rc) rc = p->plk.run[MODE_INV](p->dev, A, nullptr, nullptr, cb, nullptr, p->a_inv_stride, 0, nc, st);
+        if (rc) { p->sticky = rc; return rc; }
+        p->launches += 2;
+    }
+    return FFTB_OK;
+}
+
+int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void *stream)
+{
+    int rc = check_exec(p, d_cuboid, d_packed, nb);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char *A = p->d_mem + p->o_ws;
+    p->launches = 0;
+    for (int b0 = 0; b0 < nb; b0 += p->chunk) {
+        const int nc = nb - b0 < p->chunk ? nb - b0 : p->chunk;
+        unsigned char *pk = (unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
+        const unsigned char *cb = (const unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
+        rc = p->plk.run[MODE_FWD](p->dev, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd_stride, nc, st);
+        if (!rc) rc = p->zl.fwd(p->dev, A, pk, p->a_fwd_stride, nc, st);
+        if (rc) { p->sticky = rc; return rc; }
+        p->launches += 2;
+    }
+    return FFTB_OK;
+}
+
+int fftb_apply_vloc(fftb_plan p, const void *d_in, void *d_out, const void *d_vloc, int nb, void *stream)
+{
+    int rc = check_exec(p, d_in, d_out, nb);
+    if (rc) return rc;
+    if (!d_vloc || (uintptr_t)d_vloc % 16) return FFTB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char *Ai = p->d_mem + p->o_ws;
+    unsigned char *Af = Ai + (size_t)p->chunk * p->a_inv_stride * p->elem;
+    p->launches = 0;
+    for (int b0 = 0; b0 < nb; b0 += p->chunk) {
+        const int nc = nb - b0 < p->chunk ? nb - b0 : p->chunk;
+        const unsigned char *pi = (const unsigned char *)d_in + (size_t)b0 * p->S * p->elem;
+        unsigned char *po = (unsigned char *)d_out + (size_t)b0 * p->S * p->elem;
+        rc = p->zl.inv(p->dev, pi, Ai, p->a_inv_stride, nc, st);
+        if (!rc) rc = p->plk.run[MODE_VLOC](p->dev, Ai, Af, nullptr, nullptr, d_vloc, p->a_inv_stride, p->a_fwd_stride, nc, st);
+        if (!rc) rc = p->zl.fwd(p->dev, Af, po, p->a_fwd_stride, nc, st);
+        if (rc) { p->sticky = rc; return rc; }
+        p->launches += 3;
+    }
+    return FFTB_OK;
+}
+
+static int check_host(fftb_plan p, int nb)
+{
+    if (!p) return FFTB_EINVAL;
+    if (p->sticky) return p->sticky;
+    if (!p->d_mem) return FFTB_ESTATE;
+    if (!p->staging) return FFTB_ENOMEM;
+    if (nb < 1 || nb > p->desc.batch) return FFTB_EINVAL;
+    return FFTB_OK;
+}
+
+int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb, void *stream)
+{
+    int rc = check_host(p, nb);
+    if (rc) return rc;
+    if (!h_packed || !d_cuboid) return FFTB_EINVAL;
+    unsigned char *stg = p->d_mem + p->o_stage;
+    if (cudaMemcpyAsync(stg, h_packed, (size_t)nb * p->S * p->elem, cudaMemcpyHostToDevice, (cudaStream_t)stream) != cudaSuccess) {
+        p->sticky = FFTB_ECUDA;
+        return FFTB_ECUDA;
+    }
+    return fftb_inverse(p, stg, d_cuboid, nb, stream);
+}
+
+int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb, void *stream)
+{
+    int rc = check_host(p, nb);
+    if (rc) return rc;
+    if (!h_packed || !d_cuboid) return FFTB_EINVAL;
+    unsigned char *stg = p->d_mem + p->o_stage;
+    rc = fftb_forward(p, d_cuboid, stg, nb, stream);
+    if (rc) return rc;
+    if (cudaMemcpyAsync(h_packed, stg, (size_t)nb * p->S * p->elem, cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess) {
+        p->sticky = FFTB_ECUDA;
+        return FFTB_ECUDA;
+    }
+    return FFTB_OK;
+}
+
+int fftb_apply_vloc_host(fftb_plan p, const void *h_in, void *h_out, const void *d_vloc, int nb, void *stream)
+{
+    int rc = check_host(p, nb);
+    if (rc) return rc;
+    if (!h_in || !h_out) return FFTB_EINVAL;
+    unsigned char *stg = p->d_mem + p->o_stage;
+    const size_t bytes = (size_t)nb * p->S * p->elem;
+    if (cudaMemcpyAsync(stg, h_in, bytes, cudaMemcpyHostToDevice, (cudaStream_t)stream) != cudaSuccess) {
+        p->sticky = FFTB_ECUDA;
+        return FFTB_ECUDA;
+    }
+    rc = fftb_apply_vloc(p, stg, stg, d_vloc, nb, stream);
+    if (rc) return rc;
+    if (cudaMemcpyAsync(h_out, stg, bytes, cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess) {
+        p->sticky = FFTB_ECUDA;
+        return FFTB_ECUDA;
+    }
+    return FFTB_OK;
+}
+
+static int dense_move(fftb_plan pruned, fftb_plan dense, const void *src, void *dst, int nb, void *stream, bool extract)
+{
+    if (!pruned || !dense || !src || !dst) return FFTB_EINVAL;
+    if (pruned->sticky) return pruned->sticky;
+    if (!pruned->d_mem || !dense->dense || pruned->dense) return FFTB_ESTATE;
+    for (int d = 0; d < 3; ++d)
+        if (pruned->desc.n[d] != dense->desc.n[d]) return FFTB_ESTATE;
+    if (pruned->desc.dtype != dense->desc.dtype) return FFTB_ESTATE;
+    if (nb < 1 || nb > pruned->desc.batch || nb > dense->desc.batch) return FFTB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!extract && cudaMemsetAsync(dst, 0, (size_t)nb * dense->S * dense->elem, st) != cudaSuccess) return FFTB_ECUDA;
+    dim3 grid((pruned->nsticks + 7) / 8, nb);
+    const DevPlan &dv = pruned->dev;
+    if (pruned->elem == 16)
+        dense_embed_k<double><<<grid, 256, 0, st>>>(dv.stick, dv.nsticks, dv.S, (const double2 *)src, (double2 *)dst, dv.n1, dv.n2, dv.n3, extract);
+    else
+        dense_embed_k<float><<<grid, 256, 0, st>>>(dv.stick, dv.nsticks, dv.S, (const float2 *)src, (float2 *)dst, dv.n1, dv.n2, dv.n3, extract);
+    pruned->launches = 1;
+    return cudaGetLastError() == cudaSuccess ? FFTB_OK : FFTB_ECUDA;
+}
+
+int fftb_dense_embed(fftb_plan pruned, fftb_plan dense, const void *d_packed_pruned, void *d_packed_dense, int nb, void *stream)
+{
+    return dense_move(pruned, dense, d_packed_pruned, d_packed_dense, nb, stream, false);
+}
+int fftb_dense_extract(fftb_plan pruned, fftb_plan dense, const void *d_packed_dense, void *d_packed_pruned, int nb, void *stream)
+{
+    return dense_move(pruned, dense, d_packed_dense, d_packed_pruned, nb, stream, true);
+}
+
+int fftb_plan_last_launches(fftb_plan p) { return p ? p->launches : FFTB_EINVAL; }
+
+int fftb_plan_destroy(fftb_plan p)
+{
+    if (!p) return FFTB_EINVAL;
+    delete p;
+    return FFTB_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,242 @@
+"""GPU parity tests: the CUDA path (through the C-ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Bar (BASELINE.json north_star): relative L2 error <= 1e-12 for complex128
+and <= 1e-5 for complex64; the stick map is compared for equality in tests/test_host_cabi.py.
+"""
+import numpy as np
+import pytest
+
+from paper_2406_05577_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _rel(a, b):
+    a = np.asarray(a, dtype=np.complex128).ravel()
+    b = np.asarray(b, dtype=np.complex128).ravel()
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def fb():
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2406_05577_b200 import binding
+
+    binding.lib()  # fails loudly if libfftb.so is missing
+    return binding
+
+
+def _plan(fb, w, batch, scale="forward", dense=False, host=False):
+    p = fb.Plan(w.n, w.cutoff, batch=batch, dtype=w.dtype, scale=scale, dense=dense)
+    p.bind(host_staging=host)
+    return p
+
+
+def _small(n, a, dtype="c128", batch=3, dist="uniform", number=0):
+    return wl.Workload(number, "t", n, a, dtype, batch, dist, "inv_fwd")
+
+
+SMALL = [
+    _small((32, 32, 32), (8, 8, 8), number=1),
+    _small((32, 32, 32), (5, 8, 3)),
+    _small((64, 64, 64), (16, 16, 16), batch=5),
+    _small((64, 64, 32), (9, 16, 8)),
+    _small((32, 32, 96), (8, 8, 24)),
+    _small((96, 96, 192), (24, 24, 48), dtype="c64", batch=2, number=4),
+    _small((96, 96, 64), (24, 20, 16), dtype="c128", batch=2),
+    _small((32, 32, 192), (8, 8, 48), dtype="c128", batch=2),
+    _small((128, 128, 128), (32, 32, 32), batch=3, dist="normal_decay", number=3),
+    _small((128, 128, 64), (32, 17, 16), dtype="c64", batch=2),
+    _small((192, 192, 32), (48, 48, 8), dtype="c64", batch=2),
+    _small((192, 192, 32), (48, 40, 8), dtype="c128", batch=1),
+    _small((256, 256, 256), (64, 64, 64), batch=1, number=5),
+    _small((256, 256, 32), (64, 64, 8), dtype="c64", batch=2),
+]
+IDS = [f"{w.n[0]}x{w.n[1]}x{w.n[2]}-a{w.cutoff[0]}.{w.cutoff[1]}.{w.cutoff[2]}-{w.dtype}" for w in SMALL]
+
+
+@pytest.mark.parametrize("w", SMALL, ids=IDS)
+def test_inverse_forward_vs_oracle(fb, oracle, w):
+    p = _plan(fb, w, w.batch)
+    k = p.points()
+    ko = oracle.enum_points(w.n, w.cutoff)
+    assert all(np.array_equal(x, y) for x, y in zip(k, ko))
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    # stage check: A after the inverse z pass == oracle's z-only stage, read through the stick columns
+    d_psi = p.inverse(d_c)
+    torch.cuda.synchronize()
+    psi_ref = oracle.inverse(w.n, ko, c)
+    e_inv = _rel(d_psi.cpu().numpy(), psi_ref)
+    assert e_inv <= w.tol, f"inverse rel L2 {e_inv:.3e}"
+    # the input must be preserved
+    assert torch.equal(d_c.cpu(), torch.from_numpy(c))
+    # forward of a generic (not band-limited) cuboid
+    g = wl.cuboid(w)
+    d_g = torch.from_numpy(g).cuda()
+    d_f = p.forward(d_g)
+    torch.cuda.synchronize()
+    C = float(np.prod(w.n))
+    f_ref = oracle.forward(w.n, ko, g, 1.0 / C)
+    e_fwd = _rel(d_f.cpu().numpy(), f_ref)
+    assert e_fwd <= w.tol, f"forward rel L2 {e_fwd:.3e}"
+    assert torch.equal(d_g.cpu(), torch.from_numpy(g))
+    # round trip recovers the sphere
+    d_rt = p.forward(d_psi)
+    torch.cuda.synchronize()
+    e_rt = _rel(d_rt.cpu().numpy(), c)
+    assert e_rt <= w.tol, f"round trip rel L2 {e_rt:.3e}"
+    p.destroy()
+
+
+@pytest.mark.parametrize("w", [SMALL[0], SMALL[2], SMALL[3], SMALL[5], SMALL[8], SMALL[10], SMALL[13]],
+                         ids=[IDS[i] for i in (0, 2, 3, 5, 8, 10, 13)])
+def test_apply_vloc_vs_oracle(fb, oracle, w):
+    p = _plan(fb, w, w.batch)
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    v = wl.potential(w)
+    d_c, d_v = torch.from_numpy(c).cuda(), torch.from_numpy(v).cuda()
+    d_o = p.apply_vloc(d_c, d_v)
+    torch.cuda.synchronize()
+    C = float(np.prod(w.n))
+    ref = oracle.apply_vloc(w.n, k, c, v, 1.0 / C)
+    e = _rel(d_o.cpu().numpy(), ref)
+    assert e <= w.tol, f"vloc rel L2 {e:.3e}"
+    # in place (d_packed_in == d_packed_out is allowed)
+    d_io = d_c.clone()
+    p.apply_vloc(d_io, d_v, d_io)
+    torch.cuda.synchronize()
+    assert _rel(d_io.cpu().numpy(), ref) <= w.tol
+    p.destroy()
+
+
+def test_scale_none(fb, oracle):
+    w = SMALL[0]
+    p = _plan(fb, w, w.batch, scale="none")
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    d_rt = p.forward(p.inverse(torch.from_numpy(c).cuda()))
+    torch.cuda.synchronize()
+    assert _rel(d_rt.cpu().numpy(), float(np.prod(w.n)) * c) <= w.tol  # forward(inverse(c)) = C c (R2)
+
+
+def test_closed_forms_on_gpu(fb):
+    """Impulse -> ones, single plane wave -> exp(+2 pi j k0.i/N) (Eq. 8), without the oracle."""
+    w = SMALL[2]
+    p = _plan(fb, w, 2)
+    k = p.points()
+    S = p.S
+    c = np.zeros((2, S), np.complex128)
+    c[0, (S - 1) // 2] = 1.0
+    p0 = 1234
+    c[1, p0] = 1.0
+    psi = p.inverse(torch.from_numpy(c).cuda()).cpu().numpy()
+    assert np.abs(psi[0] - 1).max() < 1e-13
+    i3, i2, i1 = np.meshgrid(*[np.arange(w.n[d]) for d in (2, 1, 0)], indexing="ij")
+    ref = np.exp(2j * np.pi * (k[0][p0] * i1 / w.n[0] + k[1][p0] * i2 / w.n[1] + k[2][p0] * i3 / w.n[2]))
+    assert np.abs(psi[1] - ref).max() < 1e-13
+
+
+def test_batch_chunking_and_partial_batches(fb, oracle):
+    """nb smaller than, equal to and not a multiple of the plan's chunk size; plan reuse."""
+    w = _small((64, 64, 64), (16, 16, 16), batch=37)
+    p = _plan(fb, w, 37)
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    ref = oracle.inverse(w.n, k, c[:5])
+    for nb in (1, 5, 37):
+        d_psi = p.inverse(d_c[:nb].contiguous())
+        torch.cuda.synchronize()
+        m = min(nb, 5)
+        assert _rel(d_psi[:m].cpu().numpy(), ref[:m]) <= w.tol
+        rt = p.forward(d_psi)
+        torch.cuda.synchronize()
+        assert _rel(rt.cpu().numpy(), c[:nb]) <= w.tol
+    assert p.last_launches() == 2 * -(-37 // p.info["chunk_bands"])
+    with pytest.raises(fb.FftbError):
+        p.inverse(torch.zeros((38, p.S), dtype=torch.complex128, device="cuda"))
+
+
+def test_host_buffer_calls(fb, oracle):
+    w = SMALL[2]
+    p = _plan(fb, w, w.batch, host=True)
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    h_c = torch.from_numpy(c).pin_memory()
+    d_psi = torch.empty(p.cuboid_shape(w.batch), dtype=torch.complex128, device="cuda")
+    p.inverse_host(h_c, d_psi)
+    h_rt = torch.empty_like(h_c).pin_memory()
+    p.forward_host(d_psi, h_rt)
+    torch.cuda.synchronize()
+    assert _rel(h_rt.numpy(), c) <= w.tol
+    v = wl.potential(w)
+    h_o = torch.empty_like(h_c).pin_memory()
+    p.apply_vloc_host(h_c, h_o, torch.from_numpy(v).cuda())
+    torch.cuda.synchronize()
+    ref = oracle.apply_vloc(w.n, k, c, v, 1.0 / float(np.prod(w.n)))
+    assert _rel(h_o.numpy(), ref) <= w.tol
+    # without the staging area the host calls are refused
+    p2 = _plan(fb, w, w.batch, host=False)
+    with pytest.raises(fb.FftbError):
+        p2.inverse_host(h_c, d_psi)
+
+
+@pytest.mark.parametrize("n,a", [((32, 32, 32), (8, 8, 8)), ((64, 64, 64), (16, 16, 16)), ((128, 128, 128), (32, 32, 32)),
+                                 ((256, 256, 256), (64, 64, 64))])
+def test_pruned_vs_dense(fb, oracle, n, a):
+    """BASELINE config 5: the same data zero-padded to the full cuboid and transformed unpruned by
+    the product's kernels gives the same result as the pruned path."""
+    w = _small(n, a, batch=1 if n[0] >= 128 else 2)
+    pp = _plan(fb, w, w.batch)
+    pd = _plan(fb, w, w.batch, dense=True)
+    k = pp.points()
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    d_dense_in = pp.dense_embed(pd, d_c)
+    psi_p = pp.inverse(d_c)
+    psi_d = pd.inverse(d_dense_in)
+    torch.cuda.synchronize()
+    # embedding is a pure scatter: bit-exact against the oracle-side definition
+    cube = np.zeros((w.batch,) + tuple(n), np.complex128)  # [b][k1+N1/2][k2+N2/2][k3+N3/2]
+    cube[:, k[0] + n[0] // 2, k[1] + n[1] // 2, k[2] + n[2] // 2] = c
+    assert np.array_equal(d_dense_in.cpu().numpy().reshape(cube.shape), cube)
+    assert _rel(psi_d.cpu().numpy(), psi_p.cpu().numpy()) <= w.tol
+    if n[0] <= 128:
+        assert _rel(psi_d.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol
+    back_d = pp.dense_extract(pd, pd.forward(psi_d))
+    back_p = pp.forward(psi_p)
+    torch.cuda.synchronize()
+    assert _rel(back_d.cpu().numpy(), c) <= w.tol and _rel(back_p.cpu().numpy(), c) <= w.tol
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_full_size_configs_sampled_bands(fb, oracle, cfg):
+    """BASELINE.json's five configurations at full batch size, in the launch configuration bench.py
+    times; the oracle checks a sample of bands (every band is an independent transform)."""
+    w = wl.WORKLOADS[cfg]
+    p = _plan(fb, w, w.batch)
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    sample = sorted({0, w.batch // 2, w.batch - 1})
+    C = float(np.prod(w.n))
+    if w.op == "vloc":
+        v = wl.potential(w)
+        d_o = p.apply_vloc(d_c, torch.from_numpy(v).cuda())
+        torch.cuda.synchronize()
+        ref = oracle.apply_vloc(w.n, k, c[sample], v, 1.0 / C)
+        assert _rel(d_o[sample].cpu().numpy(), ref) <= w.tol
+    else:
+        d_psi = p.inverse(d_c)
+        d_rt = p.forward(d_psi)
+        torch.cuda.synchronize()
+        ref = oracle.inverse(w.n, k, c[sample])
+        assert _rel(d_psi[sample].cpu().numpy(), ref) <= w.tol
+        assert _rel(d_rt.cpu().numpy(), c) <= w.tol
+        # Parseval at full size: sum |psi|^2 = C sum |c|^2 (holds at any size)
+        e_psi = float((d_psi.abs() ** 2).sum().item())
+        e_c = float((np.abs(c.astype(np.complex128)) ** 2).sum())
+        assert abs(e_psi - C * e_c) <= 1e-6 * C * e_c

@@ -1,0 +1,110 @@
+"""CPU-only tests of the C-ABI library: it loads, exports every symbol include/fftb.h declares,
+the host plan builder reproduces the oracle's stick map bit for bit, and the error paths return
+codes instead of throwing.  No kernel is launched here."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2406_05577_b200 import binding as fb
+from paper_2406_05577_b200 import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    from paper_2406_05577_b200.build import build
+
+    build()
+
+
+def test_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "fftb.h")).read()
+    declared = set(re.findall(r"\b(fftb_[a-z_]+)\s*\(", hdr))
+    assert declared == set(fb.SYMBOLS)
+    L = ctypes.CDLL(str(fb._LIBPATH))
+    for s in declared:
+        assert hasattr(L, s), s
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_stick_map_bit_exact_vs_oracle(oracle, cfg):
+    w = wl.WORKLOADS[cfg]
+    p = fb.Plan(w.n, w.cutoff, batch=w.batch, dtype=w.dtype)
+    m, o = p.get_map(), oracle.stick_map(w.n, w.cutoff)
+    for key in ("k1", "k2", "k3lo", "len", "off"):
+        assert m[key].dtype == o[key].dtype and np.array_equal(m[key], o[key]), key
+    assert p.info["n_points"] == int(o["off"][-1]) and p.info["n_sticks"] == len(o["k1"])
+    assert p.info["n_xocc"] == 2 * w.cutoff[0] + 1
+    k = oracle.enum_points(w.n, w.cutoff)
+    pk = p.points()
+    assert all(np.array_equal(a, b) for a, b in zip(pk, k))
+    elem = 16 if w.dtype == "c128" else 8
+    assert p.info["min_bytes_per_band_dir"] == (p.S + int(np.prod(w.n))) * elem
+    p.destroy()
+
+
+def test_smaller_cutoffs_and_ellipsoids_vs_oracle(oracle):
+    for n, a in [((32, 32, 64), (5, 7, 16)), ((64, 64, 32), (16, 3, 0)), ((128, 128, 96), (1, 32, 24)),
+                 ((32, 32, 32), (0, 0, 0))]:
+        p = fb.Plan(n, a)
+        m, o = p.get_map(), oracle.stick_map(n, a)
+        for key in ("k1", "k2", "k3lo", "len", "off"):
+            assert np.array_equal(m[key], o[key]), (n, a, key)
+
+
+def test_dense_plan_map():
+    p = fb.Plan((32, 32, 64), dense=True)
+    m = p.get_map()
+    assert p.S == 32 * 32 * 64 and p.info["n_sticks"] == 1024 and p.info["n_xocc"] == 32
+    assert np.all(m["len"] == 64) and np.all(m["k3lo"] == -32)
+    assert m["k1"][0] == -16 and m["k2"][0] == -16 and m["k1"][-1] == 15 and m["k2"][33] == -15
+
+
+def _create_rc(n, a, batch=1, dtype=fb.FFTB_C128, scale=fb.FFTB_SCALE_FORWARD, flags=0):
+    d = fb.PlanDesc()
+    d.n[:] = n
+    d.cutoff[:] = a
+    d.batch, d.dtype, d.scale, d.flags = batch, dtype, scale, flags
+    h = ctypes.c_void_p()
+    rc = fb.lib().fftb_plan_create(ctypes.byref(h), ctypes.byref(d))
+    if rc == 0:
+        fb.lib().fftb_plan_destroy(h)
+    return rc
+
+
+def test_error_paths():
+    L = fb.lib()
+    assert _create_rc((32, 32, 32), (8, 8, 8)) == fb.FFTB_OK
+    assert _create_rc((32, 32, 32), (16, 8, 8)) == fb.FFTB_EINVAL        # 2a >= N aliases (R9)
+    assert _create_rc((32, 32, 32), (8, -1, 8)) == fb.FFTB_EINVAL
+    assert _create_rc((0, 32, 32), (8, 8, 8)) == fb.FFTB_EINVAL
+    assert _create_rc((32, 32, 32), (8, 8, 8), batch=0) == fb.FFTB_EINVAL
+    assert _create_rc((32, 32, 32), (8, 8, 8), dtype=7) == fb.FFTB_EINVAL
+    assert _create_rc((32, 32, 32), (8, 8, 8), flags=2) == fb.FFTB_EINVAL
+    # outside the predefined patterns
+    assert _create_rc((40, 40, 40), (8, 8, 8)) == fb.FFTB_EUNSUPPORTED
+    assert _create_rc((32, 64, 32), (8, 8, 8)) == fb.FFTB_EUNSUPPORTED
+    assert _create_rc((32, 32, 32), (12, 8, 8)) == fb.FFTB_EUNSUPPORTED   # a > N/4: not a half-band plan
+    assert L.fftb_plan_create(None, None) == fb.FFTB_EINVAL
+    assert L.fftb_plan_destroy(None) == fb.FFTB_EINVAL
+    assert L.fftb_plan_info_get(None, None) == fb.FFTB_EINVAL
+    # execute before bind
+    p = fb.Plan((32, 32, 32), (8, 8, 8))
+    buf = ctypes.create_string_buffer(64)
+    a = ctypes.c_void_p((ctypes.addressof(buf) + 15) // 16 * 16)
+    assert L.fftb_inverse(p._h, a, a, 1, None) == fb.FFTB_ESTATE
+    assert L.fftb_forward(p._h, None, a, 1, None) == fb.FFTB_EINVAL
+    assert L.fftb_plan_bind(p._h, None, 0, None) == fb.FFTB_EINVAL
+    assert fb.strerror(fb.FFTB_EUNSUPPORTED).startswith("description outside")
+    assert fb.strerror(-99) == "unknown fftb status"
+
+
+def test_missing_library_fails_loudly(monkeypatch, tmp_path):
+    monkeypatch.setattr(fb, "_lib", None)
+    monkeypatch.setattr(fb, "_LIBPATH", tmp_path / "nope.so")
+    with pytest.raises(ImportError, match="no CPU fallback"):
+        fb.lib()
