@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the sphere <-> cuboid hot path on B200 (driver contract in DESIGN.md).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input: for the default
+workload (BASELINE.json configs[2], "config 3": 128^3 grid, complex128, 128 bands, sphere radius 32)
+that is fftb_inverse followed by fftb_forward on all 128 bands, i.e. 256 band 3D-FFTs.
+Prints ONE JSON line on rank 0.  N > 1 shards BANDS over GPUs (every rank owns a full batch: weak
+scaling, no data-path collective).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2406_05577_b200 import workloads as wl  # noqa: E402
+
+METRIC = "band 3D-FFTs/sec (inv+fwd)"
+UNIT = "band-FFTs/s"
+NOMINAL_HBM_GBS = 8000.0     # BASELINE.json's "~8 TB/s" target denominator
+FALLBACK_HBM_GBS = 6650.0    # /opt/skills/guides/B200_PROFILING.md fallback
+FP64_PEAK_TFLOPS = 36.1      # probed on this pool's B200: 62 FMA/clk/SM @ 1965 MHz
+FP32_PEAK_TFLOPS = 65.9
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback"
+
+
+def nominal_flops_per_band_dir(n, info):
+    """5 N log2 N per transformed line with the pruned line counts."""
+    n1, n2, n3 = n
+    f = lambda m: 5.0 * m * math.log2(m)
+    return info["n_sticks"] * f(n3) + info["n_xocc"] * n3 * f(n2) + n2 * n3 * f(n1)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100", "-i", str(self.idx)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._pump, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle as the CPU baseline / reference arm (the one place outside tests/ that runs oracle/)
+# ------------------------------------------------------------------------------------------------
+def oracle_step(w, k, c, v, orc):
+    """One oracle pass of the workload's operation over the bands in c."""
+    C = float(np.prod(w.n))
+    if w.op == "vloc":
+        return orc.apply_vloc(w.n, k, c, v, 1.0 / C)
+    psi = orc.inverse(w.n, k, c)
+    return orc.forward(w.n, k, psi, 1.0 / C)
+
+
+def oracle_sample_bands(w):
+    # sized for roughly 10-30 s of CPU work over the default steps on the box's host cores
+    return {1: 4, 2: 16, 3: 4, 4: 2, 5: 1}[w.number]
+
+
+def time_oracle(w, steps, warmup):
+    import oracle as orc
+
+    orc.build()
+    k = orc.enum_points(w.n, w.cutoff)
+    nb = oracle_sample_bands(w)
+    c = wl.coefficients(w, *k, batch=nb)
+    v = wl.potential(w) if w.op == "vloc" else None
+    for _ in range(warmup):
+        oracle_step(w, k, c, v, orc)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(w, k, c, v, orc)
+    dt = (time.perf_counter() - t0) / steps
+    return {"value": 2 * nb / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "sample": f"{nb} of {w.batch} bands of the workload per step (inverse+forward each), oracle as it stands, "
+                      f"-O2 -fopenmp, {steps} steps after {warmup} warm-up"}, dt
+
+
+def config_dict(w, extra=None):
+    d = {"workload": f"config {w.number}: {w.name}", "grid": list(w.n), "cutoff": list(w.cutoff), "bands_per_gpu": w.batch,
+         "op": w.op, "l2": "inputs larger than L2 (cuboids %.2f GB per GPU), no flush" % (
+             w.batch * np.prod(w.n) * (16 if w.dtype == "c128" else 8) / 1e9)}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    cb, dt = time_oracle(w, steps, warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": config_dict(w, {"note": "CPU oracle on host cores, bounded sample"}),
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------------
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2406_05577_b200 import binding as fb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU path; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    fb.lib()  # fail loudly if libfftb.so is missing
+
+    nb = w.batch
+    plan = fb.Plan(w.n, w.cutoff, batch=nb, dtype=w.dtype, scale="forward").bind(host_staging=True)
+    info = plan.info
+    elem = 16 if w.dtype == "c128" else 8
+    k = plan.points()
+    # every rank owns its own batch of bands (band sharding); the seed differs per rank
+    c = wl.coefficients(w, *k, seed=1000 + w.number + 7919 * rank)
+    h_c = torch.from_numpy(c).pin_memory()
+    h_out = torch.empty_like(h_c).pin_memory()
+    d_c = h_c.cuda()
+    d_out = torch.empty_like(d_c)
+    vloc = w.op == "vloc"
+    d_v = torch.from_numpy(wl.potential(w)).cuda() if vloc else None
+    d_psi = None if vloc else torch.empty(plan.cuboid_shape(nb), dtype=plan.torch_complex, device="cuda")
+
+    def step():
+        if vloc:
+            plan.apply_vloc(d_c, d_v, d_out)
+            return plan.last_launches()
+        plan.inverse(d_c, d_psi)
+        n = plan.last_launches()
+        plan.forward(d_psi, d_out)
+        return n + plan.last_launches()
+
+    def step_e2e():
+        if vloc:
+            plan.apply_vloc_host(h_c, h_out, d_v)
+            return plan.last_launches()
+        plan.inverse_host(h_c, d_psi)
+        n = plan.last_launches()
+        plan.forward_host(d_psi, h_out)
+        return n + plan.last_launches()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed(fn, steps, warmup, sample_clocks=False, profile=False):
+        for _ in range(warmup):
+            fn()
+        barrier()
+        sampler = ClockSampler(local) if sample_clocks else None
+        if sampler:
+            sampler.start()
+            time.sleep(0.25)
+        if profile:
+            plan.profile(True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        launches = 0
+        e0.record()
+        for _ in range(steps):
+            launches += fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        clocks = sampler.stop() if sampler else None
+        prof = plan.profile_read() if profile else None
+        if profile:
+            plan.profile(False)
+        barrier()
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms / steps, clocks, prof, launches
+
+    K, W = max(1, args.steps), max(3, args.warmup)
+    ms_step, clocks, prof, launches = timed(step, K, W, sample_clocks=True, profile=True)
+    ms_e2e, _, _, _ = timed(step_e2e, K, max(1, min(W, 3)))
+
+    transforms = 2 * nb * world
+    value = transforms / (ms_step * 1e-3)
+    e2e_value = transforms / (ms_e2e * 1e-3)
+    peak, peak_kind = measured_peaks()
+    min_bytes_step = 2 * nb * info["min_bytes_per_band_dir"]           # per GPU, inverse + forward
+    step_gbs = min_bytes_step / (ms_step * 1e-3) / 1e9
+    C = int(np.prod(w.n))
+    # dominant kernel: the plane kernel with the largest total time in the timed region
+    dom = max(("plane_inv", "plane_fwd", "plane_vloc"), key=lambda kk: prof[kk][0])
+    dom_ms, dom_n = prof[dom]
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get(f"config{w.number}", {}).get(dom)
+    except Exception:
+        pass
+    if not vloc:
+        # algorithmic bytes of the plane kernel = the cuboid side of the direction (C elements per band;
+        # its other operand, the intermediate A, is not algorithmic traffic) -- DESIGN.md "Roofline"
+        bytes_total = K * nb * C * elem
+        ach = bytes_total / (dom_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "peak_kind": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})", "traffic": traffic,
+                "avg_launch_ms": dom_ms / max(dom_n, 1), "launches_timed": dom_n,
+                "bytes_per_launch": bytes_total / max(dom_n, 1)}
+    else:
+        fl = K * nb * 2 * nominal_flops_per_band_dir(w.n, info)
+        pk = FP64_PEAK_TFLOPS if w.dtype == "c128" else FP32_PEAK_TFLOPS
+        ach = fl / (dom_ms * 1e-3) / 1e12
+        roof = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
+                "peak_kind": "register-only FMA probe on this pool's B200 (DESIGN.md)", "traffic": traffic,
+                "avg_launch_ms": dom_ms / max(dom_n, 1), "launches_timed": dom_n,
+                "note": "fused vloc never writes the cuboid; flops counted as 5 N log2 N per pruned line, y and x passes twice"}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu_baseline, _ = time_oracle(w, 2, 1)
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if w.dtype == "c128" else "f32", "data": "synthetic",
+            "config": config_dict(w, {"parallelism": f"band-sharded x{world}, no collective", "chunk_bands": info["chunk_bands"]}),
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e,
+                    "h2d_bytes_per_step": int(h_c.numel() * elem), "d2h_bytes_per_step": int(h_out.numel() * elem),
+                    "api": "fftb_inverse_host + fftb_forward_host (pinned host packed arrays)" if not vloc
+                           else "fftb_apply_vloc_host (pinned host packed arrays)"},
+            "gpu_launches": int(launches),
+            "roofline": roof,
+            "step_roofline": {"min_bytes_per_step_per_gpu": int(min_bytes_step), "achieved_gbs": step_gbs,
+                              "frac_of_8000_nominal": step_gbs / NOMINAL_HBM_GBS, "frac_of_measured_copy": step_gbs / peak,
+                              "nominal_tflops_5nlog2n": 2 * nb * nominal_flops_per_band_dir(w.n, info) / (ms_step * 1e-3) / 1e12},
+            "kernel_ms_per_step": {kk: prof[kk][0] / K for kk in prof if prof[kk][1]},
+            "cpu_baseline": cpu_baseline,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)   # the paper's protocol: 10 warm-up + 10 timed
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5 (default 3, the graded one)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    w = wl.WORKLOADS[args.config]
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()

@@ -143,6 +143,14 @@ int fftb_dense_extract(fftb_plan pruned, fftb_plan dense, const void *d_packed_d
 /* Number of kernels the last execute call on this plan launched (for launch accounting). */
 int fftb_plan_last_launches(fftb_plan p);
 
+/* Per-kernel timing for benchmarks.  fftb_plan_profile(p, 1) makes every later execute call record a
+ * CUDA event pair around each kernel it launches (on the launching stream); fftb_plan_profile_read
+ * waits for them, adds the elapsed milliseconds and launch counts per kernel kind into ms[5] and
+ * count[5] -- 0 inverse z pass, 1 inverse plane, 2 forward plane, 3 forward z pass, 4 fused vloc
+ * plane -- and clears the record.  fftb_plan_profile(p, 0) switches it off. */
+int fftb_plan_profile(fftb_plan p, int enable);
+int fftb_plan_profile_read(fftb_plan p, double *ms, int64_t *count);
+
 int fftb_plan_destroy(fftb_plan p);
 
 const char *fftb_strerror(int code);

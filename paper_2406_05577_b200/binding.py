@@ -25,7 +25,7 @@ SYMBOLS = [
     "fftb_inverse", "fftb_forward", "fftb_apply_vloc",
     "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
     "fftb_dense_embed", "fftb_dense_extract",
-    "fftb_plan_last_launches", "fftb_plan_destroy", "fftb_strerror",
+    "fftb_plan_last_launches", "fftb_plan_profile", "fftb_plan_profile_read", "fftb_plan_destroy", "fftb_strerror",
 ]
 
 
@@ -69,6 +69,8 @@ def lib():
         for name in ("fftb_dense_embed", "fftb_dense_extract"):
             getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
         L.fftb_plan_last_launches.argtypes = [vp]
+        L.fftb_plan_profile.argtypes = [vp, i32]
+        L.fftb_plan_profile_read.argtypes = [vp, vp, vp]
         L.fftb_plan_destroy.argtypes = [vp]
         L.fftb_strerror.argtypes = [i32]
         L.fftb_strerror.restype = ctypes.c_char_p
@@ -238,6 +240,19 @@ class Plan:
 
     def last_launches(self) -> int:
         return int(lib().fftb_plan_last_launches(self._h))
+
+    KERNEL_KINDS = ("zpass_inv", "plane_inv", "plane_fwd", "zpass_fwd", "plane_vloc")
+
+    def profile(self, enable: bool):
+        _check(lib().fftb_plan_profile(self._h, int(bool(enable))), "fftb_plan_profile")
+
+    def profile_read(self):
+        """-> {kernel kind: (total ms, launches)} since profiling was enabled / last read."""
+        ms = np.zeros(5, dtype=np.float64)
+        cnt = np.zeros(5, dtype=np.int64)
+        _check(lib().fftb_plan_profile_read(self._h, ms.ctypes.data_as(ctypes.c_void_p),
+                                            cnt.ctypes.data_as(ctypes.c_void_p)), "fftb_plan_profile_read")
+        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(self.KERNEL_KINDS)}
 
     def destroy(self):
         if self._h:

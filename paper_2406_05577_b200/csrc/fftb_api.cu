@@ -191,7 +191,34 @@ struct fftb_plan_s {
     DevPlan dev;
     int sticky;
     int launches;
+    // optional per-kernel timing (fftb_plan_profile): event pairs recorded around every launch
+    bool prof;
+    std::vector<cudaEvent_t> ev;   // pairs
+    std::vector<int> ev_kind;      // kernel kind of each pair
+    size_t ev_used;
 };
+
+enum { K_ZINV = 0, K_PLANE_INV = 1, K_PLANE_FWD = 2, K_ZFWD = 3, K_PLANE_VLOC = 4, K_KINDS = 5 };
+
+static void prof_begin(fftb_plan p, int kind, cudaStream_t st)
+{
+    if (!p->prof) return;
+    if (p->ev_used + 2 > p->ev.size()) {
+        cudaEvent_t a, b;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { p->prof = false; return; }
+        p->ev.push_back(a);
+        p->ev.push_back(b);
+        p->ev_kind.push_back(kind);
+    }
+    p->ev_kind[p->ev_used / 2] = kind;
+    cudaEventRecord(p->ev[p->ev_used], st);
+}
+static void prof_end(fftb_plan p, cudaStream_t st)
+{
+    if (!p->prof) return;
+    cudaEventRecord(p->ev[p->ev_used + 1], st);
+    p->ev_used += 2;
+}
 
 extern "C" {
 
@@ -329,6 +356,8 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
         p->staging = false;
         p->sticky = 0;
         p->launches = 0;
+        p->prof = false;
+        p->ev_used = 0;
     } catch (const std::bad_alloc &) {
         delete p;
         return FFTB_ENOMEM;
@@ -412,8 +441,12 @@ int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void
         const int nc = nb - b0 < p->chunk ? nb - b0 : p->chunk;
         const unsigned char *pk = (const unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
         unsigned char *cb = (unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
+        prof_begin(p, K_ZINV, st);
         rc = p->zl.inv(p->dev, pk, A, p->a_inv_stride, nc, st);
+        prof_end(p, st);
+        prof_begin(p, K_PLANE_INV, st);
         if (!rc) rc = p->plk.run[MODE_INV](p->dev, A, nullptr, nullptr, cb, nullptr, p->a_inv_stride, 0, nc, st);
+        prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
         p->launches += 2;
     }
@@ -431,8 +464,12 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
         const int nc = nb - b0 < p->chunk ? nb - b0 : p->chunk;
         unsigned char *pk = (unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
         const unsigned char *cb = (const unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
+        prof_begin(p, K_PLANE_FWD, st);
         rc = p->plk.run[MODE_FWD](p->dev, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd_stride, nc, st);
+        prof_end(p, st);
+        prof_begin(p, K_ZFWD, st);
         if (!rc) rc = p->zl.fwd(p->dev, A, pk, p->a_fwd_stride, nc, st);
+        prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
         p->launches += 2;
     }
@@ -452,9 +489,15 @@ int fftb_apply_vloc(fftb_plan p, const void *d_in, void *d_out, const void *d_vl
         const int nc = nb - b0 < p->chunk ? nb - b0 : p->chunk;
         const unsigned char *pi = (const unsigned char *)d_in + (size_t)b0 * p->S * p->elem;
         unsigned char *po = (unsigned char *)d_out + (size_t)b0 * p->S * p->elem;
+        prof_begin(p, K_ZINV, st);
         rc = p->zl.inv(p->dev, pi, Ai, p->a_inv_stride, nc, st);
+        prof_end(p, st);
+        prof_begin(p, K_PLANE_VLOC, st);
         if (!rc) rc = p->plk.run[MODE_VLOC](p->dev, Ai, Af, nullptr, nullptr, d_vloc, p->a_inv_stride, p->a_fwd_stride, nc, st);
+        prof_end(p, st);
+        prof_begin(p, K_ZFWD, st);
         if (!rc) rc = p->zl.fwd(p->dev, Af, po, p->a_fwd_stride, nc, st);
+        prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
         p->launches += 3;
     }
@@ -551,9 +594,33 @@ int fftb_dense_extract(fftb_plan pruned, fftb_plan dense, const void *d_packed_d
 
 int fftb_plan_last_launches(fftb_plan p) { return p ? p->launches : FFTB_EINVAL; }
 
+int fftb_plan_profile(fftb_plan p, int enable)
+{
+    if (!p) return FFTB_EINVAL;
+    p->prof = enable != 0;
+    p->ev_used = 0;
+    return FFTB_OK;
+}
+
+int fftb_plan_profile_read(fftb_plan p, double *ms, int64_t *count)
+{
+    if (!p || !ms || !count) return FFTB_EINVAL;
+    for (int k = 0; k < K_KINDS; ++k) { ms[k] = 0.0; count[k] = 0; }
+    for (size_t i = 0; i + 1 < p->ev_used; i += 2) {
+        if (cudaEventSynchronize(p->ev[i + 1]) != cudaSuccess) return FFTB_ECUDA;
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, p->ev[i], p->ev[i + 1]) != cudaSuccess) return FFTB_ECUDA;
+        ms[p->ev_kind[i / 2]] += t;
+        count[p->ev_kind[i / 2]] += 1;
+    }
+    p->ev_used = 0;
+    return FFTB_OK;
+}
+
 int fftb_plan_destroy(fftb_plan p)
 {
     if (!p) return FFTB_EINVAL;
+    for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
     delete p;
     return FFTB_OK;
 }
