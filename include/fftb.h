@@ -83,11 +83,13 @@ typedef struct {
     int64_t device_bytes; /* smallest block fftb_plan_bind accepts (tables + workspace) */
     int64_t device_bytes_host; /* block size that also holds the staging area of the *_host calls
                                   (batch * S elements more) */
-    int64_t chunk_bands;  /* bands processed per kernel group (the workspace holds this many) */
+    int64_t chunk_bands;  /* bands per kernel group in fftb_inverse (the workspace holds this many) */
     int64_t min_bytes_per_band_dir; /* algorithmic bytes of one band, one direction: (S + C) * elem */
     int64_t workspace_offset; /* byte offset of the plane-major intermediate A inside the bind block */
     int64_t pitch;        /* row pitch of A in elements: A[band][z][pitch] after the inverse z pass */
     int64_t y_residues;   /* number of partial A planes the forward plane kernel writes per band */
+    int64_t chunk_bands_fwd;  /* bands per kernel group in fftb_forward */
+    int64_t chunk_bands_vloc; /* bands per kernel group in fftb_apply_vloc */
 } fftb_plan_info;
 
 /* Create a plan (host only, no CUDA call).  Builds the offset array -- the stick map -- from the

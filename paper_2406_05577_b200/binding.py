@@ -37,7 +37,7 @@ class PlanDesc(ctypes.Structure):
 class PlanInfo(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int64) for k in (
         "n_points", "n_sticks", "n_xocc", "device_bytes", "device_bytes_host", "chunk_bands",
-        "min_bytes_per_band_dir", "workspace_offset", "pitch", "y_residues")]
+        "min_bytes_per_band_dir", "workspace_offset", "pitch", "y_residues", "chunk_bands_fwd", "chunk_bands_vloc")]
 
 
 class FftbError(RuntimeError):

@@ -7,6 +7,7 @@
 // (FFTB_EUNSUPPORTED), and sizes the workspace.
 #include "../../include/fftb.h"
 #include "fftb_kernels.cuh"
+#include "fftb_plane_fast.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -107,6 +108,68 @@ int launch_plane(const DevPlan &pl, const void *Ain, void *Aout, const void *cin
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 
+// warp-synchronous plane kernel (fftb_plane_fast.cuh): half-band power-of-two grids
+constexpr int FAST_NW = 8;
+template <typename T, class F, int MODE>
+int launch_plane_fast(const DevPlan &pl, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
+                      long long sout, int nb, cudaStream_t st)
+{
+    auto k = plane_fast_k<T, F, FAST_NW, MODE>;
+    const size_t smem = F::smem_bytes(FAST_NW);
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    dim3 grid(2 * pl.n3, nb);
+    k<<<grid, FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
+{
+    using F = FastCfg<T, N, P1, P2>;
+    static_assert(F::smem_bytes(FAST_NW) <= 113 * 1024, "two CTAs per SM");
+    return PlaneLaunch{2, {&launch_plane_fast<T, F, MODE_INV>, &launch_plane_fast<T, F, MODE_FWD>, &launch_plane_fast<T, F, MODE_VLOC>}};
+}
+bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)
+{
+    if (dense) return false;
+    if (dtype == FFTB_C128 && n == 128) { *out = make_plane_fast<double, 128, 8, 8>(); return true; }
+    if (dtype == FFTB_C128 && n == 64) { *out = make_plane_fast<double, 64, 8, 4>(); return true; }
+    if (dtype == FFTB_C64 && n == 128) { *out = make_plane_fast<float, 128, 8, 8>(); return true; }
+    if (dtype == FFTB_C64 && n == 64) { *out = make_plane_fast<float, 64, 8, 4>(); return true; }
+    return false;
+}
+
+template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
+{
+    auto k = zpass_fast_inv_k<T, F, FAST_NW>;
+    const size_t smem = sizeof(cx<T>) * (size_t)FAST_NW * F::EXW;
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    dim3 grid((pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), nb);
+    k<<<grid, FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
+{
+    auto k = zpass_fast_fwd_k<T, F, FAST_NW>;
+    const size_t smem = sizeof(cx<T>) * (size_t)FAST_NW * F::EXW;
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    dim3 grid((pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), nb);
+    k<<<grid, FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+template <typename T, int N, int P1, int P2> ZLaunch make_z_fast()
+{
+    using F = FastCfg<T, N, P1, P2>;
+    return ZLaunch{&launch_zfast_inv<T, F>, &launch_zfast_fwd<T, F>};
+}
+bool find_z_fast(int dtype, int n, bool dense, ZLaunch *out)
+{
+    if (dense) return false;
+    if (dtype == FFTB_C128 && n == 128) { *out = make_z_fast<double, 128, 8, 8>(); return true; }
+    if (dtype == FFTB_C128 && n == 64) { *out = make_z_fast<double, 64, 8, 4>(); return true; }
+    if (dtype == FFTB_C64 && n == 128) { *out = make_z_fast<float, 128, 8, 8>(); return true; }
+    if (dtype == FFTB_C64 && n == 64) { *out = make_z_fast<float, 64, 8, 4>(); return true; }
+    return false;
+}
+
 template <typename T, int N, bool DENSE> ZLaunch make_z()
 {
     using AZ = typename ZX<N, DENSE>::type;
@@ -178,13 +241,16 @@ struct fftb_plan_s {
     std::vector<int32_t> k1, k2, k3lo, len;
     std::vector<int64_t> off;
     std::vector<int4> h_stick, h_col;
+    std::vector<int> h_colperm;
+    int n_multi;
     std::vector<unsigned char> h_tw[3];
     ZLaunch zl;
     PlaneLaunch plk;
     // device block layout
-    size_t o_stick, o_col, o_tw[3], o_ws, o_stage, bytes_min, bytes_stage;
+    size_t o_stick, o_col, o_perm, o_tw[3], o_ws, o_stage, bytes_min, bytes_stage;
     long long a_inv_stride, a_fwd_stride; // elements per band of the intermediate
-    int chunk;                            // bands per kernel pair
+    int chunk;                            // bands per kernel group (vloc: both intermediates live)
+    int chunk_inv, chunk_fwd;             // inverse / forward alone
     // bound state
     unsigned char *d_mem;
     bool staging;
@@ -253,6 +319,14 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
     ZLaunch zl;
     PlaneLaunch plk;
     if (!find_z(desc->dtype, desc->n[2], dense, &zl) || !find_plane(desc->dtype, desc->n[0], dense, &plk)) return FFTB_EUNSUPPORTED;
+    {
+        const char *gen = getenv("FFTB_GENERIC_PLANE"); // debugging aid: keep the generic plane kernel
+        PlaneLaunch fast;
+        if (!(gen && gen[0] == '1') && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) plk = fast;
+        const char *genz = getenv("FFTB_GENERIC_Z");
+        ZLaunch zfast;
+        if (!(genz && genz[0] == '1') && find_z_fast(desc->dtype, desc->n[2], dense, &zfast)) zl = zfast;
+    }
     if (!dense)
         for (int d = 0; d < 3; ++d)
             if (4 * (long long)desc->cutoff[d] > desc->n[d]) return FFTB_EUNSUPPORTED; // half-band kernels only
@@ -309,6 +383,11 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
         p->off.push_back(run);
         p->S = run;
         p->nsticks = (int)p->k1.size();
+        for (int c = 0; c < p->nxocc; ++c)
+            if (p->h_col[c].y > 1) p->h_colperm.push_back(c);
+        p->n_multi = (int)p->h_colperm.size();
+        for (int c = 0; c < p->nxocc; ++c)
+            if (p->h_col[c].y <= 1) p->h_colperm.push_back(c);
         if (p->S >= (int64_t)1 << 31) { delete p; return FFTB_EUNSUPPORTED; }
         p->pitch = (int)align_up((size_t)p->nsticks, 16);
         p->h_stick.resize(p->nsticks);
@@ -339,16 +418,23 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
         p->a_inv_stride = (long long)n3 * p->pitch;
         p->a_fwd_stride = (long long)p->ry * n3 * p->pitch;
         const size_t per_band = (size_t)(p->a_inv_stride + p->a_fwd_stride) * p->elem; // vloc needs both
-        const size_t budget = (size_t)48 << 20;
-        long long chunk = (long long)(budget / per_band);
-        if (chunk < 1) chunk = 1;
-        if (chunk > desc->batch) chunk = desc->batch;
-        p->chunk = (int)chunk;
+        size_t budget = (size_t)48 << 20;
+        if (const char *e = getenv("FFTB_WS_MB")) { long v = atol(e); if (v > 0) budget = (size_t)v << 20; }
+        auto chunk_of = [&](size_t bytes_per_band) {
+            long long c = (long long)(budget / bytes_per_band);
+            if (c < 1) c = 1;
+            if (c > desc->batch) c = desc->batch;
+            return (int)c;
+        };
+        p->chunk = chunk_of(per_band);
+        p->chunk_inv = chunk_of((size_t)p->a_inv_stride * p->elem);
+        p->chunk_fwd = chunk_of((size_t)p->a_fwd_stride * p->elem);
         size_t o = 0;
         p->o_stick = o; o = align_up(o + sizeof(int4) * p->h_stick.size(), 256);
         p->o_col = o; o = align_up(o + sizeof(int4) * p->h_col.size(), 256);
         for (int d = 0; d < 3; ++d) { p->o_tw[d] = o; o = align_up(o + p->h_tw[d].size(), 256); }
-        p->o_ws = o; o = align_up(o + per_band * (size_t)p->chunk, 256);
+        p->o_perm = o; o = align_up(o + sizeof(int) * p->h_colperm.size(), 256);
+        p->o_ws = o; o = align_up(o + (budget > per_band ? budget : per_band), 256);
         p->bytes_min = o;
         p->o_stage = o; o = align_up(o + (size_t)desc->batch * (size_t)p->S * p->elem, 256);
         p->bytes_stage = o;
@@ -374,7 +460,9 @@ int fftb_plan_info_get(fftb_plan p, fftb_plan_info *info)
     info->n_xocc = p->nxocc;
     info->device_bytes = (int64_t)p->bytes_min;
     info->device_bytes_host = (int64_t)p->bytes_stage;
-    info->chunk_bands = p->chunk;
+    info->chunk_bands = p->chunk_inv;
+    info->chunk_bands_fwd = p->chunk_fwd;
+    info->chunk_bands_vloc = p->chunk;
     info->min_bytes_per_band_dir = (p->S + p->C) * (int64_t)p->elem;
     info->workspace_offset = (int64_t)p->o_ws;
     info->pitch = p->pitch;
@@ -404,6 +492,7 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
     unsigned char *m = (unsigned char *)d_mem;
     cudaError_t e = cudaMemcpyAsync(m + p->o_stick, p->h_stick.data(), sizeof(int4) * p->h_stick.size(), cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(m + p->o_col, p->h_col.data(), sizeof(int4) * p->h_col.size(), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(m + p->o_perm, p->h_colperm.data(), sizeof(int) * p->h_colperm.size(), cudaMemcpyHostToDevice, st);
     for (int d = 0; d < 3 && e == cudaSuccess; ++d)
         e = cudaMemcpyAsync(m + p->o_tw[d], p->h_tw[d].data(), p->h_tw[d].size(), cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) { p->sticky = FFTB_ECUDA; return FFTB_ECUDA; }
@@ -414,6 +503,8 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
     dv.nsticks = p->nsticks; dv.pitch = p->pitch; dv.nxocc = p->nxocc; dv.k1lo = p->k1lo; dv.ry = p->ry;
     dv.stick = (const int4 *)(m + p->o_stick);
     dv.col = (const int4 *)(m + p->o_col);
+    dv.colperm = (const int *)(m + p->o_perm);
+    dv.n_multi = p->n_multi;
     dv.tw1 = m + p->o_tw[0]; dv.tw2 = m + p->o_tw[1]; dv.tw3 = m + p->o_tw[2];
     dv.S = p->S;
     dv.scale = p->desc.scale == FFTB_SCALE_FORWARD ? 1.0 / (double)p->C : 1.0;
@@ -437,8 +528,8 @@ int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void
     cudaStream_t st = (cudaStream_t)stream;
     unsigned char *A = p->d_mem + p->o_ws;
     p->launches = 0;
-    for (int b0 = 0; b0 < nb; b0 += p->chunk) {
-        const int nc = nb - b0 < p->chunk ? nb - b0 : p->chunk;
+    for (int b0 = 0; b0 < nb; b0 += p->chunk_inv) {
+        const int nc = nb - b0 < p->chunk_inv ? nb - b0 : p->chunk_inv;
         const unsigned char *pk = (const unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
         unsigned char *cb = (unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
         prof_begin(p, K_ZINV, st);
@@ -460,8 +551,8 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
     cudaStream_t st = (cudaStream_t)stream;
     unsigned char *A = p->d_mem + p->o_ws;
     p->launches = 0;
-    for (int b0 = 0; b0 < nb; b0 += p->chunk) {
-        const int nc = nb - b0 < p->chunk ? nb - b0 : p->chunk;
+    for (int b0 = 0; b0 < nb; b0 += p->chunk_fwd) {
+        const int nc = nb - b0 < p->chunk_fwd ? nb - b0 : p->chunk_fwd;
         unsigned char *pk = (unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
         const unsigned char *cb = (const unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
         prof_begin(p, K_PLANE_FWD, st);

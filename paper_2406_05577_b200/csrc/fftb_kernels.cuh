@@ -40,6 +40,8 @@ struct DevPlan {
     int ry;            // number of y residues = partial A planes written by the forward plane kernel
     const int4 *stick; // {off, k3lo, len, (k1 & 0xffff) | (k2 << 16)}
     const int4 *col;   // {first stick, stick count, k2lo, 0}
+    const int *colperm; // x columns with more than one stick first, then the single-stick ones
+    int n_multi;       // number of multi-stick columns
     const void *tw1, *tw2, *tw3; // exp(+j 2 pi i / N_d), i < N_d, in the plan's precision
     long long S;       // points per band
     double scale;      // applied in zpass_fwd

@@ -1,0 +1,422 @@
+// fftb_plane_fast.cuh -- warp-synchronous plane kernel for half-band power-of-two grids (sm_100a).
+//
+// Same mathematics as plane_k in fftb_kernels.cuh (y and x passes of one z-plane, one y residue per
+// CTA; PAPER.md:96 Fig. 3, :112 staged padding), restructured for the B200 SM:
+//   * a length-N half-band line is two length-M = N/2 transforms (n = 2n' + e) of
+//         u_e[k_s mod M] = x[k_s] W^{e k_s},   k_s the SIGNED frequency in [-M/2, M/2], W = exp(+2 pi j/N)
+//     (the two aliases k_s = -M/2, +M/2 share slot M/2).  No index shift and no output modulation;
+//     the e = 0 half has no arithmetic in front of it at all: that is the pruning of the first stage.
+//   * a length-M transform is done by a GROUP of P2 lanes of one warp, P1 = M/P2 values per lane,
+//     two in-register codelet stages around one exchange through a warp-private shared-memory
+//     tile: only __syncwarp, no CTA barrier inside a transform.
+//   * the inter-stage twiddles W^{2 t m} (t = lane in group) live in registers for the whole kernel;
+//     the e = 1 pre-twiddle is W^t (one register pair) times a compile-time root of order 2 P1.
+//   * the forward direction is the exact adjoint chain, so in VLOC mode the line never leaves the
+//     registers between the inverse x pass, the V(r) multiply and the forward x pass.
+//   * the only CTA-wide barriers are the two between the y and x passes (plane buffer hand-over).
+#pragma once
+#include "fftb_kernels.cuh"
+
+namespace fftb {
+
+template <typename T, int N_, int P1_, int P2_> struct FastCfg {
+    static constexpr int N = N_, P1 = P1_, P2 = P2_, M = N_ / 2;
+    static constexpr int G = 32 / P2_;   // transforms per warp
+    static constexpr int B2 = P1_ / P2_; // stage-2 codelets per lane
+    static constexpr int LW = 128 / (int)sizeof(cx<T>); // lanes per shared-memory wavefront
+    // plane buffer pitch: >= M, congruent to LW/P2 modulo LW (conflict-free column-strided reads)
+    static constexpr int YP = M + ((LW / P2_ - M % LW) + LW) % LW;
+    static constexpr int NCOL = M + 1;
+    static constexpr int FS0 = P1_ * (P2_ + 1);
+    static constexpr int FS = P2_ >= 8 ? FS0 : FS0 + ((P2_ - FS0 % 8) + 8) % 8; // tile pitch per transform
+    static constexpr int EXW = G * FS;   // exchange elements per warp
+    static_assert(P1_ * P2_ * 2 == N_ && P1_ % P2_ == 0 && 32 % P2_ == 0 && 48 % (2 * P1_) == 0, "unsupported factorisation");
+    static constexpr size_t smem_bytes(int nwarps) { return sizeof(cx<T>) * ((size_t)NCOL * YP + (size_t)nwarps * EXW); }
+};
+
+// signed frequency held by lane t in slot j (slot P1/2 of lane 0 is the -M/2 alias; +M/2 is extra)
+template <class F> __device__ __forceinline__ int ks_of(int t, int j) { return t + F::P2 * j - (j >= F::P1 / 2 ? F::M : 0); }
+// order-2P1 root index of the e = 1 pre-twiddle of slot j (the sign of the wrapped half is folded in)
+template <class F> __host__ __device__ constexpr int jroot(int j) { return j < F::P1 / 2 ? j : j + F::P1; }
+
+// e = 1 pre-twiddle (inverse): x[j] *= W^t * w_{2P1}^{jroot(j)}
+template <class F, int J, typename T> __device__ __forceinline__ void pre_inv(cx<T> (&x)[F::P1], cx<T> g)
+{
+    if constexpr (J < F::P1) {
+        x[J] = mul_root<jroot<F>(J), 2 * F::P1, +1, T>(cmul(x[J], g));
+        pre_inv<F, J + 1, T>(x, g);
+    }
+}
+// forward combine: F[j] = G0[j] + conj(W^t w^{jroot(j)}) G1[j]; returns the G1 term in g1
+template <class F, int J, typename T> __device__ __forceinline__ void post_fwd(cx<T> (&g1)[F::P1], cx<T> g)
+{
+    if constexpr (J < F::P1) {
+        g1[J] = cmulc(mul_root<jroot<F>(J), 2 * F::P1, -1, T>(g1[J]), g);
+        post_fwd<F, J + 1, T>(g1, g);
+    }
+}
+
+// conj twiddle w_{P1}^{t' b} of the forward first stage for codelet b > 0
+template <class F, int B, int TP, typename T> __device__ __forceinline__ void fwd_btw(cx<T> (&y)[F::P2])
+{
+    if constexpr (TP < F::P2) {
+        y[TP] = mul_root<TP * B, F::P1, -1, T>(y[TP]);
+        fwd_btw<F, B, TP + 1, T>(y);
+    }
+}
+template <class F, int B, typename T> __device__ __forceinline__ void fwd_btw_all(cx<T> (&y)[F::B2][F::P2])
+{
+    if constexpr (B < F::B2) {
+        if constexpr (B > 0) fwd_btw<F, B, 1, T>(y[B]);
+        fwd_btw_all<F, B + 1, T>(y);
+    }
+}
+
+// length-M inverse transform of the group: x[j] = u[t + P2 j]  ->  y[b][q] = out[(t + P2 b) + P1 q]
+template <class F, typename T>
+__device__ __forceinline__ void sub_inv(cx<T> (&x)[F::P1], cx<T> (&y)[F::B2][F::P2], const cx<T> (&tws)[F::P1], cx<T> *ex, int t)
+{
+    constexpr int P1 = F::P1, P2 = F::P2, B2 = F::B2;
+    fft_reg<P1, +1, T>(x);
+#pragma unroll
+    for (int m = 1; m < P1; ++m) x[m] = cmul(x[m], tws[m]);
+    __syncwarp();
+#pragma unroll
+    for (int m = 0; m < P1; ++m) ex[m * (P2 + 1) + t] = x[m];
+    __syncwarp();
+#pragma unroll
+    for (int b = 0; b < B2; ++b) {
+#pragma unroll
+        for (int tt = 0; tt < P2; ++tt) y[b][tt] = ex[(t + P2 * b) * (P2 + 1) + tt];
+        fft_reg<P2, +1, T>(y[b]);
+    }
+}
+
+// adjoint: y[b][q] = in[(t + P2 b) + P1 q]  ->  x[j] = G[t + P2 j]
+template <class F, typename T>
+__device__ __forceinline__ void sub_fwd(cx<T> (&y)[F::B2][F::P2], cx<T> (&x)[F::P1], const cx<T> (&tws)[F::P1], cx<T> *ex, int t)
+{
+    constexpr int P1 = F::P1, P2 = F::P2, B2 = F::B2;
+#pragma unroll
+    for (int b = 0; b < B2; ++b) {
+        fft_reg<P2, -1, T>(y[b]);
+#pragma unroll
+        for (int tt = 1; tt < P2; ++tt) y[b][tt] = cmulc(y[b][tt], tws[tt]);
+    }
+    fwd_btw_all<F, 0, T>(y);
+    __syncwarp();
+#pragma unroll
+    for (int b = 0; b < B2; ++b)
+#pragma unroll
+        for (int tt = 0; tt < P2; ++tt) ex[(t + P2 * b) * (P2 + 1) + tt] = y[b][tt];
+    __syncwarp();
+#pragma unroll
+    for (int m = 0; m < P1; ++m) x[m] = ex[m * (P2 + 1) + t];
+    fft_reg<P1, -1, T>(x);
+}
+
+// 2-element (x = 2n', 2n'+1) global accesses: 32 bytes for complex128, 16 for complex64
+__device__ __forceinline__ void st_pair(double2 *p, double2 a, double2 b)
+{
+    asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
+}
+__device__ __forceinline__ void st_pair(float2 *p, float2 a, float2 b)
+{
+    __stcs(reinterpret_cast<float4 *>(p), make_float4(a.x, a.y, b.x, b.y));
+}
+__device__ __forceinline__ void ld_pair(const double2 *p, double2 &a, double2 &b)
+{
+    asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a.x), "=d"(a.y), "=d"(b.x), "=d"(b.y) : "l"(p));
+}
+__device__ __forceinline__ void ld_pair(const float2 *p, float2 &a, float2 &b)
+{
+    const float4 v = __ldcs(reinterpret_cast<const float4 *>(p));
+    a = make_float2(v.x, v.y);
+    b = make_float2(v.z, v.w);
+}
+
+template <typename T, class F, int NW, int MODE>
+__global__ void __launch_bounds__(NW * 32, 2)
+plane_fast_k(DevPlan pl, const cx<T> *__restrict__ Ain, cx<T> *__restrict__ Aout, const cx<T> *__restrict__ cub_in,
+             cx<T> *__restrict__ cub_out, const T *__restrict__ vloc, long long a_in_stride, long long a_out_stride)
+{
+    using C = cx<T>;
+    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, YP = F::YP, NT = NW * 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *pbuf = reinterpret_cast<C *>(smem_raw);          // [NCOL][YP]: column c = k1 - k1lo, local line y'
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    C *ex = pbuf + F::NCOL * YP + warp * F::EXW + f * F::FS; // this group's exchange tile
+    const int z = blockIdx.x >> 1, r = blockIdx.x & 1, b = blockIdx.y;
+    const C *tw = reinterpret_cast<const C *>(pl.tw1);  // N1 == N2: one table
+    C tws[P1];
+#pragma unroll
+    for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
+    tws[0] = mk<T>((T)1, (T)0);
+    const C g = tw[t];
+    const int nx = pl.nxocc, k1lo = pl.k1lo;
+    const bool l0 = (t == 0);
+
+    // ------------------------------------------------------------------ inverse y pass -> pbuf
+    if constexpr (MODE != MODE_FWD) {
+        const C *src = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
+        const int ntask = (pl.n_multi + G - 1) / G;
+        for (int task = warp; task < ntask; task += NW) {
+            const int ci = task * G + f;
+            const bool act = ci < pl.n_multi;
+            const int col = act ? pl.colperm[ci] : 0;
+            const int4 co = pl.col[col];
+            C x[P1];
+#pragma unroll
+            for (int j = 0; j < P1; ++j) {
+                const int idx = ks_of<F>(t, j) - co.z;
+                x[j] = (act && (unsigned)idx < (unsigned)co.y) ? src[co.x + idx] : czero<T>();
+            }
+            const int idb = M / 2 - co.z;
+            const C bv = (act && l0 && (unsigned)idb < (unsigned)co.y) ? src[co.x + idb] : czero<T>();
+            if (r == 0) {
+                x[P1 / 2] = cadd(x[P1 / 2], bv);
+            } else {
+                x[P1 / 2] = csub(x[P1 / 2], bv);
+                pre_inv<F, 0, T>(x, g);
+            }
+            C y[B2][P2];
+            sub_inv<F, T>(x, y, tws, ex, t);
+            if (act) {
+#pragma unroll
+                for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                    for (int q = 0; q < P2; ++q) pbuf[col * YP + (t + P2 * bb) + P1 * q] = y[bb][q];
+            }
+        }
+        // single-stick columns: closed form x W^{k2 y}
+        const int n_one = nx - pl.n_multi;
+        for (int i = tid; i < n_one * M; i += NT) {
+            const int col = pl.colperm[pl.n_multi + i / M], yl = i % M;
+            const int4 co = pl.col[col];
+            pbuf[col * YP + yl] = cmul(src[co.x], tw[modn<N>(co.z * (2 * yl + r))]);
+        }
+        __syncthreads();
+    }
+
+    // ------------------------------------------------------------------ x passes, G lines per warp task
+    for (int task = warp; task < M / G; task += NW) {
+        const int yl = task * G + f;
+        const int ygl = 2 * yl + r;
+        C o0[B2][P2], o1[B2][P2]; // line values x = 2 n' + e, n' = (t + P2 b) + P1 q
+        if constexpr (MODE != MODE_FWD) {
+            C x[P1], xs[P1];
+#pragma unroll
+            for (int j = 0; j < P1; ++j) {
+                const int c = ks_of<F>(t, j) - k1lo;
+                x[j] = (unsigned)c < (unsigned)nx ? pbuf[c * YP + yl] : czero<T>();
+            }
+            const int cb = M / 2 - k1lo;
+            const C bv = (l0 && (unsigned)cb < (unsigned)nx) ? pbuf[cb * YP + yl] : czero<T>();
+#pragma unroll
+            for (int j = 0; j < P1; ++j) xs[j] = x[j];
+            xs[P1 / 2] = cadd(xs[P1 / 2], bv);
+            sub_inv<F, T>(xs, o0, tws, ex, t);
+            x[P1 / 2] = csub(x[P1 / 2], bv);
+            pre_inv<F, 0, T>(x, g);
+            sub_inv<F, T>(x, o1, tws, ex, t);
+        }
+        if constexpr (MODE == MODE_INV) {
+            C *row = cub_out + (((long long)b * pl.n3 + z) * N + ygl) * N;
+#pragma unroll
+            for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                for (int q = 0; q < P2; ++q) st_pair(row + 2 * ((t + P2 * bb) + P1 * q), o0[bb][q], o1[bb][q]);
+        }
+        if constexpr (MODE == MODE_VLOC) {
+            const T *vrow = vloc + ((long long)z * N + ygl) * N;
+#pragma unroll
+            for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                for (int q = 0; q < P2; ++q) {
+                    const int n = 2 * ((t + P2 * bb) + P1 * q);
+                    const T v0 = vrow[n], v1 = vrow[n + 1];
+                    o0[bb][q].x *= v0; o0[bb][q].y *= v0;
+                    o1[bb][q].x *= v1; o1[bb][q].y *= v1;
+                }
+        }
+        if constexpr (MODE == MODE_FWD) {
+            const C *row = cub_in + (((long long)b * pl.n3 + z) * N + ygl) * N;
+#pragma unroll
+            for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                for (int q = 0; q < P2; ++q) ld_pair(row + 2 * ((t + P2 * bb) + P1 * q), o0[bb][q], o1[bb][q]);
+        }
+        if constexpr (MODE != MODE_INV) {
+            C g0[P1], g1[P1];
+            sub_fwd<F, T>(o0, g0, tws, ex, t);
+            sub_fwd<F, T>(o1, g1, tws, ex, t);
+            post_fwd<F, 0, T>(g1, g);
+            const int cb = M / 2 - k1lo;
+            if (l0 && (unsigned)cb < (unsigned)nx) pbuf[cb * YP + yl] = csub(g0[P1 / 2], g1[P1 / 2]);
+#pragma unroll
+            for (int j = 0; j < P1; ++j) {
+                const int c = ks_of<F>(t, j) - k1lo;
+                if ((unsigned)c < (unsigned)nx) pbuf[c * YP + yl] = cadd(g0[j], g1[j]);
+            }
+        }
+    }
+
+    // ------------------------------------------------------------------ forward y pass: pbuf -> partial A
+    if constexpr (MODE != MODE_INV) {
+        __syncthreads();
+        C *dst = Aout + (long long)b * a_out_stride + ((long long)r * pl.n3 + z) * pl.pitch;
+        const int ntask = (pl.n_multi + G - 1) / G;
+        for (int task = warp; task < ntask; task += NW) {
+            const int ci = task * G + f;
+            const bool act = ci < pl.n_multi;
+            const int col = act ? pl.colperm[ci] : 0;
+            const int4 co = pl.col[col];
+            C y[B2][P2], x[P1];
+#pragma unroll
+            for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                for (int q = 0; q < P2; ++q) y[bb][q] = pbuf[col * YP + (t + P2 * bb) + P1 * q];
+            sub_fwd<F, T>(y, x, tws, ex, t);
+            if (r != 0) post_fwd<F, 0, T>(x, g); // partial of residue 1: conj(W^{k_s}) G[k]
+            if (act) {
+                const int idb = M / 2 - co.z;
+                if (l0 && (unsigned)idb < (unsigned)co.y)
+                    dst[co.x + idb] = r ? mk<T>(-x[P1 / 2].x, -x[P1 / 2].y) : x[P1 / 2];
+#pragma unroll
+                for (int j = 0; j < P1; ++j) {
+                    const int idx = ks_of<F>(t, j) - co.z;
+                    if ((unsigned)idx < (unsigned)co.y) dst[co.x + idx] = x[j];
+                }
+            }
+        }
+        // single-stick columns: one warp per column, dot product with conj(W^{k2 y})
+        const int n_one = nx - pl.n_multi;
+        for (int i = warp; i < n_one; i += NW) {
+            const int col = pl.colperm[pl.n_multi + i];
+            const int4 co = pl.col[col];
+            C acc = czero<T>();
+            for (int yl = lane; yl < M; yl += 32) acc = cadd(acc, cmulc(pbuf[col * YP + yl], tw[modn<N>(co.z * (2 * yl + r))]));
+#pragma unroll
+            for (int s = 16; s > 0; s >>= 1) {
+                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, s);
+                acc.y += __shfl_xor_sync(0xffffffffu, acc.y, s);
+            }
+            if (lane == 0) dst[co.x] = acc;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// z passes, warp-synchronous: one group of P2 lanes per stick, G sticks per warp task
+//   grid = (ceil(n_sticks / (G * NW)), bands)
+// ---------------------------------------------------------------------------------------------
+template <typename T, class F, int NW>
+__global__ void __launch_bounds__(NW * 32)
+zpass_fast_inv_k(DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride)
+{
+    using C = cx<T>;
+    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    C *ex = reinterpret_cast<C *>(smem_raw) + warp * F::EXW + f * F::FS;
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    C tws[P1];
+#pragma unroll
+    for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
+    tws[0] = mk<T>((T)1, (T)0);
+    const C g = tw[t];
+    const int s = (blockIdx.x * NW + warp) * G + f;
+    const bool act = s < pl.nsticks;
+    const int4 st = pl.stick[act ? s : 0]; // {off, k3lo, len, .}
+    const C *src = packed + (long long)blockIdx.y * pl.S + st.x;
+    C *dst = A + (long long)blockIdx.y * a_band_stride + s;
+    C x[P1], xs[P1];
+#pragma unroll
+    for (int j = 0; j < P1; ++j) {
+        const int idx = ks_of<F>(t, j) - st.y;
+        x[j] = (act && (unsigned)idx < (unsigned)st.z) ? src[idx] : czero<T>();
+    }
+    const int idb = M / 2 - st.y;
+    const C bv = (act && t == 0 && (unsigned)idb < (unsigned)st.z) ? src[idb] : czero<T>();
+#pragma unroll
+    for (int j = 0; j < P1; ++j) xs[j] = x[j];
+    xs[P1 / 2] = cadd(xs[P1 / 2], bv);
+    C y[B2][P2];
+    sub_inv<F, T>(xs, y, tws, ex, t);
+    if (act) {
+#pragma unroll
+        for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+            for (int q = 0; q < P2; ++q) dst[(long long)(2 * ((t + P2 * bb) + P1 * q)) * pl.pitch] = y[bb][q];
+    }
+    x[P1 / 2] = csub(x[P1 / 2], bv);
+    pre_inv<F, 0, T>(x, g);
+    sub_inv<F, T>(x, y, tws, ex, t);
+    if (act) {
+#pragma unroll
+        for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+            for (int q = 0; q < P2; ++q) dst[(long long)(2 * ((t + P2 * bb) + P1 * q) + 1) * pl.pitch] = y[bb][q];
+    }
+}
+
+template <typename T, class F, int NW>
+__global__ void __launch_bounds__(NW * 32)
+zpass_fast_fwd_k(DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride)
+{
+    using C = cx<T>;
+    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    C *ex = reinterpret_cast<C *>(smem_raw) + warp * F::EXW + f * F::FS;
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    C tws[P1];
+#pragma unroll
+    for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
+    tws[0] = mk<T>((T)1, (T)0);
+    const C g = tw[t];
+    const int s = (blockIdx.x * NW + warp) * G + f;
+    const bool act = s < pl.nsticks;
+    const int4 st = pl.stick[act ? s : 0];
+    const C *src = A + (long long)blockIdx.y * a_band_stride + (act ? s : 0);
+    C *dst = packed + (long long)blockIdx.y * pl.S + st.x;
+    const long long rstride = (long long)pl.n3 * pl.pitch;
+    const T scale = (T)pl.scale;
+    C y0[B2][P2], y1[B2][P2], g0[P1], g1[P1];
+#pragma unroll
+    for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+        for (int q = 0; q < P2; ++q) {
+            const long long o = (long long)(2 * ((t + P2 * bb) + P1 * q)) * pl.pitch;
+            C a = src[o], c = src[o + pl.pitch];
+            for (int p = 1; p < pl.ry; ++p) {
+                a = cadd(a, src[p * rstride + o]);
+                c = cadd(c, src[p * rstride + o + pl.pitch]);
+            }
+            y0[bb][q] = a;
+            y1[bb][q] = c;
+        }
+    sub_fwd<F, T>(y0, g0, tws, ex, t);
+    sub_fwd<F, T>(y1, g1, tws, ex, t);
+    post_fwd<F, 0, T>(g1, g);
+    if (act) {
+        const int idb = M / 2 - st.y;
+        if (t == 0 && (unsigned)idb < (unsigned)st.z) {
+            const C v = csub(g0[P1 / 2], g1[P1 / 2]);
+            dst[idb] = mk<T>(v.x * scale, v.y * scale);
+        }
+#pragma unroll
+        for (int j = 0; j < P1; ++j) {
+            const int idx = ks_of<F>(t, j) - st.y;
+            if ((unsigned)idx < (unsigned)st.z) {
+                const C v = cadd(g0[j], g1[j]);
+                dst[idx] = mk<T>(v.x * scale, v.y * scale);
+            }
+        }
+    }
+}
+
+} // namespace fftb

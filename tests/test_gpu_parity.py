@@ -155,7 +155,7 @@ def test_batch_chunking_and_partial_batches(fb, oracle):
         rt = p.forward(d_psi)
         torch.cuda.synchronize()
         assert _rel(rt.cpu().numpy(), c[:nb]) <= w.tol
-    assert p.last_launches() == 2 * -(-37 // p.info["chunk_bands"])
+    assert p.last_launches() == 2 * -(-37 // p.info["chunk_bands_fwd"])  # the last call was a forward
     with pytest.raises(fb.FftbError):
         p.inverse(torch.zeros((38, p.S), dtype=torch.complex128, device="cuda"))
 
