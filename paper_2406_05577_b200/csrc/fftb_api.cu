@@ -73,7 +73,7 @@ struct ZLaunch {
 };
 struct PlaneLaunch {
     int ry;
-    int (*run[3])(const DevPlan &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v,
+    int (*run[3])(const DevPlan &, const ColTab &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v,
                   long long sin, long long sout, int nb, cudaStream_t);
 };
 
@@ -96,7 +96,7 @@ template <typename T, class AZ> int launch_zfwd(const DevPlan &pl, const void *A
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 template <typename T, class AX, class AY, int MODE>
-int launch_plane(const DevPlan &pl, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
+int launch_plane(const DevPlan &pl, const ColTab &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
                  long long sout, int nb, cudaStream_t st)
 {
     using TU = PlaneTune<AX, AY>;
@@ -108,39 +108,65 @@ int launch_plane(const DevPlan &pl, const void *Ain, void *Aout, const void *cin
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 
-// warp-synchronous plane kernel (fftb_plane_fast.cuh): half-band power-of-two grids
-constexpr int FAST_NW = 8;
+// warp-synchronous persistent plane kernel (fftb_plane_fast.cuh): half-band power-of-two grids
+constexpr int FAST_NW = 8; // warps per CTA of the z-pass kernels
+template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 16 : 4; }; // x tasks per half plane = N/2 / G
+
+static int g_sm_count = 0;
+static int sm_count()
+{
+    if (!g_sm_count) {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+            g_sm_count = n;
+        else
+            g_sm_count = 148;
+    }
+    return g_sm_count;
+}
+
 template <typename T, class F, int MODE>
-int launch_plane_fast(const DevPlan &pl, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
+int launch_plane_fast(const DevPlan &pl, const ColTab &ct, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
                       long long sout, int nb, cudaStream_t st)
 {
-    auto k = plane_fast_k<T, F, FAST_NW, MODE>;
-    const size_t smem = F::smem_bytes(FAST_NW);
-    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-    dim3 grid(2 * pl.n3, nb);
-    k<<<grid, FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout);
+    constexpr int NW = PlaneNW<F::N>::value;
+    auto k = plane_fast_k<T, F, NW, MODE>;
+    const size_t smem = PlaneFast<T, F, NW>::smem_bytes;
+    static int per_sm = 0; // CTAs per SM of this instantiation
+    if (!per_sm) {
+        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, NW * 32, smem) != cudaSuccess || occ < 1) return FFTB_ECUDA;
+        per_sm = occ;
+    }
+    const int ntasks = 2 * pl.n3 * nb;
+    int grid = sm_count() * per_sm;
+    if (grid > ntasks) grid = ntasks;
+    k<<<grid, NW * 32, smem, st>>>(pl, ct, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout, ntasks);
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
 {
     using F = FastCfg<T, N, P1, P2>;
-    static_assert(F::smem_bytes(FAST_NW) <= 113 * 1024, "two CTAs per SM");
+    static_assert(PlaneFast<T, F, PlaneNW<N>::value>::smem_bytes <= 227 * 1024, "plane buffers do not fit in shared memory");
     return PlaneLaunch{2, {&launch_plane_fast<T, F, MODE_INV>, &launch_plane_fast<T, F, MODE_FWD>, &launch_plane_fast<T, F, MODE_VLOC>}};
 }
 bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)
 {
     if (dense) return false;
     if (dtype == FFTB_C128 && n == 128) { *out = make_plane_fast<double, 128, 8, 8>(); return true; }
+#ifndef FFTB_DEV
     if (dtype == FFTB_C128 && n == 64) { *out = make_plane_fast<double, 64, 8, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 128) { *out = make_plane_fast<float, 128, 8, 8>(); return true; }
     if (dtype == FFTB_C64 && n == 64) { *out = make_plane_fast<float, 64, 8, 4>(); return true; }
+#endif
     return false;
 }
 
 template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
 {
     auto k = zpass_fast_inv_k<T, F, FAST_NW>;
-    const size_t smem = sizeof(cx<T>) * (size_t)FAST_NW * F::EXW;
+    const size_t smem = ZFast<T, F, FAST_NW>::smem_bytes;
     if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
     dim3 grid((pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), nb);
     k<<<grid, FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
@@ -149,7 +175,7 @@ template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const voi
 template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
 {
     auto k = zpass_fast_fwd_k<T, F, FAST_NW>;
-    const size_t smem = sizeof(cx<T>) * (size_t)FAST_NW * F::EXW;
+    const size_t smem = ZFast<T, F, FAST_NW>::smem_bytes;
     if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
     dim3 grid((pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), nb);
     k<<<grid, FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);
@@ -164,9 +190,11 @@ bool find_z_fast(int dtype, int n, bool dense, ZLaunch *out)
 {
     if (dense) return false;
     if (dtype == FFTB_C128 && n == 128) { *out = make_z_fast<double, 128, 8, 8>(); return true; }
+#ifndef FFTB_DEV
     if (dtype == FFTB_C128 && n == 64) { *out = make_z_fast<double, 64, 8, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 128) { *out = make_z_fast<float, 128, 8, 8>(); return true; }
     if (dtype == FFTB_C64 && n == 64) { *out = make_z_fast<float, 64, 8, 4>(); return true; }
+#endif
     return false;
 }
 
@@ -189,12 +217,15 @@ bool find_z(int dtype, int n, bool dense, ZLaunch *out)
 {
 #define ZCASE(T, DT, N, D) \
     if (dtype == DT && n == N && dense == D) { *out = make_z<T, N, D>(); return true; }
+    ZCASE(double, FFTB_C128, 128, false)
+#ifndef FFTB_DEV /* development builds (-DFFTB_DEV) instantiate the 128^3 complex128 kernels only */
     ZCASE(double, FFTB_C128, 32, false) ZCASE(double, FFTB_C128, 64, false) ZCASE(double, FFTB_C128, 96, false)
-    ZCASE(double, FFTB_C128, 128, false) ZCASE(double, FFTB_C128, 192, false) ZCASE(double, FFTB_C128, 256, false)
+    ZCASE(double, FFTB_C128, 192, false) ZCASE(double, FFTB_C128, 256, false)
     ZCASE(float, FFTB_C64, 32, false) ZCASE(float, FFTB_C64, 64, false) ZCASE(float, FFTB_C64, 96, false)
     ZCASE(float, FFTB_C64, 128, false) ZCASE(float, FFTB_C64, 192, false) ZCASE(float, FFTB_C64, 256, false)
     ZCASE(double, FFTB_C128, 32, true) ZCASE(double, FFTB_C128, 64, true) ZCASE(double, FFTB_C128, 128, true)
     ZCASE(double, FFTB_C128, 256, true)
+#endif
 #undef ZCASE
     return false;
 }
@@ -202,12 +233,15 @@ bool find_plane(int dtype, int n, bool dense, PlaneLaunch *out)
 {
 #define PCASE(T, DT, N, D) \
     if (dtype == DT && n == N && dense == D) { *out = make_plane<T, N, D>(); return true; }
+    PCASE(double, FFTB_C128, 128, false)
+#ifndef FFTB_DEV
     PCASE(double, FFTB_C128, 32, false) PCASE(double, FFTB_C128, 64, false) PCASE(double, FFTB_C128, 96, false)
-    PCASE(double, FFTB_C128, 128, false) PCASE(double, FFTB_C128, 192, false) PCASE(double, FFTB_C128, 256, false)
+    PCASE(double, FFTB_C128, 192, false) PCASE(double, FFTB_C128, 256, false)
     PCASE(float, FFTB_C64, 32, false) PCASE(float, FFTB_C64, 64, false) PCASE(float, FFTB_C64, 96, false)
     PCASE(float, FFTB_C64, 128, false) PCASE(float, FFTB_C64, 192, false) PCASE(float, FFTB_C64, 256, false)
     PCASE(double, FFTB_C128, 32, true) PCASE(double, FFTB_C128, 64, true) PCASE(double, FFTB_C128, 128, true)
     PCASE(double, FFTB_C128, 256, true)
+#endif
 #undef PCASE
     return false;
 }
@@ -255,6 +289,7 @@ struct fftb_plan_s {
     unsigned char *d_mem;
     bool staging;
     DevPlan dev;
+    ColTab coltab; // the column table again, as a by-value kernel parameter of the fast plane kernel
     int sticky;
     int launches;
     // optional per-kernel timing (fftb_plan_profile): event pairs recorded around every launch
@@ -389,6 +424,9 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
         for (int c = 0; c < p->nxocc; ++c)
             if (p->h_col[c].y <= 1) p->h_colperm.push_back(c);
         if (p->S >= (int64_t)1 << 31) { delete p; return FFTB_EUNSUPPORTED; }
+        memset(&p->coltab, 0, sizeof(p->coltab));
+        if (p->nxocc <= FAST_MAXCOL)
+            for (int c = 0; c < p->nxocc; ++c) { p->coltab.col[c] = p->h_col[c]; p->coltab.perm[c] = p->h_colperm[c]; }
         p->pitch = (int)align_up((size_t)p->nsticks, 16);
         p->h_stick.resize(p->nsticks);
         for (int s = 0; s < p->nsticks; ++s) {
@@ -508,6 +546,9 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
     dv.tw1 = m + p->o_tw[0]; dv.tw2 = m + p->o_tw[1]; dv.tw3 = m + p->o_tw[2];
     dv.S = p->S;
     dv.scale = p->desc.scale == FFTB_SCALE_FORWARD ? 1.0 / (double)p->C : 1.0;
+#ifdef FFTB_DEV
+    dv.dbg = getenv("FFTB_DBG") ? atoi(getenv("FFTB_DBG")) : 0;
+#endif
     return FFTB_OK;
 }
 
@@ -536,7 +577,7 @@ int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void
         rc = p->zl.inv(p->dev, pk, A, p->a_inv_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_PLANE_INV, st);
-        if (!rc) rc = p->plk.run[MODE_INV](p->dev, A, nullptr, nullptr, cb, nullptr, p->a_inv_stride, 0, nc, st);
+        if (!rc) rc = p->plk.run[MODE_INV](p->dev, p->coltab, A, nullptr, nullptr, cb, nullptr, p->a_inv_stride, 0, nc, st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
         p->launches += 2;
@@ -556,7 +597,7 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
         unsigned char *pk = (unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
         const unsigned char *cb = (const unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
         prof_begin(p, K_PLANE_FWD, st);
-        rc = p->plk.run[MODE_FWD](p->dev, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd_stride, nc, st);
+        rc = p->plk.run[MODE_FWD](p->dev, p->coltab, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_ZFWD, st);
         if (!rc) rc = p->zl.fwd(p->dev, A, pk, p->a_fwd_stride, nc, st);
@@ -584,7 +625,7 @@ int fftb_apply_vloc(fftb_plan p, const void *d_in, void *d_out, const void *d_vl
         rc = p->zl.inv(p->dev, pi, Ai, p->a_inv_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_PLANE_VLOC, st);
-        if (!rc) rc = p->plk.run[MODE_VLOC](p->dev, Ai, Af, nullptr, nullptr, d_vloc, p->a_inv_stride, p->a_fwd_stride, nc, st);
+        if (!rc) rc = p->plk.run[MODE_VLOC](p->dev, p->coltab, Ai, Af, nullptr, nullptr, d_vloc, p->a_inv_stride, p->a_fwd_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_ZFWD, st);
         if (!rc) rc = p->zl.fwd(p->dev, Af, po, p->a_fwd_stride, nc, st);
@@ -684,6 +725,16 @@ int fftb_dense_extract(fftb_plan pruned, fftb_plan dense, const void *d_packed_d
 }
 
 int fftb_plan_last_launches(fftb_plan p) { return p ? p->launches : FFTB_EINVAL; }
+
+#ifdef FFTB_DEV
+int fftb_dev_clk(unsigned long long *out, int reset)
+{
+    cudaDeviceSynchronize();
+    if (cudaMemcpyFromSymbol(out, g_fftb_clk, sizeof(unsigned long long) * 16) != cudaSuccess) return -1;
+    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_fftb_clk, z, sizeof(z)); }
+    return 0;
+}
+#endif
 
 int fftb_plan_profile(fftb_plan p, int enable)
 {

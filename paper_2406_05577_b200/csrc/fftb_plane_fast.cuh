@@ -34,6 +34,14 @@ template <typename T, int N_, int P1_, int P2_> struct FastCfg {
     static constexpr size_t smem_bytes(int nwarps) { return sizeof(cx<T>) * ((size_t)NCOL * YP + (size_t)nwarps * EXW); }
 };
 
+// Column table of the y pass, passed BY VALUE as a kernel parameter (constant bank): no dependent
+// global loads stand between the start of a CTA and its first loads of the intermediate A.
+constexpr int FAST_MAXCOL = 65; // N <= 128: at most N/2 + 1 occupied k1 columns
+struct ColTab {
+    int4 col[FAST_MAXCOL];  // {first stick, stick count, k2lo, 0} per occupied k1 column
+    int perm[FAST_MAXCOL];  // multi-stick columns first, then the single-stick ones
+};
+
 // signed frequency held by lane t in slot j (slot P1/2 of lane 0 is the -M/2 alias; +M/2 is extra)
 template <class F> __device__ __forceinline__ int ks_of(int t, int j) { return t + F::P2 * j - (j >= F::P1 / 2 ? F::M : 0); }
 // order-2P1 root index of the e = 1 pre-twiddle of slot j (the sign of the wrapped half is folded in)
@@ -135,19 +143,48 @@ __device__ __forceinline__ void ld_pair(const float2 *p, float2 &a, float2 &b)
     b = make_float2(v.z, v.w);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Persistent plane kernel.  A TASK is one half z-plane: (band b, plane z, y residue r), numbered
+// id = (b * n3 + z) * 2 + r; CTA c of a grid of G CTAs owns tasks c, c + G, c + 2G, ...  The plane
+// buffer is double-buffered so that, inside one iteration, the x pass of one task and the y pass of
+// the neighbouring task are independent; odd warps run them in the opposite order to the even warps,
+// so that the loads of one half of the CTA are covered by the arithmetic of the other half.  One
+// CTA-wide barrier per iteration is the only synchronisation.
+//   INV   it: y_inv(task it)   -> buf[it&1]      | x_inv(task it-1) : buf[(it-1)&1] -> cuboid
+//   FWD   it: x_fwd(task it)   -> buf[it&1]      | y_fwd(task it-1) : buf[(it-1)&1] -> A
+//   VLOC  it: y_fwd(task it-2) : buf[it&1] -> A, then y_inv(task it) -> buf[it&1] (same warp, same
+//             columns, in this order)             | x_vloc(task it-1) in place in buf[(it-1)&1]
+// ---------------------------------------------------------------------------------------------
+#ifdef FFTB_DEV
+__device__ unsigned long long g_fftb_clk[16];
+#define FFTB_CLK_DECL unsigned long long clk_acc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}; long long clk_t = clock64();
+#define FFTB_CLK(i) { const long long clk_n = clock64(); clk_acc[i] += (unsigned long long)(clk_n - clk_t); clk_t = clk_n; }
+#define FFTB_CLK_FLUSH if (lane == 0) { for (int i = 0; i < 10; ++i) atomicAdd(&g_fftb_clk[i], clk_acc[i]); }
+#else
+#define FFTB_CLK_DECL
+#define FFTB_CLK(i)
+#define FFTB_CLK_FLUSH
+#endif
+
+template <typename T, class F, int NW> struct PlaneFast {
+    static constexpr int PB = F::NCOL * F::YP; // elements of one plane buffer
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * (2 * (size_t)PB + (size_t)NW * F::EXW);
+};
+
 template <typename T, class F, int NW, int MODE>
-__global__ void __launch_bounds__(NW * 32, 2)
-plane_fast_k(DevPlan pl, const cx<T> *__restrict__ Ain, cx<T> *__restrict__ Aout, const cx<T> *__restrict__ cub_in,
-             cx<T> *__restrict__ cub_out, const T *__restrict__ vloc, long long a_in_stride, long long a_out_stride)
+__global__ void __launch_bounds__(NW * 32, 1)
+plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct, const cx<T> *__restrict__ Ain,
+             cx<T> *__restrict__ Aout, const cx<T> *__restrict__ cub_in, cx<T> *__restrict__ cub_out,
+             const T *__restrict__ vloc, long long a_in_stride, long long a_out_stride, int ntasks)
 {
     using C = cx<T>;
-    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, YP = F::YP, NT = NW * 32;
+    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, YP = F::YP;
+    constexpr int PB = PlaneFast<T, F, NW>::PB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    C *pbuf = reinterpret_cast<C *>(smem_raw);          // [NCOL][YP]: column c = k1 - k1lo, local line y'
+    C *pbuf0 = reinterpret_cast<C *>(smem_raw); // [2][NCOL][YP]: column c = k1 - k1lo, local line y'
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    C *ex = pbuf + F::NCOL * YP + warp * F::EXW + f * F::FS; // this group's exchange tile
-    const int z = blockIdx.x >> 1, r = blockIdx.x & 1, b = blockIdx.y;
+    C *ex = pbuf0 + 2 * PB + warp * F::EXW + f * F::FS; // this group's exchange tile
     const C *tw = reinterpret_cast<const C *>(pl.tw1);  // N1 == N2: one table
     C tws[P1];
 #pragma unroll
@@ -156,251 +193,361 @@ plane_fast_k(DevPlan pl, const cx<T> *__restrict__ Ain, cx<T> *__restrict__ Aout
     const C g = tw[t];
     const int nx = pl.nxocc, k1lo = pl.k1lo;
     const bool l0 = (t == 0);
+    const int n_one = nx - pl.n_multi;
+    const int ntask_y = (pl.n_multi + G - 1) / G;
+    const int ktasks = ntasks > (int)blockIdx.x ? (ntasks - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    constexpr int LAG = (MODE == MODE_VLOC) ? 2 : 1; // iterations between the first and the last stage of a task
+#ifdef FFTB_EXP_PREFETCH
+    const int swap = (MODE == MODE_INV) ? 1 : (warp & 1);
+#else
+    const int swap = warp & 1;
+#endif
+    FFTB_CLK_DECL
 
-    // ------------------------------------------------------------------ inverse y pass -> pbuf
-    if constexpr (MODE != MODE_FWD) {
-        const C *src = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
-        const int ntask = (pl.n_multi + G - 1) / G;
-        for (int task = warp; task < ntask; task += NW) {
-            const int ci = task * G + f;
-            const bool act = ci < pl.n_multi;
-            const int col = act ? pl.colperm[ci] : 0;
-            const int4 co = pl.col[col];
-            C x[P1];
-#pragma unroll
-            for (int j = 0; j < P1; ++j) {
-                const int idx = ks_of<F>(t, j) - co.z;
-                x[j] = (act && (unsigned)idx < (unsigned)co.y) ? src[co.x + idx] : czero<T>();
-            }
-            const int idb = M / 2 - co.z;
-            const C bv = (act && l0 && (unsigned)idb < (unsigned)co.y) ? src[co.x + idb] : czero<T>();
-            if (r == 0) {
-                x[P1 / 2] = cadd(x[P1 / 2], bv);
-            } else {
-                x[P1 / 2] = csub(x[P1 / 2], bv);
-                pre_inv<F, 0, T>(x, g);
-            }
-            C y[B2][P2];
-            sub_inv<F, T>(x, y, tws, ex, t);
-            if (act) {
-#pragma unroll
-                for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                    for (int q = 0; q < P2; ++q) pbuf[col * YP + (t + P2 * bb) + P1 * q] = y[bb][q];
-            }
-        }
-        // single-stick columns: closed form x W^{k2 y}
-        const int n_one = nx - pl.n_multi;
-        for (int i = tid; i < n_one * M; i += NT) {
-            const int col = pl.colperm[pl.n_multi + i / M], yl = i % M;
-            const int4 co = pl.col[col];
-            pbuf[col * YP + yl] = cmul(src[co.x], tw[modn<N>(co.z * (2 * yl + r))]);
-        }
-        __syncthreads();
-    }
-
-    // ------------------------------------------------------------------ x passes, G lines per warp task
-    for (int task = warp; task < M / G; task += NW) {
-        const int yl = task * G + f;
-        const int ygl = 2 * yl + r;
-        C o0[B2][P2], o1[B2][P2]; // line values x = 2 n' + e, n' = (t + P2 b) + P1 q
-        if constexpr (MODE != MODE_FWD) {
-            C x[P1], xs[P1];
-#pragma unroll
-            for (int j = 0; j < P1; ++j) {
-                const int c = ks_of<F>(t, j) - k1lo;
-                x[j] = (unsigned)c < (unsigned)nx ? pbuf[c * YP + yl] : czero<T>();
-            }
-            const int cb = M / 2 - k1lo;
-            const C bv = (l0 && (unsigned)cb < (unsigned)nx) ? pbuf[cb * YP + yl] : czero<T>();
-#pragma unroll
-            for (int j = 0; j < P1; ++j) xs[j] = x[j];
-            xs[P1 / 2] = cadd(xs[P1 / 2], bv);
-            sub_inv<F, T>(xs, o0, tws, ex, t);
-            x[P1 / 2] = csub(x[P1 / 2], bv);
-            pre_inv<F, 0, T>(x, g);
-            sub_inv<F, T>(x, o1, tws, ex, t);
-        }
+#pragma unroll 1
+    for (int it = 0; it < ktasks + LAG; ++it) {
+#ifdef FFTB_EXP_PREFETCH
+        C xp[P1], bvp = czero<T>();
         if constexpr (MODE == MODE_INV) {
-            C *row = cub_out + (((long long)b * pl.n3 + z) * N + ygl) * N;
-#pragma unroll
-            for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                for (int q = 0; q < P2; ++q) st_pair(row + 2 * ((t + P2 * bb) + P1 * q), o0[bb][q], o1[bb][q]);
-        }
-        if constexpr (MODE == MODE_VLOC) {
-            const T *vrow = vloc + ((long long)z * N + ygl) * N;
-#pragma unroll
-            for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                for (int q = 0; q < P2; ++q) {
-                    const int n = 2 * ((t + P2 * bb) + P1 * q);
-                    const T v0 = vrow[n], v1 = vrow[n + 1];
-                    o0[bb][q].x *= v0; o0[bb][q].y *= v0;
-                    o1[bb][q].x *= v1; o1[bb][q].y *= v1;
-                }
-        }
-        if constexpr (MODE == MODE_FWD) {
-            const C *row = cub_in + (((long long)b * pl.n3 + z) * N + ygl) * N;
-#pragma unroll
-            for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                for (int q = 0; q < P2; ++q) ld_pair(row + 2 * ((t + P2 * bb) + P1 * q), o0[bb][q], o1[bb][q]);
-        }
-        if constexpr (MODE != MODE_INV) {
-            C g0[P1], g1[P1];
-            sub_fwd<F, T>(o0, g0, tws, ex, t);
-            sub_fwd<F, T>(o1, g1, tws, ex, t);
-            post_fwd<F, 0, T>(g1, g);
-            const int cb = M / 2 - k1lo;
-            if (l0 && (unsigned)cb < (unsigned)nx) pbuf[cb * YP + yl] = csub(g0[P1 / 2], g1[P1 / 2]);
-#pragma unroll
-            for (int j = 0; j < P1; ++j) {
-                const int c = ks_of<F>(t, j) - k1lo;
-                if ((unsigned)c < (unsigned)nx) pbuf[c * YP + yl] = cadd(g0[j], g1[j]);
-            }
-        }
-    }
-
-    // ------------------------------------------------------------------ forward y pass: pbuf -> partial A
-    if constexpr (MODE != MODE_INV) {
-        __syncthreads();
-        C *dst = Aout + (long long)b * a_out_stride + ((long long)r * pl.n3 + z) * pl.pitch;
-        const int ntask = (pl.n_multi + G - 1) / G;
-        for (int task = warp; task < ntask; task += NW) {
-            const int ci = task * G + f;
-            const bool act = ci < pl.n_multi;
-            const int col = act ? pl.colperm[ci] : 0;
-            const int4 co = pl.col[col];
-            C y[B2][P2], x[P1];
-#pragma unroll
-            for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                for (int q = 0; q < P2; ++q) y[bb][q] = pbuf[col * YP + (t + P2 * bb) + P1 * q];
-            sub_fwd<F, T>(y, x, tws, ex, t);
-            if (r != 0) post_fwd<F, 0, T>(x, g); // partial of residue 1: conj(W^{k_s}) G[k]
-            if (act) {
-                const int idb = M / 2 - co.z;
-                if (l0 && (unsigned)idb < (unsigned)co.y)
-                    dst[co.x + idb] = r ? mk<T>(-x[P1 / 2].x, -x[P1 / 2].y) : x[P1 / 2];
+            if (it < ktasks) {
+                const int id = blockIdx.x + it * gridDim.x;
+                const int z = (id >> 1) % pl.n3, b = (id >> 1) / pl.n3;
+                const C *src = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
+                const int ci = warp * G + f;
+                const bool act = ci < pl.n_multi;
+                const int4 co = ct.col[ct.perm[act ? ci : 0]];
 #pragma unroll
                 for (int j = 0; j < P1; ++j) {
                     const int idx = ks_of<F>(t, j) - co.z;
-                    if ((unsigned)idx < (unsigned)co.y) dst[co.x + idx] = x[j];
+                    xp[j] = (act && (unsigned)idx < (unsigned)co.y) ? __ldcg(src + co.x + idx) : czero<T>();
+                }
+                const int idb = M / 2 - co.z;
+                bvp = (act && l0 && (unsigned)idb < (unsigned)co.y) ? __ldcg(src + co.x + idb) : czero<T>();
+            }
+        }
+#endif
+#pragma unroll 1
+        for (int step = 0; step < 2; ++step) {
+            if ((step ^ swap) == 0) {
+                // ============================================================ y stage(s)
+                if constexpr (MODE != MODE_INV) {
+                    // -------- forward y pass: buf -> partial A of residue r
+                    const int k = (MODE == MODE_FWD) ? it - 1 : it - 2;
+                    if (k >= 0 && k < ktasks) {
+                        const int id = blockIdx.x + k * gridDim.x;
+                        const int r = id & 1, z = (id >> 1) % pl.n3, b = (id >> 1) / pl.n3;
+                        const C *pbuf = pbuf0 + (k & 1) * PB;
+                        C *dst = Aout + (long long)b * a_out_stride + ((long long)r * pl.n3 + z) * pl.pitch;
+                        for (int task = warp; task < ntask_y; task += NW) {
+                            const int ci = task * G + f;
+                            const bool act = ci < pl.n_multi;
+                            const int col = ct.perm[act ? ci : 0];
+                            const int4 co = ct.col[col];
+                            C y[B2][P2], x[P1];
+#pragma unroll
+                            for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                                for (int q = 0; q < P2; ++q) y[bb][q] = pbuf[col * YP + (t + P2 * bb) + P1 * q];
+                            sub_fwd<F, T>(y, x, tws, ex, t);
+                            if (r != 0) post_fwd<F, 0, T>(x, g); // partial of residue 1: conj(W^{k_s}) G[k]
+                            if (act) {
+                                const int idb = M / 2 - co.z;
+                                if (l0 && (unsigned)idb < (unsigned)co.y)
+                                    dst[co.x + idb] = r ? mk<T>(-x[P1 / 2].x, -x[P1 / 2].y) : x[P1 / 2];
+#pragma unroll
+                                for (int j = 0; j < P1; ++j) {
+                                    const int idx = ks_of<F>(t, j) - co.z;
+                                    if ((unsigned)idx < (unsigned)co.y) dst[co.x + idx] = x[j];
+                                }
+                            }
+                        }
+                        // single-stick columns: one warp per column, dot product with conj(W^{k2 y})
+                        for (int i = warp; i < n_one; i += NW) {
+                            const int col = ct.perm[pl.n_multi + i];
+                            const int4 co = ct.col[col];
+                            C acc = czero<T>();
+                            for (int yl = lane; yl < M; yl += 32)
+                                acc = cadd(acc, cmulc(pbuf[col * YP + yl], tw[modn<N>(co.z * (2 * yl + r))]));
+#pragma unroll
+                            for (int sft = 16; sft > 0; sft >>= 1) {
+                                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, sft);
+                                acc.y += __shfl_xor_sync(0xffffffffu, acc.y, sft);
+                            }
+                            if (lane == 0) dst[co.x] = acc;
+                        }
+                    }
+                }
+                if constexpr (MODE != MODE_FWD) {
+                    // -------- inverse y pass: A row of plane z -> buf
+                    const int k = it;
+                    if (k < ktasks) {
+                        const int id = blockIdx.x + k * gridDim.x;
+                        const int r = id & 1, z = (id >> 1) % pl.n3, b = (id >> 1) / pl.n3;
+                        C *pbuf = pbuf0 + (k & 1) * PB;
+                        const C *src = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
+                        for (int task = warp; task < ntask_y; task += NW) {
+                            const int ci = task * G + f;
+                            const bool act = ci < pl.n_multi;
+                            const int col = ct.perm[act ? ci : 0];
+                            const int4 co = ct.col[col];
+                            C x[P1];
+#ifdef FFTB_EXP_PREFETCH
+#pragma unroll
+                            for (int j = 0; j < P1; ++j) x[j] = xp[j];
+                            const C bv = bvp;
+#else
+#pragma unroll
+                            for (int j = 0; j < P1; ++j) {
+                                const int idx = ks_of<F>(t, j) - co.z;
+                                x[j] = (act && (unsigned)idx < (unsigned)co.y) ? __ldcg(src + co.x + idx) : czero<T>();
+                            }
+                            const int idb = M / 2 - co.z;
+                            const C bv = (act && l0 && (unsigned)idb < (unsigned)co.y) ? __ldcg(src + co.x + idb) : czero<T>();
+#endif
+                            FFTB_CLK(0)
+                            if (r == 0) {
+                                x[P1 / 2] = cadd(x[P1 / 2], bv);
+                            } else {
+                                x[P1 / 2] = csub(x[P1 / 2], bv);
+                                pre_inv<F, 0, T>(x, g);
+                            }
+                            FFTB_CLK(1)
+                            C y[B2][P2];
+                            sub_inv<F, T>(x, y, tws, ex, t);
+                            FFTB_CLK(2)
+                            if (act) {
+#pragma unroll
+                                for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                                    for (int q = 0; q < P2; ++q) pbuf[col * YP + (t + P2 * bb) + P1 * q] = y[bb][q];
+                            }
+                        }
+                        // single-stick columns (same warp as in the forward pass): closed form x W^{k2 y}
+                        for (int i = warp; i < n_one; i += NW) {
+                            const int col = ct.perm[pl.n_multi + i];
+                            const int4 co = ct.col[col];
+                            const C v = __ldcg(src + co.x);
+                            __syncwarp();
+                            for (int yl = lane; yl < M; yl += 32) pbuf[col * YP + yl] = cmul(v, tw[modn<N>(co.z * (2 * yl + r))]);
+                        }
+                        FFTB_CLK(3)
+                    }
+                }
+            } else {
+                // ============================================================ x stage, G lines per warp task
+                const int k = (MODE == MODE_FWD) ? it : it - 1;
+                if (k >= 0 && k < ktasks) {
+                    const int id = blockIdx.x + k * gridDim.x;
+                    const int r = id & 1, z = (id >> 1) % pl.n3, b = (id >> 1) / pl.n3;
+                    C *pbuf = pbuf0 + (k & 1) * PB;
+                    for (int task = warp; task < M / G; task += NW) {
+                        const int yl = task * G + f;
+                        const int ygl = 2 * yl + r;
+                        FFTB_CLK(4)
+                        C o0[B2][P2], o1[B2][P2]; // line values x = 2 n' + e, n' = (t + P2 b) + P1 q
+                        if constexpr (MODE != MODE_FWD) {
+                            C x[P1], xs[P1];
+#pragma unroll
+                            for (int j = 0; j < P1; ++j) {
+                                const int c = ks_of<F>(t, j) - k1lo;
+                                x[j] = (unsigned)c < (unsigned)nx ? pbuf[c * YP + yl] : czero<T>();
+                            }
+                            const int cb = M / 2 - k1lo;
+                            const C bv = (l0 && (unsigned)cb < (unsigned)nx) ? pbuf[cb * YP + yl] : czero<T>();
+#pragma unroll
+                            for (int j = 0; j < P1; ++j) xs[j] = x[j];
+                            xs[P1 / 2] = cadd(xs[P1 / 2], bv);
+                            FFTB_CLK(5)
+                            sub_inv<F, T>(xs, o0, tws, ex, t);
+                            x[P1 / 2] = csub(x[P1 / 2], bv);
+                            pre_inv<F, 0, T>(x, g);
+                            sub_inv<F, T>(x, o1, tws, ex, t);
+                            FFTB_CLK(6)
+                        }
+                        if constexpr (MODE == MODE_INV) {
+                            C *row = cub_out + (((long long)b * pl.n3 + z) * N + ygl) * N;
+#pragma unroll
+                            for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                                for (int q = 0; q < P2; ++q) st_pair(row + 2 * ((t + P2 * bb) + P1 * q), o0[bb][q], o1[bb][q]);
+                            FFTB_CLK(7)
+                        }
+                        if constexpr (MODE == MODE_VLOC) {
+                            const T *vrow = vloc + ((long long)z * N + ygl) * N;
+#pragma unroll
+                            for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                                for (int q = 0; q < P2; ++q) {
+                                    const int n = 2 * ((t + P2 * bb) + P1 * q);
+                                    const T v0 = vrow[n], v1 = vrow[n + 1];
+                                    o0[bb][q].x *= v0; o0[bb][q].y *= v0;
+                                    o1[bb][q].x *= v1; o1[bb][q].y *= v1;
+                                }
+                        }
+                        if constexpr (MODE == MODE_FWD) {
+                            const C *row = cub_in + (((long long)b * pl.n3 + z) * N + ygl) * N;
+#pragma unroll
+                            for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+                                for (int q = 0; q < P2; ++q) ld_pair(row + 2 * ((t + P2 * bb) + P1 * q), o0[bb][q], o1[bb][q]);
+                        }
+                        if constexpr (MODE != MODE_INV) {
+                            C g0[P1], g1[P1];
+                            sub_fwd<F, T>(o0, g0, tws, ex, t);
+                            sub_fwd<F, T>(o1, g1, tws, ex, t);
+                            post_fwd<F, 0, T>(g1, g);
+                            const int cb = M / 2 - k1lo;
+                            if (l0 && (unsigned)cb < (unsigned)nx) pbuf[cb * YP + yl] = csub(g0[P1 / 2], g1[P1 / 2]);
+#pragma unroll
+                            for (int j = 0; j < P1; ++j) {
+                                const int c = ks_of<F>(t, j) - k1lo;
+                                if ((unsigned)c < (unsigned)nx) pbuf[c * YP + yl] = cadd(g0[j], g1[j]);
+                            }
+                        }
+                    }
                 }
             }
         }
-        // single-stick columns: one warp per column, dot product with conj(W^{k2 y})
-        const int n_one = nx - pl.n_multi;
-        for (int i = warp; i < n_one; i += NW) {
-            const int col = pl.colperm[pl.n_multi + i];
-            const int4 co = pl.col[col];
-            C acc = czero<T>();
-            for (int yl = lane; yl < M; yl += 32) acc = cadd(acc, cmulc(pbuf[col * YP + yl], tw[modn<N>(co.z * (2 * yl + r))]));
-#pragma unroll
-            for (int s = 16; s > 0; s >>= 1) {
-                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, s);
-                acc.y += __shfl_xor_sync(0xffffffffu, acc.y, s);
-            }
-            if (lane == 0) dst[co.x] = acc;
-        }
+        FFTB_CLK(8)
+        __syncthreads();
+        FFTB_CLK(9)
     }
+    FFTB_CLK_FLUSH
 }
 
 // ---------------------------------------------------------------------------------------------
-// z passes, warp-synchronous: one group of P2 lanes per stick, G sticks per warp task
-//   grid = (ceil(n_sticks / (G * NW)), bands)
+// z passes, warp-synchronous: one group of P2 lanes per stick, G sticks per warp, TS = G * NW
+// consecutive sticks per CTA.  The transposition between "one stick, all z" (what a transform
+// produces / consumes) and the plane-major intermediate A[z][stick] goes through a shared-memory
+// tile [N][TS] so that every global access to A is a run of TS consecutive elements of one z row
+// (512 bytes for complex128); element (z, sl) sits in column (sl + z/2) mod TS, which makes the
+// strided accesses of the transforms bank-conflict-free.
+//   grid = (ceil(n_sticks / TS), bands)
 // ---------------------------------------------------------------------------------------------
+template <typename T, class F, int NW> struct ZFast {
+    static constexpr int TS = F::G * NW;
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)F::N * TS + (size_t)NW * F::EXW);
+    __device__ static __forceinline__ int swz(int z, int sl) { return z * TS + ((sl + (z >> 1)) & (TS - 1)); }
+};
+
 template <typename T, class F, int NW>
-__global__ void __launch_bounds__(NW * 32)
-zpass_fast_inv_k(DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride)
+__global__ void __launch_bounds__(NW * 32, 2)
+zpass_fast_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride)
 {
     using C = cx<T>;
-    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G;
+    using Z = ZFast<T, F, NW>;
+    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *tile = reinterpret_cast<C *>(smem_raw); // [N][TS], swizzled
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    C *ex = reinterpret_cast<C *>(smem_raw) + warp * F::EXW + f * F::FS;
+    C *ex = tile + N * TS + warp * F::EXW + f * F::FS;
     const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    const int s0 = blockIdx.x * TS, sl = warp * G + f, s = s0 + sl;
+    const bool act = s < pl.nsticks;
+    const int4 st = pl.stick[act ? s : 0]; // {off, k3lo, len, .}
+    const C *src = packed + (long long)blockIdx.y * pl.S + st.x;
+    C x[P1], xs[P1];
+#pragma unroll
+    for (int j = 0; j < P1; ++j) {
+        const int idx = ks_of<F>(t, j) - st.y;
+        x[j] = (act && (unsigned)idx < (unsigned)st.z) ? __ldcs(src + idx) : czero<T>();
+    }
+    const int idb = M / 2 - st.y;
+    const C bv = (act && t == 0 && (unsigned)idb < (unsigned)st.z) ? __ldcs(src + idb) : czero<T>();
     C tws[P1];
 #pragma unroll
     for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
     tws[0] = mk<T>((T)1, (T)0);
     const C g = tw[t];
-    const int s = (blockIdx.x * NW + warp) * G + f;
-    const bool act = s < pl.nsticks;
-    const int4 st = pl.stick[act ? s : 0]; // {off, k3lo, len, .}
-    const C *src = packed + (long long)blockIdx.y * pl.S + st.x;
-    C *dst = A + (long long)blockIdx.y * a_band_stride + s;
-    C x[P1], xs[P1];
-#pragma unroll
-    for (int j = 0; j < P1; ++j) {
-        const int idx = ks_of<F>(t, j) - st.y;
-        x[j] = (act && (unsigned)idx < (unsigned)st.z) ? src[idx] : czero<T>();
-    }
-    const int idb = M / 2 - st.y;
-    const C bv = (act && t == 0 && (unsigned)idb < (unsigned)st.z) ? src[idb] : czero<T>();
 #pragma unroll
     for (int j = 0; j < P1; ++j) xs[j] = x[j];
     xs[P1 / 2] = cadd(xs[P1 / 2], bv);
     C y[B2][P2];
     sub_inv<F, T>(xs, y, tws, ex, t);
-    if (act) {
 #pragma unroll
-        for (int bb = 0; bb < B2; ++bb)
+    for (int bb = 0; bb < B2; ++bb)
 #pragma unroll
-            for (int q = 0; q < P2; ++q) dst[(long long)(2 * ((t + P2 * bb) + P1 * q)) * pl.pitch] = y[bb][q];
-    }
+        for (int q = 0; q < P2; ++q) tile[Z::swz(2 * ((t + P2 * bb) + P1 * q), sl)] = y[bb][q];
     x[P1 / 2] = csub(x[P1 / 2], bv);
     pre_inv<F, 0, T>(x, g);
     sub_inv<F, T>(x, y, tws, ex, t);
-    if (act) {
 #pragma unroll
-        for (int bb = 0; bb < B2; ++bb)
+    for (int bb = 0; bb < B2; ++bb)
 #pragma unroll
-            for (int q = 0; q < P2; ++q) dst[(long long)(2 * ((t + P2 * bb) + P1 * q) + 1) * pl.pitch] = y[bb][q];
+        for (int q = 0; q < P2; ++q) tile[Z::swz(2 * ((t + P2 * bb) + P1 * q) + 1, sl)] = y[bb][q];
+    __syncthreads();
+    C *dst = A + (long long)blockIdx.y * a_band_stride + s0;
+#pragma unroll 4
+    for (int i = tid; i < N * TS; i += NT) {
+        const int z = i / TS, c = i % TS;
+        const int l = (c - (z >> 1)) & (TS - 1);
+        if (s0 + l < pl.nsticks) dst[(long long)z * pl.pitch + l] = tile[i];
     }
 }
 
 template <typename T, class F, int NW>
-__global__ void __launch_bounds__(NW * 32)
-zpass_fast_fwd_k(DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride)
+__global__ void __launch_bounds__(NW * 32, 2)
+zpass_fast_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride)
 {
     using C = cx<T>;
-    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G;
+    using Z = ZFast<T, F, NW>;
+    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *tile = reinterpret_cast<C *>(smem_raw);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    C *ex = reinterpret_cast<C *>(smem_raw) + warp * F::EXW + f * F::FS;
+    C *ex = tile + N * TS + warp * F::EXW + f * F::FS;
     const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    const int s0 = blockIdx.x * TS, sl = warp * G + f, s = s0 + sl;
+    const bool act = s < pl.nsticks;
+    // ---- A[z][s0 .. s0+TS) -> tile, summing the ry partial planes of the forward plane kernel
+    {
+        const C *src = A + (long long)blockIdx.y * a_band_stride + s0;
+        const long long rstride = (long long)pl.n3 * pl.pitch;
+        constexpr int U = 8;
+        static_assert((N * TS) % (NT * U) == 0, "tile copy is unrolled by U");
+        for (int i0 = tid; i0 < N * TS; i0 += NT * U) {
+            C v[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int i = i0 + u * NT, z = i / TS, l = i % TS;
+                v[u] = (s0 + l < pl.nsticks) ? __ldcs(src + (long long)z * pl.pitch + l) : czero<T>();
+            }
+            for (int p = 1; p < pl.ry; ++p) {
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const int i = i0 + u * NT, z = i / TS, l = i % TS;
+                    if (s0 + l < pl.nsticks) v[u] = cadd(v[u], __ldcs(src + p * rstride + (long long)z * pl.pitch + l));
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int i = i0 + u * NT, z = i / TS, l = i % TS;
+                tile[Z::swz(z, l)] = v[u];
+            }
+        }
+    }
     C tws[P1];
 #pragma unroll
     for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
     tws[0] = mk<T>((T)1, (T)0);
     const C g = tw[t];
-    const int s = (blockIdx.x * NW + warp) * G + f;
-    const bool act = s < pl.nsticks;
     const int4 st = pl.stick[act ? s : 0];
-    const C *src = A + (long long)blockIdx.y * a_band_stride + (act ? s : 0);
     C *dst = packed + (long long)blockIdx.y * pl.S + st.x;
-    const long long rstride = (long long)pl.n3 * pl.pitch;
     const T scale = (T)pl.scale;
-    C y0[B2][P2], y1[B2][P2], g0[P1], g1[P1];
+    __syncthreads();
+    C y[B2][P2], g0[P1], g1[P1];
 #pragma unroll
     for (int bb = 0; bb < B2; ++bb)
 #pragma unroll
-        for (int q = 0; q < P2; ++q) {
-            const long long o = (long long)(2 * ((t + P2 * bb) + P1 * q)) * pl.pitch;
-            C a = src[o], c = src[o + pl.pitch];
-            for (int p = 1; p < pl.ry; ++p) {
-                a = cadd(a, src[p * rstride + o]);
-                c = cadd(c, src[p * rstride + o + pl.pitch]);
-            }
-            y0[bb][q] = a;
-            y1[bb][q] = c;
-        }
-    sub_fwd<F, T>(y0, g0, tws, ex, t);
-    sub_fwd<F, T>(y1, g1, tws, ex, t);
+        for (int q = 0; q < P2; ++q) y[bb][q] = tile[Z::swz(2 * ((t + P2 * bb) + P1 * q), sl)];
+    sub_fwd<F, T>(y, g0, tws, ex, t);
+#pragma unroll
+    for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+        for (int q = 0; q < P2; ++q) y[bb][q] = tile[Z::swz(2 * ((t + P2 * bb) + P1 * q) + 1, sl)];
+    sub_fwd<F, T>(y, g1, tws, ex, t);
     post_fwd<F, 0, T>(g1, g);
     if (act) {
         const int idb = M / 2 - st.y;
