@@ -353,11 +353,12 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
     if (desc->n[0] != desc->n[1]) return FFTB_EUNSUPPORTED;
     ZLaunch zl;
     PlaneLaunch plk;
+    bool fast_plane = false;
     if (!find_z(desc->dtype, desc->n[2], dense, &zl) || !find_plane(desc->dtype, desc->n[0], dense, &plk)) return FFTB_EUNSUPPORTED;
     {
         const char *gen = getenv("FFTB_GENERIC_PLANE"); // debugging aid: keep the generic plane kernel
         PlaneLaunch fast;
-        if (!(gen && gen[0] == '1') && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) plk = fast;
+        if (!(gen && gen[0] == '1') && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) { plk = fast; fast_plane = true; }
         const char *genz = getenv("FFTB_GENERIC_Z");
         ZLaunch zfast;
         if (!(genz && genz[0] == '1') && find_z_fast(desc->dtype, desc->n[2], dense, &zfast)) zl = zfast;
@@ -452,11 +453,14 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
                 }
             }
         }
-        // ---- workspace: the plane-major intermediate for `chunk` bands, sized to stay in L2
+        // ---- workspace: the plane-major intermediate for `chunk` bands.  The generic kernels are launched
+        // per chunk and want it to stay in L2 between the two kernels of a chunk; the persistent fast
+        // kernels gain more from few, long launches (measured on config 3: 48 MB -> 4.3 ms, whole batch
+        // -> 3.9 ms per step), so their budget covers the whole batch whenever 4 GiB allow it.
         p->a_inv_stride = (long long)n3 * p->pitch;
         p->a_fwd_stride = (long long)p->ry * n3 * p->pitch;
         const size_t per_band = (size_t)(p->a_inv_stride + p->a_fwd_stride) * p->elem; // vloc needs both
-        size_t budget = (size_t)48 << 20;
+        size_t budget = fast_plane ? (size_t)4 << 30 : (size_t)48 << 20;
         if (const char *e = getenv("FFTB_WS_MB")) { long v = atol(e); if (v > 0) budget = (size_t)v << 20; }
         auto chunk_of = [&](size_t bytes_per_band) {
             long long c = (long long)(budget / bytes_per_band);
@@ -472,7 +476,12 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
         p->o_col = o; o = align_up(o + sizeof(int4) * p->h_col.size(), 256);
         for (int d = 0; d < 3; ++d) { p->o_tw[d] = o; o = align_up(o + p->h_tw[d].size(), 256); }
         p->o_perm = o; o = align_up(o + sizeof(int) * p->h_colperm.size(), 256);
-        p->o_ws = o; o = align_up(o + (budget > per_band ? budget : per_band), 256);
+        {
+            size_t ws = (size_t)desc->batch * per_band;
+            if (ws > budget) ws = budget;
+            if (ws < per_band) ws = per_band;
+            p->o_ws = o; o = align_up(o + ws, 256);
+        }
         p->bytes_min = o;
         p->o_stage = o; o = align_up(o + (size_t)desc->batch * (size_t)p->S * p->elem, 256);
         p->bytes_stage = o;
@@ -546,9 +555,6 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
     dv.tw1 = m + p->o_tw[0]; dv.tw2 = m + p->o_tw[1]; dv.tw3 = m + p->o_tw[2];
     dv.S = p->S;
     dv.scale = p->desc.scale == FFTB_SCALE_FORWARD ? 1.0 / (double)p->C : 1.0;
-#ifdef FFTB_DEV
-    dv.dbg = getenv("FFTB_DBG") ? atoi(getenv("FFTB_DBG")) : 0;
-#endif
     return FFTB_OK;
 }
 
@@ -726,15 +732,6 @@ int fftb_dense_extract(fftb_plan pruned, fftb_plan dense, const void *d_packed_d
 
 int fftb_plan_last_launches(fftb_plan p) { return p ? p->launches : FFTB_EINVAL; }
 
-#ifdef FFTB_DEV
-int fftb_dev_clk(unsigned long long *out, int reset)
-{
-    cudaDeviceSynchronize();
-    if (cudaMemcpyFromSymbol(out, g_fftb_clk, sizeof(unsigned long long) * 16) != cudaSuccess) return -1;
-    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_fftb_clk, z, sizeof(z)); }
-    return 0;
-}
-#endif
 
 int fftb_plan_profile(fftb_plan p, int enable)
 {

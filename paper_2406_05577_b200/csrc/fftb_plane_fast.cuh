@@ -155,17 +155,6 @@ __device__ __forceinline__ void ld_pair(const float2 *p, float2 &a, float2 &b)
 //   VLOC  it: y_fwd(task it-2) : buf[it&1] -> A, then y_inv(task it) -> buf[it&1] (same warp, same
 //             columns, in this order)             | x_vloc(task it-1) in place in buf[(it-1)&1]
 // ---------------------------------------------------------------------------------------------
-#ifdef FFTB_DEV
-__device__ unsigned long long g_fftb_clk[16];
-#define FFTB_CLK_DECL unsigned long long clk_acc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}; long long clk_t = clock64();
-#define FFTB_CLK(i) { const long long clk_n = clock64(); clk_acc[i] += (unsigned long long)(clk_n - clk_t); clk_t = clk_n; }
-#define FFTB_CLK_FLUSH if (lane == 0) { for (int i = 0; i < 10; ++i) atomicAdd(&g_fftb_clk[i], clk_acc[i]); }
-#else
-#define FFTB_CLK_DECL
-#define FFTB_CLK(i)
-#define FFTB_CLK_FLUSH
-#endif
-
 template <typename T, class F, int NW> struct PlaneFast {
     static constexpr int PB = F::NCOL * F::YP; // elements of one plane buffer
     static constexpr size_t smem_bytes = sizeof(cx<T>) * (2 * (size_t)PB + (size_t)NW * F::EXW);
@@ -197,35 +186,10 @@ plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab 
     const int ntask_y = (pl.n_multi + G - 1) / G;
     const int ktasks = ntasks > (int)blockIdx.x ? (ntasks - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     constexpr int LAG = (MODE == MODE_VLOC) ? 2 : 1; // iterations between the first and the last stage of a task
-#ifdef FFTB_EXP_PREFETCH
-    const int swap = (MODE == MODE_INV) ? 1 : (warp & 1);
-#else
     const int swap = warp & 1;
-#endif
-    FFTB_CLK_DECL
 
 #pragma unroll 1
     for (int it = 0; it < ktasks + LAG; ++it) {
-#ifdef FFTB_EXP_PREFETCH
-        C xp[P1], bvp = czero<T>();
-        if constexpr (MODE == MODE_INV) {
-            if (it < ktasks) {
-                const int id = blockIdx.x + it * gridDim.x;
-                const int z = (id >> 1) % pl.n3, b = (id >> 1) / pl.n3;
-                const C *src = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
-                const int ci = warp * G + f;
-                const bool act = ci < pl.n_multi;
-                const int4 co = ct.col[ct.perm[act ? ci : 0]];
-#pragma unroll
-                for (int j = 0; j < P1; ++j) {
-                    const int idx = ks_of<F>(t, j) - co.z;
-                    xp[j] = (act && (unsigned)idx < (unsigned)co.y) ? __ldcg(src + co.x + idx) : czero<T>();
-                }
-                const int idb = M / 2 - co.z;
-                bvp = (act && l0 && (unsigned)idb < (unsigned)co.y) ? __ldcg(src + co.x + idb) : czero<T>();
-            }
-        }
-#endif
 #pragma unroll 1
         for (int step = 0; step < 2; ++step) {
             if ((step ^ swap) == 0) {
@@ -291,11 +255,6 @@ plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab 
                             const int col = ct.perm[act ? ci : 0];
                             const int4 co = ct.col[col];
                             C x[P1];
-#ifdef FFTB_EXP_PREFETCH
-#pragma unroll
-                            for (int j = 0; j < P1; ++j) x[j] = xp[j];
-                            const C bv = bvp;
-#else
 #pragma unroll
                             for (int j = 0; j < P1; ++j) {
                                 const int idx = ks_of<F>(t, j) - co.z;
@@ -303,18 +262,14 @@ plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab 
                             }
                             const int idb = M / 2 - co.z;
                             const C bv = (act && l0 && (unsigned)idb < (unsigned)co.y) ? __ldcg(src + co.x + idb) : czero<T>();
-#endif
-                            FFTB_CLK(0)
                             if (r == 0) {
                                 x[P1 / 2] = cadd(x[P1 / 2], bv);
                             } else {
                                 x[P1 / 2] = csub(x[P1 / 2], bv);
                                 pre_inv<F, 0, T>(x, g);
                             }
-                            FFTB_CLK(1)
                             C y[B2][P2];
                             sub_inv<F, T>(x, y, tws, ex, t);
-                            FFTB_CLK(2)
                             if (act) {
 #pragma unroll
                                 for (int bb = 0; bb < B2; ++bb)
@@ -330,7 +285,6 @@ plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab 
                             __syncwarp();
                             for (int yl = lane; yl < M; yl += 32) pbuf[col * YP + yl] = cmul(v, tw[modn<N>(co.z * (2 * yl + r))]);
                         }
-                        FFTB_CLK(3)
                     }
                 }
             } else {
@@ -343,7 +297,6 @@ plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab 
                     for (int task = warp; task < M / G; task += NW) {
                         const int yl = task * G + f;
                         const int ygl = 2 * yl + r;
-                        FFTB_CLK(4)
                         C o0[B2][P2], o1[B2][P2]; // line values x = 2 n' + e, n' = (t + P2 b) + P1 q
                         if constexpr (MODE != MODE_FWD) {
                             C x[P1], xs[P1];
@@ -357,12 +310,10 @@ plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab 
 #pragma unroll
                             for (int j = 0; j < P1; ++j) xs[j] = x[j];
                             xs[P1 / 2] = cadd(xs[P1 / 2], bv);
-                            FFTB_CLK(5)
                             sub_inv<F, T>(xs, o0, tws, ex, t);
                             x[P1 / 2] = csub(x[P1 / 2], bv);
                             pre_inv<F, 0, T>(x, g);
                             sub_inv<F, T>(x, o1, tws, ex, t);
-                            FFTB_CLK(6)
                         }
                         if constexpr (MODE == MODE_INV) {
                             C *row = cub_out + (((long long)b * pl.n3 + z) * N + ygl) * N;
@@ -370,7 +321,6 @@ plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab 
                             for (int bb = 0; bb < B2; ++bb)
 #pragma unroll
                                 for (int q = 0; q < P2; ++q) st_pair(row + 2 * ((t + P2 * bb) + P1 * q), o0[bb][q], o1[bb][q]);
-                            FFTB_CLK(7)
                         }
                         if constexpr (MODE == MODE_VLOC) {
                             const T *vrow = vloc + ((long long)z * N + ygl) * N;
@@ -408,11 +358,8 @@ plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab 
                 }
             }
         }
-        FFTB_CLK(8)
         __syncthreads();
-        FFTB_CLK(9)
     }
-    FFTB_CLK_FLUSH
 }
 
 // ---------------------------------------------------------------------------------------------
