@@ -8,6 +8,7 @@
 #include "../../include/fftb.h"
 #include "fftb_kernels.cuh"
 #include "fftb_plane_fast.cuh"
+#include "fftb_plane_pf.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -110,7 +111,7 @@ int launch_plane(const DevPlan &pl, const ColTab &, const void *Ain, void *Aout,
 
 // warp-synchronous persistent plane kernel (fftb_plane_fast.cuh): half-band power-of-two grids
 constexpr int FAST_NW = 8; // warps per CTA of the z-pass kernels
-template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 16 : 4; }; // x tasks per half plane = N/2 / G
+template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 8 : 2; }; // half the x tasks of a half plane
 
 static int g_sm_count = 0;
 static int sm_count()
@@ -130,8 +131,8 @@ int launch_plane_fast(const DevPlan &pl, const ColTab &ct, const void *Ain, void
                       long long sout, int nb, cudaStream_t st)
 {
     constexpr int NW = PlaneNW<F::N>::value;
-    auto k = plane_fast_k<T, F, NW, MODE>;
-    const size_t smem = PlaneFast<T, F, NW>::smem_bytes;
+    auto k = plane_pf_k<T, F, NW, MODE>;
+    const size_t smem = PlanePF<T, F, NW>::smem_bytes;
     static int per_sm = 0; // CTAs per SM of this instantiation
     if (!per_sm) {
         if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
@@ -148,7 +149,7 @@ int launch_plane_fast(const DevPlan &pl, const ColTab &ct, const void *Ain, void
 template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
 {
     using F = FastCfg<T, N, P1, P2>;
-    static_assert(PlaneFast<T, F, PlaneNW<N>::value>::smem_bytes <= 227 * 1024, "plane buffers do not fit in shared memory");
+    static_assert(PlanePF<T, F, PlaneNW<N>::value>::smem_bytes <= 227 * 1024, "plane buffers do not fit in shared memory");
     return PlaneLaunch{2, {&launch_plane_fast<T, F, MODE_INV>, &launch_plane_fast<T, F, MODE_FWD>, &launch_plane_fast<T, F, MODE_VLOC>}};
 }
 bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)

@@ -1,4 +1,5 @@
-// fftb_plane_fast.cuh -- warp-synchronous plane kernel for half-band power-of-two grids (sm_100a).
+// fftb_plane_fast.cuh -- warp-synchronous building blocks and z-pass kernels for half-band power-of-two
+// grids (sm_100a); the plane kernel built from them is in fftb_plane_pf.cuh.
 //
 // Same mathematics as plane_k in fftb_kernels.cuh (y and x passes of one z-plane, one y residue per
 // CTA; PAPER.md:96 Fig. 3, :112 staged padding), restructured for the B200 SM:
@@ -141,225 +142,6 @@ __device__ __forceinline__ void ld_pair(const float2 *p, float2 &a, float2 &b)
     const float4 v = __ldcs(reinterpret_cast<const float4 *>(p));
     a = make_float2(v.x, v.y);
     b = make_float2(v.z, v.w);
-}
-
-// ---------------------------------------------------------------------------------------------
-// Persistent plane kernel.  A TASK is one half z-plane: (band b, plane z, y residue r), numbered
-// id = (b * n3 + z) * 2 + r; CTA c of a grid of G CTAs owns tasks c, c + G, c + 2G, ...  The plane
-// buffer is double-buffered so that, inside one iteration, the x pass of one task and the y pass of
-// the neighbouring task are independent; odd warps run them in the opposite order to the even warps,
-// so that the loads of one half of the CTA are covered by the arithmetic of the other half.  One
-// CTA-wide barrier per iteration is the only synchronisation.
-//   INV   it: y_inv(task it)   -> buf[it&1]      | x_inv(task it-1) : buf[(it-1)&1] -> cuboid
-//   FWD   it: x_fwd(task it)   -> buf[it&1]      | y_fwd(task it-1) : buf[(it-1)&1] -> A
-//   VLOC  it: y_fwd(task it-2) : buf[it&1] -> A, then y_inv(task it) -> buf[it&1] (same warp, same
-//             columns, in this order)             | x_vloc(task it-1) in place in buf[(it-1)&1]
-// ---------------------------------------------------------------------------------------------
-template <typename T, class F, int NW> struct PlaneFast {
-    static constexpr int PB = F::NCOL * F::YP; // elements of one plane buffer
-    static constexpr size_t smem_bytes = sizeof(cx<T>) * (2 * (size_t)PB + (size_t)NW * F::EXW);
-};
-
-template <typename T, class F, int NW, int MODE>
-__global__ void __launch_bounds__(NW * 32, 1)
-plane_fast_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct, const cx<T> *__restrict__ Ain,
-             cx<T> *__restrict__ Aout, const cx<T> *__restrict__ cub_in, cx<T> *__restrict__ cub_out,
-             const T *__restrict__ vloc, long long a_in_stride, long long a_out_stride, int ntasks)
-{
-    using C = cx<T>;
-    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, YP = F::YP;
-    constexpr int PB = PlaneFast<T, F, NW>::PB;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    C *pbuf0 = reinterpret_cast<C *>(smem_raw); // [2][NCOL][YP]: column c = k1 - k1lo, local line y'
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int f = lane / P2, t = lane % P2;
-    C *ex = pbuf0 + 2 * PB + warp * F::EXW + f * F::FS; // this group's exchange tile
-    const C *tw = reinterpret_cast<const C *>(pl.tw1);  // N1 == N2: one table
-    C tws[P1];
-#pragma unroll
-    for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
-    tws[0] = mk<T>((T)1, (T)0);
-    const C g = tw[t];
-    const int nx = pl.nxocc, k1lo = pl.k1lo;
-    const bool l0 = (t == 0);
-    const int n_one = nx - pl.n_multi;
-    const int ntask_y = (pl.n_multi + G - 1) / G;
-    const int ktasks = ntasks > (int)blockIdx.x ? (ntasks - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
-    constexpr int LAG = (MODE == MODE_VLOC) ? 2 : 1; // iterations between the first and the last stage of a task
-    const int swap = warp & 1;
-
-#pragma unroll 1
-    for (int it = 0; it < ktasks + LAG; ++it) {
-#pragma unroll 1
-        for (int step = 0; step < 2; ++step) {
-            if ((step ^ swap) == 0) {
-                // ============================================================ y stage(s)
-                if constexpr (MODE != MODE_INV) {
-                    // -------- forward y pass: buf -> partial A of residue r
-                    const int k = (MODE == MODE_FWD) ? it - 1 : it - 2;
-                    if (k >= 0 && k < ktasks) {
-                        const int id = blockIdx.x + k * gridDim.x;
-                        const int r = id & 1, z = (id >> 1) % pl.n3, b = (id >> 1) / pl.n3;
-                        const C *pbuf = pbuf0 + (k & 1) * PB;
-                        C *dst = Aout + (long long)b * a_out_stride + ((long long)r * pl.n3 + z) * pl.pitch;
-                        for (int task = warp; task < ntask_y; task += NW) {
-                            const int ci = task * G + f;
-                            const bool act = ci < pl.n_multi;
-                            const int col = ct.perm[act ? ci : 0];
-                            const int4 co = ct.col[col];
-                            C y[B2][P2], x[P1];
-#pragma unroll
-                            for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                                for (int q = 0; q < P2; ++q) y[bb][q] = pbuf[col * YP + (t + P2 * bb) + P1 * q];
-                            sub_fwd<F, T>(y, x, tws, ex, t);
-                            if (r != 0) post_fwd<F, 0, T>(x, g); // partial of residue 1: conj(W^{k_s}) G[k]
-                            if (act) {
-                                const int idb = M / 2 - co.z;
-                                if (l0 && (unsigned)idb < (unsigned)co.y)
-                                    dst[co.x + idb] = r ? mk<T>(-x[P1 / 2].x, -x[P1 / 2].y) : x[P1 / 2];
-#pragma unroll
-                                for (int j = 0; j < P1; ++j) {
-                                    const int idx = ks_of<F>(t, j) - co.z;
-                                    if ((unsigned)idx < (unsigned)co.y) dst[co.x + idx] = x[j];
-                                }
-                            }
-                        }
-                        // single-stick columns: one warp per column, dot product with conj(W^{k2 y})
-                        for (int i = warp; i < n_one; i += NW) {
-                            const int col = ct.perm[pl.n_multi + i];
-                            const int4 co = ct.col[col];
-                            C acc = czero<T>();
-                            for (int yl = lane; yl < M; yl += 32)
-                                acc = cadd(acc, cmulc(pbuf[col * YP + yl], tw[modn<N>(co.z * (2 * yl + r))]));
-#pragma unroll
-                            for (int sft = 16; sft > 0; sft >>= 1) {
-                                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, sft);
-                                acc.y += __shfl_xor_sync(0xffffffffu, acc.y, sft);
-                            }
-                            if (lane == 0) dst[co.x] = acc;
-                        }
-                    }
-                }
-                if constexpr (MODE != MODE_FWD) {
-                    // -------- inverse y pass: A row of plane z -> buf
-                    const int k = it;
-                    if (k < ktasks) {
-                        const int id = blockIdx.x + k * gridDim.x;
-                        const int r = id & 1, z = (id >> 1) % pl.n3, b = (id >> 1) / pl.n3;
-                        C *pbuf = pbuf0 + (k & 1) * PB;
-                        const C *src = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
-                        for (int task = warp; task < ntask_y; task += NW) {
-                            const int ci = task * G + f;
-                            const bool act = ci < pl.n_multi;
-                            const int col = ct.perm[act ? ci : 0];
-                            const int4 co = ct.col[col];
-                            C x[P1];
-#pragma unroll
-                            for (int j = 0; j < P1; ++j) {
-                                const int idx = ks_of<F>(t, j) - co.z;
-                                x[j] = (act && (unsigned)idx < (unsigned)co.y) ? __ldcg(src + co.x + idx) : czero<T>();
-                            }
-                            const int idb = M / 2 - co.z;
-                            const C bv = (act && l0 && (unsigned)idb < (unsigned)co.y) ? __ldcg(src + co.x + idb) : czero<T>();
-                            if (r == 0) {
-                                x[P1 / 2] = cadd(x[P1 / 2], bv);
-                            } else {
-                                x[P1 / 2] = csub(x[P1 / 2], bv);
-                                pre_inv<F, 0, T>(x, g);
-                            }
-                            C y[B2][P2];
-                            sub_inv<F, T>(x, y, tws, ex, t);
-                            if (act) {
-#pragma unroll
-                                for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                                    for (int q = 0; q < P2; ++q) pbuf[col * YP + (t + P2 * bb) + P1 * q] = y[bb][q];
-                            }
-                        }
-                        // single-stick columns (same warp as in the forward pass): closed form x W^{k2 y}
-                        for (int i = warp; i < n_one; i += NW) {
-                            const int col = ct.perm[pl.n_multi + i];
-                            const int4 co = ct.col[col];
-                            const C v = __ldcg(src + co.x);
-                            __syncwarp();
-                            for (int yl = lane; yl < M; yl += 32) pbuf[col * YP + yl] = cmul(v, tw[modn<N>(co.z * (2 * yl + r))]);
-                        }
-                    }
-                }
-            } else {
-                // ============================================================ x stage, G lines per warp task
-                const int k = (MODE == MODE_FWD) ? it : it - 1;
-                if (k >= 0 && k < ktasks) {
-                    const int id = blockIdx.x + k * gridDim.x;
-                    const int r = id & 1, z = (id >> 1) % pl.n3, b = (id >> 1) / pl.n3;
-                    C *pbuf = pbuf0 + (k & 1) * PB;
-                    for (int task = warp; task < M / G; task += NW) {
-                        const int yl = task * G + f;
-                        const int ygl = 2 * yl + r;
-                        C o0[B2][P2], o1[B2][P2]; // line values x = 2 n' + e, n' = (t + P2 b) + P1 q
-                        if constexpr (MODE != MODE_FWD) {
-                            C x[P1], xs[P1];
-#pragma unroll
-                            for (int j = 0; j < P1; ++j) {
-                                const int c = ks_of<F>(t, j) - k1lo;
-                                x[j] = (unsigned)c < (unsigned)nx ? pbuf[c * YP + yl] : czero<T>();
-                            }
-                            const int cb = M / 2 - k1lo;
-                            const C bv = (l0 && (unsigned)cb < (unsigned)nx) ? pbuf[cb * YP + yl] : czero<T>();
-#pragma unroll
-                            for (int j = 0; j < P1; ++j) xs[j] = x[j];
-                            xs[P1 / 2] = cadd(xs[P1 / 2], bv);
-                            sub_inv<F, T>(xs, o0, tws, ex, t);
-                            x[P1 / 2] = csub(x[P1 / 2], bv);
-                            pre_inv<F, 0, T>(x, g);
-                            sub_inv<F, T>(x, o1, tws, ex, t);
-                        }
-                        if constexpr (MODE == MODE_INV) {
-                            C *row = cub_out + (((long long)b * pl.n3 + z) * N + ygl) * N;
-#pragma unroll
-                            for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                                for (int q = 0; q < P2; ++q) st_pair(row + 2 * ((t + P2 * bb) + P1 * q), o0[bb][q], o1[bb][q]);
-                        }
-                        if constexpr (MODE == MODE_VLOC) {
-                            const T *vrow = vloc + ((long long)z * N + ygl) * N;
-#pragma unroll
-                            for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                                for (int q = 0; q < P2; ++q) {
-                                    const int n = 2 * ((t + P2 * bb) + P1 * q);
-                                    const T v0 = vrow[n], v1 = vrow[n + 1];
-                                    o0[bb][q].x *= v0; o0[bb][q].y *= v0;
-                                    o1[bb][q].x *= v1; o1[bb][q].y *= v1;
-                                }
-                        }
-                        if constexpr (MODE == MODE_FWD) {
-                            const C *row = cub_in + (((long long)b * pl.n3 + z) * N + ygl) * N;
-#pragma unroll
-                            for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-                                for (int q = 0; q < P2; ++q) ld_pair(row + 2 * ((t + P2 * bb) + P1 * q), o0[bb][q], o1[bb][q]);
-                        }
-                        if constexpr (MODE != MODE_INV) {
-                            C g0[P1], g1[P1];
-                            sub_fwd<F, T>(o0, g0, tws, ex, t);
-                            sub_fwd<F, T>(o1, g1, tws, ex, t);
-                            post_fwd<F, 0, T>(g1, g);
-                            const int cb = M / 2 - k1lo;
-                            if (l0 && (unsigned)cb < (unsigned)nx) pbuf[cb * YP + yl] = csub(g0[P1 / 2], g1[P1 / 2]);
-#pragma unroll
-                            for (int j = 0; j < P1; ++j) {
-                                const int c = ks_of<F>(t, j) - k1lo;
-                                if ((unsigned)c < (unsigned)nx) pbuf[c * YP + yl] = cadd(g0[j], g1[j]);
-                            }
-                        }
-                    }
-                }
-            }
-        }
-        __syncthreads();
-    }
 }
 
 // ---------------------------------------------------------------------------------------------
