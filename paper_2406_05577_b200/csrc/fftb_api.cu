@@ -132,9 +132,12 @@ int launch_plane_fast(const DevPlan &pl, const ColTab &ct, const void *Ain, void
 {
     constexpr int NW = PlaneNW<F::N>::value;
     auto k = plane_pf_k<T, F, NW, MODE>;
-    const size_t smem = PlanePF<T, F, NW>::smem_bytes;
-    static int per_sm = 0; // CTAs per SM of this instantiation
-    if (!per_sm) {
+    const size_t smem = PlanePF<T, F, NW>::smem_bytes_mode(MODE, pl.pitch);
+    if (smem > 227 * 1024) return FFTB_EUNSUPPORTED;
+    static int per_sm = 0;    // CTAs per SM of this instantiation
+    static size_t smem_set = 0;
+    if (!per_sm || smem != smem_set) {
+        smem_set = smem;
         if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
         int occ = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, NW * 32, smem) != cudaSuccess || occ < 1) return FFTB_ECUDA;

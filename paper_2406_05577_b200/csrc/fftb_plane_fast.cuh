@@ -81,9 +81,26 @@ template <class F, int B, typename T> __device__ __forceinline__ void fwd_btw_al
     }
 }
 
+// Where a group exchanges its M values between the two codelet stages: element (i, j), i < P1 the
+// stage-1 output index, j < P2 the lane.  ExTile is a warp-private tile of pitch P2+1; ExSkew uses M
+// slots that lie STRIDE elements apart (a line or a column of the plane buffer, exchanged in place),
+// rotated by i so that both access directions touch P2 different 16-byte bank groups.
+template <typename T, int P2> struct ExTile {
+    cx<T> *p;
+    __device__ __forceinline__ void put(int i, int j, cx<T> v) const { p[i * (P2 + 1) + j] = v; }
+    __device__ __forceinline__ cx<T> get(int i, int j) const { return p[i * (P2 + 1) + j]; }
+};
+template <typename T, int P2, int STRIDE> struct ExSkew {
+    cx<T> *p;
+    bool on; // a group without work must not scribble over somebody else's line or column
+    __device__ __forceinline__ int slot(int i, int j) const { return (P2 * i + ((j + i) & (P2 - 1))) * STRIDE; }
+    __device__ __forceinline__ void put(int i, int j, cx<T> v) const { if (on) p[slot(i, j)] = v; }
+    __device__ __forceinline__ cx<T> get(int i, int j) const { return p[slot(i, j)]; }
+};
+
 // length-M inverse transform of the group: x[j] = u[t + P2 j]  ->  y[b][q] = out[(t + P2 b) + P1 q]
-template <class F, typename T>
-__device__ __forceinline__ void sub_inv(cx<T> (&x)[F::P1], cx<T> (&y)[F::B2][F::P2], const cx<T> (&tws)[F::P1], cx<T> *ex, int t)
+template <class F, typename T, class EX>
+__device__ __forceinline__ void sub_inv(cx<T> (&x)[F::P1], cx<T> (&y)[F::B2][F::P2], const cx<T> (&tws)[F::P1], EX ex, int t)
 {
     constexpr int P1 = F::P1, P2 = F::P2, B2 = F::B2;
     fft_reg<P1, +1, T>(x);
@@ -91,19 +108,19 @@ __device__ __forceinline__ void sub_inv(cx<T> (&x)[F::P1], cx<T> (&y)[F::B2][F::
     for (int m = 1; m < P1; ++m) x[m] = cmul(x[m], tws[m]);
     __syncwarp();
 #pragma unroll
-    for (int m = 0; m < P1; ++m) ex[m * (P2 + 1) + t] = x[m];
+    for (int m = 0; m < P1; ++m) ex.put(m, t, x[m]);
     __syncwarp();
 #pragma unroll
     for (int b = 0; b < B2; ++b) {
 #pragma unroll
-        for (int tt = 0; tt < P2; ++tt) y[b][tt] = ex[(t + P2 * b) * (P2 + 1) + tt];
+        for (int tt = 0; tt < P2; ++tt) y[b][tt] = ex.get(t + P2 * b, tt);
         fft_reg<P2, +1, T>(y[b]);
     }
 }
 
 // adjoint: y[b][q] = in[(t + P2 b) + P1 q]  ->  x[j] = G[t + P2 j]
-template <class F, typename T>
-__device__ __forceinline__ void sub_fwd(cx<T> (&y)[F::B2][F::P2], cx<T> (&x)[F::P1], const cx<T> (&tws)[F::P1], cx<T> *ex, int t)
+template <class F, typename T, class EX>
+__device__ __forceinline__ void sub_fwd(cx<T> (&y)[F::B2][F::P2], cx<T> (&x)[F::P1], const cx<T> (&tws)[F::P1], EX ex, int t)
 {
     constexpr int P1 = F::P1, P2 = F::P2, B2 = F::B2;
 #pragma unroll
@@ -117,10 +134,10 @@ __device__ __forceinline__ void sub_fwd(cx<T> (&y)[F::B2][F::P2], cx<T> (&x)[F::
 #pragma unroll
     for (int b = 0; b < B2; ++b)
 #pragma unroll
-        for (int tt = 0; tt < P2; ++tt) ex[(t + P2 * b) * (P2 + 1) + tt] = y[b][tt];
+        for (int tt = 0; tt < P2; ++tt) ex.put(t + P2 * b, tt, y[b][tt]);
     __syncwarp();
 #pragma unroll
-    for (int m = 0; m < P1; ++m) x[m] = ex[m * (P2 + 1) + t];
+    for (int m = 0; m < P1; ++m) x[m] = ex.get(m, t);
     fft_reg<P1, -1, T>(x);
 }
 
@@ -170,7 +187,7 @@ zpass_fast_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
     C *tile = reinterpret_cast<C *>(smem_raw); // [N][TS], swizzled
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    C *ex = tile + N * TS + warp * F::EXW + f * F::FS;
+    const ExTile<T, P2> ex{tile + N * TS + warp * F::EXW + f * F::FS};
     const C *tw = reinterpret_cast<const C *>(pl.tw3);
     const int s0 = blockIdx.x * TS, sl = warp * G + f, s = s0 + sl;
     const bool act = s < pl.nsticks;
@@ -226,7 +243,7 @@ zpass_fast_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
     C *tile = reinterpret_cast<C *>(smem_raw);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    C *ex = tile + N * TS + warp * F::EXW + f * F::FS;
+    const ExTile<T, P2> ex{tile + N * TS + warp * F::EXW + f * F::FS};
     const C *tw = reinterpret_cast<const C *>(pl.tw3);
     const int s0 = blockIdx.x * TS, sl = warp * G + f, s = s0 + sl;
     const bool act = s < pl.nsticks;
