@@ -111,7 +111,8 @@ int launch_plane(const DevPlan &pl, const ColTab &, const void *Ain, void *Aout,
 
 // warp-synchronous persistent plane kernel (fftb_plane_fast.cuh): half-band power-of-two grids
 constexpr int FAST_NW = 8; // warps per CTA of the z-pass kernels
-template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 8 : 2; }; // half the x tasks of a half plane
+// warps per CTA of the plane kernel: a quarter of the x tasks of a plane
+template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 8 : 2; };
 
 static int g_sm_count = 0;
 static int sm_count()
@@ -143,17 +144,16 @@ int launch_plane_fast(const DevPlan &pl, const ColTab &ct, const void *Ain, void
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, NW * 32, smem) != cudaSuccess || occ < 1) return FFTB_ECUDA;
         per_sm = occ;
     }
-    const int ntasks = 2 * pl.n3 * nb;
+    const int nplanes = pl.n3 * nb;
     int grid = sm_count() * per_sm;
-    if (grid > ntasks) grid = ntasks;
-    k<<<grid, NW * 32, smem, st>>>(pl, ct, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout, ntasks);
+    if (grid > nplanes) grid = nplanes;
+    k<<<grid, NW * 32, smem, st>>>(pl, ct, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout, nplanes);
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
 {
     using F = FastCfg<T, N, P1, P2>;
-    static_assert(PlanePF<T, F, PlaneNW<N>::value>::smem_bytes <= 227 * 1024, "plane buffers do not fit in shared memory");
-    return PlaneLaunch{2, {&launch_plane_fast<T, F, MODE_INV>, &launch_plane_fast<T, F, MODE_FWD>, &launch_plane_fast<T, F, MODE_VLOC>}};
+    return PlaneLaunch{1, {&launch_plane_fast<T, F, MODE_INV>, &launch_plane_fast<T, F, MODE_FWD>, &launch_plane_fast<T, F, MODE_VLOC>}};
 }
 bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)
 {
