@@ -176,38 +176,35 @@ template <typename T, class F, int NW> struct ZFast {
     __device__ static __forceinline__ int swz(int z, int sl) { return z * TS + ((sl + (z >> 1)) & (TS - 1)); }
 };
 
+// One tile (TS consecutive sticks starting at s0 = j TS) of one band, called by all NW warps of a CTA;
+// `smem` holds the tile [N][TS] and the warps' exchange tiles (ZFast::smem_bytes); tws / g are the caller's
+// twiddle registers for the z axis.  Both contain CTA barriers; the caller must put one more between
+// two calls (or any other use of `smem`).
 template <typename T, class F, int NW>
-__global__ void __launch_bounds__(NW * 32, 2)
-zpass_fast_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride)
+__device__ __forceinline__ void z_inv_tile(const DevPlan &pl, const cx<T> *__restrict__ packed_band, cx<T> *__restrict__ A_band, int j,
+                                           cx<T> *smem, const cx<T> (&tws)[F::P1], cx<T> g)
 {
     using C = cx<T>;
     using Z = ZFast<T, F, NW>;
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    C *tile = reinterpret_cast<C *>(smem_raw); // [N][TS], swizzled
+    C *tile = smem; // [N][TS], swizzled
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
     const ExTile<T, P2> ex{tile + N * TS + warp * F::EXW + f * F::FS};
-    const C *tw = reinterpret_cast<const C *>(pl.tw3);
-    const int s0 = blockIdx.x * TS, sl = warp * G + f, s = s0 + sl;
+    const int s0 = j * TS, sl = warp * G + f, s = s0 + sl;
     const bool act = s < pl.nsticks;
     const int4 st = pl.stick[act ? s : 0]; // {off, k3lo, len, .}
-    const C *src = packed + (long long)blockIdx.y * pl.S + st.x;
+    const C *src = packed_band + st.x;
     C x[P1], xs[P1];
 #pragma unroll
-    for (int j = 0; j < P1; ++j) {
-        const int idx = ks_of<F>(t, j) - st.y;
-        x[j] = (act && (unsigned)idx < (unsigned)st.z) ? __ldcs(src + idx) : czero<T>();
+    for (int jj = 0; jj < P1; ++jj) {
+        const int idx = ks_of<F>(t, jj) - st.y;
+        x[jj] = (act && (unsigned)idx < (unsigned)st.z) ? __ldcs(src + idx) : czero<T>();
     }
     const int idb = M / 2 - st.y;
     const C bv = (act && t == 0 && (unsigned)idb < (unsigned)st.z) ? __ldcs(src + idb) : czero<T>();
-    C tws[P1];
 #pragma unroll
-    for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
-    tws[0] = mk<T>((T)1, (T)0);
-    const C g = tw[t];
-#pragma unroll
-    for (int j = 0; j < P1; ++j) xs[j] = x[j];
+    for (int jj = 0; jj < P1; ++jj) xs[jj] = x[jj];
     xs[P1 / 2] = cadd(xs[P1 / 2], bv);
     C y[B2][P2];
     sub_inv<F, T>(xs, y, tws, ex, t);
@@ -223,7 +220,7 @@ zpass_fast_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
 #pragma unroll
         for (int q = 0; q < P2; ++q) tile[Z::swz(2 * ((t + P2 * bb) + P1 * q) + 1, sl)] = y[bb][q];
     __syncthreads();
-    C *dst = A + (long long)blockIdx.y * a_band_stride + s0;
+    C *dst = A_band + s0;
 #pragma unroll 4
     for (int i = tid; i < N * TS; i += NT) {
         const int z = i / TS, c = i % TS;
@@ -233,23 +230,21 @@ zpass_fast_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
 }
 
 template <typename T, class F, int NW>
-__global__ void __launch_bounds__(NW * 32, 2)
-zpass_fast_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride)
+__device__ __forceinline__ void z_fwd_tile(const DevPlan &pl, const cx<T> *__restrict__ A_band, cx<T> *__restrict__ packed_band, int j,
+                                           cx<T> *smem, const cx<T> (&tws)[F::P1], cx<T> g)
 {
     using C = cx<T>;
     using Z = ZFast<T, F, NW>;
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    C *tile = reinterpret_cast<C *>(smem_raw);
+    C *tile = smem;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
     const ExTile<T, P2> ex{tile + N * TS + warp * F::EXW + f * F::FS};
-    const C *tw = reinterpret_cast<const C *>(pl.tw3);
-    const int s0 = blockIdx.x * TS, sl = warp * G + f, s = s0 + sl;
+    const int s0 = j * TS, sl = warp * G + f, s = s0 + sl;
     const bool act = s < pl.nsticks;
-    // ---- A[z][s0 .. s0+TS) -> tile, summing the ry partial planes of the forward plane kernel
+    // ---- A[z][s0 .. s0+TS) -> tile, summing the ry partial planes of the generic forward plane kernel
     {
-        const C *src = A + (long long)blockIdx.y * a_band_stride + s0;
+        const C *src = A_band + s0;
         const long long rstride = (long long)pl.n3 * pl.pitch;
         constexpr int U = 8;
         static_assert((N * TS) % (NT * U) == 0, "tile copy is unrolled by U");
@@ -258,13 +253,13 @@ zpass_fast_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int i = i0 + u * NT, z = i / TS, l = i % TS;
-                v[u] = (s0 + l < pl.nsticks) ? __ldcs(src + (long long)z * pl.pitch + l) : czero<T>();
+                v[u] = (s0 + l < pl.nsticks) ? __ldcg(src + (long long)z * pl.pitch + l) : czero<T>();
             }
             for (int p = 1; p < pl.ry; ++p) {
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
                     const int i = i0 + u * NT, z = i / TS, l = i % TS;
-                    if (s0 + l < pl.nsticks) v[u] = cadd(v[u], __ldcs(src + p * rstride + (long long)z * pl.pitch + l));
+                    if (s0 + l < pl.nsticks) v[u] = cadd(v[u], __ldcg(src + p * rstride + (long long)z * pl.pitch + l));
                 }
             }
 #pragma unroll
@@ -274,13 +269,8 @@ zpass_fast_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
             }
         }
     }
-    C tws[P1];
-#pragma unroll
-    for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
-    tws[0] = mk<T>((T)1, (T)0);
-    const C g = tw[t];
     const int4 st = pl.stick[act ? s : 0];
-    C *dst = packed + (long long)blockIdx.y * pl.S + st.x;
+    C *dst = packed_band + st.x;
     const T scale = (T)pl.scale;
     __syncthreads();
     C y[B2][P2], g0[P1], g1[P1];
@@ -302,14 +292,47 @@ zpass_fast_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
             dst[idb] = mk<T>(v.x * scale, v.y * scale);
         }
 #pragma unroll
-        for (int j = 0; j < P1; ++j) {
-            const int idx = ks_of<F>(t, j) - st.y;
+        for (int jj = 0; jj < P1; ++jj) {
+            const int idx = ks_of<F>(t, jj) - st.y;
             if ((unsigned)idx < (unsigned)st.z) {
-                const C v = cadd(g0[j], g1[j]);
+                const C v = cadd(g0[jj], g1[jj]);
                 dst[idx] = mk<T>(v.x * scale, v.y * scale);
             }
         }
     }
+}
+
+// stand-alone z-pass kernels: one tile per CTA, grid = (ceil(n_sticks / TS), bands)
+template <typename T, class F, int NW>
+__global__ void __launch_bounds__(NW * 32, 2)
+zpass_fast_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride)
+{
+    using C = cx<T>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int t = (threadIdx.x & 31) % F::P2;
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    C tws[F::P1];
+#pragma unroll
+    for (int m = 1; m < F::P1; ++m) tws[m] = tw[modn<F::N>(2 * t * m)];
+    tws[0] = mk<T>((T)1, (T)0);
+    z_inv_tile<T, F, NW>(pl, packed + (long long)blockIdx.y * pl.S, A + (long long)blockIdx.y * a_band_stride, blockIdx.x,
+                         reinterpret_cast<C *>(smem_raw), tws, tw[t]);
+}
+
+template <typename T, class F, int NW>
+__global__ void __launch_bounds__(NW * 32, 2)
+zpass_fast_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride)
+{
+    using C = cx<T>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int t = (threadIdx.x & 31) % F::P2;
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    C tws[F::P1];
+#pragma unroll
+    for (int m = 1; m < F::P1; ++m) tws[m] = tw[modn<F::N>(2 * t * m)];
+    tws[0] = mk<T>((T)1, (T)0);
+    z_fwd_tile<T, F, NW>(pl, A + (long long)blockIdx.y * a_band_stride, packed + (long long)blockIdx.y * pl.S, blockIdx.x,
+                         reinterpret_cast<C *>(smem_raw), tws, tw[t]);
 }
 
 } // namespace fftb
