@@ -110,9 +110,9 @@ int launch_plane(const DevPlan &pl, const ColTab &, const void *Ain, void *Aout,
 }
 
 // warp-synchronous persistent plane kernel (fftb_plane_fast.cuh): half-band power-of-two grids
-constexpr int FAST_NW = 8; // warps per CTA of the z-pass kernels
+constexpr int FAST_NW = 4; // warps per CTA of the z-pass kernels (4 CTAs per SM)
 // warps per CTA of the plane kernel: a quarter of the x tasks of a plane
-template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 8 : 2; };
+template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 8 : 2; }; // must divide N / G
 
 static int g_sm_count = 0;
 static int sm_count()
@@ -163,6 +163,8 @@ bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)
     if (dtype == FFTB_C128 && n == 64) { *out = make_plane_fast<double, 64, 8, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 128) { *out = make_plane_fast<float, 128, 8, 8>(); return true; }
     if (dtype == FFTB_C64 && n == 64) { *out = make_plane_fast<float, 64, 8, 4>(); return true; }
+    if (dtype == FFTB_C64 && n == 96) { *out = make_plane_fast<float, 96, 12, 4>(); return true; }   // 48 = 12 x 4
+    if (dtype == FFTB_C128 && n == 96) { *out = make_plane_fast<double, 96, 12, 4>(); return true; }
 #endif
     return false;
 }
@@ -198,6 +200,9 @@ bool find_z_fast(int dtype, int n, bool dense, ZLaunch *out)
     if (dtype == FFTB_C128 && n == 64) { *out = make_z_fast<double, 64, 8, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 128) { *out = make_z_fast<float, 128, 8, 8>(); return true; }
     if (dtype == FFTB_C64 && n == 64) { *out = make_z_fast<float, 64, 8, 4>(); return true; }
+    if (dtype == FFTB_C64 && n == 96) { *out = make_z_fast<float, 96, 12, 4>(); return true; }
+    if (dtype == FFTB_C128 && n == 96) { *out = make_z_fast<double, 96, 12, 4>(); return true; }
+    if (dtype == FFTB_C64 && n == 192) { *out = make_z_fast<float, 192, 24, 4>(); return true; }     // 96 = 24 x 4
 #endif
     return false;
 }

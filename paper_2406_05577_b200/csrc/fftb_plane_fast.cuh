@@ -304,7 +304,7 @@ __device__ __forceinline__ void z_fwd_tile(const DevPlan &pl, const cx<T> *__res
 
 // stand-alone z-pass kernels: one tile per CTA, grid = (ceil(n_sticks / TS), bands)
 template <typename T, class F, int NW>
-__global__ void __launch_bounds__(NW * 32, 2)
+__global__ void __launch_bounds__(NW * 32, F::P1 > 16 ? 2 : 16 / NW)
 zpass_fast_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride)
 {
     using C = cx<T>;
@@ -320,7 +320,7 @@ zpass_fast_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
 }
 
 template <typename T, class F, int NW>
-__global__ void __launch_bounds__(NW * 32, 2)
+__global__ void __launch_bounds__(NW * 32, F::P1 > 16 ? 2 : 16 / NW)
 zpass_fast_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride)
 {
     using C = cx<T>;
