@@ -102,6 +102,18 @@ typedef struct {
  *   - FFTB_C128 with N1 = 192 and dense FFTB_C128 beyond what fits one SM's shared memory. */
 int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc);
 
+/* Create a plan from an EXPLICIT stick map instead of a cut-off: the paper's general domain with an
+ * offset array (PAPER.md:183-185: "x and y dense, only z compressed", :201 `offsets` argument), e.g. the
+ * g-vector list of a plane-wave code whose sphere is shifted by a k-point.  Stick s is the k3 run
+ * k3lo[s] .. k3lo[s]+len[s]-1 of column (k1[s], k2[s]); `desc->cutoff` is ignored, FFTB_FLAG_DENSE is not
+ * allowed.  The arrays (host, n_sticks entries each) are copied.
+ *   FFTB_EINVAL        a point outside [-N_d/2, N_d/2), len < 1, sticks not strictly ascending in (k1, k2)
+ *   FFTB_EUNSUPPORTED  outside the predefined patterns of fftb_plan_create, or: a frequency beyond
+ *                      |k_d| <= N_d/4 (half-band kernels), a hole in the occupied k1 range, or a k1 whose
+ *                      k2 values are not one contiguous run. */
+int fftb_plan_create_explicit(fftb_plan *out, const fftb_plan_desc *desc, int64_t n_sticks, const int32_t *k1,
+                              const int32_t *k2, const int32_t *k3lo, const int32_t *len);
+
 int fftb_plan_info_get(fftb_plan p, fftb_plan_info *info);
 
 /* Copy the stick map to host arrays supplied by the caller (any may be NULL):

@@ -21,7 +21,7 @@ FFTB_OK, FFTB_EINVAL, FFTB_EUNSUPPORTED, FFTB_ENOMEM, FFTB_ECUDA, FFTB_ESTATE = 
 
 # every symbol include/fftb.h declares
 SYMBOLS = [
-    "fftb_plan_create", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
+    "fftb_plan_create", "fftb_plan_create_explicit", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
     "fftb_inverse", "fftb_forward", "fftb_apply_vloc",
     "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
     "fftb_dense_embed", "fftb_dense_extract",
@@ -59,6 +59,7 @@ def lib():
         L = ctypes.CDLL(str(_LIBPATH))
         vp, i32 = ctypes.c_void_p, ctypes.c_int
         L.fftb_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc)]
+        L.fftb_plan_create_explicit.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc), ctypes.c_int64, vp, vp, vp, vp]
         L.fftb_plan_info_get.argtypes = [vp, ctypes.POINTER(PlanInfo)]
         L.fftb_plan_get_map.argtypes = [vp, vp, vp, vp, vp, vp]
         L.fftb_plan_bind.argtypes = [vp, vp, ctypes.c_size_t, vp]
@@ -98,7 +99,8 @@ class Plan:
     """fftb_plan_create / bind / execute / destroy.  Tensors are torch CUDA tensors (or pinned host
     tensors for the *_host calls); shapes follow include/fftb.h: packed (nb, S), cuboid (nb, N3, N2, N1)."""
 
-    def __init__(self, n, cutoff=(0, 0, 0), batch=1, dtype="c128", scale="forward", dense=False):
+    def __init__(self, n, cutoff=(0, 0, 0), batch=1, dtype="c128", scale="forward", dense=False, stick_map=None):
+        """stick_map = (k1, k2, k3lo, len) int arrays: fftb_plan_create_explicit instead of a cut-off."""
         d = PlanDesc()
         d.n[:] = [int(x) for x in n]
         d.cutoff[:] = [int(x) for x in cutoff]
@@ -107,7 +109,13 @@ class Plan:
         d.scale = FFTB_SCALE_FORWARD if scale == "forward" else FFTB_SCALE_NONE
         d.flags = FFTB_FLAG_DENSE if dense else 0
         self._h = ctypes.c_void_p()
-        _check(lib().fftb_plan_create(ctypes.byref(self._h), ctypes.byref(d)), "fftb_plan_create")
+        if stick_map is None:
+            _check(lib().fftb_plan_create(ctypes.byref(self._h), ctypes.byref(d)), "fftb_plan_create")
+        else:
+            m = [np.ascontiguousarray(x, dtype=np.int32) for x in stick_map]
+            assert len(m) == 4 and all(x.shape == m[0].shape and x.ndim == 1 for x in m)
+            _check(lib().fftb_plan_create_explicit(ctypes.byref(self._h), ctypes.byref(d), ctypes.c_int64(m[0].size),
+                                                   *[x.ctypes.data_as(ctypes.c_void_p) for x in m]), "fftb_plan_create_explicit")
         self.n = tuple(int(x) for x in n)
         self.batch = int(batch)
         self.dtype = dtype

@@ -345,18 +345,32 @@ const char *fftb_strerror(int code)
     }
 }
 
-int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
+struct ExplicitMap { int64_t n; const int32_t *k1, *k2, *k3lo, *len; };
+
+static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const ExplicitMap *xm)
 {
     if (!out || !desc) return FFTB_EINVAL;
     *out = nullptr;
     const bool dense = (desc->flags & FFTB_FLAG_DENSE) != 0;
+    if (xm && (dense || xm->n < 1 || xm->n > (int64_t)1 << 24 || !xm->k1 || !xm->k2 || !xm->k3lo || !xm->len)) return FFTB_EINVAL;
     if (desc->flags & ~(uint32_t)FFTB_FLAG_DENSE) return FFTB_EINVAL;
     if (desc->dtype != FFTB_C64 && desc->dtype != FFTB_C128) return FFTB_EINVAL;
     if (desc->scale != FFTB_SCALE_NONE && desc->scale != FFTB_SCALE_FORWARD) return FFTB_EINVAL;
     if (desc->batch < 1) return FFTB_EINVAL;
     for (int d = 0; d < 3; ++d) {
         if (desc->n[d] < 1) return FFTB_EINVAL;
-        if (!dense && (desc->cutoff[d] < 0 || 2 * (long long)desc->cutoff[d] >= desc->n[d])) return FFTB_EINVAL;
+        if (!dense && !xm && (desc->cutoff[d] < 0 || 2 * (long long)desc->cutoff[d] >= desc->n[d])) return FFTB_EINVAL;
+    }
+    if (xm) {
+        // every point inside [-N_d/2, N_d/2) (EINVAL otherwise), strictly ascending (k1, k2), len >= 1
+        for (int64_t s = 0; s < xm->n; ++s) {
+            const long long lo = xm->k3lo[s], hi = lo + xm->len[s] - 1;
+            if (xm->len[s] < 1) return FFTB_EINVAL;
+            if (2 * (long long)xm->k1[s] < -desc->n[0] || 2 * (long long)xm->k1[s] >= desc->n[0]) return FFTB_EINVAL;
+            if (2 * (long long)xm->k2[s] < -desc->n[1] || 2 * (long long)xm->k2[s] >= desc->n[1]) return FFTB_EINVAL;
+            if (2 * lo < -desc->n[2] || 2 * hi >= desc->n[2]) return FFTB_EINVAL;
+            if (s > 0 && !(xm->k1[s - 1] < xm->k1[s] || (xm->k1[s - 1] == xm->k1[s] && xm->k2[s - 1] < xm->k2[s]))) return FFTB_EINVAL;
+        }
     }
     // predefined patterns
     if (desc->n[0] != desc->n[1]) return FFTB_EUNSUPPORTED;
@@ -372,9 +386,16 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
         ZLaunch zfast;
         if (!(genz && genz[0] == '1') && find_z_fast(desc->dtype, desc->n[2], dense, &zfast)) zl = zfast;
     }
-    if (!dense)
+    if (!dense && !xm)
         for (int d = 0; d < 3; ++d)
             if (4 * (long long)desc->cutoff[d] > desc->n[d]) return FFTB_EUNSUPPORTED; // half-band kernels only
+    if (xm) { // half-band kernels only: every frequency within [-N_d/4, N_d/4]
+        for (int64_t s = 0; s < xm->n; ++s) {
+            const long long lo = xm->k3lo[s], hi = lo + xm->len[s] - 1;
+            if (4 * llabs((long long)xm->k1[s]) > desc->n[0] || 4 * llabs((long long)xm->k2[s]) > desc->n[1]) return FFTB_EUNSUPPORTED;
+            if (4 * lo < -desc->n[2] || 4 * hi > desc->n[2]) return FFTB_EUNSUPPORTED;
+        }
+    }
 
     fftb_plan_s *p = new (std::nothrow) fftb_plan_s();
     if (!p) return FFTB_ENOMEM;
@@ -388,40 +409,55 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
         const int n1 = desc->n[0], n2 = desc->n[1], n3 = desc->n[2];
         p->C = (int64_t)n1 * n2 * n3;
         int32_t a[3] = {desc->cutoff[0], desc->cutoff[1], desc->cutoff[2]};
-        // ---- stick map: k1 major, k2 minor, both ascending over signed values (reading R5)
-        const int k1a = dense ? -(n1 / 2) : -a[0], k1b = dense ? (n1 + 1) / 2 - 1 : a[0];
-        const int k2a = dense ? -(n2 / 2) : -a[1], k2b = dense ? (n2 + 1) / 2 - 1 : a[1];
-        p->k1lo = k1a;
+        // ---- stick map: k1 major, k2 minor, both ascending over signed values (reading R5); either
+        // generated from the cut-off (Eq. 9) or given explicitly
+        std::vector<int32_t> ck1, ck2, clo, cln;
+        if (xm) {
+            ck1.assign(xm->k1, xm->k1 + xm->n);
+            ck2.assign(xm->k2, xm->k2 + xm->n);
+            clo.assign(xm->k3lo, xm->k3lo + xm->n);
+            cln.assign(xm->len, xm->len + xm->n);
+            a[0] = a[1] = a[2] = 0;
+        } else {
+            const int k1a = dense ? -(n1 / 2) : -a[0], k1b = dense ? (n1 + 1) / 2 - 1 : a[0];
+            const int k2a = dense ? -(n2 / 2) : -a[1], k2b = dense ? (n2 + 1) / 2 - 1 : a[1];
+            for (int q1 = k1a; q1 <= k1b; ++q1)
+                for (int q2 = k2a; q2 <= k2b; ++q2) {
+                    int lo, ln;
+                    if (dense) {
+                        lo = -(n3 / 2);
+                        ln = n3;
+                    } else {
+                        if (!inside(q1, q2, 0, a)) continue;
+                        int top = 0; // the column is symmetric in k3 and convex: grow from 0
+                        while (top + 1 <= a[2] && inside(q1, q2, top + 1, a)) ++top;
+                        lo = -top;
+                        ln = 2 * top + 1;
+                    }
+                    ck1.push_back(q1); ck2.push_back(q2); clo.push_back(lo); cln.push_back(ln);
+                }
+        }
+        if (ck1.empty()) { delete p; return FFTB_EUNSUPPORTED; }
+        // the kernels need (R6): the occupied k1 form one contiguous range, the k2 of a k1 one contiguous run
+        p->k1lo = ck1.front();
         p->nxocc = 0;
         int64_t run = 0;
-        for (int q1 = k1a; q1 <= k1b; ++q1) {
-            int first = (int)p->k1.size(), cnt = 0, k2lo = 0, k2prev = 0;
-            for (int q2 = k2a; q2 <= k2b; ++q2) {
-                int lo, ln;
-                if (dense) {
-                    lo = -(n3 / 2);
-                    ln = n3;
-                } else {
-                    if (!inside(q1, q2, 0, a)) continue;
-                    int top = 0; // the column is symmetric in k3 and convex: grow from 0
-                    while (top + 1 <= a[2] && inside(q1, q2, top + 1, a)) ++top;
-                    lo = -top;
-                    ln = 2 * top + 1;
-                }
-                if (cnt == 0) k2lo = q2;
-                else if (q2 != k2prev + 1) { delete p; return FFTB_EUNSUPPORTED; } // non-contiguous k2 run (R6)
-                k2prev = q2;
-                ++cnt;
+        for (size_t s = 0; s < ck1.size();) {
+            const int q1 = ck1[s];
+            if (q1 != p->k1lo + p->nxocc) { delete p; return FFTB_EUNSUPPORTED; } // hole in the occupied k1 range
+            const int first = (int)p->k1.size();
+            int cnt = 0;
+            for (; s < ck1.size() && ck1[s] == q1; ++s, ++cnt) {
+                if (cnt > 0 && ck2[s] != ck2[s - 1] + 1) { delete p; return FFTB_EUNSUPPORTED; } // non-contiguous k2 run
                 p->k1.push_back(q1);
-                p->k2.push_back(q2);
-                p->k3lo.push_back(lo);
-                p->len.push_back(ln);
+                p->k2.push_back(ck2[s]);
+                p->k3lo.push_back(clo[s]);
+                p->len.push_back(cln[s]);
                 p->off.push_back(run);
-                run += ln;
+                run += cln[s];
             }
-            if (cnt == 0) { delete p; return FFTB_EUNSUPPORTED; } // hole in the occupied k1 range
             int4 c;
-            c.x = first; c.y = cnt; c.z = k2lo; c.w = 0;
+            c.x = first; c.y = cnt; c.z = p->k2[first]; c.w = 0;
             p->h_col.push_back(c);
             ++p->nxocc;
         }
@@ -506,6 +542,15 @@ int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc)
     }
     *out = p;
     return FFTB_OK;
+}
+
+int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc) { return plan_create_impl(out, desc, nullptr); }
+
+int fftb_plan_create_explicit(fftb_plan *out, const fftb_plan_desc *desc, int64_t n_sticks, const int32_t *k1, const int32_t *k2,
+                              const int32_t *k3lo, const int32_t *len)
+{
+    const ExplicitMap xm = {n_sticks, k1, k2, k3lo, len};
+    return plan_create_impl(out, desc, &xm);
 }
 
 int fftb_plan_info_get(fftb_plan p, fftb_plan_info *info)

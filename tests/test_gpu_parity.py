@@ -240,3 +240,36 @@ def test_full_size_configs_sampled_bands(fb, oracle, cfg):
         e_psi = float((d_psi.abs() ** 2).sum().item())
         e_c = float((np.abs(c.astype(np.complex128)) ** 2).sum())
         assert abs(e_psi - C * e_c) <= 1e-6 * C * e_c
+
+
+@pytest.mark.parametrize("n,radius,centre,dtype,trim", [((64, 64, 64), 11, (2, -3, 4), "c128", 7), ((128, 128, 128), 27, (-3, 4, 2), "c128", None),
+                                                        ((32, 32, 96), 6, (1, 1, -9), "c64", 3), ((96, 96, 64), 13, (3, -2, 1), "c128", 5)])
+def test_explicit_stick_map_vs_oracle(fb, oracle, n, radius, centre, dtype, trim):
+    """plans from an explicit stick map, here a k-point-shifted
+    ball with (optionally) randomly shortened sticks, against the oracle's plain definition evaluated on
+    the point list the TEST expands from the map."""
+    from test_host_cabi import _shifted_ball_map
+
+    sm = _shifted_ball_map(n, radius, centre, trim_seed=trim)
+    nb = 3
+    p = fb.Plan(n, batch=nb, dtype=dtype, stick_map=sm).bind()
+    rep = np.repeat(np.arange(sm[0].size), sm[3])
+    off = np.concatenate([[0], np.cumsum(sm[3])])[:-1]
+    k = (sm[0][rep], sm[1][rep], (sm[2][rep] + (np.arange(rep.size) - off[rep])).astype(np.int32))
+    assert all(np.array_equal(a, b) for a, b in zip(p.points(), k))
+    w = wl.Workload(0, "explicit", n, (0, 0, 0), dtype, nb, "uniform", "inv_fwd")
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    d_psi = p.inverse(d_c)
+    torch.cuda.synchronize()
+    assert _rel(d_psi.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol
+    g = wl.cuboid(w)
+    d_f = p.forward(torch.from_numpy(g).cuda())
+    torch.cuda.synchronize()
+    C = float(np.prod(n))
+    assert _rel(d_f.cpu().numpy(), oracle.forward(n, k, g, 1.0 / C)) <= w.tol
+    v = wl.potential(w)
+    d_o = p.apply_vloc(d_c, torch.from_numpy(v).cuda())
+    torch.cuda.synchronize()
+    assert _rel(d_o.cpu().numpy(), oracle.apply_vloc(n, k, c, v, 1.0 / C)) <= w.tol
+    p.destroy()

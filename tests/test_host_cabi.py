@@ -108,3 +108,62 @@ def test_missing_library_fails_loudly(monkeypatch, tmp_path):
     monkeypatch.setattr(fb, "_LIBPATH", tmp_path / "nope.so")
     with pytest.raises(ImportError, match="no CPU fallback"):
         fb.lib()
+
+
+def _shifted_ball_map(n, radius, centre, trim_seed=None):
+    """Sticks of the ball |k - centre| <= radius (a k-point-shifted sphere), written out in numpy as
+    mask + sort (independent of both the plan builder and the oracle's cut-off enumeration); with
+    trim_seed the sticks are shortened at random, so the map is no cut-off of any kind."""
+    r = radius + max(abs(c) for c in centre)
+    g = np.arange(-r, r + 1)
+    k1, k2, k3 = np.meshgrid(g, g, g, indexing="ij")
+    inside = (k1 - centre[0]) ** 2 + (k2 - centre[1]) ** 2 + (k3 - centre[2]) ** 2 <= radius ** 2
+    cols = inside.any(axis=2)
+    m1, m2 = k1[:, :, 0][cols], k2[:, :, 0][cols]
+    lo = np.array([g[inside[a + r, b + r]].min() for a, b in zip(m1, m2)])
+    hi = np.array([g[inside[a + r, b + r]].max() for a, b in zip(m1, m2)])
+    if trim_seed is not None:
+        rng = np.random.default_rng(trim_seed)
+        cut_lo = rng.integers(0, 3, size=lo.size)
+        cut_hi = rng.integers(0, 3, size=lo.size)
+        lo2, hi2 = lo + cut_lo, hi - cut_hi
+        keep = lo2 <= hi2
+        lo, hi = np.where(keep, lo2, lo), np.where(keep, hi2, hi)
+    return m1.astype(np.int32), m2.astype(np.int32), lo.astype(np.int32), (hi - lo + 1).astype(np.int32)
+
+
+def test_explicit_stick_map_round_trip_and_errors():
+    """fftb_plan_create_explicit (PAPER.md:183-185, :201): the map given is the map kept, bit for bit;
+    maps outside the predefined patterns are refused with a code."""
+    n = (64, 64, 64)
+    sm = _shifted_ball_map(n, 11, (2, -3, 4), trim_seed=7)
+    p = fb.Plan(n, batch=2, stick_map=sm)
+    m = p.get_map()
+    for key, ref in zip(("k1", "k2", "k3lo", "len"), sm):
+        assert np.array_equal(m[key], ref), key
+    assert np.array_equal(m["off"], np.concatenate([[0], np.cumsum(sm[3])]))
+    assert p.S == int(sm[3].sum()) and p.info["n_sticks"] == sm[0].size
+    p.destroy()
+    k1, k2, lo, ln = [x.copy() for x in sm]
+    with pytest.raises(fb.FftbError) as e:      # not ascending
+        fb.Plan(n, stick_map=(k1[::-1].copy(), k2[::-1].copy(), lo[::-1].copy(), ln[::-1].copy()))
+    assert e.value.code == fb.FFTB_EINVAL
+    bad = ln.copy(); bad[3] = 0
+    with pytest.raises(fb.FftbError) as e:      # empty stick
+        fb.Plan(n, stick_map=(k1, k2, lo, bad))
+    assert e.value.code == fb.FFTB_EINVAL
+    far = lo.copy(); far[0] = 40
+    with pytest.raises(fb.FftbError) as e:      # outside [-N/2, N/2)
+        fb.Plan(n, stick_map=(k1, k2, far, ln))
+    assert e.value.code == fb.FFTB_EINVAL
+    wide = ln.copy(); wide[0] = 17 - lo[0] + 1
+    with pytest.raises(fb.FftbError) as e:      # beyond the half band |k| <= N/4
+        fb.Plan(n, stick_map=(k1, k2, lo, wide))
+    assert e.value.code == fb.FFTB_EUNSUPPORTED
+    hole = np.ones(k1.size, bool); hole[np.flatnonzero(k1 == k1[k1.size // 2])[1]] = False
+    with pytest.raises(fb.FftbError) as e:      # a k2 run with a hole
+        fb.Plan(n, stick_map=(k1[hole], k2[hole], lo[hole], ln[hole]))
+    assert e.value.code == fb.FFTB_EUNSUPPORTED
+    with pytest.raises(fb.FftbError) as e:      # dense + explicit
+        fb.Plan(n, stick_map=sm, dense=True)
+    assert e.value.code == fb.FFTB_EINVAL
