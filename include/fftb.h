@@ -139,8 +139,11 @@ int fftb_apply_vloc(fftb_plan p, const void *d_packed_in, void *d_packed_out, co
                     void *stream);
 
 /* The same three operations with the PACKED arrays in host memory (pinned memory makes the copies
- * asynchronous): the library copies them through the staging area inside the bind block
- * (cudaMemcpyAsync on `stream`), cuboid and vloc stay device pointers. */
+ * asynchronous): the library copies them through the staging area inside the bind block, cuboid and vloc
+ * stay device pointers.  Large batches cross PCIe in band chunks on two copy streams owned by the plan
+ * (created in fftb_plan_bind), overlapped with the transforms of the neighbouring chunks; the calls stay
+ * ordered on `stream`: work queued on it earlier is finished before the first copy, work queued later
+ * sees the complete result. */
 int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb, void *stream);
 int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb, void *stream);
 int fftb_apply_vloc_host(fftb_plan p, const void *h_packed_in, void *h_packed_out, const void *d_vloc, int nb,

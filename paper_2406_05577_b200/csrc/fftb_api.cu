@@ -297,6 +297,11 @@ struct fftb_plan_s {
     // bound state
     unsigned char *d_mem;
     bool staging;
+    // *_host calls: the packed arrays cross PCIe in HOST_PIPE band chunks on two private copy streams, so
+    // that a chunk's copy runs while its neighbours are transformed (created once in fftb_plan_bind)
+    cudaStream_t cs_in, cs_out;
+    cudaEvent_t hev_start, hev_done, hev_in[8], hev_out[8];
+    bool pipe_ok;
     DevPlan dev;
     ColTab coltab; // the column table again, as a by-value kernel parameter of the fast plane kernel
     int sticky;
@@ -532,6 +537,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         p->bytes_stage = o;
         p->d_mem = nullptr;
         p->staging = false;
+        p->pipe_ok = false;
         p->sticky = 0;
         p->launches = 0;
         p->prof = false;
@@ -599,6 +605,17 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
     if (e != cudaSuccess) { p->sticky = FFTB_ECUDA; return FFTB_ECUDA; }
     p->d_mem = m;
     p->staging = bytes >= p->bytes_stage;
+    if (p->staging && !p->pipe_ok) {
+        bool ok = cudaStreamCreateWithFlags(&p->cs_in, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaStreamCreateWithFlags(&p->cs_out, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&p->hev_start, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&p->hev_done, cudaEventDisableTiming) == cudaSuccess;
+        for (int i = 0; i < 8 && ok; ++i)
+            ok = cudaEventCreateWithFlags(&p->hev_in[i], cudaEventDisableTiming) == cudaSuccess &&
+                 cudaEventCreateWithFlags(&p->hev_out[i], cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) { p->sticky = FFTB_ECUDA; return FFTB_ECUDA; }
+        p->pipe_ok = true;
+    }
     DevPlan &dv = p->dev;
     dv.n1 = p->desc.n[0]; dv.n2 = p->desc.n[1]; dv.n3 = p->desc.n[2];
     dv.nsticks = p->nsticks; dv.pitch = p->pitch; dv.nxocc = p->nxocc; dv.k1lo = p->k1lo; dv.ry = p->ry;
@@ -706,17 +723,44 @@ static int check_host(fftb_plan p, int nb)
     return FFTB_OK;
 }
 
+// Band chunks of the *_host calls: HOST_PIPE chunks when the batch is large enough to keep the persistent
+// kernels efficient, otherwise one.
+static int host_chunks(fftb_plan p, int nb)
+{
+    const int HOST_PIPE = 4;
+    return (p->pipe_ok && nb >= 8 * HOST_PIPE) ? HOST_PIPE : 1;
+}
+#define FFTB_CU(call) do { if ((call) != cudaSuccess) { p->sticky = FFTB_ECUDA; return FFTB_ECUDA; } } while (0)
+
 int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb, void *stream)
 {
     int rc = check_host(p, nb);
     if (rc) return rc;
     if (!h_packed || !d_cuboid) return FFTB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
     unsigned char *stg = p->d_mem + p->o_stage;
-    if (cudaMemcpyAsync(stg, h_packed, (size_t)nb * p->S * p->elem, cudaMemcpyHostToDevice, (cudaStream_t)stream) != cudaSuccess) {
-        p->sticky = FFTB_ECUDA;
-        return FFTB_ECUDA;
+    const int K = host_chunks(p, nb);
+    const size_t band = (size_t)p->S * p->elem, cband = (size_t)p->C * p->elem;
+    if (K == 1) {
+        FFTB_CU(cudaMemcpyAsync(stg, h_packed, (size_t)nb * band, cudaMemcpyHostToDevice, st));
+        return fftb_inverse(p, stg, d_cuboid, nb, stream);
     }
-    return fftb_inverse(p, stg, d_cuboid, nb, stream);
+    // the copies start after everything already queued on the caller's stream (it may still read the staging area)
+    FFTB_CU(cudaEventRecord(p->hev_start, st));
+    FFTB_CU(cudaStreamWaitEvent(p->cs_in, p->hev_start, 0));
+    int launches = 0;
+    for (int k = 0; k < K; ++k) {
+        const int b0 = (int)((long long)nb * k / K), b1 = (int)((long long)nb * (k + 1) / K);
+        FFTB_CU(cudaMemcpyAsync(stg + b0 * band, (const unsigned char *)h_packed + b0 * band, (size_t)(b1 - b0) * band,
+                                cudaMemcpyHostToDevice, p->cs_in));
+        FFTB_CU(cudaEventRecord(p->hev_in[k], p->cs_in));
+        FFTB_CU(cudaStreamWaitEvent(st, p->hev_in[k], 0));
+        rc = fftb_inverse(p, stg + b0 * band, (unsigned char *)d_cuboid + b0 * cband, b1 - b0, stream);
+        if (rc) return rc;
+        launches += p->launches;
+    }
+    p->launches = launches;
+    return FFTB_OK;
 }
 
 int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb, void *stream)
@@ -724,13 +768,31 @@ int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb,
     int rc = check_host(p, nb);
     if (rc) return rc;
     if (!h_packed || !d_cuboid) return FFTB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
     unsigned char *stg = p->d_mem + p->o_stage;
-    rc = fftb_forward(p, d_cuboid, stg, nb, stream);
-    if (rc) return rc;
-    if (cudaMemcpyAsync(h_packed, stg, (size_t)nb * p->S * p->elem, cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess) {
-        p->sticky = FFTB_ECUDA;
-        return FFTB_ECUDA;
+    const int K = host_chunks(p, nb);
+    const size_t band = (size_t)p->S * p->elem, cband = (size_t)p->C * p->elem;
+    if (K == 1) {
+        rc = fftb_forward(p, d_cuboid, stg, nb, stream);
+        if (rc) return rc;
+        FFTB_CU(cudaMemcpyAsync(h_packed, stg, (size_t)nb * band, cudaMemcpyDeviceToHost, st));
+        return FFTB_OK;
     }
+    int launches = 0;
+    for (int k = 0; k < K; ++k) {
+        const int b0 = (int)((long long)nb * k / K), b1 = (int)((long long)nb * (k + 1) / K);
+        rc = fftb_forward(p, (const unsigned char *)d_cuboid + b0 * cband, stg + b0 * band, b1 - b0, stream);
+        if (rc) return rc;
+        launches += p->launches;
+        FFTB_CU(cudaEventRecord(p->hev_out[k], st));
+        FFTB_CU(cudaStreamWaitEvent(p->cs_out, p->hev_out[k], 0));
+        FFTB_CU(cudaMemcpyAsync((unsigned char *)h_packed + b0 * band, stg + b0 * band, (size_t)(b1 - b0) * band,
+                                cudaMemcpyDeviceToHost, p->cs_out));
+    }
+    // the call completes, in the caller's stream order, when the last chunk is in host memory
+    FFTB_CU(cudaEventRecord(p->hev_done, p->cs_out));
+    FFTB_CU(cudaStreamWaitEvent(st, p->hev_done, 0));
+    p->launches = launches;
     return FFTB_OK;
 }
 
@@ -739,18 +801,37 @@ int fftb_apply_vloc_host(fftb_plan p, const void *h_in, void *h_out, const void 
     int rc = check_host(p, nb);
     if (rc) return rc;
     if (!h_in || !h_out) return FFTB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
     unsigned char *stg = p->d_mem + p->o_stage;
-    const size_t bytes = (size_t)nb * p->S * p->elem;
-    if (cudaMemcpyAsync(stg, h_in, bytes, cudaMemcpyHostToDevice, (cudaStream_t)stream) != cudaSuccess) {
-        p->sticky = FFTB_ECUDA;
-        return FFTB_ECUDA;
+    const int K = host_chunks(p, nb);
+    const size_t band = (size_t)p->S * p->elem;
+    if (K == 1) {
+        FFTB_CU(cudaMemcpyAsync(stg, h_in, (size_t)nb * band, cudaMemcpyHostToDevice, st));
+        rc = fftb_apply_vloc(p, stg, stg, d_vloc, nb, stream);
+        if (rc) return rc;
+        FFTB_CU(cudaMemcpyAsync(h_out, stg, (size_t)nb * band, cudaMemcpyDeviceToHost, st));
+        return FFTB_OK;
     }
-    rc = fftb_apply_vloc(p, stg, stg, d_vloc, nb, stream);
-    if (rc) return rc;
-    if (cudaMemcpyAsync(h_out, stg, bytes, cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess) {
-        p->sticky = FFTB_ECUDA;
-        return FFTB_ECUDA;
+    FFTB_CU(cudaEventRecord(p->hev_start, st));
+    FFTB_CU(cudaStreamWaitEvent(p->cs_in, p->hev_start, 0));
+    int launches = 0;
+    for (int k = 0; k < K; ++k) {
+        const int b0 = (int)((long long)nb * k / K), b1 = (int)((long long)nb * (k + 1) / K);
+        FFTB_CU(cudaMemcpyAsync(stg + b0 * band, (const unsigned char *)h_in + b0 * band, (size_t)(b1 - b0) * band,
+                                cudaMemcpyHostToDevice, p->cs_in));
+        FFTB_CU(cudaEventRecord(p->hev_in[k], p->cs_in));
+        FFTB_CU(cudaStreamWaitEvent(st, p->hev_in[k], 0));
+        rc = fftb_apply_vloc(p, stg + b0 * band, stg + b0 * band, d_vloc, b1 - b0, stream);
+        if (rc) return rc;
+        launches += p->launches;
+        FFTB_CU(cudaEventRecord(p->hev_out[k], st));
+        FFTB_CU(cudaStreamWaitEvent(p->cs_out, p->hev_out[k], 0));
+        FFTB_CU(cudaMemcpyAsync((unsigned char *)h_out + b0 * band, stg + b0 * band, (size_t)(b1 - b0) * band,
+                                cudaMemcpyDeviceToHost, p->cs_out));
     }
+    FFTB_CU(cudaEventRecord(p->hev_done, p->cs_out));
+    FFTB_CU(cudaStreamWaitEvent(st, p->hev_done, 0));
+    p->launches = launches;
     return FFTB_OK;
 }
 
@@ -814,6 +895,13 @@ int fftb_plan_destroy(fftb_plan p)
 {
     if (!p) return FFTB_EINVAL;
     for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
+    if (p->pipe_ok) {
+        cudaStreamDestroy(p->cs_in);
+        cudaStreamDestroy(p->cs_out);
+        cudaEventDestroy(p->hev_start);
+        cudaEventDestroy(p->hev_done);
+        for (int i = 0; i < 8; ++i) { cudaEventDestroy(p->hev_in[i]); cudaEventDestroy(p->hev_out[i]); }
+    }
     delete p;
     return FFTB_OK;
 }
