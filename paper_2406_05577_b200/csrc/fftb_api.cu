@@ -112,7 +112,7 @@ int launch_plane(const DevPlan &pl, const ColTab &, const void *Ain, void *Aout,
 // warp-synchronous persistent plane kernel (fftb_plane_fast.cuh): half-band power-of-two grids
 constexpr int FAST_NW = 4; // warps per CTA of the z-pass kernels (4 CTAs per SM)
 // warps per CTA of the plane kernel: a quarter of the x tasks of a plane
-template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 8 : 2; }; // must divide N / G
+template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 8 : (N == 96 ? 4 : 2); }; // must divide N / G; measured best
 
 static int g_sm_count = 0;
 static int sm_count()
