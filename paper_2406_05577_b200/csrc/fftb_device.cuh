@@ -147,4 +147,24 @@ template <int N> __device__ __forceinline__ int modn(int x)
 template <typename C> __device__ __forceinline__ C ldg_stream(const C *p) { return __ldcs(p); }
 template <typename C> __device__ __forceinline__ void stg_stream(C *p, C v) { __stcs(p, v); }
 
+// 2-element (x = 2n', 2n'+1) global accesses: 32 bytes for complex128, 16 for complex64
+__device__ __forceinline__ void st_pair(double2 *p, double2 a, double2 b)
+{
+    asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
+}
+__device__ __forceinline__ void st_pair(float2 *p, float2 a, float2 b)
+{
+    __stcs(reinterpret_cast<float4 *>(p), make_float4(a.x, a.y, b.x, b.y));
+}
+__device__ __forceinline__ void ld_pair(const double2 *p, double2 &a, double2 &b)
+{
+    asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a.x), "=d"(a.y), "=d"(b.x), "=d"(b.y) : "l"(p));
+}
+__device__ __forceinline__ void ld_pair(const float2 *p, float2 &a, float2 &b)
+{
+    const float4 v = __ldcs(reinterpret_cast<const float4 *>(p));
+    a = make_float2(v.x, v.y);
+    b = make_float2(v.z, v.w);
+}
+
 } // namespace fftb

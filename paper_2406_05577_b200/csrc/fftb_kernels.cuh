@@ -370,9 +370,13 @@ __global__ void __launch_bounds__(NT) plane_k(DevPlan pl, const cx<T> *__restric
                 if (act2) {
                     C *row = cub_out + (((long long)b * pl.n3 + z) * N2 + ygl) * N1;
 #pragma unroll
-                    for (int q = 0; q < P2; ++q)
+                    for (int q = 0; q < P2; ++q) {
+                        if constexpr (RX == 2) st_pair(row + 2 * (ml + P1 * q), reg[0][q], reg[1][q]); // one 32-byte store
+                        else {
 #pragma unroll
-                        for (int e = 0; e < RX; ++e) stg_stream(row + RX * (ml + P1 * q) + e, reg[e][q]);
+                            for (int e = 0; e < RX; ++e) stg_stream(row + RX * (ml + P1 * q) + e, reg[e][q]);
+                        }
+                    }
                 }
             }
         }
@@ -393,9 +397,13 @@ __global__ void __launch_bounds__(NT) plane_k(DevPlan pl, const cx<T> *__restric
             if (act2) {
                 const C *row = cub_in + (((long long)b * pl.n3 + z) * N2 + ygl) * N1;
 #pragma unroll
-                for (int q = 0; q < P2; ++q)
+                for (int q = 0; q < P2; ++q) {
+                    if constexpr (RX == 2) ld_pair(row + 2 * (ml + P1 * q), reg[0][q], reg[1][q]);
+                    else {
 #pragma unroll
-                    for (int e = 0; e < RX; ++e) reg[e][q] = ldg_stream(row + RX * (ml + P1 * q) + e);
+                        for (int e = 0; e < RX; ++e) reg[e][q] = ldg_stream(row + RX * (ml + P1 * q) + e);
+                    }
+                }
             }
         }
         if constexpr (MODE != MODE_INV) {
