@@ -295,7 +295,8 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
     }
     __syncthreads();
     T vq0[B2][P2], vq1[B2][P2]; // V(r) of the next x task (VLOC)
-    int id = blockIdx.x, z = id % pl.n3, b = id / pl.n3; // current plane
+    int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;          // current plane
+    const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;      // step to this CTA's next plane
     if (kplanes > 0) {
         if constexpr (MODE == MODE_FWD) line_issue(b, z, warp);
         else if (tid == 0) stage_issue(b, z);
@@ -303,7 +304,7 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
     }
 #pragma unroll 1
     for (int i = 0; i < kplanes; ++i) {
-        const int idn = id + gridDim.x, zn = idn % pl.n3, bn = idn / pl.n3; // this CTA's next plane
+        const int zc = z + dz, zn = zc >= pl.n3 ? zc - pl.n3 : zc, bn = b + db + (zc >= pl.n3 ? 1 : 0); // next plane
         const bool more = i + 1 < kplanes;
         if constexpr (MODE != MODE_FWD) {
             // ======================================================== inverse y pass: staged row -> both buffers
@@ -364,7 +365,7 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
             // touches the same columns from the same warp, no barrier needed.
             if constexpr (MODE == MODE_FWD) __syncthreads();
         }
-        id = idn; z = zn; b = bn;
+        z = zn; b = bn;
     }
 }
 
