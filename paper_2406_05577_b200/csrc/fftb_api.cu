@@ -9,6 +9,7 @@
 #include "fftb_kernels.cuh"
 #include "fftb_plane_fast.cuh"
 #include "fftb_plane_pf.cuh"
+#include "fftb_plane_r4.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -72,9 +73,10 @@ struct ZLaunch {
     int (*inv)(const DevPlan &, const void *packed, void *A, long long stride, int nb, cudaStream_t);
     int (*fwd)(const DevPlan &, const void *A, void *packed, long long stride, int nb, cudaStream_t);
 };
+struct PlanTabs { ColTab ct; ColTab4 ct4; }; // column tables passed by value to the fast kernels
 struct PlaneLaunch {
     int ry;
-    int (*run[3])(const DevPlan &, const ColTab &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v,
+    int (*run[3])(const DevPlan &, const PlanTabs &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v,
                   long long sin, long long sout, int nb, cudaStream_t);
 };
 
@@ -97,7 +99,7 @@ template <typename T, class AZ> int launch_zfwd(const DevPlan &pl, const void *A
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 template <typename T, class AX, class AY, int MODE>
-int launch_plane(const DevPlan &pl, const ColTab &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
+int launch_plane(const DevPlan &pl, const PlanTabs &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
                  long long sout, int nb, cudaStream_t st)
 {
     using TU = PlaneTune<AX, AY>;
@@ -128,7 +130,7 @@ static int sm_count()
 }
 
 template <typename T, class F, int MODE>
-int launch_plane_fast(const DevPlan &pl, const ColTab &ct, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
+int launch_plane_fast(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
                       long long sout, int nb, cudaStream_t st)
 {
     constexpr int NW = PlaneNW<F::N>::value;
@@ -147,7 +149,7 @@ int launch_plane_fast(const DevPlan &pl, const ColTab &ct, const void *Ain, void
     const int nplanes = pl.n3 * nb;
     int grid = sm_count() * per_sm;
     if (grid > nplanes) grid = nplanes;
-    k<<<grid, NW * 32, smem, st>>>(pl, ct, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout, nplanes);
+    k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout, nplanes);
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
@@ -155,6 +157,26 @@ template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
     using F = FastCfg<T, N, P1, P2>;
     return PlaneLaunch{1, {&launch_plane_fast<T, F, MODE_INV>, &launch_plane_fast<T, F, MODE_FWD>, &launch_plane_fast<T, F, MODE_VLOC>}};
 }
+// inverse plane kernel of the 256 pattern (fftb_plane_r4.cuh)
+template <typename T>
+int launch_plane_r4_inv(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *, const void *, void *cout, const void *, long long sin,
+                        long long, int nb, cudaStream_t st)
+{
+    constexpr int NW = 8;
+    auto k = plane_r4_inv_k<T, NW>;
+    const size_t smem = PlaneR4<T, NW>::smem_bytes;
+    static bool ready = false;
+    if (!ready) {
+        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+        ready = true;
+    }
+    const int nplanes = pl.n3 * nb;
+    int grid = sm_count();
+    if (grid > nplanes) grid = nplanes;
+    k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)Ain, (cx<T> *)cout, sin, nplanes);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+
 bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)
 {
     if (dense) return false;
@@ -303,7 +325,7 @@ struct fftb_plan_s {
     cudaEvent_t hev_start, hev_done, hev_in[8], hev_out[8];
     bool pipe_ok;
     DevPlan dev;
-    ColTab coltab; // the column table again, as a by-value kernel parameter of the fast plane kernel
+    PlanTabs tabs; // the column table again, as a by-value kernel parameter of the fast plane kernels
     int sticky;
     int launches;
     // optional per-kernel timing (fftb_plan_profile): event pairs recorded around every launch
@@ -387,6 +409,8 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         const char *gen = getenv("FFTB_GENERIC_PLANE"); // debugging aid: keep the generic plane kernel
         PlaneLaunch fast;
         if (!(gen && gen[0] == '1') && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) { plk = fast; fast_plane = true; }
+        // 256 pattern, complex128: the inverse plane pass has its own persistent kernel (four-way split)
+        if (!(gen && gen[0] == '1') && !dense && desc->dtype == FFTB_C128 && desc->n[0] == 256) plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
         const char *genz = getenv("FFTB_GENERIC_Z");
         ZLaunch zfast;
         if (!(genz && genz[0] == '1') && find_z_fast(desc->dtype, desc->n[2], dense, &zfast)) zl = zfast;
@@ -475,9 +499,11 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         for (int c = 0; c < p->nxocc; ++c)
             if (p->h_col[c].y <= 1) p->h_colperm.push_back(c);
         if (p->S >= (int64_t)1 << 31) { delete p; return FFTB_EUNSUPPORTED; }
-        memset(&p->coltab, 0, sizeof(p->coltab));
+        memset(&p->tabs, 0, sizeof(p->tabs));
         if (p->nxocc <= FAST_MAXCOL)
-            for (int c = 0; c < p->nxocc; ++c) { p->coltab.col[c] = p->h_col[c]; p->coltab.perm[c] = p->h_colperm[c]; }
+            for (int c = 0; c < p->nxocc; ++c) { p->tabs.ct.col[c] = p->h_col[c]; p->tabs.ct.perm[c] = p->h_colperm[c]; }
+        if (p->nxocc <= R4_MAXCOL)
+            for (int c = 0; c < p->nxocc; ++c) { p->tabs.ct4.col[c] = p->h_col[c]; p->tabs.ct4.perm[c] = p->h_colperm[c]; }
         p->pitch = (int)align_up((size_t)p->nsticks, 16);
         p->h_stick.resize(p->nsticks);
         for (int s = 0; s < p->nsticks; ++s) {
@@ -654,7 +680,7 @@ int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void
         rc = p->zl.inv(p->dev, pk, A, p->a_inv_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_PLANE_INV, st);
-        if (!rc) rc = p->plk.run[MODE_INV](p->dev, p->coltab, A, nullptr, nullptr, cb, nullptr, p->a_inv_stride, 0, nc, st);
+        if (!rc) rc = p->plk.run[MODE_INV](p->dev, p->tabs, A, nullptr, nullptr, cb, nullptr, p->a_inv_stride, 0, nc, st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
         p->launches += 2;
@@ -674,7 +700,7 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
         unsigned char *pk = (unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
         const unsigned char *cb = (const unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
         prof_begin(p, K_PLANE_FWD, st);
-        rc = p->plk.run[MODE_FWD](p->dev, p->coltab, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd_stride, nc, st);
+        rc = p->plk.run[MODE_FWD](p->dev, p->tabs, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_ZFWD, st);
         if (!rc) rc = p->zl.fwd(p->dev, A, pk, p->a_fwd_stride, nc, st);
@@ -702,7 +728,7 @@ int fftb_apply_vloc(fftb_plan p, const void *d_in, void *d_out, const void *d_vl
         rc = p->zl.inv(p->dev, pi, Ai, p->a_inv_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_PLANE_VLOC, st);
-        if (!rc) rc = p->plk.run[MODE_VLOC](p->dev, p->coltab, Ai, Af, nullptr, nullptr, d_vloc, p->a_inv_stride, p->a_fwd_stride, nc, st);
+        if (!rc) rc = p->plk.run[MODE_VLOC](p->dev, p->tabs, Ai, Af, nullptr, nullptr, d_vloc, p->a_inv_stride, p->a_fwd_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_ZFWD, st);
         if (!rc) rc = p->zl.fwd(p->dev, Af, po, p->a_fwd_stride, nc, st);

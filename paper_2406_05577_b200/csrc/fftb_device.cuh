@@ -55,42 +55,55 @@ template <typename C> __device__ __forceinline__ C mul_jpow(C a, int p)
     return r;
 }
 
-// cos / sin of 2 pi q / 48, q in [0, 48): every twiddle of the P <= 16 codelets
-__host__ __device__ constexpr double cos48_first(int q)
+// cos / sin of 2 pi q / 96, q in [0, 96): every root of order 2, 3, 4, 6, 8, 12, 16, 24, 32, 48 the
+// codelets and the pre-/post-twiddles need, as correctly rounded literals
+__host__ __device__ constexpr double cos96_first(int q)
 {
     return q == 0 ? 1.0
-         : q == 1 ? 0.9914448613738104111445575
-         : q == 2 ? 0.9659258262890682867497432
-         : q == 3 ? 0.9238795325112867561281832
-         : q == 4 ? 0.8660254037844386467637232
-         : q == 5 ? 0.793353340291235164579777
-         : q == 6 ? 0.7071067811865475244008444
-         : q == 7 ? 0.6087614290087206394160975
-         : q == 8 ? 0.5
-         : q == 9 ? 0.38268343236508977172846
-         : q == 10 ? 0.2588190451025207623488988
-         : q == 11 ? 0.1305261922200515915484062
+         : q == 1 ? 0.9978589232386035067380698
+         : q == 2 ? 0.9914448613738104111445575
+         : q == 3 ? 0.9807852804032304491261822
+         : q == 4 ? 0.9659258262890682867497432
+         : q == 5 ? 0.9469301294951056642558043
+         : q == 6 ? 0.9238795325112867561281832
+         : q == 7 ? 0.8968727415326883038941039
+         : q == 8 ? 0.8660254037844386467637232
+         : q == 9 ? 0.8314696123025452370787884
+         : q == 10 ? 0.793353340291235164579777
+         : q == 11 ? 0.7518398074789773964075194
+         : q == 12 ? 0.7071067811865475244008444
+         : q == 13 ? 0.6593458151000688684251246
+         : q == 14 ? 0.6087614290087206394160975
+         : q == 15 ? 0.5555702330196022247428308
+         : q == 16 ? 0.5
+         : q == 17 ? 0.442288690219001281995239
+         : q == 18 ? 0.38268343236508977172846
+         : q == 19 ? 0.3214394653031615807010576
+         : q == 20 ? 0.2588190451025207623488988
+         : q == 21 ? 0.1950903220161282678482849
+         : q == 22 ? 0.1305261922200515915484062
+         : q == 23 ? 0.06540312923014306681531556
          : 0.0;
 }
-__host__ __device__ constexpr double cos48(int q)
+__host__ __device__ constexpr double cos96(int q)
 {
-    q = ((q % 48) + 48) % 48;
-    return q <= 12 ? cos48_first(q) : q <= 24 ? -cos48_first(24 - q) : q <= 36 ? -cos48_first(q - 24) : cos48_first(48 - q);
+    q = ((q % 96) + 96) % 96;
+    return q <= 24 ? cos96_first(q) : q <= 48 ? -cos96_first(48 - q) : q <= 72 ? -cos96_first(q - 48) : cos96_first(96 - q);
 }
-__host__ __device__ constexpr double sin48(int q) { return cos48(q - 12); }
+__host__ __device__ constexpr double sin96(int q) { return cos96(q - 24); }
 
 // a * exp(SIGN j 2 pi K / P), K and P compile-time
 template <int K, int P, int SIGN, typename T> __device__ __forceinline__ cx<T> mul_root(cx<T> a)
 {
-    static_assert(48 % P == 0, "codelet radix must divide 48");
-    constexpr int q = ((K * (48 / P)) % 48 + 48) % 48;
+    static_assert(96 % P == 0, "root order must divide 96");
+    constexpr int q = ((K * (96 / P)) % 96 + 96) % 96;
     if constexpr (q == 0) return a;
-    else if constexpr (q == 24) return mk<T>(-a.x, -a.y);
-    else if constexpr (q == 12) return SIGN > 0 ? mk<T>(-a.y, a.x) : mk<T>(a.y, -a.x);
-    else if constexpr (q == 36) return SIGN > 0 ? mk<T>(a.y, -a.x) : mk<T>(-a.y, a.x);
+    else if constexpr (q == 48) return mk<T>(-a.x, -a.y);
+    else if constexpr (q == 24) return SIGN > 0 ? mk<T>(-a.y, a.x) : mk<T>(a.y, -a.x);
+    else if constexpr (q == 72) return SIGN > 0 ? mk<T>(a.y, -a.x) : mk<T>(-a.y, a.x);
     else {
-        constexpr T c = (T)cos48(q);
-        constexpr T s = (T)(SIGN * sin48(q));
+        constexpr T c = (T)cos96(q);
+        constexpr T s = (T)(SIGN * sin96(q));
         return mk<T>(a.x * c - a.y * s, a.x * s + a.y * c);
     }
 }

@@ -31,7 +31,7 @@ template <typename T, int N_, int P1_, int P2_> struct FastCfg {
     static constexpr int FS0 = P1_ * (P2_ + 1);
     static constexpr int FS = P2_ >= 8 ? FS0 : FS0 + ((P2_ - FS0 % 8) + 8) % 8; // tile pitch per transform
     static constexpr int EXW = G * FS;   // exchange elements per warp
-    static_assert(P1_ * P2_ * 2 == N_ && P1_ % P2_ == 0 && 32 % P2_ == 0 && 48 % (2 * P1_) == 0, "unsupported factorisation");
+    static_assert(P1_ * P2_ * 2 == N_ && P1_ % P2_ == 0 && 32 % P2_ == 0 && 96 % (2 * P1_) == 0, "unsupported factorisation");
     static constexpr size_t smem_bytes(int nwarps) { return sizeof(cx<T>) * ((size_t)NCOL * YP + (size_t)nwarps * EXW); }
 };
 

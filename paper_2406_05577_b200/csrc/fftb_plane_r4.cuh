@@ -1,0 +1,215 @@
+// fftb_plane_r4.cuh -- persistent inverse plane kernel for grids of 4 x 64 = 256 points per axis (sm_100a).
+//
+// The 256^3 / radius-64 problem is the paper's own workload shape ("256^3 grid ... sphere
+// diameter 128").  A z-plane of both y residues (532 KB in complex128) does not fit the schedule of
+// fftb_plane_pf.cuh, so the half-band axis is split FOUR ways instead of two: with n = 4 n' + e,
+//     out[4 n' + e] = sum_k (x[k] W^{e k}) w_64^{k n'},   W = exp(2 pi j / 256),  k in [-64, 64],
+// i.e. four length-64 transforms u_e of the input folded onto 64 slots: slot s = k mod 64 receives
+// b = x[s] and a = x[s - 64] (and slot 0 the alias c = x[+64]):
+//     u_e[s] = W^{e s} (b + (-j)^e a)  [+ (+j)^e c for s = 0].
+// e = 0 costs one addition per slot, the others one complex multiplication more: 15% more FP64 work
+// than a two-level split, but every transform is the 8 x 8 length-64 core of fftb_plane_fast.cuh and a
+// QUARTER plane (129 columns x 64 lines, 134 KB) fits in shared memory next to the TMA landing zones.
+//
+// Schedule: persistent grid, CTA c owns the planes c, c + G, ...; per plane four quarters r = 0..3:
+//     Y_r: every occupied k1 column -> u_r -> length-64 transform -> pbuf[column][y'] (y = 4 y' + r) | barrier
+//     X_r: each of the 64 lines y = 4 y' + r: 129 inputs read once, four folded transforms, 64-byte
+//          runs (x = 4 n' .. 4 n' + 3) stored as two 32-byte stores                                  | barrier
+// The stick values of a column group arrive by TMA bulk copies in a per-warp landing zone, one y task
+// ahead (cp.async.bulk + mbarrier); the row of A is read four times per plane, from L2.
+// The forward direction and the fused vloc of this pattern still run on the generic plane kernel.
+#pragma once
+#include "fftb_plane_pf.cuh"
+
+namespace fftb {
+
+constexpr int R4_MAXCOL = 129;
+struct ColTab4 {
+    int4 col[R4_MAXCOL]; // {first stick, stick count, k2lo, 0} per occupied k1 column
+    int perm[R4_MAXCOL]; // multi-stick columns first, then the single-stick ones
+};
+
+template <typename T, int NW> struct PlaneR4 {
+    using F = FastCfg<T, 128, 8, 8>;              // the length-64 core: 8 lanes x 8 values
+    static constexpr int N = 256, M = 64;
+    static constexpr int NCOL = 2 * M + 1, YP = F::YP;
+    static constexpr int PB = NCOL * YP;          // one quarter plane
+    static constexpr int ZCOL = 2 * M + 2;        // landing zone pitch per column (129 values, even)
+    static constexpr int ZONE = F::G * ZCOL;      // per warp: the G columns of its next y task
+    static constexpr int NXT = M / F::G;          // x tasks per quarter (G lines each)
+    static_assert(NXT % NW == 0, "x tasks must divide evenly over the warps");
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)PB + (size_t)NW * ZONE);
+};
+
+// u_e of one lane: slots s = t + 8 j; a = x[s - 64], b = x[s], c = x[+64] (lane 0, slot 0 only, else 0)
+template <int E, int J, typename T>
+__device__ __forceinline__ void r4_fold_inv(const cx<T> (&a)[8], const cx<T> (&b)[8], cx<T> c, cx<T> (&u)[8], cx<T> wte)
+{
+    if constexpr (J < 8) {
+        cx<T> v = cadd(b[J], mul_root<(32 - 8 * E) % 32, 32, +1, T>(a[J])); // (-j)^E a
+        if constexpr (J == 0) v = cadd(v, mul_root<(8 * E) % 32, 32, +1, T>(c)); // (+j)^E c
+        if constexpr (E > 0) v = mul_root<(E * J) % 32, 32, +1, T>(cmul(v, wte)); // W^{E (t + 8 J)}
+        u[J] = v;
+        r4_fold_inv<E, J + 1, T>(a, b, c, u, wte);
+    }
+}
+
+template <typename T, int NW>
+__global__ void __launch_bounds__(NW * 32, 1)
+plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab4 ct, const cx<T> *__restrict__ Ain,
+               cx<T> *__restrict__ cub_out, long long a_in_stride, int nplanes)
+{
+    using C = cx<T>;
+    using R4 = PlaneR4<T, NW>;
+    using F = typename R4::F;
+    constexpr int N = R4::N, M = R4::M, P2 = F::P2, G = F::G, YP = R4::YP, ZCOL = R4::ZCOL;
+    constexpr int XT = R4::NXT / NW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *pbuf = reinterpret_cast<C *>(smem_raw); // [NCOL][YP]: column c = k1 - k1lo, line y' of the current quarter
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    C *zone = pbuf + R4::PB + warp * R4::ZONE;  // landing zone of this warp's next y task
+    __shared__ __align__(8) unsigned long long bar_zone[NW];
+    unsigned zone_par = 0;
+    const C *tw = reinterpret_cast<const C *>(pl.tw1); // exp(+2 pi j i / 256)
+    C tws[8];
+#pragma unroll
+    for (int m = 1; m < 8; ++m) tws[m] = tw[(4 * t * m) & (N - 1)]; // w_64^{t m}
+    tws[0] = mk<T>((T)1, (T)0);
+    C wt[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) wt[e] = tw[e * t]; // W^{e t}
+    const int nx = pl.nxocc, k1lo = pl.k1lo;
+    const int n_one = nx - pl.n_multi;
+    const int ntask_y = (pl.n_multi + G - 1) / G;
+    const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    const int ytasks_w = ntask_y > warp ? (ntask_y - warp + NW - 1) / NW : 0; // y tasks of this warp per quarter
+
+    struct YCol { bool act; int col; int4 co; };
+    auto ycol = [&](int task) -> YCol {
+        YCol c;
+        const int ci = task * G + f;
+        c.act = ci < pl.n_multi;
+        c.col = ct.perm[c.act ? ci : 0];
+        c.co = ct.col[c.col];
+        return c;
+    };
+    // TMA: the stick runs of the G columns of y task `task` of plane (b, z) -> this warp's landing zone
+    auto zone_issue = [&](int b, int z, int task) {
+        const C *row = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
+        int bytes = 0;
+        int4 co = make_int4(0, 0, 0, 0);
+        if (lane < G) {
+            const int ci = task * G + lane;
+            if (ci < pl.n_multi) {
+                co = ct.col[ct.perm[ci]];
+                bytes = co.y * (int)sizeof(C);
+            }
+        }
+        int total = bytes;
+#pragma unroll
+        for (int sft = 1; sft < G; sft <<= 1) total += __shfl_xor_sync(0xffffffffu, total, sft);
+        if (lane == 0) mbar_expect_tx(&bar_zone[warp], (unsigned)total);
+        __syncwarp();
+        if (bytes > 0) bulk_load(zone + lane * ZCOL, row + co.x, (unsigned)bytes, &bar_zone[warp]);
+    };
+
+    if (tid == 0) {
+        for (int w = 0; w < NW; ++w) mbar_init(&bar_zone[w], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;
+    const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;
+    if (kplanes > 0 && ytasks_w > 0) zone_issue(b, z, warp);
+
+#pragma unroll 1
+    for (int i = 0; i < kplanes; ++i) {
+        const int zc = z + dz, zn = zc >= pl.n3 ? zc - pl.n3 : zc, bn = b + db + (zc >= pl.n3 ? 1 : 0); // next plane
+        const bool more = i + 1 < kplanes;
+        const C *row = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
+        auto quarter = [&](auto rc) {
+            constexpr int R = decltype(rc)::value;
+            // ================================================== Y_R: columns -> pbuf (lines y = 4 y' + R)
+            C sv = czero<T>(); // single-stick column of this warp: its value, loaded while the y tasks run
+            int4 sco = make_int4(0, 0, 0, 0);
+            int scol = 0;
+            if (warp < n_one) {
+                scol = ct.perm[pl.n_multi + warp];
+                sco = ct.col[scol];
+                sv = __ldcg(row + sco.x);
+            }
+#pragma unroll 1
+            for (int k = 0; k < ytasks_w; ++k) {
+                const int task = warp + k * NW;
+                const YCol c = ycol(task);
+                mbar_wait(&bar_zone[warp], zone_par);
+                zone_par ^= 1u;
+                const C *src = zone + f * ZCOL;
+                C a[8], bq[8], u[8], y[1][8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
+                    a[j] = (c.act && (unsigned)ia < (unsigned)c.co.y) ? src[ia] : czero<T>();
+                    bq[j] = (c.act && (unsigned)ib < (unsigned)c.co.y) ? src[ib] : czero<T>();
+                }
+                const int ic = M - c.co.z;
+                const C cv = (c.act && t == 0 && (unsigned)ic < (unsigned)c.co.y) ? src[ic] : czero<T>();
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp(); // every lane has its values: the landing zone may be refilled
+                // next y task of this warp: same quarter, next quarter (same row again), or the next plane
+                if (k + 1 < ytasks_w) zone_issue(b, z, task + NW);
+                else if (R < 3) zone_issue(b, z, warp);
+                else if (more) zone_issue(bn, zn, warp);
+                r4_fold_inv<R, 0, T>(a, bq, cv, u, wt[R]);
+                C *pc = pbuf + c.col * YP;
+                sub_inv<F, T>(u, y, tws, ExSkew<T, P2, 1>{pc, c.act}, t); // exchanged in place in the column
+                __syncwarp();
+                if (c.act) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) pc[t + 8 * q] = y[0][q];
+                }
+            }
+            if (warp < n_one) // closed form x W^{k2 y}
+                for (int yl = lane; yl < M; yl += 32) pbuf[scol * YP + yl] = cmul(sv, tw[(sco.z * (4 * yl + R)) & (N - 1)]);
+            __syncthreads();
+            // ================================================== X_R: 64 lines y = 4 y' + R -> cuboid
+#pragma unroll 1
+            for (int v = 0; v < XT; ++v) {
+                const int yl = (warp + v * NW) * G + f;
+                C a[8], bq[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int ca = (t + 8 * j) - M - k1lo, cb = (t + 8 * j) - k1lo;
+                    a[j] = (unsigned)ca < (unsigned)nx ? pbuf[ca * YP + yl] : czero<T>();
+                    bq[j] = (unsigned)cb < (unsigned)nx ? pbuf[cb * YP + yl] : czero<T>();
+                }
+                const int cc = M - k1lo;
+                const C cv = (t == 0 && (unsigned)cc < (unsigned)nx) ? pbuf[cc * YP + yl] : czero<T>();
+                C *rowo = cub_out + (((long long)b * pl.n3 + z) * N + (4 * yl + R)) * N;
+                const ExSkew<T, P2, YP> ex{pbuf + yl, true}; // the line's slots are dead: exchanged in them
+                C u[8], o0[1][8], o1[1][8];
+                r4_fold_inv<0, 0, T>(a, bq, cv, u, wt[0]);
+                sub_inv<F, T>(u, o0, tws, ex, t);
+                r4_fold_inv<1, 0, T>(a, bq, cv, u, wt[1]);
+                sub_inv<F, T>(u, o1, tws, ex, t);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) st_pair(rowo + 4 * (t + 8 * q), o0[0][q], o1[0][q]);
+                r4_fold_inv<2, 0, T>(a, bq, cv, u, wt[2]);
+                sub_inv<F, T>(u, o0, tws, ex, t);
+                r4_fold_inv<3, 0, T>(a, bq, cv, u, wt[3]);
+                sub_inv<F, T>(u, o1, tws, ex, t);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) st_pair(rowo + 4 * (t + 8 * q) + 2, o0[0][q], o1[0][q]);
+            }
+            __syncthreads();
+        };
+        quarter(std::integral_constant<int, 0>{});
+        quarter(std::integral_constant<int, 1>{});
+        quarter(std::integral_constant<int, 2>{});
+        quarter(std::integral_constant<int, 3>{});
+        z = zn; b = bn;
+    }
+}
+
+} // namespace fftb
