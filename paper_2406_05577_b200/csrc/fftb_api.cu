@@ -214,9 +214,31 @@ template <typename T, int N, int P1, int P2> ZLaunch make_z_fast()
     using F = FastCfg<T, N, P1, P2>;
     return ZLaunch{&launch_zfast_inv<T, F>, &launch_zfast_fwd<T, F>};
 }
+// z passes of the 256 pattern (fftb_plane_r4.cuh)
+constexpr int R4Z_NW = 4;
+template <typename T> int launch_zr4_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
+{
+    auto k = zpass_r4_inv_k<T, R4Z_NW>;
+    const size_t smem = ZR4<T, R4Z_NW>::smem_bytes;
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    dim3 grid((pl.nsticks + ZR4<T, R4Z_NW>::TS - 1) / ZR4<T, R4Z_NW>::TS, nb);
+    k<<<grid, R4Z_NW * 32, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
+{
+    auto k = zpass_r4_fwd_k<T, R4Z_NW>;
+    const size_t smem = ZR4<T, R4Z_NW>::smem_bytes;
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    dim3 grid((pl.nsticks + ZR4<T, R4Z_NW>::TS - 1) / ZR4<T, R4Z_NW>::TS, nb);
+    k<<<grid, R4Z_NW * 32, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+
 bool find_z_fast(int dtype, int n, bool dense, ZLaunch *out)
 {
     if (dense) return false;
+    if (dtype == FFTB_C128 && n == 256) { *out = ZLaunch{&launch_zr4_inv<double>, &launch_zr4_fwd<double>}; return true; }
     if (dtype == FFTB_C128 && n == 128) { *out = make_z_fast<double, 128, 8, 8>(); return true; }
 #ifndef FFTB_DEV
     if (dtype == FFTB_C128 && n == 64) { *out = make_z_fast<double, 64, 8, 4>(); return true; }

@@ -212,4 +212,179 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     }
 }
 
+// adjoint of r4_fold_inv: accumulate F[k] = sum_e conj(W^{e k}) G_e[k mod 64] for k = s - 64 (fa), s (fb), +64 (fc)
+template <int E, int J, typename T>
+__device__ __forceinline__ void r4_fold_fwd(const cx<T> (&gq)[8], cx<T> (&fa)[8], cx<T> (&fb)[8], cx<T> &fc, cx<T> wte)
+{
+    if constexpr (J < 8) {
+        cx<T> h = gq[J];
+        if constexpr (E > 0) h = cmulc(mul_root<(E * J) % 32, 32, -1, T>(h), wte); // conj(W^{E (t + 8 J)}) G
+        if constexpr (E == 0) {
+            fa[J] = h;
+            fb[J] = h;
+            if constexpr (J == 0) fc = h;
+        } else {
+            fb[J] = cadd(fb[J], h);
+            fa[J] = cadd(fa[J], mul_root<(8 * E) % 32, 32, +1, T>(h));            // conj((-j)^E) = (+j)^E
+            if constexpr (J == 0) fc = cadd(fc, mul_root<(32 - 8 * E) % 32, 32, +1, T>(h)); // conj((+j)^E)
+        }
+        r4_fold_fwd<E, J + 1, T>(gq, fa, fb, fc, wte);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// z passes of the 256 pattern: one group of 8 lanes per stick, TS = 4 NW sticks per CTA, the same
+// tile transposition as the z-pass kernels of fftb_plane_fast.cuh (element (z, sl) in column
+// (sl + z/4) mod TS: the strided accesses z = 4 n' + e of the transforms are conflict-free).
+//   grid = (ceil(n_sticks / TS), bands)
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NW> struct ZR4 {
+    using F = FastCfg<T, 128, 8, 8>;
+    static constexpr int N = 256, M = 64, TS = F::G * NW;
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)N * TS + (size_t)NW * F::EXW);
+    __device__ static __forceinline__ int swz(int z, int sl) { return z * TS + ((sl + (z >> 2)) & (TS - 1)); }
+};
+
+template <typename T, int NW>
+__global__ void __launch_bounds__(NW * 32, 2)
+zpass_r4_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride)
+{
+    using C = cx<T>;
+    using Z = ZR4<T, NW>;
+    using F = typename Z::F;
+    constexpr int N = Z::N, M = Z::M, P2 = F::P2, G = F::G, TS = Z::TS, NT = NW * 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *tile = reinterpret_cast<C *>(smem_raw); // [N][TS], swizzled
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    const ExTile<T, P2> ex{tile + N * TS + warp * F::EXW + f * F::FS};
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    const int s0 = blockIdx.x * TS, sl = warp * G + f, s = s0 + sl;
+    const bool act = s < pl.nsticks;
+    const int4 st = pl.stick[act ? s : 0]; // {off, k3lo, len, .}
+    const C *src = packed + (long long)blockIdx.y * pl.S + st.x;
+    C a[8], bq[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const int ia = (t + 8 * j) - M - st.y, ib = (t + 8 * j) - st.y;
+        a[j] = (act && (unsigned)ia < (unsigned)st.z) ? __ldcs(src + ia) : czero<T>();
+        bq[j] = (act && (unsigned)ib < (unsigned)st.z) ? __ldcs(src + ib) : czero<T>();
+    }
+    const int ic = M - st.y;
+    const C cv = (act && t == 0 && (unsigned)ic < (unsigned)st.z) ? __ldcs(src + ic) : czero<T>();
+    C tws[8], wt[4];
+#pragma unroll
+    for (int m = 1; m < 8; ++m) tws[m] = tw[(4 * t * m) & (N - 1)];
+    tws[0] = mk<T>((T)1, (T)0);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
+    C u[8], y[1][8];
+    r4_fold_inv<0, 0, T>(a, bq, cv, u, wt[0]);
+    sub_inv<F, T>(u, y, tws, ex, t);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) tile[Z::swz(4 * (t + 8 * q), sl)] = y[0][q];
+    r4_fold_inv<1, 0, T>(a, bq, cv, u, wt[1]);
+    sub_inv<F, T>(u, y, tws, ex, t);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) tile[Z::swz(4 * (t + 8 * q) + 1, sl)] = y[0][q];
+    r4_fold_inv<2, 0, T>(a, bq, cv, u, wt[2]);
+    sub_inv<F, T>(u, y, tws, ex, t);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) tile[Z::swz(4 * (t + 8 * q) + 2, sl)] = y[0][q];
+    r4_fold_inv<3, 0, T>(a, bq, cv, u, wt[3]);
+    sub_inv<F, T>(u, y, tws, ex, t);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) tile[Z::swz(4 * (t + 8 * q) + 3, sl)] = y[0][q];
+    __syncthreads();
+    C *dst = A + (long long)blockIdx.y * a_band_stride + s0;
+#pragma unroll 4
+    for (int i = tid; i < N * TS; i += NT) {
+        const int z = i / TS, c = i % TS;
+        const int l = (c - (z >> 2)) & (TS - 1);
+        if (s0 + l < pl.nsticks) dst[(long long)z * pl.pitch + l] = tile[i];
+    }
+}
+
+template <typename T, int NW>
+__global__ void __launch_bounds__(NW * 32, 2)
+zpass_r4_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride)
+{
+    using C = cx<T>;
+    using Z = ZR4<T, NW>;
+    using F = typename Z::F;
+    constexpr int N = Z::N, M = Z::M, P2 = F::P2, G = F::G, TS = Z::TS, NT = NW * 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *tile = reinterpret_cast<C *>(smem_raw);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    const ExTile<T, P2> ex{tile + N * TS + warp * F::EXW + f * F::FS};
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    const int s0 = blockIdx.x * TS, sl = warp * G + f, s = s0 + sl;
+    const bool act = s < pl.nsticks;
+    // ---- A[z][s0 .. s0+TS) -> tile, summing the ry partial planes of the forward plane kernel
+    {
+        const C *src = A + (long long)blockIdx.y * a_band_stride + s0;
+        const long long rstride = (long long)pl.n3 * pl.pitch;
+        constexpr int U = 8;
+        static_assert((N * TS) % (NT * U) == 0, "tile copy is unrolled by U");
+        for (int i0 = tid; i0 < N * TS; i0 += NT * U) {
+            C v[U];
+#pragma unroll
+            for (int uu = 0; uu < U; ++uu) {
+                const int i = i0 + uu * NT, z = i / TS, l = i % TS;
+                v[uu] = (s0 + l < pl.nsticks) ? __ldcg(src + (long long)z * pl.pitch + l) : czero<T>();
+            }
+            for (int p = 1; p < pl.ry; ++p) {
+#pragma unroll
+                for (int uu = 0; uu < U; ++uu) {
+                    const int i = i0 + uu * NT, z = i / TS, l = i % TS;
+                    if (s0 + l < pl.nsticks) v[uu] = cadd(v[uu], __ldcg(src + p * rstride + (long long)z * pl.pitch + l));
+                }
+            }
+#pragma unroll
+            for (int uu = 0; uu < U; ++uu) {
+                const int i = i0 + uu * NT, z = i / TS, l = i % TS;
+                tile[Z::swz(z, l)] = v[uu];
+            }
+        }
+    }
+    C tws[8], wt[4];
+#pragma unroll
+    for (int m = 1; m < 8; ++m) tws[m] = tw[(4 * t * m) & (N - 1)];
+    tws[0] = mk<T>((T)1, (T)0);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
+    const int4 st = pl.stick[act ? s : 0];
+    C *dst = packed + (long long)blockIdx.y * pl.S + st.x;
+    const T scale = (T)pl.scale;
+    __syncthreads();
+    C y[1][8], gq[8], fa[8], fb[8], fc;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) y[0][q] = tile[Z::swz(4 * (t + 8 * q), sl)];
+    sub_fwd<F, T>(y, gq, tws, ex, t);
+    r4_fold_fwd<0, 0, T>(gq, fa, fb, fc, wt[0]);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) y[0][q] = tile[Z::swz(4 * (t + 8 * q) + 1, sl)];
+    sub_fwd<F, T>(y, gq, tws, ex, t);
+    r4_fold_fwd<1, 0, T>(gq, fa, fb, fc, wt[1]);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) y[0][q] = tile[Z::swz(4 * (t + 8 * q) + 2, sl)];
+    sub_fwd<F, T>(y, gq, tws, ex, t);
+    r4_fold_fwd<2, 0, T>(gq, fa, fb, fc, wt[2]);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) y[0][q] = tile[Z::swz(4 * (t + 8 * q) + 3, sl)];
+    sub_fwd<F, T>(y, gq, tws, ex, t);
+    r4_fold_fwd<3, 0, T>(gq, fa, fb, fc, wt[3]);
+    if (act) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int ia = (t + 8 * j) - M - st.y, ib = (t + 8 * j) - st.y;
+            if ((unsigned)ia < (unsigned)st.z) dst[ia] = mk<T>(fa[j].x * scale, fa[j].y * scale);
+            if ((unsigned)ib < (unsigned)st.z) dst[ib] = mk<T>(fb[j].x * scale, fb[j].y * scale);
+        }
+        const int ic = M - st.y;
+        if (t == 0 && (unsigned)ic < (unsigned)st.z) dst[ic] = mk<T>(fc.x * scale, fc.y * scale);
+    }
+}
+
 } // namespace fftb
