@@ -432,7 +432,10 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         PlaneLaunch fast;
         if (!(gen && gen[0] == '1') && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) { plk = fast; fast_plane = true; }
         // 256 pattern, complex128: the inverse plane pass has its own persistent kernel (four-way split)
-        if (!(gen && gen[0] == '1') && !dense && desc->dtype == FFTB_C128 && desc->n[0] == 256) plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
+        if (!(gen && gen[0] == '1') && !dense && desc->dtype == FFTB_C128 && desc->n[0] == 256) {
+            plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
+            fast_plane = true; // persistent kernel: whole-batch launches (256 planes per band on 148 CTAs would waste half a wave)
+        }
         const char *genz = getenv("FFTB_GENERIC_Z");
         ZLaunch zfast;
         if (!(genz && genz[0] == '1') && find_z_fast(desc->dtype, desc->n[2], dense, &zfast)) zl = zfast;
