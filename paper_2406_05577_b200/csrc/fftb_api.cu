@@ -177,6 +177,25 @@ int launch_plane_r4_inv(const DevPlan &pl, const PlanTabs &tabs, const void *Ain
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 
+template <typename T>
+int launch_plane_r4_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *, void *Aout, const void *cin, void *, const void *, long long,
+                        long long sout, int nb, cudaStream_t st)
+{
+    constexpr int NW = 8;
+    auto k = plane_r4_fwd_k<T, NW>;
+    const size_t smem = sizeof(cx<T>) * (size_t)PlaneR4<T, NW>::PB;
+    static bool ready = false;
+    if (!ready) {
+        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+        ready = true;
+    }
+    const int nplanes = pl.n3 * nb;
+    int grid = sm_count();
+    if (grid > nplanes) grid = nplanes;
+    k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)cin, (cx<T> *)Aout, sout, nplanes);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+
 bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)
 {
     if (dense) return false;
@@ -434,6 +453,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         // 256 pattern, complex128: the inverse plane pass has its own persistent kernel (four-way split)
         if (!(gen && gen[0] == '1') && !dense && desc->dtype == FFTB_C128 && desc->n[0] == 256) {
             plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
+            plk.run[MODE_FWD] = &launch_plane_r4_fwd<double>; // writes the generic kernel's four partial planes (plk.ry = 4)
             fast_plane = true; // persistent kernel: whole-batch launches (256 planes per band on 148 CTAs would waste half a wave)
         }
         const char *genz = getenv("FFTB_GENERIC_Z");

@@ -17,7 +17,8 @@
 //          runs (x = 4 n' .. 4 n' + 3) stored as two 32-byte stores                                  | barrier
 // The stick values of a column group arrive by TMA bulk copies in a per-warp landing zone, one y task
 // ahead (cp.async.bulk + mbarrier); the row of A is read four times per plane, from L2.
-// The forward direction and the fused vloc of this pattern still run on the generic plane kernel.
+// The forward kernel (plane_r4_fwd_k below) is the adjoint chain; the fused vloc of this pattern still
+// runs on the generic plane kernel.
 #pragma once
 #include "fftb_plane_pf.cuh"
 
@@ -229,6 +230,144 @@ __device__ __forceinline__ void r4_fold_fwd(const cx<T> (&gq)[8], cx<T> (&fa)[8]
             if constexpr (J == 0) fc = cadd(fc, mul_root<(32 - 8 * E) % 32, 32, +1, T>(h)); // conj((+j)^E)
         }
         r4_fold_fwd<E, J + 1, T>(gq, fa, fb, fc, wte);
+    }
+}
+
+// the part of residue R of F[k] (one partial plane per y residue, summed by the forward z pass):
+// conj(W^{R k}) G_R[k mod 64] for k = s - 64 (pa), s (pb), +64 (pc)
+template <int R, int J, typename T>
+__device__ __forceinline__ void r4_part_fwd(const cx<T> (&gq)[8], cx<T> (&pa)[8], cx<T> (&pb)[8], cx<T> &pc, cx<T> wte)
+{
+    if constexpr (J < 8) {
+        cx<T> h = gq[J];
+        if constexpr (R > 0) h = cmulc(mul_root<(R * J) % 32, 32, -1, T>(h), wte);
+        pb[J] = h;
+        pa[J] = mul_root<(8 * R) % 32, 32, +1, T>(h);
+        if constexpr (J == 0) pc = mul_root<(32 - 8 * R) % 32, 32, +1, T>(h);
+        r4_part_fwd<R, J + 1, T>(gq, pa, pb, pc, wte);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// forward plane kernel of the 256 pattern: the adjoint chain, quarter by quarter.
+//     X_r: each of the 64 lines y = 4 y' + r: (x, x+1) pairs loaded in two batches (e = 0,1 and e = 2,3),
+//          four length-64 transforms, F[k1] accumulated over e -> the occupied k1 columns of pbuf    | barrier
+//     Y_r: every column: length-64 transform over y', the part of residue r of F[k2] -> partial plane
+//          A[b][r][z][.] (the layout of the generic plane kernel: the z pass sums the four planes)  | barrier
+// The quarter-plane buffer leaves no room for a TMA landing zone of G = 4 lines of 4 KB per warp, so
+// the cuboid lines are loaded straight into registers here.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NW>
+__global__ void __launch_bounds__(NW * 32, 1)
+plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab4 ct, const cx<T> *__restrict__ cub_in,
+               cx<T> *__restrict__ Aout, long long a_out_stride, int nplanes)
+{
+    using C = cx<T>;
+    using R4 = PlaneR4<T, NW>;
+    using F = typename R4::F;
+    constexpr int N = R4::N, M = R4::M, P2 = F::P2, G = F::G, YP = R4::YP;
+    constexpr int XT = R4::NXT / NW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *pbuf = reinterpret_cast<C *>(smem_raw);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    const C *tw = reinterpret_cast<const C *>(pl.tw1);
+    C tws[8];
+#pragma unroll
+    for (int m = 1; m < 8; ++m) tws[m] = tw[(4 * t * m) & (N - 1)];
+    tws[0] = mk<T>((T)1, (T)0);
+    C wt[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
+    const int nx = pl.nxocc, k1lo = pl.k1lo;
+    const int n_one = nx - pl.n_multi;
+    const int ntask_y = (pl.n_multi + G - 1) / G;
+    const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;
+    const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;
+
+#pragma unroll 1
+    for (int i = 0; i < kplanes; ++i) {
+        auto quarter = [&](auto rc) {
+            constexpr int R = decltype(rc)::value;
+            // ================================================== X_R: 64 lines y = 4 y' + R -> pbuf
+#pragma unroll 1
+            for (int v = 0; v < XT; ++v) {
+                const int yl = (warp + v * NW) * G + f;
+                const C *rowi = cub_in + (((long long)b * pl.n3 + z) * N + (4 * yl + R)) * N;
+                const ExSkew<T, P2, YP> ex{pbuf + yl, true}; // the line's slots are still unused: exchanged in them
+                C o0[1][8], o1[1][8], gq[8], fa[8], fb[8], fc;
+#pragma unroll
+                for (int q = 0; q < 8; ++q) ld_pair(rowi + 4 * (t + 8 * q), o0[0][q], o1[0][q]);
+                sub_fwd<F, T>(o0, gq, tws, ex, t);
+                r4_fold_fwd<0, 0, T>(gq, fa, fb, fc, wt[0]);
+                sub_fwd<F, T>(o1, gq, tws, ex, t);
+                r4_fold_fwd<1, 0, T>(gq, fa, fb, fc, wt[1]);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) ld_pair(rowi + 4 * (t + 8 * q) + 2, o0[0][q], o1[0][q]);
+                sub_fwd<F, T>(o0, gq, tws, ex, t);
+                r4_fold_fwd<2, 0, T>(gq, fa, fb, fc, wt[2]);
+                sub_fwd<F, T>(o1, gq, tws, ex, t);
+                r4_fold_fwd<3, 0, T>(gq, fa, fb, fc, wt[3]);
+                __syncwarp(); // the last exchange has been read by every lane: the slots take the results
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int ca = (t + 8 * j) - M - k1lo, cb = (t + 8 * j) - k1lo;
+                    if ((unsigned)ca < (unsigned)nx) pbuf[ca * YP + yl] = fa[j];
+                    if ((unsigned)cb < (unsigned)nx) pbuf[cb * YP + yl] = fb[j];
+                }
+                const int cc = M - k1lo;
+                if (t == 0 && (unsigned)cc < (unsigned)nx) pbuf[cc * YP + yl] = fc;
+            }
+            __syncthreads();
+            // ================================================== Y_R: columns -> partial plane R of A
+            C *dst = Aout + (long long)b * a_out_stride + ((long long)R * pl.n3 + z) * pl.pitch;
+#pragma unroll 1
+            for (int task = warp; task < ntask_y; task += NW) {
+                const int ci = task * G + f;
+                const bool act = ci < pl.n_multi;
+                const int col = ct.perm[act ? ci : 0];
+                const int4 co = ct.col[col];
+                C *pc = pbuf + col * YP;
+                C y[1][8], gq[8], pa[8], pb[8], pcv;
+#pragma unroll
+                for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
+                sub_fwd<F, T>(y, gq, tws, ExSkew<T, P2, 1>{pc, act}, t); // exchanged in place in the column
+                r4_part_fwd<R, 0, T>(gq, pa, pb, pcv, wt[R]);
+                if (act) {
+                    C *d = dst + co.x;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
+                        if ((unsigned)ia < (unsigned)co.y) d[ia] = pa[j];
+                        if ((unsigned)ib < (unsigned)co.y) d[ib] = pb[j];
+                    }
+                    const int ic = M - co.z;
+                    if (t == 0 && (unsigned)ic < (unsigned)co.y) d[ic] = pcv;
+                }
+            }
+            // single-stick columns: one warp per column, dot product with conj(W^{k2 y}) over the quarter's lines
+            for (int k = warp; k < n_one; k += NW) {
+                const int col = ct.perm[pl.n_multi + k];
+                const int4 co = ct.col[col];
+                C acc = czero<T>();
+                for (int yl = lane; yl < M; yl += 32) acc = cadd(acc, cmulc(pbuf[col * YP + yl], tw[(co.z * (4 * yl + R)) & (N - 1)]));
+#pragma unroll
+                for (int sft = 16; sft > 0; sft >>= 1) {
+                    acc.x += __shfl_xor_sync(0xffffffffu, acc.x, sft);
+                    acc.y += __shfl_xor_sync(0xffffffffu, acc.y, sft);
+                }
+                if (lane == 0) dst[co.x] = acc;
+            }
+            __syncthreads();
+        };
+        quarter(std::integral_constant<int, 0>{});
+        quarter(std::integral_constant<int, 1>{});
+        quarter(std::integral_constant<int, 2>{});
+        quarter(std::integral_constant<int, 3>{});
+        const int zc = z + dz;
+        b += db + (zc >= pl.n3 ? 1 : 0);
+        z = zc >= pl.n3 ? zc - pl.n3 : zc;
     }
 }
 
