@@ -52,6 +52,7 @@ SMALL = [
     _small((192, 192, 32), (48, 40, 8), dtype="c128", batch=1),
     _small((256, 256, 256), (64, 64, 64), batch=1, number=5),
     _small((256, 256, 32), (64, 64, 8), dtype="c64", batch=2),
+    _small((256, 256, 64), (40, 50, 16), dtype="c128", batch=2),   # four-way split kernels, partly filled columns
 ]
 IDS = [f"{w.n[0]}x{w.n[1]}x{w.n[2]}-a{w.cutoff[0]}.{w.cutoff[1]}.{w.cutoff[2]}-{w.dtype}" for w in SMALL]
 
@@ -90,8 +91,8 @@ def test_inverse_forward_vs_oracle(fb, oracle, w):
     p.destroy()
 
 
-@pytest.mark.parametrize("w", [SMALL[0], SMALL[2], SMALL[3], SMALL[5], SMALL[8], SMALL[10], SMALL[13]],
-                         ids=[IDS[i] for i in (0, 2, 3, 5, 8, 10, 13)])
+@pytest.mark.parametrize("w", [SMALL[0], SMALL[2], SMALL[3], SMALL[5], SMALL[8], SMALL[10], SMALL[13], SMALL[14]],
+                         ids=[IDS[i] for i in (0, 2, 3, 5, 8, 10, 13, 14)])
 def test_apply_vloc_vs_oracle(fb, oracle, w):
     p = _plan(fb, w, w.batch)
     k = p.points()
