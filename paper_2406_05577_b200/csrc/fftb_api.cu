@@ -354,7 +354,9 @@ struct fftb_plan_s {
     PlaneLaunch plk;
     // device block layout
     size_t o_stick, o_col, o_perm, o_tw[3], o_ws, o_stage, bytes_min, bytes_stage;
-    long long a_inv_stride, a_fwd_stride; // elements per band of the intermediate
+    long long a_inv_stride, a_fwd_stride; // elements per band of the intermediate (a_fwd_stride: vloc and generic forward)
+    int ry_fwd;                           // partial A planes written by fftb_forward's plane kernel (1: it accumulates itself)
+    long long a_fwd1_stride;              // elements per band of the forward intermediate of fftb_forward
     int chunk;                            // bands per kernel group (vloc: both intermediates live)
     int chunk_inv, chunk_fwd;             // inverse / forward alone
     // bound state
@@ -444,7 +446,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
     if (desc->n[0] != desc->n[1]) return FFTB_EUNSUPPORTED;
     ZLaunch zl;
     PlaneLaunch plk;
-    bool fast_plane = false;
+    bool fast_plane = false, fwd_accumulates = false;
     if (!find_z(desc->dtype, desc->n[2], dense, &zl) || !find_plane(desc->dtype, desc->n[0], dense, &plk)) return FFTB_EUNSUPPORTED;
     {
         const char *gen = getenv("FFTB_GENERIC_PLANE"); // debugging aid: keep the generic plane kernel
@@ -453,7 +455,8 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         // 256 pattern, complex128: the inverse plane pass has its own persistent kernel (four-way split)
         if (!(gen && gen[0] == '1') && !dense && desc->dtype == FFTB_C128 && desc->n[0] == 256) {
             plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
-            plk.run[MODE_FWD] = &launch_plane_r4_fwd<double>; // writes the generic kernel's four partial planes (plk.ry = 4)
+            plk.run[MODE_FWD] = &launch_plane_r4_fwd<double>; // accumulates the four y residues into ONE plane of A
+            fwd_accumulates = true;                           // (the generic vloc kernel of this plan still writes plk.ry = 4)
             fast_plane = true; // persistent kernel: whole-batch launches (256 planes per band on 148 CTAs would waste half a wave)
         }
         const char *genz = getenv("FFTB_GENERIC_Z");
@@ -580,6 +583,8 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         // -> 3.9 ms per step), so their budget covers the whole batch whenever 4 GiB allow it.
         p->a_inv_stride = (long long)n3 * p->pitch;
         p->a_fwd_stride = (long long)p->ry * n3 * p->pitch;
+        p->ry_fwd = fwd_accumulates ? 1 : p->ry;
+        p->a_fwd1_stride = (long long)p->ry_fwd * n3 * p->pitch;
         const size_t per_band = (size_t)(p->a_inv_stride + p->a_fwd_stride) * p->elem; // vloc needs both
         size_t budget = fast_plane ? (size_t)4 << 30 : (size_t)48 << 20;
         if (const char *e = getenv("FFTB_WS_MB")) { long v = atol(e); if (v > 0) budget = (size_t)v << 20; }
@@ -591,7 +596,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         };
         p->chunk = chunk_of(per_band);
         p->chunk_inv = chunk_of((size_t)p->a_inv_stride * p->elem);
-        p->chunk_fwd = chunk_of((size_t)p->a_fwd_stride * p->elem);
+        p->chunk_fwd = chunk_of((size_t)p->a_fwd1_stride * p->elem);
         size_t o = 0;
         p->o_stick = o; o = align_up(o + sizeof(int4) * p->h_stick.size(), 256);
         p->o_col = o; o = align_up(o + sizeof(int4) * p->h_col.size(), 256);
@@ -745,10 +750,12 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
         unsigned char *pk = (unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
         const unsigned char *cb = (const unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
         prof_begin(p, K_PLANE_FWD, st);
-        rc = p->plk.run[MODE_FWD](p->dev, p->tabs, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd_stride, nc, st);
+        DevPlan dv = p->dev;
+        dv.ry = p->ry_fwd;
+        rc = p->plk.run[MODE_FWD](dv, p->tabs, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd1_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_ZFWD, st);
-        if (!rc) rc = p->zl.fwd(p->dev, A, pk, p->a_fwd_stride, nc, st);
+        if (!rc) rc = p->zl.fwd(dv, A, pk, p->a_fwd1_stride, nc, st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
         p->launches += 2;

@@ -233,7 +233,7 @@ __device__ __forceinline__ void r4_fold_fwd(const cx<T> (&gq)[8], cx<T> (&fa)[8]
     }
 }
 
-// the part of residue R of F[k] (one partial plane per y residue, summed by the forward z pass):
+// the part of residue R of F[k] (added into the one plane of A by plane_r4_fwd_k):
 // conj(W^{R k}) G_R[k mod 64] for k = s - 64 (pa), s (pb), +64 (pc)
 template <int R, int J, typename T>
 __device__ __forceinline__ void r4_part_fwd(const cx<T> (&gq)[8], cx<T> (&pa)[8], cx<T> (&pb)[8], cx<T> &pc, cx<T> wte)
@@ -252,8 +252,8 @@ __device__ __forceinline__ void r4_part_fwd(const cx<T> (&gq)[8], cx<T> (&pa)[8]
 // forward plane kernel of the 256 pattern: the adjoint chain, quarter by quarter.
 //     X_r: each of the 64 lines y = 4 y' + r: (x, x+1) pairs loaded in two batches (e = 0,1 and e = 2,3),
 //          four length-64 transforms, F[k1] accumulated over e -> the occupied k1 columns of pbuf    | barrier
-//     Y_r: every column: length-64 transform over y', the part of residue r of F[k2] -> partial plane
-//          A[b][r][z][.] (the layout of the generic plane kernel: the z pass sums the four planes)  | barrier
+//     Y_r: every column: length-64 transform over y', the part of residue r of F[k2] is ADDED to the one
+//          plane A[b][z][.] (r = 0 stores; the same lane wrote the same addresses one quarter earlier)  | barrier
 // The quarter-plane buffer leaves no room for a TMA landing zone of G = 4 lines of 4 KB per warp, so
 // the cuboid lines are loaded straight into registers here.
 // ---------------------------------------------------------------------------------------------
@@ -321,7 +321,9 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             }
             __syncthreads();
             // ================================================== Y_R: columns -> partial plane R of A
-            C *dst = Aout + (long long)b * a_out_stride + ((long long)R * pl.n3 + z) * pl.pitch;
+            // One plane of A: residue 0 stores, residues 1..3 add to what the SAME lane stored one quarter ago
+            // (still in L2; the loads are issued before the transform whose result they are added to).
+            C *dst = Aout + (long long)b * a_out_stride + (long long)z * pl.pitch;
 #pragma unroll 1
             for (int task = warp; task < ntask_y; task += NW) {
                 const int ci = task * G + f;
@@ -329,21 +331,31 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
                 const int col = ct.perm[act ? ci : 0];
                 const int4 co = ct.col[col];
                 C *pc = pbuf + col * YP;
-                C y[1][8], gq[8], pa[8], pb[8], pcv;
+                C *d = dst + co.x;
+                const int ic = M - co.z;
+                const bool hc = act && t == 0 && (unsigned)ic < (unsigned)co.y;
+                C y[1][8], gq[8], pa[8], pb[8], pcv, oa[8], ob[8], oc = czero<T>();
+                if constexpr (R > 0) {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
+                        oa[j] = (act && (unsigned)ia < (unsigned)co.y) ? __ldcg(d + ia) : czero<T>();
+                        ob[j] = (act && (unsigned)ib < (unsigned)co.y) ? __ldcg(d + ib) : czero<T>();
+                    }
+                    if (hc) oc = __ldcg(d + ic);
+                }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
                 sub_fwd<F, T>(y, gq, tws, ExSkew<T, P2, 1>{pc, act}, t); // exchanged in place in the column
                 r4_part_fwd<R, 0, T>(gq, pa, pb, pcv, wt[R]);
                 if (act) {
-                    C *d = dst + co.x;
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
-                        if ((unsigned)ia < (unsigned)co.y) d[ia] = pa[j];
-                        if ((unsigned)ib < (unsigned)co.y) d[ib] = pb[j];
+                        if ((unsigned)ia < (unsigned)co.y) d[ia] = R > 0 ? cadd(oa[j], pa[j]) : pa[j];
+                        if ((unsigned)ib < (unsigned)co.y) d[ib] = R > 0 ? cadd(ob[j], pb[j]) : pb[j];
                     }
-                    const int ic = M - co.z;
-                    if (t == 0 && (unsigned)ic < (unsigned)co.y) d[ic] = pcv;
+                    if (hc) d[ic] = R > 0 ? cadd(oc, pcv) : pcv;
                 }
             }
             // single-stick columns: one warp per column, dot product with conj(W^{k2 y}) over the quarter's lines
@@ -357,7 +369,7 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
                     acc.x += __shfl_xor_sync(0xffffffffu, acc.x, sft);
                     acc.y += __shfl_xor_sync(0xffffffffu, acc.y, sft);
                 }
-                if (lane == 0) dst[co.x] = acc;
+                if (lane == 0) dst[co.x] = R > 0 ? cadd(__ldcg(dst + co.x), acc) : acc;
             }
             __syncthreads();
         };
