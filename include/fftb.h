@@ -87,7 +87,8 @@ typedef struct {
     int64_t min_bytes_per_band_dir; /* algorithmic bytes of one band, one direction: (S + C) * elem */
     int64_t workspace_offset; /* byte offset of the plane-major intermediate A inside the bind block */
     int64_t pitch;        /* row pitch of A in elements: A[band][z][pitch] after the inverse z pass */
-    int64_t y_residues;   /* number of partial A planes the forward plane kernel writes per band */
+    int64_t y_residues;   /* largest number of partial A planes a forward-side plane kernel of this plan writes
+                             per band (the fast kernels accumulate the y residues themselves and write one) */
     int64_t chunk_bands_fwd;  /* bands per kernel group in fftb_forward */
     int64_t chunk_bands_vloc; /* bands per kernel group in fftb_apply_vloc */
 } fftb_plan_info;
