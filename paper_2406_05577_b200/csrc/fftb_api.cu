@@ -258,6 +258,7 @@ bool find_z_fast(int dtype, int n, bool dense, ZLaunch *out)
 {
     if (dense) return false;
     if (dtype == FFTB_C128 && n == 256) { *out = ZLaunch{&launch_zr4_inv<double>, &launch_zr4_fwd<double>}; return true; }
+    if (dtype == FFTB_C64 && n == 256) { *out = ZLaunch{&launch_zr4_inv<float>, &launch_zr4_fwd<float>}; return true; }
     if (dtype == FFTB_C128 && n == 128) { *out = make_z_fast<double, 128, 8, 8>(); return true; }
 #ifndef FFTB_DEV
     if (dtype == FFTB_C128 && n == 64) { *out = make_z_fast<double, 64, 8, 4>(); return true; }
@@ -453,9 +454,15 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         PlaneLaunch fast;
         if (!(gen && gen[0] == '1') && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) { plk = fast; fast_plane = true; }
         // 256 pattern, complex128: the inverse plane pass has its own persistent kernel (four-way split)
-        if (!(gen && gen[0] == '1') && !dense && desc->dtype == FFTB_C128 && desc->n[0] == 256) {
-            plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
-            plk.run[MODE_FWD] = &launch_plane_r4_fwd<double>; // accumulates the four y residues into ONE plane of A
+        if (!(gen && gen[0] == '1') && !dense && desc->n[0] == 256) {
+            if (desc->dtype == FFTB_C128) {
+                plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
+                plk.run[MODE_FWD] = &launch_plane_r4_fwd<double>;
+            } else {
+                plk.run[MODE_INV] = &launch_plane_r4_inv<float>;
+                plk.run[MODE_FWD] = &launch_plane_r4_fwd<float>;
+            }
+            // the forward kernel accumulates the four y residues into ONE plane of A
             fwd_accumulates = true;                           // (the generic vloc kernel of this plan still writes plk.ry = 4)
             fast_plane = true; // persistent kernel: whole-batch launches (256 planes per band on 148 CTAs would waste half a wave)
         }
@@ -801,12 +808,15 @@ static int check_host(fftb_plan p, int nb)
     return FFTB_OK;
 }
 
-// Band chunks of the *_host calls: HOST_PIPE chunks when the batch is large enough to keep the persistent
-// kernels efficient, otherwise one.
+// Band chunks of the *_host calls.
 static int host_chunks(fftb_plan p, int nb)
 {
-    const int HOST_PIPE = 4;
-    return (p->pipe_ok && nb >= 8 * HOST_PIPE) ? HOST_PIPE : 1;
+    // at least 1024 z-planes per chunk keep the persistent kernels efficient; at most 4 chunks
+    if (!p->pipe_ok) return 1;
+    long long k = (long long)nb * p->desc.n[2] / 1024;
+    if (k > 4) k = 4;
+    if (k > nb) k = nb;
+    return k < 1 ? 1 : (int)k;
 }
 #define FFTB_CU(call) do { if ((call) != cudaSuccess) { p->sticky = FFTB_ECUDA; return FFTB_ECUDA; } } while (0)
 

@@ -35,7 +35,7 @@ template <typename T, int NW> struct PlaneR4 {
     static constexpr int N = 256, M = 64;
     static constexpr int NCOL = 2 * M + 1, YP = F::YP;
     static constexpr int PB = NCOL * YP;          // one quarter plane
-    static constexpr int ZCOL = 2 * M + 2;        // landing zone pitch per column (129 values, even)
+    static constexpr int ZCOL = 2 * M + 4;        // landing zone pitch per column (129 values + alignment slack, 16-byte multiple)
     static constexpr int ZONE = F::G * ZCOL;      // per warp: the G columns of its next y task
     static constexpr int NXT = M / F::G;          // x tasks per quarter (G lines each)
     static_assert(NXT % NW == 0, "x tasks must divide evenly over the warps");
@@ -104,6 +104,12 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             const int ci = task * G + lane;
             if (ci < pl.n_multi) {
                 co = ct.col[ct.perm[ci]];
+                // bulk copies move 16-byte multiples from 16-byte aligned addresses: for 8-byte elements the run is
+                // widened to even element indices (the row's pitch is even, so the widened run stays inside the row)
+                const int sh = sizeof(C) == 8 ? (co.x & 1) : 0;
+                co.x -= sh;
+                co.y += sh;
+                if (sizeof(C) == 8) co.y = (co.y + 1) & ~1;
                 bytes = co.y * (int)sizeof(C);
             }
         }
@@ -146,7 +152,7 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
                 const YCol c = ycol(task);
                 mbar_wait(&bar_zone[warp], zone_par);
                 zone_par ^= 1u;
-                const C *src = zone + f * ZCOL;
+                const C *src = zone + f * ZCOL + (sizeof(C) == 8 ? (c.co.x & 1) : 0); // see zone_issue
                 C a[8], bq[8], u[8], y[1][8];
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
