@@ -178,6 +178,25 @@ int launch_plane_r4_inv(const DevPlan &pl, const PlanTabs &tabs, const void *Ain
 }
 
 template <typename T>
+int launch_plane_r4_vloc(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *Aout, const void *, void *, const void *v, long long sin,
+                         long long sout, int nb, cudaStream_t st)
+{
+    constexpr int NW = 8;
+    auto k = plane_r4_vloc_k<T, NW>;
+    const size_t smem = PlaneR4<T, NW>::smem_bytes;
+    static bool ready = false;
+    if (!ready) {
+        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+        ready = true;
+    }
+    const int nplanes = pl.n3 * nb;
+    int grid = sm_count();
+    if (grid > nplanes) grid = nplanes;
+    k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)Ain, (cx<T> *)Aout, (const T *)v, sin, sout, nplanes);
+    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+}
+
+template <typename T>
 int launch_plane_r4_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *, void *Aout, const void *cin, void *, const void *, long long,
                         long long sout, int nb, cudaStream_t st)
 {
@@ -291,6 +310,9 @@ bool find_z(int dtype, int n, bool dense, ZLaunch *out)
 #define ZCASE(T, DT, N, D) \
     if (dtype == DT && n == N && dense == D) { *out = make_z<T, N, D>(); return true; }
     ZCASE(double, FFTB_C128, 128, false)
+#ifdef FFTB_DEV256
+    ZCASE(double, FFTB_C128, 256, false)
+#endif
 #ifndef FFTB_DEV /* development builds (-DFFTB_DEV) instantiate the 128^3 complex128 kernels only */
     ZCASE(double, FFTB_C128, 32, false) ZCASE(double, FFTB_C128, 64, false) ZCASE(double, FFTB_C128, 96, false)
     ZCASE(double, FFTB_C128, 192, false) ZCASE(double, FFTB_C128, 256, false)
@@ -307,6 +329,9 @@ bool find_plane(int dtype, int n, bool dense, PlaneLaunch *out)
 #define PCASE(T, DT, N, D) \
     if (dtype == DT && n == N && dense == D) { *out = make_plane<T, N, D>(); return true; }
     PCASE(double, FFTB_C128, 128, false)
+#ifdef FFTB_DEV256
+    PCASE(double, FFTB_C128, 256, false)
+#endif
 #ifndef FFTB_DEV
     PCASE(double, FFTB_C128, 32, false) PCASE(double, FFTB_C128, 64, false) PCASE(double, FFTB_C128, 96, false)
     PCASE(double, FFTB_C128, 192, false) PCASE(double, FFTB_C128, 256, false)
@@ -356,8 +381,6 @@ struct fftb_plan_s {
     // device block layout
     size_t o_stick, o_col, o_perm, o_tw[3], o_ws, o_stage, bytes_min, bytes_stage;
     long long a_inv_stride, a_fwd_stride; // elements per band of the intermediate (a_fwd_stride: vloc and generic forward)
-    int ry_fwd;                           // partial A planes written by fftb_forward's plane kernel (1: it accumulates itself)
-    long long a_fwd1_stride;              // elements per band of the forward intermediate of fftb_forward
     int chunk;                            // bands per kernel group (vloc: both intermediates live)
     int chunk_inv, chunk_fwd;             // inverse / forward alone
     // bound state
@@ -447,23 +470,24 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
     if (desc->n[0] != desc->n[1]) return FFTB_EUNSUPPORTED;
     ZLaunch zl;
     PlaneLaunch plk;
-    bool fast_plane = false, fwd_accumulates = false;
+    bool fast_plane = false;
     if (!find_z(desc->dtype, desc->n[2], dense, &zl) || !find_plane(desc->dtype, desc->n[0], dense, &plk)) return FFTB_EUNSUPPORTED;
     {
         const char *gen = getenv("FFTB_GENERIC_PLANE"); // debugging aid: keep the generic plane kernel
         PlaneLaunch fast;
         if (!(gen && gen[0] == '1') && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) { plk = fast; fast_plane = true; }
-        // 256 pattern, complex128: the inverse plane pass has its own persistent kernel (four-way split)
+        // 256 pattern: persistent plane kernels of their own (four-way split, fftb_plane_r4.cuh)
         if (!(gen && gen[0] == '1') && !dense && desc->n[0] == 256) {
             if (desc->dtype == FFTB_C128) {
                 plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
                 plk.run[MODE_FWD] = &launch_plane_r4_fwd<double>;
+                plk.run[MODE_VLOC] = &launch_plane_r4_vloc<double>;
             } else {
                 plk.run[MODE_INV] = &launch_plane_r4_inv<float>;
                 plk.run[MODE_FWD] = &launch_plane_r4_fwd<float>;
+                plk.run[MODE_VLOC] = &launch_plane_r4_vloc<float>;
             }
-            // the forward kernel accumulates the four y residues into ONE plane of A
-            fwd_accumulates = true;                           // (the generic vloc kernel of this plan still writes plk.ry = 4)
+            plk.ry = 1; // the forward and vloc kernels accumulate the four y residues into ONE plane of A themselves
             fast_plane = true; // persistent kernel: whole-batch launches (256 planes per band on 148 CTAs would waste half a wave)
         }
         const char *genz = getenv("FFTB_GENERIC_Z");
@@ -590,8 +614,6 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         // -> 3.9 ms per step), so their budget covers the whole batch whenever 4 GiB allow it.
         p->a_inv_stride = (long long)n3 * p->pitch;
         p->a_fwd_stride = (long long)p->ry * n3 * p->pitch;
-        p->ry_fwd = fwd_accumulates ? 1 : p->ry;
-        p->a_fwd1_stride = (long long)p->ry_fwd * n3 * p->pitch;
         const size_t per_band = (size_t)(p->a_inv_stride + p->a_fwd_stride) * p->elem; // vloc needs both
         size_t budget = fast_plane ? (size_t)4 << 30 : (size_t)48 << 20;
         if (const char *e = getenv("FFTB_WS_MB")) { long v = atol(e); if (v > 0) budget = (size_t)v << 20; }
@@ -603,7 +625,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         };
         p->chunk = chunk_of(per_band);
         p->chunk_inv = chunk_of((size_t)p->a_inv_stride * p->elem);
-        p->chunk_fwd = chunk_of((size_t)p->a_fwd1_stride * p->elem);
+        p->chunk_fwd = chunk_of((size_t)p->a_fwd_stride * p->elem);
         size_t o = 0;
         p->o_stick = o; o = align_up(o + sizeof(int4) * p->h_stick.size(), 256);
         p->o_col = o; o = align_up(o + sizeof(int4) * p->h_col.size(), 256);
@@ -757,12 +779,10 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
         unsigned char *pk = (unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
         const unsigned char *cb = (const unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
         prof_begin(p, K_PLANE_FWD, st);
-        DevPlan dv = p->dev;
-        dv.ry = p->ry_fwd;
-        rc = p->plk.run[MODE_FWD](dv, p->tabs, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd1_stride, nc, st);
+        rc = p->plk.run[MODE_FWD](p->dev, p->tabs, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_ZFWD, st);
-        if (!rc) rc = p->zl.fwd(dv, A, pk, p->a_fwd1_stride, nc, st);
+        if (!rc) rc = p->zl.fwd(p->dev, A, pk, p->a_fwd_stride, nc, st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
         p->launches += 2;

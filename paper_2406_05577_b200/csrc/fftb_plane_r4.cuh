@@ -17,8 +17,7 @@
 //          runs (x = 4 n' .. 4 n' + 3) stored as two 32-byte stores                                  | barrier
 // The stick values of a column group arrive by TMA bulk copies in a per-warp landing zone, one y task
 // ahead (cp.async.bulk + mbarrier); the row of A is read four times per plane, from L2.
-// The forward kernel (plane_r4_fwd_k below) is the adjoint chain; the fused vloc of this pattern still
-// runs on the generic plane kernel.
+// plane_r4_fwd_k below is the adjoint chain, plane_r4_vloc_k the fused local-potential apply.
 #pragma once
 #include "fftb_plane_pf.cuh"
 
@@ -135,9 +134,9 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
         const int zc = z + dz, zn = zc >= pl.n3 ? zc - pl.n3 : zc, bn = b + db + (zc >= pl.n3 ? 1 : 0); // next plane
         const bool more = i + 1 < kplanes;
         const C *row = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
-        auto quarter = [&](auto rc) {
+        // ================================================== Y_R: columns -> pbuf (lines y = 4 y' + R)
+        auto yphase = [&](auto rc) {
             constexpr int R = decltype(rc)::value;
-            // ================================================== Y_R: columns -> pbuf (lines y = 4 y' + R)
             C sv = czero<T>(); // single-stick column of this warp: its value, loaded while the y tasks run
             int4 sco = make_int4(0, 0, 0, 0);
             int scol = 0;
@@ -179,8 +178,17 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             }
             if (warp < n_one) // closed form x W^{k2 y}
                 for (int yl = lane; yl < M; yl += 32) pbuf[scol * YP + yl] = cmul(sv, tw[(sco.z * (4 * yl + R)) & (N - 1)]);
-            __syncthreads();
-            // ================================================== X_R: 64 lines y = 4 y' + R -> cuboid
+            for (int k = warp + NW; k < n_one; k += NW) { // more single-stick columns than warps (explicit maps)
+                const int col = ct.perm[pl.n_multi + k];
+                const int4 co = ct.col[col];
+                const C xv = __ldcg(row + co.x);
+                for (int yl = lane; yl < M; yl += 32) pbuf[col * YP + yl] = cmul(xv, tw[(co.z * (4 * yl + R)) & (N - 1)]);
+            }
+        };
+        // ================================================== X_r: 64 lines y = 4 y' + r -> cuboid
+        // (r is a run-time value: the x phase is most of the code and exists once -- with the four quarters
+        // unrolled the kernel outgrows the instruction caches)
+        auto xphase = [&](int r) {
 #pragma unroll 1
             for (int v = 0; v < XT; ++v) {
                 const int yl = (warp + v * NW) * G + f;
@@ -193,7 +201,7 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
                 }
                 const int cc = M - k1lo;
                 const C cv = (t == 0 && (unsigned)cc < (unsigned)nx) ? pbuf[cc * YP + yl] : czero<T>();
-                C *rowo = cub_out + (((long long)b * pl.n3 + z) * N + (4 * yl + R)) * N;
+                C *rowo = cub_out + (((long long)b * pl.n3 + z) * N + (4 * yl + r)) * N;
                 const ExSkew<T, P2, YP> ex{pbuf + yl, true}; // the line's slots are dead: exchanged in them
                 C u[8], o0[1][8], o1[1][8];
                 r4_fold_inv<0, 0, T>(a, bq, cv, u, wt[0]);
@@ -209,12 +217,19 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
 #pragma unroll
                 for (int q = 0; q < 8; ++q) st_pair(rowo + 4 * (t + 8 * q) + 2, o0[0][q], o1[0][q]);
             }
-            __syncthreads();
         };
-        quarter(std::integral_constant<int, 0>{});
-        quarter(std::integral_constant<int, 1>{});
-        quarter(std::integral_constant<int, 2>{});
-        quarter(std::integral_constant<int, 3>{});
+#pragma unroll 1
+        for (int r = 0; r < 4; ++r) {
+            switch (r) {
+            case 0: yphase(std::integral_constant<int, 0>{}); break;
+            case 1: yphase(std::integral_constant<int, 1>{}); break;
+            case 2: yphase(std::integral_constant<int, 2>{}); break;
+            default: yphase(std::integral_constant<int, 3>{}); break;
+            }
+            __syncthreads();
+            xphase(r);
+            __syncthreads();
+        }
         z = zn; b = bn;
     }
 }
@@ -294,13 +309,13 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
 
 #pragma unroll 1
     for (int i = 0; i < kplanes; ++i) {
-        auto quarter = [&](auto rc) {
-            constexpr int R = decltype(rc)::value;
-            // ================================================== X_R: 64 lines y = 4 y' + R -> pbuf
+        // ================================================== X_r: 64 lines y = 4 y' + r -> pbuf
+        // (r is a run-time value: the x phase exists once, see plane_r4_inv_k)
+        auto xphase = [&](int r) {
 #pragma unroll 1
             for (int v = 0; v < XT; ++v) {
                 const int yl = (warp + v * NW) * G + f;
-                const C *rowi = cub_in + (((long long)b * pl.n3 + z) * N + (4 * yl + R)) * N;
+                const C *rowi = cub_in + (((long long)b * pl.n3 + z) * N + (4 * yl + r)) * N;
                 const ExSkew<T, P2, YP> ex{pbuf + yl, true}; // the line's slots are still unused: exchanged in them
                 C o0[1][8], o1[1][8], gq[8], fa[8], fb[8], fc;
 #pragma unroll
@@ -325,8 +340,10 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
                 const int cc = M - k1lo;
                 if (t == 0 && (unsigned)cc < (unsigned)nx) pbuf[cc * YP + yl] = fc;
             }
-            __syncthreads();
-            // ================================================== Y_R: columns -> partial plane R of A
+        };
+        // ================================================== Y_R: columns -> partial plane R of A
+        auto yphase = [&](auto rc) {
+            constexpr int R = decltype(rc)::value;
             // One plane of A: residue 0 stores, residues 1..3 add to what the SAME lane stored one quarter ago
             // (still in L2; the loads are issued before the transform whose result they are added to).
             C *dst = Aout + (long long)b * a_out_stride + (long long)z * pl.pitch;
@@ -377,15 +394,294 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
                 }
                 if (lane == 0) dst[co.x] = R > 0 ? cadd(__ldcg(dst + co.x), acc) : acc;
             }
-            __syncthreads();
         };
-        quarter(std::integral_constant<int, 0>{});
-        quarter(std::integral_constant<int, 1>{});
-        quarter(std::integral_constant<int, 2>{});
-        quarter(std::integral_constant<int, 3>{});
+#pragma unroll 1
+        for (int r = 0; r < 4; ++r) {
+            xphase(r);
+            __syncthreads();
+            switch (r) {
+            case 0: yphase(std::integral_constant<int, 0>{}); break;
+            case 1: yphase(std::integral_constant<int, 1>{}); break;
+            case 2: yphase(std::integral_constant<int, 2>{}); break;
+            default: yphase(std::integral_constant<int, 3>{}); break;
+            }
+            __syncthreads();
+        }
         const int zc = z + dz;
         b += db + (zc >= pl.n3 ? 1 : 0);
         z = zc >= pl.n3 ? zc - pl.n3 : zc;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// fused local-potential apply of the 256 pattern: per quarter r
+//     Y_inv_r (as plane_r4_inv_k)                                                        | barrier
+//     X_r: a line's 129 inputs -> e = 0, 1: two transforms, times V(r), two adjoint transforms, F[k1]
+//          accumulated; the inputs are read AGAIN from the plane buffer for e = 2, 3 (they would not fit in
+//          registers next to F), so the exchanges go through the warp's landing zone instead of the line's
+//          slots; finally F[k1] replaces the line in the plane buffer                      | barrier
+//     Y_fwd_r (as plane_r4_fwd_k: added into one plane of A), then the Y_inv of the next quarter on the
+//          same columns by the same warp, no barrier in between.
+// The cuboid is never written (I6').  The landing zone is scratch during X_r, so the first y task of
+// a quarter is requested after X_{r-1} and lands during Y_fwd_{r-1}.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NW>
+__global__ void __launch_bounds__(NW * 32, 1)
+plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab4 ct, const cx<T> *__restrict__ Ain,
+                cx<T> *__restrict__ Aout, const T *__restrict__ vloc, long long a_in_stride, long long a_out_stride, int nplanes)
+{
+    using C = cx<T>;
+    using R4 = PlaneR4<T, NW>;
+    using F = typename R4::F;
+    constexpr int N = R4::N, M = R4::M, P2 = F::P2, G = F::G, YP = R4::YP, ZCOL = R4::ZCOL;
+    constexpr int XT = R4::NXT / NW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *pbuf = reinterpret_cast<C *>(smem_raw);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    C *zone = pbuf + R4::PB + warp * R4::ZONE;
+    __shared__ __align__(8) unsigned long long bar_zone[NW];
+    unsigned zone_par = 0;
+    const C *tw = reinterpret_cast<const C *>(pl.tw1);
+    C tws[8];
+#pragma unroll
+    for (int m = 1; m < 8; ++m) tws[m] = tw[(4 * t * m) & (N - 1)];
+    tws[0] = mk<T>((T)1, (T)0);
+    C wt[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
+    const int nx = pl.nxocc, k1lo = pl.k1lo;
+    const int n_one = nx - pl.n_multi;
+    const int ntask_y = (pl.n_multi + G - 1) / G;
+    const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    const int ytasks_w = ntask_y > warp ? (ntask_y - warp + NW - 1) / NW : 0;
+
+    struct YCol { bool act; int col; int4 co; };
+    auto ycol = [&](int task) -> YCol {
+        YCol c;
+        const int ci = task * G + f;
+        c.act = ci < pl.n_multi;
+        c.col = ct.perm[c.act ? ci : 0];
+        c.co = ct.col[c.col];
+        return c;
+    };
+    auto zone_issue = [&](int b, int z, int task) {
+        const C *row = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
+        int bytes = 0;
+        int4 co = make_int4(0, 0, 0, 0);
+        if (lane < G) {
+            const int ci = task * G + lane;
+            if (ci < pl.n_multi) {
+                co = ct.col[ct.perm[ci]];
+                const int sh = sizeof(C) == 8 ? (co.x & 1) : 0; // see plane_r4_inv_k
+                co.x -= sh;
+                co.y += sh;
+                if (sizeof(C) == 8) co.y = (co.y + 1) & ~1;
+                bytes = co.y * (int)sizeof(C);
+            }
+        }
+        int total = bytes;
+#pragma unroll
+        for (int sft = 1; sft < G; sft <<= 1) total += __shfl_xor_sync(0xffffffffu, total, sft);
+        if (lane == 0) mbar_expect_tx(&bar_zone[warp], (unsigned)total);
+        __syncwarp();
+        if (bytes > 0) bulk_load(zone + lane * ZCOL, row + co.x, (unsigned)bytes, &bar_zone[warp]);
+    };
+
+    if (tid == 0) {
+        for (int w = 0; w < NW; ++w) mbar_init(&bar_zone[w], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;
+    const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;
+    if (kplanes > 0 && ytasks_w > 0) zone_issue(b, z, warp);
+
+#pragma unroll 1
+    for (int i = 0; i < kplanes; ++i) {
+        const int zc = z + dz, zn = zc >= pl.n3 ? zc - pl.n3 : zc, bn = b + db + (zc >= pl.n3 ? 1 : 0);
+        const bool more = i + 1 < kplanes;
+        const C *row = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
+        C *dst = Aout + (long long)b * a_out_stride + (long long)z * pl.pitch;
+        // ================================================== Y_inv_R: columns -> pbuf
+        auto yinv = [&](auto rc) {
+            constexpr int R = decltype(rc)::value;
+            C sv = czero<T>();
+            int4 sco = make_int4(0, 0, 0, 0);
+            int scol = 0;
+            if (warp < n_one) {
+                scol = ct.perm[pl.n_multi + warp];
+                sco = ct.col[scol];
+                sv = __ldcg(row + sco.x);
+            }
+#pragma unroll 1
+            for (int k = 0; k < ytasks_w; ++k) {
+                const int task = warp + k * NW;
+                const YCol c = ycol(task);
+                mbar_wait(&bar_zone[warp], zone_par);
+                zone_par ^= 1u;
+                const C *src = zone + f * ZCOL + (sizeof(C) == 8 ? (c.co.x & 1) : 0);
+                C a[8], bq[8], u[8], y[1][8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
+                    a[j] = (c.act && (unsigned)ia < (unsigned)c.co.y) ? src[ia] : czero<T>();
+                    bq[j] = (c.act && (unsigned)ib < (unsigned)c.co.y) ? src[ib] : czero<T>();
+                }
+                const int ic = M - c.co.z;
+                const C cv = (c.act && t == 0 && (unsigned)ic < (unsigned)c.co.y) ? src[ic] : czero<T>();
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (k + 1 < ytasks_w) zone_issue(b, z, task + NW); // within the y phase the zone is a landing zone only
+                r4_fold_inv<R, 0, T>(a, bq, cv, u, wt[R]);
+                C *pc = pbuf + c.col * YP;
+                sub_inv<F, T>(u, y, tws, ExSkew<T, P2, 1>{pc, c.act}, t);
+                __syncwarp();
+                if (c.act) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) pc[t + 8 * q] = y[0][q];
+                }
+            }
+            if (warp < n_one)
+                for (int yl = lane; yl < M; yl += 32) pbuf[scol * YP + yl] = cmul(sv, tw[(sco.z * (4 * yl + R)) & (N - 1)]);
+            for (int k = warp + NW; k < n_one; k += NW) { // more single-stick columns than warps (explicit maps)
+                const int col = ct.perm[pl.n_multi + k];
+                const int4 co = ct.col[col];
+                const C xv = __ldcg(row + co.x);
+                for (int yl = lane; yl < M; yl += 32) pbuf[col * YP + yl] = cmul(xv, tw[(co.z * (4 * yl + R)) & (N - 1)]);
+            }
+        };
+        // ================================================== X_r: inverse, V(r), forward, in place in pbuf
+        // (r is a run-time value here: this is the bulk of the code and it exists once, see the note on the
+        // instruction cache in DESIGN.md 6.4)
+        auto xphase = [&](int r) {
+#pragma unroll 1
+            for (int v = 0; v < XT; ++v) {
+                const int yl = (warp + v * NW) * G + f;
+                const T *vrow = vloc + ((long long)z * N + (4 * yl + r)) * N;
+                const ExSkew<T, P2, 1> ex{zone + f * ZCOL, true}; // the line must stay intact for the second read
+                C fa[8], fb[8], fc;
+                auto pass = [&](auto ec) {
+                    constexpr int E0 = decltype(ec)::value; // this pass does e = E0, E0 + 1
+                    T v0[8], v1[8];
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) { // V at x = 4 n' + E0, + 1: one load per pair
+                        const C vv = __ldg(reinterpret_cast<const C *>(vrow + 4 * (t + 8 * q) + E0));
+                        v0[q] = vv.x;
+                        v1[q] = vv.y;
+                    }
+                    C a[8], bq[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int ca = (t + 8 * j) - M - k1lo, cb = (t + 8 * j) - k1lo;
+                        a[j] = (unsigned)ca < (unsigned)nx ? pbuf[ca * YP + yl] : czero<T>();
+                        bq[j] = (unsigned)cb < (unsigned)nx ? pbuf[cb * YP + yl] : czero<T>();
+                    }
+                    const int cc = M - k1lo;
+                    const C cv = (t == 0 && (unsigned)cc < (unsigned)nx) ? pbuf[cc * YP + yl] : czero<T>();
+                    C u[8], o0[1][8], o1[1][8], gq[8];
+                    r4_fold_inv<E0, 0, T>(a, bq, cv, u, wt[E0]);
+                    sub_inv<F, T>(u, o0, tws, ex, t);
+                    r4_fold_inv<E0 + 1, 0, T>(a, bq, cv, u, wt[E0 + 1]);
+                    sub_inv<F, T>(u, o1, tws, ex, t);
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) {
+                        o0[0][q].x *= v0[q]; o0[0][q].y *= v0[q];
+                        o1[0][q].x *= v1[q]; o1[0][q].y *= v1[q];
+                    }
+                    sub_fwd<F, T>(o0, gq, tws, ex, t);
+                    r4_fold_fwd<E0, 0, T>(gq, fa, fb, fc, wt[E0]);
+                    sub_fwd<F, T>(o1, gq, tws, ex, t);
+                    r4_fold_fwd<E0 + 1, 0, T>(gq, fa, fb, fc, wt[E0 + 1]);
+                };
+                pass(std::integral_constant<int, 0>{});
+                pass(std::integral_constant<int, 2>{});
+                __syncwarp(); // every lane has read the line twice: it takes the result
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int ca = (t + 8 * j) - M - k1lo, cb = (t + 8 * j) - k1lo;
+                    if ((unsigned)ca < (unsigned)nx) pbuf[ca * YP + yl] = fa[j];
+                    if ((unsigned)cb < (unsigned)nx) pbuf[cb * YP + yl] = fb[j];
+                }
+                const int cc = M - k1lo;
+                if (t == 0 && (unsigned)cc < (unsigned)nx) pbuf[cc * YP + yl] = fc;
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); // generic-proxy writes to the zone before the next bulk copy
+        };
+        // ================================================== Y_fwd_R: columns -> added into the one plane of A
+        auto yfwd = [&](auto rc) {
+            constexpr int R = decltype(rc)::value;
+#pragma unroll 1
+            for (int task = warp; task < ntask_y; task += NW) {
+                const YCol c = ycol(task);
+                C *pc = pbuf + c.col * YP;
+                C *d = dst + c.co.x;
+                const int ic = M - c.co.z;
+                const bool hc = c.act && t == 0 && (unsigned)ic < (unsigned)c.co.y;
+                C y[1][8], gq[8], pa[8], pb[8], pcv, oa[8], ob[8], oc = czero<T>();
+                if constexpr (R > 0) {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
+                        oa[j] = (c.act && (unsigned)ia < (unsigned)c.co.y) ? __ldcg(d + ia) : czero<T>();
+                        ob[j] = (c.act && (unsigned)ib < (unsigned)c.co.y) ? __ldcg(d + ib) : czero<T>();
+                    }
+                    if (hc) oc = __ldcg(d + ic);
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
+                sub_fwd<F, T>(y, gq, tws, ExSkew<T, P2, 1>{pc, c.act}, t);
+                r4_part_fwd<R, 0, T>(gq, pa, pb, pcv, wt[R]);
+                if (c.act) {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
+                        if ((unsigned)ia < (unsigned)c.co.y) d[ia] = R > 0 ? cadd(oa[j], pa[j]) : pa[j];
+                        if ((unsigned)ib < (unsigned)c.co.y) d[ib] = R > 0 ? cadd(ob[j], pb[j]) : pb[j];
+                    }
+                    if (hc) d[ic] = R > 0 ? cadd(oc, pcv) : pcv;
+                }
+            }
+            for (int k = warp; k < n_one; k += NW) {
+                const int col = ct.perm[pl.n_multi + k];
+                const int4 co = ct.col[col];
+                C acc = czero<T>();
+                for (int yl = lane; yl < M; yl += 32) acc = cadd(acc, cmulc(pbuf[col * YP + yl], tw[(co.z * (4 * yl + R)) & (N - 1)]));
+#pragma unroll
+                for (int sft = 16; sft > 0; sft >>= 1) {
+                    acc.x += __shfl_xor_sync(0xffffffffu, acc.x, sft);
+                    acc.y += __shfl_xor_sync(0xffffffffu, acc.y, sft);
+                }
+                if (lane == 0) dst[co.x] = R > 0 ? cadd(__ldcg(dst + co.x), acc) : acc;
+            }
+        };
+        using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>;
+        using I2 = std::integral_constant<int, 2>; using I3 = std::integral_constant<int, 3>;
+#pragma unroll 1
+        for (int r = 0; r < 4; ++r) {
+            switch (r) {
+            case 0: yinv(I0{}); break;
+            case 1: yinv(I1{}); break;
+            case 2: yinv(I2{}); break;
+            default: yinv(I3{}); break;
+            }
+            __syncthreads();
+            xphase(r);
+            __syncthreads();
+            // the zone is a landing zone again: the first y task of the next quarter (or plane) lands during Y_fwd_r
+            if (ytasks_w > 0) {
+                if (r < 3) zone_issue(b, z, warp);
+                else if (more) zone_issue(bn, zn, warp);
+            }
+            switch (r) {
+            case 0: yfwd(I0{}); break;
+            case 1: yfwd(I1{}); break;
+            case 2: yfwd(I2{}); break;
+            default: yfwd(I3{}); break;
+            }
+            // no barrier: the next Y_inv touches the same columns from the same warp
+        }
+        z = zn; b = bn;
     }
 }
 
