@@ -285,6 +285,36 @@ def test_explicit_stick_map_vs_oracle(fb, oracle, n, radius, centre, dtype, trim
     p.destroy()
 
 
+def test_explicit_map_many_single_stick_columns_256(fb, oracle):
+    """An explicit map on a 256 x 256 grid whose k1 columns mostly hold ONE stick (more such columns than
+    the plane kernels have warps): they take the closed-form path of the four-way-split kernels."""
+    n = (256, 256, 32)
+    k1, k2, k3lo, ln = [], [], [], []
+    for a in range(-21, 22):
+        run = range(-4, 5) if abs(a) <= 3 else [a % 7 - 3]
+        for b in run:
+            k1.append(a); k2.append(b); k3lo.append(-3 - (a + b) % 3); ln.append(5 + (a * b) % 4)
+    sm = tuple(np.asarray(x, dtype=np.int32) for x in (k1, k2, k3lo, ln))
+    nb = 2
+    p = fb.Plan(n, batch=nb, dtype="c128", stick_map=sm).bind()
+    k = p.points()
+    w = wl.Workload(0, "explicit", n, (0, 0, 0), "c128", nb, "uniform", "inv_fwd")
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    d_psi = p.inverse(d_c)
+    torch.cuda.synchronize()
+    assert _rel(d_psi.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol
+    C = float(np.prod(n))
+    g = wl.cuboid(w)
+    d_f = p.forward(torch.from_numpy(g).cuda())
+    v = wl.potential(w)
+    d_o = p.apply_vloc(d_c, torch.from_numpy(v).cuda())
+    torch.cuda.synchronize()
+    assert _rel(d_f.cpu().numpy(), oracle.forward(n, k, g, 1.0 / C)) <= w.tol
+    assert _rel(d_o.cpu().numpy(), oracle.apply_vloc(n, k, c, v, 1.0 / C)) <= w.tol
+    p.destroy()
+
+
 def test_host_buffer_calls_pipelined(fb, oracle):
     """Batches of 32 bands and more cross PCIe in chunks on the plan's copy streams, overlapped with the
     transforms: same results as the device-pointer calls, complete when the caller's stream is."""
