@@ -325,8 +325,13 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5 (default 3, the graded one)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--op", default="config", choices=["config", "inv_fwd", "vloc"],
+                    help="operation of the step: the config's own (default), or the same grid and batch with the other one")
     args = ap.parse_args()
     w = wl.WORKLOADS[args.config]
+    if args.op != "config" and args.op != w.op:
+        import dataclasses
+        w = dataclasses.replace(w, op=args.op, name=f"{w.name} [--op {args.op}]")
     if args.impl == "reference":
         run_reference(args, w)
     else:
