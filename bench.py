@@ -118,7 +118,7 @@ def oracle_step(w, k, c, v, orc):
 
 def oracle_sample_bands(w):
     # sized for roughly 10-30 s of CPU work over the default steps on the box's host cores
-    return {1: 4, 2: 16, 3: 4, 4: 2, 5: 1}[w.number]
+    return {1: 4, 2: 16, 3: 16, 4: 4, 5: 2}[w.number]
 
 
 def time_oracle(w, steps, warmup):
