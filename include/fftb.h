@@ -158,6 +158,15 @@ int fftb_dense_embed(fftb_plan pruned, fftb_plan dense, const void *d_packed_pru
 int fftb_dense_extract(fftb_plan pruned, fftb_plan dense, const void *d_packed_dense, void *d_packed_pruned, int nb,
                        void *stream);
 
+/* Packed arrays in the paper's batch-fastest order (Fig. 8 "b x y z": the band index
+ * is the fastest one, element [point][band], nb bands) and in this library's order [band][point]
+ * (north_star: "packed z-sticks per band"): to_band_slowest != 0 copies d_in = [S][nb] to
+ * d_out = [nb][S], to_band_slowest == 0 the other way.  Both are device pointers, 16-byte aligned,
+ * S * nb elements of the plan's dtype, owned by the caller; in place is not supported
+ * (FFTB_EINVAL), nb is not limited by the plan's batch.  One kernel, both sides coalesced; this is
+ * how a caller that keeps its coefficients batch-fastest uses the transforms. */
+int fftb_packed_transpose(fftb_plan p, const void *d_in, void *d_out, int nb, int to_band_slowest, void *stream);
+
 /* Number of kernels the last execute call on this plan launched (for launch accounting). */
 int fftb_plan_last_launches(fftb_plan p);
 

@@ -24,7 +24,7 @@ SYMBOLS = [
     "fftb_plan_create", "fftb_plan_create_explicit", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
     "fftb_inverse", "fftb_forward", "fftb_apply_vloc",
     "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
-    "fftb_dense_embed", "fftb_dense_extract",
+    "fftb_dense_embed", "fftb_dense_extract", "fftb_packed_transpose",
     "fftb_plan_last_launches", "fftb_plan_profile", "fftb_plan_profile_read", "fftb_plan_destroy", "fftb_strerror",
 ]
 
@@ -69,6 +69,7 @@ def lib():
             getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
         for name in ("fftb_dense_embed", "fftb_dense_extract"):
             getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
+        L.fftb_packed_transpose.argtypes = [vp, vp, vp, i32, i32, vp]
         L.fftb_plan_last_launches.argtypes = [vp]
         L.fftb_plan_profile.argtypes = [vp, i32]
         L.fftb_plan_profile_read.argtypes = [vp, vp, vp]
@@ -245,6 +246,28 @@ class Plan:
         _check(lib().fftb_dense_extract(self._h, dense_plan._h, dense_plan._chk(packed_dense, (nb, dense_plan.S)),
                                         self._chk(packed, (nb, self.S)), nb, _stream_ptr(stream)), "fftb_dense_extract")
         return packed
+
+    def packed_to_band_slowest(self, packed_sb, out=None, stream=None):
+        """[S][nb] (the paper's batch-fastest order) -> [nb][S] (this library's order)."""
+        import torch
+
+        nb = packed_sb.shape[1]
+        if out is None:
+            out = torch.empty((nb, self.S), dtype=self.torch_complex, device=packed_sb.device)
+        _check(lib().fftb_packed_transpose(self._h, self._chk(packed_sb, (self.S, nb)), self._chk(out, (nb, self.S)), nb, 1,
+                                           _stream_ptr(stream)), "fftb_packed_transpose")
+        return out
+
+    def packed_to_band_fastest(self, packed_bs, out=None, stream=None):
+        """[nb][S] -> [S][nb]."""
+        import torch
+
+        nb = packed_bs.shape[0]
+        if out is None:
+            out = torch.empty((self.S, nb), dtype=self.torch_complex, device=packed_bs.device)
+        _check(lib().fftb_packed_transpose(self._h, self._chk(packed_bs, (nb, self.S)), self._chk(out, (self.S, nb)), nb, 0,
+                                           _stream_ptr(stream)), "fftb_packed_transpose")
+        return out
 
     def last_launches(self) -> int:
         return int(lib().fftb_plan_last_launches(self._h))

@@ -973,6 +973,25 @@ int fftb_dense_extract(fftb_plan pruned, fftb_plan dense, const void *d_packed_d
     return dense_move(pruned, dense, d_packed_dense, d_packed_pruned, nb, stream, true);
 }
 
+int fftb_packed_transpose(fftb_plan p, const void *d_in, void *d_out, int nb, int to_band_slowest, void *stream)
+{
+    if (!p || !d_in || !d_out || d_in == d_out) return FFTB_EINVAL;
+    if (p->sticky) return p->sticky;
+    if (nb < 1 || (uintptr_t)d_in % 16 || (uintptr_t)d_out % 16) return FFTB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    // to_band_slowest: in = [S][nb] -> out = [nb][S]; otherwise in = [nb][S] -> out = [S][nb]
+    const long long R = to_band_slowest ? p->S : nb, Cn = to_band_slowest ? nb : p->S;
+    const long long tiles = ((Cn + 31) / 32) * ((R + 31) / 32);
+    if (tiles > 0x7fffffffLL) return FFTB_EUNSUPPORTED;
+    const unsigned grid = (unsigned)tiles;
+    if (p->elem == 16)
+        transpose_k<double2><<<grid, 256, 0, st>>>((const double2 *)d_in, (double2 *)d_out, R, Cn);
+    else
+        transpose_k<float2><<<grid, 256, 0, st>>>((const float2 *)d_in, (float2 *)d_out, R, Cn);
+    p->launches = 1;
+    return cudaGetLastError() == cudaSuccess ? FFTB_OK : FFTB_ECUDA;
+}
+
 int fftb_plan_last_launches(fftb_plan p) { return p ? p->launches : FFTB_EINVAL; }
 
 

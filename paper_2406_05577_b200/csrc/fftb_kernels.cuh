@@ -542,4 +542,25 @@ __global__ void dense_embed_k(const int4 *__restrict__ stick, int nsticks, long 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// packed arrays between the paper's batch-fastest order (Fig. 8 "b x y z": element
+// [point][band]) and this library's band-slowest order [band][point]: out[c][r] = in[r][c] for an
+// R x Cn matrix, 32 x 32 tiles through shared memory, both sides coalesced.
+// ---------------------------------------------------------------------------------------------
+template <typename E>
+__global__ void __launch_bounds__(256) transpose_k(const E *__restrict__ in, E *__restrict__ out, long long R, long long Cn)
+{
+    __shared__ E tile[32][33];
+    const long long tcols = (Cn + 31) / 32; // one-dimensional grid of tiles: either side may be the long one
+    const long long c0 = ((long long)blockIdx.x % tcols) * 32, r0 = ((long long)blockIdx.x / tcols) * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+#pragma unroll
+    for (int i = ty; i < 32; i += 8)
+        if (r0 + i < R && c0 + tx < Cn) tile[i][tx] = in[(r0 + i) * Cn + c0 + tx];
+    __syncthreads();
+#pragma unroll
+    for (int i = ty; i < 32; i += 8)
+        if (c0 + i < Cn && r0 + tx < R) out[(c0 + i) * R + r0 + tx] = tile[tx][i];
+}
+
 } // namespace fftb

@@ -315,6 +315,32 @@ def test_explicit_map_many_single_stick_columns_256(fb, oracle):
     p.destroy()
 
 
+@pytest.mark.parametrize("dtype,nb", [("c128", 37), ("c64", 64), ("c128", 1)])
+def test_batch_fastest_packed_layout(fb, oracle, dtype, nb):
+    """PAPER.md:219-221 (Fig. 8, "b x y z"): coefficients held with the band index fastest go through
+    fftb_packed_transpose: bit-exact transposition both ways (ragged tiles), and the fused local potential
+    applied to batch-fastest data equals the oracle's result transposed."""
+    w = _small((64, 64, 32), (16, 11, 8), dtype=dtype, batch=nb)
+    p = _plan(fb, w, nb)
+    k = p.points()
+    c = wl.coefficients(w, *k)                                   # [nb][S]
+    c_sb = np.ascontiguousarray(c.T)                             # [S][nb], batch fastest
+    d_sb = torch.from_numpy(c_sb).cuda()
+    d_bs = p.packed_to_band_slowest(d_sb)
+    torch.cuda.synchronize()
+    assert torch.equal(d_bs.cpu(), torch.from_numpy(c))
+    assert torch.equal(p.packed_to_band_fastest(d_bs).cpu(), torch.from_numpy(c_sb))
+    v = wl.potential(w)
+    d_o = p.packed_to_band_fastest(p.apply_vloc(d_bs, torch.from_numpy(v).cuda()))
+    torch.cuda.synchronize()
+    ref = oracle.apply_vloc(w.n, k, c, v, 1.0 / float(np.prod(w.n)))
+    assert _rel(d_o.cpu().numpy(), np.ascontiguousarray(ref.T)) <= w.tol
+    # in place is refused
+    with pytest.raises(fb.FftbError):
+        p.packed_to_band_slowest(d_sb, out=d_sb.view(nb, p.S))
+    p.destroy()
+
+
 def test_host_buffer_calls_pipelined(fb, oracle):
     """Batches of 32 bands and more cross PCIe in chunks on the plan's copy streams, overlapped with the
     transforms: same results as the device-pointer calls, complete when the caller's stream is."""
