@@ -113,6 +113,37 @@ def test_apply_vloc_vs_oracle(fb, oracle, w):
     p.destroy()
 
 
+DEGENERATE = [((64, 64, 64), (0, 0, 0)), ((64, 64, 64), (1, 1, 1)), ((128, 128, 128), (2, 1, 3)), ((32, 32, 32), (1, 8, 1)),
+              ((128, 128, 128), (0, 5, 0)), ((256, 256, 64), (1, 1, 1)), ((256, 256, 256), (0, 0, 7)), ((96, 96, 64), (0, 24, 0)),
+              ((128, 128, 128), (32, 0, 0)), ((256, 256, 32), (64, 1, 0))]
+
+
+@pytest.mark.timeout(120)
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("n,a", DEGENERATE, ids=[f"{n[0]}x{n[1]}x{n[2]}-a{a[0]}.{a[1]}.{a[2]}" for n, a in DEGENERATE])
+def test_degenerate_spheres(fb, oracle, n, a, dtype):
+    """The degenerate cut-offs: a single point, a single stick, a single column, a single plane of sticks,
+    columns that all hold one stick (no y task at all in the persistent kernels)."""
+    w = _small(n, a, dtype=dtype, batch=2)
+    p = _plan(fb, w, w.batch)
+    k = p.points()
+    assert all(np.array_equal(x, y) for x, y in zip(k, oracle.enum_points(n, a)))
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    d_psi = p.inverse(d_c)
+    torch.cuda.synchronize()
+    assert _rel(d_psi.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol
+    C = float(np.prod(n))
+    g = wl.cuboid(w)
+    d_f = p.forward(torch.from_numpy(g).cuda())
+    v = wl.potential(w)
+    d_o = p.apply_vloc(d_c, torch.from_numpy(v).cuda())
+    torch.cuda.synchronize()
+    assert _rel(d_f.cpu().numpy(), oracle.forward(n, k, g, 1.0 / C)) <= w.tol
+    assert _rel(d_o.cpu().numpy(), oracle.apply_vloc(n, k, c, v, 1.0 / C)) <= w.tol
+    p.destroy()
+
+
 def test_scale_none(fb, oracle):
     w = SMALL[0]
     p = _plan(fb, w, w.batch, scale="none")
