@@ -127,6 +127,11 @@ int fftb_plan_get_map(fftb_plan p, int32_t *k1, int32_t *k2, int32_t *k3lo, int3
  * plan-owned host memory) and returns; later execute calls on the same stream are ordered after it. */
 int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream);
 
+/* The three device-pointer execute calls below only enqueue kernels on `stream`: no allocation, no
+ * synchronisation, no host-side dependence on the data.  They may therefore be captured in a CUDA
+ * graph by the caller (stream capture) and replayed; the *_host variants use plan-owned copy streams
+ * and events and are not meant for capture. */
+
 /* inverse: d_packed [nb][S] -> d_cuboid [nb][N3][N2][N1].  unpack + pruned z pass on the sticks,
  * y pass on the occupied x columns only, x pass last (Fig. 3, 112: staged padding). */
 int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void *stream);

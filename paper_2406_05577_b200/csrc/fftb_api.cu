@@ -117,6 +117,13 @@ constexpr int FAST_NW = 4; // warps per CTA of the z-pass kernels (4 CTAs per SM
 template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 8 : (N == 96 ? 4 : 2); }; // must divide N / G; measured best
 
 static int g_sm_count = 0;
+static int current_device()
+{
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return dev;
+}
+
 static int sm_count()
 {
     if (!g_sm_count) {
@@ -139,8 +146,11 @@ int launch_plane_fast(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, 
     if (smem > 227 * 1024) return FFTB_EUNSUPPORTED;
     static int per_sm = 0;    // CTAs per SM of this instantiation
     static size_t smem_set = 0;
-    if (!per_sm || smem != smem_set) {
+    static int dev_set = -1;  // attribute and occupancy are per device
+    const int dev = current_device();
+    if (!per_sm || smem != smem_set || dev != dev_set) {
         smem_set = smem;
+        dev_set = dev;
         if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
         int occ = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, NW * 32, smem) != cudaSuccess || occ < 1) return FFTB_ECUDA;
@@ -165,10 +175,11 @@ int launch_plane_r4_inv(const DevPlan &pl, const PlanTabs &tabs, const void *Ain
     constexpr int NW = 8;
     auto k = plane_r4_inv_k<T, NW>;
     const size_t smem = PlaneR4<T, NW>::smem_bytes;
-    static bool ready = false;
-    if (!ready) {
+    static int ready_dev = -1; // the attribute is per device: set again when the calling thread's device changes
+    const int dev = current_device();
+    if (ready_dev != dev) {
         if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-        ready = true;
+        ready_dev = dev;
     }
     const int nplanes = pl.n3 * nb;
     int grid = sm_count();
@@ -184,10 +195,11 @@ int launch_plane_r4_vloc(const DevPlan &pl, const PlanTabs &tabs, const void *Ai
     constexpr int NW = 8;
     auto k = plane_r4_vloc_k<T, NW>;
     const size_t smem = PlaneR4<T, NW>::smem_bytes;
-    static bool ready = false;
-    if (!ready) {
+    static int ready_dev = -1; // the attribute is per device: set again when the calling thread's device changes
+    const int dev = current_device();
+    if (ready_dev != dev) {
         if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-        ready = true;
+        ready_dev = dev;
     }
     const int nplanes = pl.n3 * nb;
     int grid = sm_count();
@@ -203,10 +215,11 @@ int launch_plane_r4_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *, v
     constexpr int NW = 8;
     auto k = plane_r4_fwd_k<T, NW>;
     const size_t smem = sizeof(cx<T>) * (size_t)PlaneR4<T, NW>::PB;
-    static bool ready = false;
-    if (!ready) {
+    static int ready_dev = -1; // the attribute is per device: set again when the calling thread's device changes
+    const int dev = current_device();
+    if (ready_dev != dev) {
         if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-        ready = true;
+        ready_dev = dev;
     }
     const int nplanes = pl.n3 * nb;
     int grid = sm_count();

@@ -372,6 +372,42 @@ def test_batch_fastest_packed_layout(fb, oracle, dtype, nb):
     p.destroy()
 
 
+def test_device_calls_are_graph_capturable(fb):
+    """fftb_inverse / fftb_forward / fftb_apply_vloc only enqueue kernels on the caller's stream (no allocation,
+    no synchronisation), so a caller may capture them in a CUDA graph: replay gives the same bits."""
+    w = SMALL[2]
+    p = _plan(fb, w, w.batch)
+    k = p.points()
+    d_c = torch.from_numpy(wl.coefficients(w, *k)).cuda()
+    d_v = torch.from_numpy(wl.potential(w)).cuda()
+    d_psi = torch.empty(p.cuboid_shape(w.batch), dtype=p.torch_complex, device="cuda")
+    d_rt, d_o = torch.empty_like(d_c), torch.empty_like(d_c)
+
+    def step():
+        p.inverse(d_c, d_psi)
+        p.forward(d_psi, d_rt)
+        p.apply_vloc(d_c, d_v, d_o)
+
+    step()
+    torch.cuda.synchronize()
+    ref = (d_psi.clone(), d_rt.clone(), d_o.clone())
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        step()
+        s.synchronize()
+        with torch.cuda.graph(g, stream=s):
+            step()
+    torch.cuda.synchronize()
+    for t in (d_psi, d_rt, d_o):
+        t.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert all(torch.equal(a, b) for a, b in zip((d_psi, d_rt, d_o), ref))
+    del g
+    p.destroy()
+
+
 def test_host_buffer_calls_pipelined(fb, oracle):
     """Batches of 32 bands and more cross PCIe in chunks on the plan's copy streams, overlapped with the
     transforms: same results as the device-pointer calls, complete when the caller's stream is."""
