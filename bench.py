@@ -293,6 +293,8 @@ def run_ours(args, w):
     # what a caller with a launch-bound loop gets; informational, `value` stays the plain-call number
     graph_info = None
     try:
+        if world > 1:
+            raise RuntimeError("single-GPU runs only (a rank-local failure must not unbalance the collectives)")
         gs = torch.cuda.Stream()
         graph = torch.cuda.CUDAGraph()
         with torch.cuda.stream(gs):
