@@ -73,7 +73,11 @@ __device__ __forceinline__ void bulk_load(void *sdst, const void *gsrc, unsigned
                  "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
-
+// ask for `bytes` (a multiple of 16) at gsrc to be brought into L2; no completion is signalled
+__device__ __forceinline__ void bulk_prefetch_l2(const void *gsrc, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gsrc), "r"(bytes) : "memory");
+}
 
 template <typename T, class F, int NW, int MODE>
 __global__ void __launch_bounds__(NW * 32, 1)

@@ -307,8 +307,21 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;
     const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;
 
+    // the lines of an x task are loaded into registers when the task starts; one task earlier they are
+    // requested into L2 (measured: 0.92 -> 0.90 ms on config 5; gathering the (x, x + 1) pairs of a batch
+    // into a landing zone with 16-byte cp.async copies instead was measured at 1.20 ms)
+    auto lines_prefetch = [&](int b, int z, int r, int v) {
+        if (lane < G) {
+            const int yl = (warp + v * NW) * G + lane;
+            bulk_prefetch_l2(cub_in + (((long long)b * pl.n3 + z) * N + (4 * yl + r)) * N, (unsigned)(N * sizeof(C)));
+        }
+    };
+    if (kplanes > 0) lines_prefetch(b, z, 0, 0);
+
 #pragma unroll 1
     for (int i = 0; i < kplanes; ++i) {
+        const int zc = z + dz, zn = zc >= pl.n3 ? zc - pl.n3 : zc, bn = b + db + (zc >= pl.n3 ? 1 : 0); // next plane
+        const bool more = i + 1 < kplanes;
         // ================================================== X_r: 64 lines y = 4 y' + r -> pbuf
         // (r is a run-time value: the x phase exists once, see plane_r4_inv_k)
         auto xphase = [&](int r) {
@@ -316,6 +329,9 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             for (int v = 0; v < XT; ++v) {
                 const int yl = (warp + v * NW) * G + f;
                 const C *rowi = cub_in + (((long long)b * pl.n3 + z) * N + (4 * yl + r)) * N;
+                if (v + 1 < XT) lines_prefetch(b, z, r, v + 1);
+                else if (r < 3) lines_prefetch(b, z, r + 1, 0);
+                else if (more) lines_prefetch(bn, zn, 0, 0);
                 const ExSkew<T, P2, YP> ex{pbuf + yl, true}; // the line's slots are still unused: exchanged in them
                 C o0[1][8], o1[1][8], gq[8], fa[8], fb[8], fc;
 #pragma unroll
@@ -407,9 +423,7 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             }
             __syncthreads();
         }
-        const int zc = z + dz;
-        b += db + (zc >= pl.n3 ? 1 : 0);
-        z = zc >= pl.n3 ? zc - pl.n3 : zc;
+        z = zn; b = bn;
     }
 }
 
