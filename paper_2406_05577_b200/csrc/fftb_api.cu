@@ -50,7 +50,6 @@ template <> struct YA<128, true> { using type = Axis<128, 2, 8, 8, false>; };
 template <> struct YA<256, true> { using type = Axis<256, 8, 8, 4, false>; };
 
 constexpr int cmax(int a, int b) { return a > b ? a : b; }
-constexpr int cmin(int a, int b) { return a < b ? a : b; }
 // largest divisor of m that does not exceed cap
 constexpr int div_le(int m, int cap)
 {
