@@ -154,7 +154,12 @@ __device__ __forceinline__ void sub_fwd(cx<T> (&y)[F::B2][F::P2], cx<T> (&x)[F::
 template <typename T, class F, int NW> struct ZFast {
     static constexpr int TS = F::G * NW;
     static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)F::N * TS + (size_t)NW * F::EXW);
-    __device__ static __forceinline__ int swz(int z, int sl) { return z * TS + ((sl + (z >> 1)) & (TS - 1)); }
+    // a shared-memory wavefront covers GW = LW / P2 lane groups (sticks) x P2 lanes (rows z, z+2, ...): the row
+    // rotation steps by GW so that those LW accesses fall into different banks in either precision
+    static constexpr int GW = F::LW / F::P2 < 1 ? 1 : F::LW / F::P2;
+    static_assert(TS >= F::LW, "tile row shorter than a wavefront");
+    __device__ static __forceinline__ int rot(int z) { return (z >> 1) * GW; }
+    __device__ static __forceinline__ int swz(int z, int sl) { return z * TS + ((sl + rot(z)) & (TS - 1)); }
 };
 
 // One tile (TS consecutive sticks starting at s0 = j TS) of one band, called by all NW warps of a CTA;
@@ -205,7 +210,7 @@ __device__ __forceinline__ void z_inv_tile(const DevPlan &pl, const cx<T> *__res
 #pragma unroll 4
     for (int i = tid; i < N * TS; i += NT) {
         const int z = i / TS, c = i % TS;
-        const int l = (c - (z >> 1)) & (TS - 1);
+        const int l = (c - Z::rot(z)) & (TS - 1);
         if (s0 + l < pl.nsticks) dst[(long long)z * pl.pitch + l] = tile[i];
     }
 }

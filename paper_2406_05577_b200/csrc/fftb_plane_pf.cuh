@@ -26,7 +26,13 @@
 namespace fftb {
 
 template <typename T, class F, int NW> struct PlanePF {
-    static constexpr int PB = F::NCOL * F::YP; // elements of one plane buffer (one y residue)
+    // elements of one plane buffer (one y residue).  The two buffers hold the even and the odd lines, and a
+    // shared-memory wavefront covers GW = LW / P2 lane groups = lines y, y+1 (one row of BOTH buffers), y+2, ...:
+    // with YP congruent to GW (FastCfg) the buffers must be GW/2 apart modulo LW for those accesses to
+    // fall into different banks (complex64, and complex128 with 4 lanes per transform)
+    static constexpr int GW = F::LW / F::P2;
+    static constexpr int PB0 = F::NCOL * F::YP;
+    static constexpr int PB = GW < 2 ? PB0 : PB0 + ((GW / 2 - PB0 % F::LW) + F::LW) % F::LW;
     static constexpr int NXT = F::N / F::G;    // x tasks per plane (G consecutive lines each)
     static constexpr int XT = NXT / NW;        // x tasks per warp and plane
     static_assert(NXT % NW == 0 && XT >= 1, "x tasks must divide evenly over the warps");

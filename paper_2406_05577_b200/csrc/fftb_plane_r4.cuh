@@ -709,7 +709,10 @@ template <typename T, int NW> struct ZR4 {
     using F = FastCfg<T, 128, 8, 8>;
     static constexpr int N = 256, M = 64, TS = F::G * NW;
     static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)N * TS + (size_t)NW * F::EXW);
-    __device__ static __forceinline__ int swz(int z, int sl) { return z * TS + ((sl + (z >> 2)) & (TS - 1)); }
+    static constexpr int GW = F::LW / F::P2 < 1 ? 1 : F::LW / F::P2; // lane groups per wavefront, see ZFast
+    static_assert(TS >= F::LW, "tile row shorter than a wavefront");
+    __device__ static __forceinline__ int rot(int z) { return (z >> 2) * GW; }
+    __device__ static __forceinline__ int swz(int z, int sl) { return z * TS + ((sl + rot(z)) & (TS - 1)); }
 };
 
 template <typename T, int NW>
@@ -767,7 +770,7 @@ zpass_r4_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ pac
 #pragma unroll 4
     for (int i = tid; i < N * TS; i += NT) {
         const int z = i / TS, c = i % TS;
-        const int l = (c - (z >> 2)) & (TS - 1);
+        const int l = (c - Z::rot(z)) & (TS - 1);
         if (s0 + l < pl.nsticks) dst[(long long)z * pl.pitch + l] = tile[i];
     }
 }
