@@ -43,6 +43,29 @@ struct ColTab {
     int perm[FAST_MAXCOL];  // multi-stick columns first, then the single-stick ones
 };
 
+// Column (index into the plan's column permutation) of lane group f in y task `task`, and the number of y tasks.
+// A shared-memory wavefront covers GW = LW / P2 lane groups x P2 consecutive elements of their columns.  The
+// plane-buffer pitch is congruent to GW modulo LW (what the x pass needs), so the GW columns of one wavefront
+// must be D = P2 / GW columns apart to fall into different banks: the y tasks take their columns from blocks of
+// GW x D columns, wavefront r of a block the columns r, r + D, ...  (identity when GW = 1 or D = 1).
+template <class F> __device__ __forceinline__ int ycol_index(int task, int f)
+{
+    constexpr int GW = F::LW / F::P2 < 1 ? 1 : F::LW / F::P2, D = F::P2 / GW;
+    if constexpr (GW <= 1 || D <= 1) {
+        return task * F::G + f;
+    } else {
+        static_assert(F::G % GW == 0, "lane groups per warp must be a multiple of the groups per wavefront");
+        const int u = f % GW, w = task * (F::G / GW) + f / GW;
+        return (w / D) * (GW * D) + u * D + (w % D);
+    }
+}
+template <class F> __host__ __device__ __forceinline__ int ycol_tasks(int n_multi)
+{
+    constexpr int GW = F::LW / F::P2 < 1 ? 1 : F::LW / F::P2, D = F::P2 / GW;
+    constexpr int BLK = (GW <= 1 || D <= 1) ? 1 : GW * D;
+    return ((n_multi + BLK - 1) / BLK * BLK + F::G - 1) / F::G;
+}
+
 // signed frequency held by lane t in slot j (slot P1/2 of lane 0 is the -M/2 alias; +M/2 is extra)
 template <class F> __device__ __forceinline__ int ks_of(int t, int j) { return t + F::P2 * j - (j >= F::P1 / 2 ? F::M : 0); }
 // order-2P1 root index of the e = 1 pre-twiddle of slot j (the sign of the wrapped half is folded in)

@@ -113,14 +113,14 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
     const int nx = pl.nxocc, k1lo = pl.k1lo;
     const bool l0 = (t == 0);
     const int n_one = nx - pl.n_multi;
-    const int ntask_y = (pl.n_multi + G - 1) / G;
+    const int ntask_y = ycol_tasks<F>(pl.n_multi);
     const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
 
     // column group of this lane in y task `task`
     struct YCol { bool act; int col; int4 co; };
     auto ycol = [&](int task) -> YCol {
         YCol c;
-        const int ci = task * G + f;
+        const int ci = ycol_index<F>(task, f);
         c.act = task < ntask_y && ci < pl.n_multi;
         c.col = ct.perm[c.act ? ci : 0];
         c.co = ct.col[c.col];

@@ -81,14 +81,14 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     for (int e = 0; e < 4; ++e) wt[e] = tw[e * t]; // W^{e t}
     const int nx = pl.nxocc, k1lo = pl.k1lo;
     const int n_one = nx - pl.n_multi;
-    const int ntask_y = (pl.n_multi + G - 1) / G;
+    const int ntask_y = ycol_tasks<F>(pl.n_multi);
     const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int ytasks_w = ntask_y > warp ? (ntask_y - warp + NW - 1) / NW : 0; // y tasks of this warp per quarter
 
     struct YCol { bool act; int col; int4 co; };
     auto ycol = [&](int task) -> YCol {
         YCol c;
-        const int ci = task * G + f;
+        const int ci = ycol_index<F>(task, f);
         c.act = ci < pl.n_multi;
         c.col = ct.perm[c.act ? ci : 0];
         c.co = ct.col[c.col];
@@ -100,7 +100,7 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
         int bytes = 0;
         int4 co = make_int4(0, 0, 0, 0);
         if (lane < G) {
-            const int ci = task * G + lane;
+            const int ci = ycol_index<F>(task, lane);
             if (ci < pl.n_multi) {
                 co = ct.col[ct.perm[ci]];
                 // bulk copies move 16-byte multiples from 16-byte aligned addresses: for 8-byte elements the run is
@@ -302,7 +302,7 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
     const int nx = pl.nxocc, k1lo = pl.k1lo;
     const int n_one = nx - pl.n_multi;
-    const int ntask_y = (pl.n_multi + G - 1) / G;
+    const int ntask_y = ycol_tasks<F>(pl.n_multi);
     const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;
     const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;
@@ -365,7 +365,7 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             C *dst = Aout + (long long)b * a_out_stride + (long long)z * pl.pitch;
 #pragma unroll 1
             for (int task = warp; task < ntask_y; task += NW) {
-                const int ci = task * G + f;
+                const int ci = ycol_index<F>(task, f);
                 const bool act = ci < pl.n_multi;
                 const int col = ct.perm[act ? ci : 0];
                 const int4 co = ct.col[col];
@@ -466,14 +466,14 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
     for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
     const int nx = pl.nxocc, k1lo = pl.k1lo;
     const int n_one = nx - pl.n_multi;
-    const int ntask_y = (pl.n_multi + G - 1) / G;
+    const int ntask_y = ycol_tasks<F>(pl.n_multi);
     const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int ytasks_w = ntask_y > warp ? (ntask_y - warp + NW - 1) / NW : 0;
 
     struct YCol { bool act; int col; int4 co; };
     auto ycol = [&](int task) -> YCol {
         YCol c;
-        const int ci = task * G + f;
+        const int ci = ycol_index<F>(task, f);
         c.act = ci < pl.n_multi;
         c.col = ct.perm[c.act ? ci : 0];
         c.co = ct.col[c.col];
@@ -484,7 +484,7 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
         int bytes = 0;
         int4 co = make_int4(0, 0, 0, 0);
         if (lane < G) {
-            const int ci = task * G + lane;
+            const int ci = ycol_index<F>(task, lane);
             if (ci < pl.n_multi) {
                 co = ct.col[ct.perm[ci]];
                 const int sh = sizeof(C) == 8 ? (co.x & 1) : 0; // see plane_r4_inv_k
