@@ -10,6 +10,7 @@
 #include "fftb_plane_fast.cuh"
 #include "fftb_plane_pf.cuh"
 #include "fftb_plane_r4.cuh"
+#include "fftb_zpass_pf.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -241,22 +242,54 @@ bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)
     return false;
 }
 
+// resident CTAs per SM of a persistent z-pass kernel (shared memory decides: 3 at N3 = 64, 128; 2 at 96)
+template <class K> static int zpers_grid(K kp, size_t smem, int total)
+{
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kp, FAST_NW * 32, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    const int cap = sm_count() * per_sm;
+    return total < cap ? total : cap;
+}
+
 template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
 {
-    auto k = zpass_fast_inv_k<T, F, FAST_NW>;
-    const size_t smem = ZFast<T, F, FAST_NW>::smem_bytes;
-    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-    dim3 grid((pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), nb);
-    k<<<grid, FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
+    const int ntiles = (pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW);
+    if constexpr (sizeof(cx<T>) == 16) {
+        // 16-byte elements: persistent kernel, global memory moved by the TMA engine only
+        using ZP = ZPers<T, F, FAST_NW>;
+        auto kp = zpass_pers_inv_k<T, F, FAST_NW>;
+        static int grid_cap = 0;
+        if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
+        if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
+        const int total = ntiles * nb;
+        kp<<<total < grid_cap ? total : grid_cap, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
+    } else {
+        auto k = zpass_fast_inv_k<T, F, FAST_NW>;
+        const size_t smem = ZFast<T, F, FAST_NW>::smem_bytes;
+        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+        k<<<dim3(ntiles, nb), FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
+    }
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
 {
+    const int ntiles = (pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW);
+    if constexpr (sizeof(cx<T>) == 16) {
+        if (pl.ry == 1) { // one plane of A (fast plane kernels): persistent kernel
+            using ZP = ZPers<T, F, FAST_NW>;
+            auto kp = zpass_pers_fwd_k<T, F, FAST_NW>;
+            static int grid_cap = 0;
+            if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
+            if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
+            const int total = ntiles * nb;
+            kp<<<total < grid_cap ? total : grid_cap, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
+            return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+        }
+    }
     auto k = zpass_fast_fwd_k<T, F, FAST_NW>;
     const size_t smem = ZFast<T, F, FAST_NW>::smem_bytes;
     if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-    dim3 grid((pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), nb);
-    k<<<grid, FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);
+    k<<<dim3(ntiles, nb), FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 template <typename T, int N, int P1, int P2> ZLaunch make_z_fast()

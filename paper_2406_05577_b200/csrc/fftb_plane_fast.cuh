@@ -176,14 +176,36 @@ __device__ __forceinline__ void sub_fwd(cx<T> (&y)[F::B2][F::P2], cx<T> (&x)[F::
 // ---------------------------------------------------------------------------------------------
 template <typename T, class F, int NW> struct ZFast {
     static constexpr int TS = F::G * NW;
-    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)F::N * TS + (size_t)NW * F::EXW);
     // a shared-memory wavefront covers GW = LW / P2 lane groups (sticks) x P2 lanes (rows z, z+2, ...): the row
     // rotation steps by GW so that those LW accesses fall into different banks in either precision
     static constexpr int GW = F::LW / F::P2 < 1 ? 1 : F::LW / F::P2;
     static_assert(TS >= F::LW, "tile row shorter than a wavefront");
     __device__ static __forceinline__ int rot(int z) { return (z >> 1) * GW; }
     __device__ static __forceinline__ int swz(int z, int sl) { return z * TS + ((sl + rot(z)) & (TS - 1)); }
+    // tile of the persistent kernels (fftb_zpass_pf.cuh; rows move by TMA bulk copies, so every row must be one
+    // contiguous, 16-byte aligned run):
+    // the rows z = 2m, 2m + 1 form a pair of pitch RP = 2 TS + GW elements; the P2 lanes of a group write the
+    // rows z, z + 2, ... of one column, GW groups per wavefront the neighbouring columns: (m RP + sl) mod LW
+    // takes LW different values
+    static constexpr int RP = 2 * TS + GW;
+    static_assert((RP * sizeof(cx<T>)) % 16 == 0 && (TS * sizeof(cx<T>)) % 16 == 0, "bulk copies need 16-byte aligned rows");
+    __device__ static __forceinline__ int lin(int z, int sl) { return (z >> 1) * RP + (z & 1) * TS + sl; }
+    static constexpr int TILE = (F::N / 2) * RP; // >= N TS: both layouts fit
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)TILE + (size_t)NW * F::EXW);
 };
+
+// TMA bulk store shared -> global (bulk async-group completion)
+__device__ __forceinline__ void bulk_store(void *gdst, const void *ssrc, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst),
+                 "r"((unsigned)__cvta_generic_to_shared(ssrc)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_store_commit_wait_read()
+{
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
 
 // One tile (TS consecutive sticks starting at s0 = j TS) of one band, called by all NW warps of a CTA;
 // `smem` holds the tile [N][TS] and the warps' exchange tiles (ZFast::smem_bytes); tws / g are the caller's
@@ -199,7 +221,7 @@ __device__ __forceinline__ void z_inv_tile(const DevPlan &pl, const cx<T> *__res
     C *tile = smem; // [N][TS], swizzled
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    const ExTile<T, P2> ex{tile + N * TS + warp * F::EXW + f * F::FS};
+    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
     const int s0 = j * TS, sl = warp * G + f, s = s0 + sl;
     const bool act = s < pl.nsticks;
     const int4 st = pl.stick[act ? s : 0]; // {off, k3lo, len, .}
@@ -228,8 +250,8 @@ __device__ __forceinline__ void z_inv_tile(const DevPlan &pl, const cx<T> *__res
     for (int bb = 0; bb < B2; ++bb)
 #pragma unroll
         for (int q = 0; q < P2; ++q) tile[Z::swz(2 * ((t + P2 * bb) + P1 * q) + 1, sl)] = y[bb][q];
-    __syncthreads();
     C *dst = A_band + s0;
+    __syncthreads();
 #pragma unroll 4
     for (int i = tid; i < N * TS; i += NT) {
         const int z = i / TS, c = i % TS;
@@ -248,7 +270,7 @@ __device__ __forceinline__ void z_fwd_tile(const DevPlan &pl, const cx<T> *__res
     C *tile = smem;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    const ExTile<T, P2> ex{tile + N * TS + warp * F::EXW + f * F::FS};
+    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
     const int s0 = j * TS, sl = warp * G + f, s = s0 + sl;
     const bool act = s < pl.nsticks;
     // ---- A[z][s0 .. s0+TS) -> tile, summing the ry partial planes of the generic forward plane kernel

@@ -1,0 +1,214 @@
+// fftb_zpass_pf.cuh -- persistent z passes of the fast path for 16-byte elements (sm_100a).
+//
+// Same transform and the same tile as zpass_fast_inv_k (fftb_plane_fast.cuh; unpack I1 + pruned z-DFT I2 + layout
+// change I3 of SURVEY.md 8(a), PAPER.md:96 Fig. 3, :112), but global memory is touched by the TMA engine only:
+//   * the packed values of the TS consecutive sticks of a tile are ONE contiguous range of the band (CSR offsets,
+//     PAPER.md:183-185); it is requested into a landing zone one tile ahead (cp.async.bulk + mbarrier), so no warp
+//     waits for a global load with a scoreboard slot;
+//   * the rows of the tile leave as bulk stores (one 16 TS byte run per z row).
+// A CTA loops over the tiles w = blockIdx.x, blockIdx.x + gridDim.x, ... of the whole batch (w = band * ntiles + j).
+#pragma once
+#include "fftb_plane_pf.cuh"
+
+namespace fftb {
+
+template <typename T, class F, int NW> struct ZPers {
+    using Z = ZFast<T, F, NW>;
+    static constexpr int LZ = Z::TS * (F::M + 1);   // landing zone: TS sticks of at most M + 1 values
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)Z::TILE + (size_t)NW * F::EXW + (size_t)LZ);
+    static constexpr int CTAS_PER_SM = 3;
+};
+
+template <typename T, class F, int NW>
+__global__ void __launch_bounds__(NW * 32, ZPers<T, F, NW>::CTAS_PER_SM)
+zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride,
+                 int ntiles, int total)
+{
+    using C = cx<T>;
+    using Z = ZFast<T, F, NW>;
+    static_assert(sizeof(C) == 16, "bulk copies of packed ranges need 16-byte elements");
+    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
+    C *land = tile + Z::TILE + NW * F::EXW;               // packed values of the tile's sticks
+    __shared__ __align__(8) unsigned long long bar;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
+    const int sl = warp * G + f;
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    C tws[P1];
+#pragma unroll
+    for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
+    tws[0] = mk<T>((T)1, (T)0);
+    const C g = tw[t];
+
+    // thread 0: ask for the packed range of tile w
+    auto issue = [&](int w) {
+        const int band = w / ntiles, s0 = (w % ntiles) * TS, s1 = s0 + TS;
+        const long long e0 = pl.stick[s0].x, e1 = s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S;
+        const unsigned bytes = (unsigned)((e1 - e0) * (long long)sizeof(C));
+        mbar_expect_tx(&bar, bytes);
+        bulk_load(land, packed + (long long)band * pl.S + e0, bytes, &bar);
+    };
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int w = blockIdx.x;
+    if (tid == 0 && w < total) issue(w);
+    unsigned par = 0;
+#pragma unroll 1
+    for (; w < total; w += gridDim.x) {
+        const int band = w / ntiles, s0 = (w % ntiles) * TS, s = s0 + sl;
+        const bool act = s < pl.nsticks;
+        const int4 st = pl.stick[act ? s : s0]; // {off, k3lo, len, .}
+        const int base = pl.stick[s0].x;
+        mbar_wait(&bar, par);
+        par ^= 1u;
+        const C *src = land + (st.x - base);
+        C x[P1], xs[P1];
+#pragma unroll
+        for (int jj = 0; jj < P1; ++jj) {
+            const int idx = ks_of<F>(t, jj) - st.y;
+            x[jj] = (act && (unsigned)idx < (unsigned)st.z) ? src[idx] : czero<T>();
+        }
+        const int idb = M / 2 - st.y;
+        const C bv = (act && t == 0 && (unsigned)idb < (unsigned)st.z) ? src[idb] : czero<T>();
+        // the previous tile's bulk stores must have read the tile before it is overwritten
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads(); // every thread holds its inputs: the landing zone may be refilled, the tile rewritten
+        if (tid == 0 && w + (int)gridDim.x < total) issue(w + (int)gridDim.x);
+#pragma unroll
+        for (int jj = 0; jj < P1; ++jj) xs[jj] = x[jj];
+        xs[P1 / 2] = cadd(xs[P1 / 2], bv);
+        C y[B2][P2];
+        sub_inv<F, T>(xs, y, tws, ex, t);
+#pragma unroll
+        for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+            for (int q = 0; q < P2; ++q) tile[Z::lin(2 * ((t + P2 * bb) + P1 * q), sl)] = y[bb][q];
+        x[P1 / 2] = csub(x[P1 / 2], bv);
+        pre_inv<F, 0, T>(x, g);
+        sub_inv<F, T>(x, y, tws, ex, t);
+#pragma unroll
+        for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+            for (int q = 0; q < P2; ++q) tile[Z::lin(2 * ((t + P2 * bb) + P1 * q) + 1, sl)] = y[bb][q];
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        C *dst = A + (long long)band * a_band_stride + s0;
+        const int ncol = pl.pitch - s0 < TS ? pl.pitch - s0 : TS;
+        for (int z = tid; z < N; z += NT) bulk_store(dst + (long long)z * pl.pitch, tile + Z::lin(z, 0), (unsigned)(ncol * sizeof(C)));
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+
+// Forward (F5 z-DFT keeping the stick's k3, scale, F6 pack): the N rows A[z][s0 .. s0 + TS) of the next tile are
+// requested as bulk loads as soon as every thread holds its tile values; the results of a tile are collected in the
+// landing zone in packed order and leave as ONE bulk store (the packed range of TS consecutive sticks is contiguous).
+// Only for one plane of A (ry == 1).
+template <typename T, class F, int NW>
+__global__ void __launch_bounds__(NW * 32, ZPers<T, F, NW>::CTAS_PER_SM)
+zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride,
+                 int ntiles, int total)
+{
+    using C = cx<T>;
+    using Z = ZFast<T, F, NW>;
+    static_assert(sizeof(C) == 16, "bulk copies of packed ranges need 16-byte elements");
+    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
+    C *land = tile + Z::TILE + NW * F::EXW;               // results of the tile's sticks in packed order
+    __shared__ __align__(8) unsigned long long bar;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
+    const int sl = warp * G + f;
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    C tws[P1];
+#pragma unroll
+    for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
+    tws[0] = mk<T>((T)1, (T)0);
+    const C g = tw[t];
+    const T scale = (T)pl.scale;
+
+    auto ncol_of = [&](int s0) { return pl.pitch - s0 < TS ? pl.pitch - s0 : TS; };
+    // thread 0 announces the bytes of tile w, then (after a CTA barrier) every thread asks for its rows
+    auto expect = [&](int w) { mbar_expect_tx(&bar, (unsigned)(N * ncol_of((w % ntiles) * TS) * (int)sizeof(C))); };
+    auto issue_rows = [&](int w) {
+        const int band = w / ntiles, s0 = (w % ntiles) * TS;
+        const C *src = A + (long long)band * a_band_stride + s0;
+        const unsigned bytes = (unsigned)(ncol_of(s0) * (int)sizeof(C));
+        for (int z = tid; z < N; z += NT) bulk_load(tile + Z::lin(z, 0), src + (long long)z * pl.pitch, bytes, &bar);
+    };
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int w = blockIdx.x;
+    if (w < total) {
+        if (tid == 0) expect(w);
+        __syncthreads();
+        issue_rows(w);
+    }
+    unsigned par = 0;
+#pragma unroll 1
+    for (; w < total; w += gridDim.x) {
+        const int band = w / ntiles, s0 = (w % ntiles) * TS, s = s0 + sl;
+        const bool act = s < pl.nsticks;
+        const int4 st = pl.stick[act ? s : s0];
+        const long long e0 = pl.stick[s0].x, e1 = s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S;
+        const bool more = w + (int)gridDim.x < total;
+        mbar_wait(&bar, par);
+        par ^= 1u;
+        C y[B2][P2], y1[B2][P2], g0[P1], g1[P1];
+#pragma unroll
+        for (int bb = 0; bb < B2; ++bb)
+#pragma unroll
+            for (int q = 0; q < P2; ++q) {
+                y[bb][q] = tile[Z::lin(2 * ((t + P2 * bb) + P1 * q), sl)];
+                y1[bb][q] = tile[Z::lin(2 * ((t + P2 * bb) + P1 * q) + 1, sl)];
+            }
+        // the previous tile's packed store must have read the landing zone before it is rewritten
+        if (tid == 0) {
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            if (more) expect(w + (int)gridDim.x);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads(); // every thread holds its tile values: the next tile's rows may land
+        if (more) issue_rows(w + (int)gridDim.x);
+        sub_fwd<F, T>(y, g0, tws, ex, t);
+        sub_fwd<F, T>(y1, g1, tws, ex, t);
+        post_fwd<F, 0, T>(g1, g);
+        if (act) {
+            C *dst = land + (st.x - (int)e0);
+            const int idb = M / 2 - st.y;
+            if (t == 0 && (unsigned)idb < (unsigned)st.z) {
+                const C v = csub(g0[P1 / 2], g1[P1 / 2]);
+                dst[idb] = mk<T>(v.x * scale, v.y * scale);
+            }
+#pragma unroll
+            for (int jj = 0; jj < P1; ++jj) {
+                const int idx = ks_of<F>(t, jj) - st.y;
+                if ((unsigned)idx < (unsigned)st.z) {
+                    const C v = cadd(g0[jj], g1[jj]);
+                    dst[idx] = mk<T>(v.x * scale, v.y * scale);
+                }
+            }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (tid == 0) {
+            bulk_store(packed + (long long)band * pl.S + e0, land, (unsigned)((e1 - e0) * (long long)sizeof(C)));
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+    }
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+
+} // namespace fftb
