@@ -253,40 +253,29 @@ template <class K> static int zpers_grid(K kp, size_t smem, int total)
 
 template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
 {
-    const int ntiles = (pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW);
-    if constexpr (sizeof(cx<T>) == 16) {
-        // 16-byte elements: persistent kernel, global memory moved by the TMA engine only
-        using ZP = ZPers<T, F, FAST_NW>;
-        auto kp = zpass_pers_inv_k<T, F, FAST_NW>;
-        static int grid_cap = 0;
-        if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
-        if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
-        const int total = ntiles * nb;
-        kp<<<total < grid_cap ? total : grid_cap, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
-    } else {
-        auto k = zpass_fast_inv_k<T, F, FAST_NW>;
-        const size_t smem = ZFast<T, F, FAST_NW>::smem_bytes;
-        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-        k<<<dim3(ntiles, nb), FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
-    }
+    // persistent kernel, global memory moved by the TMA engine only
+    const int ntiles = (pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), total = ntiles * nb;
+    using ZP = ZPers<T, F, FAST_NW>;
+    auto kp = zpass_pers_inv_k<T, F, FAST_NW>;
+    static int grid_cap = 0;
+    if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
+    if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
+    kp<<<total < grid_cap ? total : grid_cap, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
 {
-    const int ntiles = (pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW);
-    if constexpr (sizeof(cx<T>) == 16) {
-        if (pl.ry == 1) { // one plane of A (fast plane kernels): persistent kernel
-            using ZP = ZPers<T, F, FAST_NW>;
-            auto kp = zpass_pers_fwd_k<T, F, FAST_NW>;
-            static int grid_cap = 0;
-            if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
-            if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
-            const int total = ntiles * nb;
-            kp<<<total < grid_cap ? total : grid_cap, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
-            return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
-        }
+    const int ntiles = (pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), total = ntiles * nb;
+    if (pl.ry == 1) { // one plane of A (fast plane kernels): persistent kernel
+        using ZP = ZPers<T, F, FAST_NW>;
+        auto kp = zpass_pers_fwd_k<T, F, FAST_NW>;
+        static int grid_cap = 0;
+        if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
+        if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
+        kp<<<total < grid_cap ? total : grid_cap, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
+        return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
     }
-    auto k = zpass_fast_fwd_k<T, F, FAST_NW>;
+    auto k = zpass_fast_fwd_k<T, F, FAST_NW>; // partial planes of the generic plane kernel are summed here
     const size_t smem = ZFast<T, F, FAST_NW>::smem_bytes;
     if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
     k<<<dim3(ntiles, nb), FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);

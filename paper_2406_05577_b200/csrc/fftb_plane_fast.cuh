@@ -209,57 +209,8 @@ __device__ __forceinline__ void bulk_store_commit_wait_read()
 
 // One tile (TS consecutive sticks starting at s0 = j TS) of one band, called by all NW warps of a CTA;
 // `smem` holds the tile [N][TS] and the warps' exchange tiles (ZFast::smem_bytes); tws / g are the caller's
-// twiddle registers for the z axis.  Both contain CTA barriers; the caller must put one more between
-// two calls (or any other use of `smem`).
-template <typename T, class F, int NW>
-__device__ __forceinline__ void z_inv_tile(const DevPlan &pl, const cx<T> *__restrict__ packed_band, cx<T> *__restrict__ A_band, int j,
-                                           cx<T> *smem, const cx<T> (&tws)[F::P1], cx<T> g)
-{
-    using C = cx<T>;
-    using Z = ZFast<T, F, NW>;
-    constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
-    C *tile = smem; // [N][TS], swizzled
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int f = lane / P2, t = lane % P2;
-    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
-    const int s0 = j * TS, sl = warp * G + f, s = s0 + sl;
-    const bool act = s < pl.nsticks;
-    const int4 st = pl.stick[act ? s : 0]; // {off, k3lo, len, .}
-    const C *src = packed_band + st.x;
-    C x[P1], xs[P1];
-#pragma unroll
-    for (int jj = 0; jj < P1; ++jj) {
-        const int idx = ks_of<F>(t, jj) - st.y;
-        x[jj] = (act && (unsigned)idx < (unsigned)st.z) ? __ldcs(src + idx) : czero<T>();
-    }
-    const int idb = M / 2 - st.y;
-    const C bv = (act && t == 0 && (unsigned)idb < (unsigned)st.z) ? __ldcs(src + idb) : czero<T>();
-#pragma unroll
-    for (int jj = 0; jj < P1; ++jj) xs[jj] = x[jj];
-    xs[P1 / 2] = cadd(xs[P1 / 2], bv);
-    C y[B2][P2];
-    sub_inv<F, T>(xs, y, tws, ex, t);
-#pragma unroll
-    for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-        for (int q = 0; q < P2; ++q) tile[Z::swz(2 * ((t + P2 * bb) + P1 * q), sl)] = y[bb][q];
-    x[P1 / 2] = csub(x[P1 / 2], bv);
-    pre_inv<F, 0, T>(x, g);
-    sub_inv<F, T>(x, y, tws, ex, t);
-#pragma unroll
-    for (int bb = 0; bb < B2; ++bb)
-#pragma unroll
-        for (int q = 0; q < P2; ++q) tile[Z::swz(2 * ((t + P2 * bb) + P1 * q) + 1, sl)] = y[bb][q];
-    C *dst = A_band + s0;
-    __syncthreads();
-#pragma unroll 4
-    for (int i = tid; i < N * TS; i += NT) {
-        const int z = i / TS, c = i % TS;
-        const int l = (c - Z::rot(z)) & (TS - 1);
-        if (s0 + l < pl.nsticks) dst[(long long)z * pl.pitch + l] = tile[i];
-    }
-}
-
+// twiddle registers for the z axis.  Contains CTA barriers.  Forward only: the inverse z pass and the forward one
+// with a single plane of A are the persistent kernels of fftb_zpass_pf.cuh.
 template <typename T, class F, int NW>
 __device__ __forceinline__ void z_fwd_tile(const DevPlan &pl, const cx<T> *__restrict__ A_band, cx<T> *__restrict__ packed_band, int j,
                                            cx<T> *smem, const cx<T> (&tws)[F::P1], cx<T> g)
@@ -333,23 +284,7 @@ __device__ __forceinline__ void z_fwd_tile(const DevPlan &pl, const cx<T> *__res
     }
 }
 
-// stand-alone z-pass kernels: one tile per CTA, grid = (ceil(n_sticks / TS), bands)
-template <typename T, class F, int NW>
-__global__ void __launch_bounds__(NW * 32, F::P1 > 16 ? 2 : 16 / NW)
-zpass_fast_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride)
-{
-    using C = cx<T>;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int t = (threadIdx.x & 31) % F::P2;
-    const C *tw = reinterpret_cast<const C *>(pl.tw3);
-    C tws[F::P1];
-#pragma unroll
-    for (int m = 1; m < F::P1; ++m) tws[m] = tw[modn<F::N>(2 * t * m)];
-    tws[0] = mk<T>((T)1, (T)0);
-    z_inv_tile<T, F, NW>(pl, packed + (long long)blockIdx.y * pl.S, A + (long long)blockIdx.y * a_band_stride, blockIdx.x,
-                         reinterpret_cast<C *>(smem_raw), tws, tw[t]);
-}
-
+// stand-alone forward z-pass kernel: one tile per CTA, grid = (ceil(n_sticks / TS), bands)
 template <typename T, class F, int NW>
 __global__ void __launch_bounds__(NW * 32, F::P1 > 16 ? 2 : 16 / NW)
 zpass_fast_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride)

@@ -1,11 +1,17 @@
-// fftb_zpass_pf.cuh -- persistent z passes of the fast path for 16-byte elements (sm_100a).
+// fftb_zpass_pf.cuh -- persistent z passes of the fast path (sm_100a).
 //
-// Same transform and the same tile as zpass_fast_inv_k (fftb_plane_fast.cuh; unpack I1 + pruned z-DFT I2 + layout
-// change I3 of SURVEY.md 8(a), PAPER.md:96 Fig. 3, :112), but global memory is touched by the TMA engine only:
+// Inverse: unpack I1 + pruned z-DFT I2 + layout change I3 of SURVEY.md 8(a) (PAPER.md:96 Fig. 3, :112); forward: F5 +
+// F6.  Work item = a tile of TS consecutive sticks of one band, one group of P2 lanes per stick (sub_inv / sub_fwd of
+// fftb_plane_fast.cuh); the transposition between "one stick, all z" and the plane-major intermediate A[z][stick]
+// goes through a shared-memory tile.  Global memory is touched by the TMA engine only:
 //   * the packed values of the TS consecutive sticks of a tile are ONE contiguous range of the band (CSR offsets,
-//     PAPER.md:183-185); it is requested into a landing zone one tile ahead (cp.async.bulk + mbarrier), so no warp
-//     waits for a global load with a scoreboard slot;
-//   * the rows of the tile leave as bulk stores (one 16 TS byte run per z row).
+//     PAPER.md:183-185); the inverse kernel requests it into a landing zone one tile ahead (cp.async.bulk +
+//     mbarrier), so no warp waits for a global load with a scoreboard slot; the forward kernel collects its results
+//     there and stores the range with one bulk store;
+//   * the rows of the tile leave / arrive as bulk copies (one run of TS elements per z row).
+// complex64: a packed range may begin and end on an odd 8-byte element while bulk copies move 16-byte units; loads
+// are widened (the neighbours' values are ignored), stores cover the aligned interior and the odd edge elements are
+// stored by the lanes that own them.
 // A CTA loops over the tiles w = blockIdx.x, blockIdx.x + gridDim.x, ... of the whole batch (w = band * ntiles + j).
 #pragma once
 #include "fftb_plane_pf.cuh"
@@ -14,9 +20,10 @@ namespace fftb {
 
 template <typename T, class F, int NW> struct ZPers {
     using Z = ZFast<T, F, NW>;
-    static constexpr int LZ = Z::TS * (F::M + 1);   // landing zone: TS sticks of at most M + 1 values
+    static constexpr int EA = 16 / (int)sizeof(cx<T>);      // elements per 16 bytes, the granularity of a bulk copy
+    static constexpr int LZ = Z::TS * (F::M + 1) + 2 * (EA - 1); // landing zone: TS sticks of at most M + 1 values (+ alignment slack)
     static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)Z::TILE + (size_t)NW * F::EXW + (size_t)LZ);
-    static constexpr int CTAS_PER_SM = 3;
+    static constexpr int CTAS_PER_SM = F::P1 > 16 ? 2 : 3;
 };
 
 template <typename T, class F, int NW>
@@ -26,8 +33,8 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
 {
     using C = cx<T>;
     using Z = ZFast<T, F, NW>;
-    static_assert(sizeof(C) == 16, "bulk copies of packed ranges need 16-byte elements");
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
+    constexpr long long EA = ZPers<T, F, NW>::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
     C *land = tile + Z::TILE + NW * F::EXW;               // packed values of the tile's sticks
@@ -43,13 +50,31 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
     tws[0] = mk<T>((T)1, (T)0);
     const C g = tw[t];
 
-    // thread 0: ask for the packed range of tile w
-    auto issue = [&](int w) {
-        const int band = w / ntiles, s0 = (w % ntiles) * TS, s1 = s0 + TS;
-        const long long e0 = pl.stick[s0].x, e1 = s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S;
-        const unsigned bytes = (unsigned)((e1 - e0) * (long long)sizeof(C));
+    // Descriptor of tile w, loaded one iteration before it is used (the stick table is in global memory): this
+    // lane's stick and the packed range of the tile in elements of the whole batch, widened to 16-byte boundaries
+    // [a0, a1) (complex64: a range may begin and end on an odd element; the neighbours' values that come along are
+    // not used).  The batch ends at nall: an odd last element is not covered (a1 < end of the range) and is read
+    // straight from global.
+    const long long nall = (long long)(total / ntiles) * pl.S;
+    struct Tile { int4 st; long long a0, a1; int band, s0; bool act; };
+    auto describe = [&](int w) -> Tile {
+        Tile d;
+        d.band = w / ntiles, d.s0 = (w % ntiles) * TS;
+        const int s = d.s0 + sl, s1 = d.s0 + TS;
+        d.act = s < pl.nsticks;
+        d.st = pl.stick[d.act ? s : d.s0]; // {off, k3lo, len, .}
+        const long long g0 = (long long)d.band * pl.S + pl.stick[d.s0].x;
+        const long long g1 = (long long)d.band * pl.S + (s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S);
+        d.a0 = g0 & ~(EA - 1);
+        d.a1 = (g1 + EA - 1) & ~(EA - 1);
+        if (d.a1 > nall) d.a1 = nall & ~(EA - 1);
+        return d;
+    };
+    // thread 0: ask for the packed range of a tile
+    auto issue = [&](const Tile &d) {
+        const unsigned bytes = (unsigned)((d.a1 - d.a0) * (long long)sizeof(C));
         mbar_expect_tx(&bar, bytes);
-        bulk_load(land, packed + (long long)band * pl.S + e0, bytes, &bar);
+        bulk_load(land, packed + d.a0, bytes, &bar);
     };
     if (tid == 0) {
         mbar_init(&bar, 1);
@@ -57,30 +82,39 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
     }
     __syncthreads();
     int w = blockIdx.x;
-    if (tid == 0 && w < total) issue(w);
+    Tile cur = describe(w < total ? w : 0), nxt = cur;
+    if (tid == 0 && w < total) issue(cur);
     unsigned par = 0;
 #pragma unroll 1
     for (; w < total; w += gridDim.x) {
-        const int band = w / ntiles, s0 = (w % ntiles) * TS, s = s0 + sl;
-        const bool act = s < pl.nsticks;
-        const int4 st = pl.stick[act ? s : s0]; // {off, k3lo, len, .}
-        const int base = pl.stick[s0].x;
+        const bool more = w + (int)gridDim.x < total;
+        if (more) nxt = describe(w + (int)gridDim.x);
+        const int band = cur.band, s0 = cur.s0;
+        const bool act = cur.act;
+        const int4 st = cur.st;
+        const long long a0 = cur.a0, a1 = cur.a1;
         mbar_wait(&bar, par);
         par ^= 1u;
-        const C *src = land + (st.x - base);
+        const long long gs = (long long)band * pl.S + st.x; // the stick's first element in the batch
+        const C *src = land + (gs - a0);
+        const int lim = (int)(a1 - gs);                      // elements of the stick from here on are not in the landing zone
+        auto fetch = [&](int idx) -> C {
+            if constexpr (EA == 1) return src[idx];
+            else return idx < lim ? src[idx] : __ldcs(packed + gs + idx);
+        };
         C x[P1], xs[P1];
 #pragma unroll
         for (int jj = 0; jj < P1; ++jj) {
             const int idx = ks_of<F>(t, jj) - st.y;
-            x[jj] = (act && (unsigned)idx < (unsigned)st.z) ? src[idx] : czero<T>();
+            x[jj] = (act && (unsigned)idx < (unsigned)st.z) ? fetch(idx) : czero<T>();
         }
         const int idb = M / 2 - st.y;
-        const C bv = (act && t == 0 && (unsigned)idb < (unsigned)st.z) ? src[idb] : czero<T>();
+        const C bv = (act && t == 0 && (unsigned)idb < (unsigned)st.z) ? fetch(idb) : czero<T>();
         // the previous tile's bulk stores must have read the tile before it is overwritten
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads(); // every thread holds its inputs: the landing zone may be refilled, the tile rewritten
-        if (tid == 0 && w + (int)gridDim.x < total) issue(w + (int)gridDim.x);
+        if (tid == 0 && more) issue(nxt);
 #pragma unroll
         for (int jj = 0; jj < P1; ++jj) xs[jj] = x[jj];
         xs[P1 / 2] = cadd(xs[P1 / 2], bv);
@@ -103,6 +137,7 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
         const int ncol = pl.pitch - s0 < TS ? pl.pitch - s0 : TS;
         for (int z = tid; z < N; z += NT) bulk_store(dst + (long long)z * pl.pitch, tile + Z::lin(z, 0), (unsigned)(ncol * sizeof(C)));
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        cur = nxt;
     }
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
@@ -118,8 +153,8 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
 {
     using C = cx<T>;
     using Z = ZFast<T, F, NW>;
-    static_assert(sizeof(C) == 16, "bulk copies of packed ranges need 16-byte elements");
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
+    constexpr long long EA = ZPers<T, F, NW>::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
     C *land = tile + Z::TILE + NW * F::EXW;               // results of the tile's sticks in packed order
@@ -159,14 +194,19 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
     unsigned par = 0;
 #pragma unroll 1
     for (; w < total; w += gridDim.x) {
+        const bool more = w + (int)gridDim.x < total;
         const int band = w / ntiles, s0 = (w % ntiles) * TS, s = s0 + sl;
         const bool act = s < pl.nsticks;
         const int4 st = pl.stick[act ? s : s0];
-        const long long e0 = pl.stick[s0].x, e1 = s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S;
-        const bool more = w + (int)gridDim.x < total;
+        // the tile's packed range [g0, g1) in elements of the whole batch (used after the transforms: loading the table
+        // one tile ahead was measured 3% slower); its 16-byte aligned interior [b0, b1) leaves as one bulk store from the
+        // landing zone (origin al), an odd first / last element (complex64) by a plain store
+        const long long g0 = (long long)band * pl.S + pl.stick[s0].x;
+        const long long g1 = (long long)band * pl.S + (s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S);
+        const long long al = g0 & ~(EA - 1), b0 = (g0 + EA - 1) & ~(EA - 1), b1 = g1 & ~(EA - 1);
         mbar_wait(&bar, par);
         par ^= 1u;
-        C y[B2][P2], y1[B2][P2], g0[P1], g1[P1];
+        C y[B2][P2], y1[B2][P2], h0[P1], h1[P1];
 #pragma unroll
         for (int bb = 0; bb < B2; ++bb)
 #pragma unroll
@@ -182,29 +222,31 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads(); // every thread holds its tile values: the next tile's rows may land
         if (more) issue_rows(w + (int)gridDim.x);
-        sub_fwd<F, T>(y, g0, tws, ex, t);
-        sub_fwd<F, T>(y1, g1, tws, ex, t);
-        post_fwd<F, 0, T>(g1, g);
+        sub_fwd<F, T>(y, h0, tws, ex, t);
+        sub_fwd<F, T>(y1, h1, tws, ex, t);
+        post_fwd<F, 0, T>(h1, g);
         if (act) {
-            C *dst = land + (st.x - (int)e0);
+            const long long gs = (long long)band * pl.S + st.x;
+            C *dst = land + (gs - al);
+            const int lo = (int)(b0 - gs), hi = (int)(b1 - gs); // stick elements [lo, hi) belong to the bulk store
+            auto put = [&](int idx, C v) {
+                v = mk<T>(v.x * scale, v.y * scale);
+                if constexpr (EA == 1) dst[idx] = v;
+                else if (idx >= lo && idx < hi) dst[idx] = v;
+                else packed[gs + idx] = v;
+            };
             const int idb = M / 2 - st.y;
-            if (t == 0 && (unsigned)idb < (unsigned)st.z) {
-                const C v = csub(g0[P1 / 2], g1[P1 / 2]);
-                dst[idb] = mk<T>(v.x * scale, v.y * scale);
-            }
+            if (t == 0 && (unsigned)idb < (unsigned)st.z) put(idb, csub(h0[P1 / 2], h1[P1 / 2]));
 #pragma unroll
             for (int jj = 0; jj < P1; ++jj) {
                 const int idx = ks_of<F>(t, jj) - st.y;
-                if ((unsigned)idx < (unsigned)st.z) {
-                    const C v = cadd(g0[jj], g1[jj]);
-                    dst[idx] = mk<T>(v.x * scale, v.y * scale);
-                }
+                if ((unsigned)idx < (unsigned)st.z) put(idx, cadd(h0[jj], h1[jj]));
             }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
-        if (tid == 0) {
-            bulk_store(packed + (long long)band * pl.S + e0, land, (unsigned)((e1 - e0) * (long long)sizeof(C)));
+        if (tid == 0 && b1 > b0) {
+            bulk_store(packed + b0, land + (b0 - al), (unsigned)((b1 - b0) * (long long)sizeof(C)));
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
     }

@@ -431,3 +431,28 @@ def test_host_buffer_calls_pipelined(fb, oracle):
     sample = [0, 21, 42]
     ref = oracle.apply_vloc(w.n, k, c[sample], v, 1.0 / float(np.prod(w.n)))
     assert _rel(h_o.numpy()[sample], ref) <= w.tol
+
+
+@pytest.mark.parametrize("n,a", [((64, 64, 64), (16, 16, 16)), ((128, 128, 128), (32, 32, 32)), ((96, 96, 192), (24, 24, 48))],
+                         ids=["64", "128", "96x96x192"])
+def test_complex64_odd_packed_ranges(fb, oracle, n, a):
+    """complex64 z passes move the packed ranges of a tile by 16-byte bulk copies although a range may begin and end on
+    an odd 8-byte element: S and nb odd, so ranges of both parities occur and the batch itself ends on an odd element;
+    the packed output sits between sentinels that must survive (no store outside [0, nb S))."""
+    w = _small(n, a, dtype="c64", batch=3)
+    p = _plan(fb, w, 3)
+    assert p.S % 2 == 1
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    d_psi = p.inverse(torch.from_numpy(c).cuda())
+    torch.cuda.synchronize()
+    assert _rel(d_psi.cpu().numpy(), oracle.inverse(w.n, k, c)) <= w.tol
+    guard = 2  # complex64 elements = 16 bytes: the view stays 16-byte aligned
+    buf = torch.full((guard + 3 * p.S + guard,), 777.0 - 555.0j, dtype=torch.complex64, device="cuda")
+    out = buf[guard:guard + 3 * p.S].view(3, p.S)
+    p.forward(d_psi, out)
+    torch.cuda.synchronize()
+    h = buf.cpu().numpy()
+    assert (h[:guard] == np.complex64(777.0 - 555.0j)).all() and (h[-guard:] == np.complex64(777.0 - 555.0j)).all()
+    assert _rel(h[guard:-guard].reshape(3, p.S), c) <= w.tol
+    p.destroy()
