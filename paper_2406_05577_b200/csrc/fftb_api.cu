@@ -290,11 +290,13 @@ template <typename T, int N, int P1, int P2> ZLaunch make_z_fast()
 constexpr int R4Z_NW = 4;
 template <typename T> int launch_zr4_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
 {
-    auto k = zpass_r4_inv_k<T, R4Z_NW>;
-    const size_t smem = ZR4<T, R4Z_NW>::smem_bytes;
-    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-    dim3 grid((pl.nsticks + ZR4<T, R4Z_NW>::TS - 1) / ZR4<T, R4Z_NW>::TS, nb);
-    k<<<grid, R4Z_NW * 32, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
+    using ZP = ZPersR4<T, R4Z_NW>;
+    auto kp = zpass_r4_pers_inv_k<T, R4Z_NW>;
+    const int ntiles = (pl.nsticks + ZP::TS - 1) / ZP::TS, total = ntiles * nb;
+    static int grid_cap = 0;
+    if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
+    if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
+    kp<<<total < grid_cap ? total : grid_cap, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
     return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
 }
 template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)

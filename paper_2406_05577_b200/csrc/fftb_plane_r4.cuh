@@ -717,66 +717,6 @@ template <typename T, int NW> struct ZR4 {
 
 template <typename T, int NW>
 __global__ void __launch_bounds__(NW * 32, 2)
-zpass_r4_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride)
-{
-    using C = cx<T>;
-    using Z = ZR4<T, NW>;
-    using F = typename Z::F;
-    constexpr int N = Z::N, M = Z::M, P2 = F::P2, G = F::G, TS = Z::TS, NT = NW * 32;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    C *tile = reinterpret_cast<C *>(smem_raw); // [N][TS], swizzled
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int f = lane / P2, t = lane % P2;
-    const ExTile<T, P2> ex{tile + N * TS + warp * F::EXW + f * F::FS};
-    const C *tw = reinterpret_cast<const C *>(pl.tw3);
-    const int s0 = blockIdx.x * TS, sl = warp * G + f, s = s0 + sl;
-    const bool act = s < pl.nsticks;
-    const int4 st = pl.stick[act ? s : 0]; // {off, k3lo, len, .}
-    const C *src = packed + (long long)blockIdx.y * pl.S + st.x;
-    C a[8], bq[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        const int ia = (t + 8 * j) - M - st.y, ib = (t + 8 * j) - st.y;
-        a[j] = (act && (unsigned)ia < (unsigned)st.z) ? __ldcs(src + ia) : czero<T>();
-        bq[j] = (act && (unsigned)ib < (unsigned)st.z) ? __ldcs(src + ib) : czero<T>();
-    }
-    const int ic = M - st.y;
-    const C cv = (act && t == 0 && (unsigned)ic < (unsigned)st.z) ? __ldcs(src + ic) : czero<T>();
-    C tws[8], wt[4];
-#pragma unroll
-    for (int m = 1; m < 8; ++m) tws[m] = tw[(4 * t * m) & (N - 1)];
-    tws[0] = mk<T>((T)1, (T)0);
-#pragma unroll
-    for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
-    C u[8], y[1][8];
-    r4_fold_inv<0, 0, T>(a, bq, cv, u, wt[0]);
-    sub_inv<F, T>(u, y, tws, ex, t);
-#pragma unroll
-    for (int q = 0; q < 8; ++q) tile[Z::swz(4 * (t + 8 * q), sl)] = y[0][q];
-    r4_fold_inv<1, 0, T>(a, bq, cv, u, wt[1]);
-    sub_inv<F, T>(u, y, tws, ex, t);
-#pragma unroll
-    for (int q = 0; q < 8; ++q) tile[Z::swz(4 * (t + 8 * q) + 1, sl)] = y[0][q];
-    r4_fold_inv<2, 0, T>(a, bq, cv, u, wt[2]);
-    sub_inv<F, T>(u, y, tws, ex, t);
-#pragma unroll
-    for (int q = 0; q < 8; ++q) tile[Z::swz(4 * (t + 8 * q) + 2, sl)] = y[0][q];
-    r4_fold_inv<3, 0, T>(a, bq, cv, u, wt[3]);
-    sub_inv<F, T>(u, y, tws, ex, t);
-#pragma unroll
-    for (int q = 0; q < 8; ++q) tile[Z::swz(4 * (t + 8 * q) + 3, sl)] = y[0][q];
-    __syncthreads();
-    C *dst = A + (long long)blockIdx.y * a_band_stride + s0;
-#pragma unroll 4
-    for (int i = tid; i < N * TS; i += NT) {
-        const int z = i / TS, c = i % TS;
-        const int l = (c - Z::rot(z)) & (TS - 1);
-        if (s0 + l < pl.nsticks) dst[(long long)z * pl.pitch + l] = tile[i];
-    }
-}
-
-template <typename T, int NW>
-__global__ void __launch_bounds__(NW * 32, 2)
 zpass_r4_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride)
 {
     using C = cx<T>;

@@ -15,6 +15,7 @@
 // A CTA loops over the tiles w = blockIdx.x, blockIdx.x + gridDim.x, ... of the whole batch (w = band * ntiles + j).
 #pragma once
 #include "fftb_plane_pf.cuh"
+#include "fftb_plane_r4.cuh"
 
 namespace fftb {
 
@@ -251,6 +252,141 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
         }
     }
     if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
+// 256 pattern (four-way split z = 4 n' + e, fftb_plane_r4.cuh): the same persistent schedule, but a tile of all 256
+// rows (66 KB) next to the landing zone (16 x 129 values) would leave one CTA per SM, so the shared-memory tile
+// holds HALF of the rows: the residues e = 0, 1 are transformed, written and sent; the residues e = 2, 3 are
+// transformed while the TMA engine reads the tile and take its place.  Row (n', e & 1) of a half sits at
+// n' RP + (e & 1) TS (ZFast::lin with z = 2 n' + (e & 1)).
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NW> struct ZPersR4 {
+    using F = FastCfg<T, 128, 8, 8>;
+    using Z = ZFast<T, F, NW>;                               // tile of 128 rows = half of the 256
+    static constexpr int N = 256, M = 64, TS = Z::TS;
+    static constexpr int EA = 16 / (int)sizeof(cx<T>);
+    static constexpr int LZ = TS * (2 * M + 1) + 2 * (EA - 1);
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)Z::TILE + (size_t)NW * F::EXW + (size_t)LZ);
+};
+
+template <typename T, int NW>
+__global__ void __launch_bounds__(NW * 32, 2)
+zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride,
+                    int ntiles, int total)
+{
+    using C = cx<T>;
+    using ZP = ZPersR4<T, NW>;
+    using F = typename ZP::F;
+    using Z = typename ZP::Z;
+    constexpr int M = ZP::M, P2 = F::P2, G = F::G, TS = ZP::TS, NT = NW * 32;
+    constexpr long long EA = ZP::EA;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *tile = reinterpret_cast<C *>(smem_raw);            // half tile: rows (n', e & 1)
+    C *land = tile + Z::TILE + NW * F::EXW;               // packed values of the tile's sticks
+    __shared__ __align__(8) unsigned long long bar;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
+    const int sl = warp * G + f;
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    C tws[8], wt[4];
+#pragma unroll
+    for (int m = 1; m < 8; ++m) tws[m] = tw[(4 * t * m) & (ZP::N - 1)];
+    tws[0] = mk<T>((T)1, (T)0);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
+
+    const long long nall = (long long)(total / ntiles) * pl.S;
+    auto range = [&](int w, long long &a0, long long &a1) { // see zpass_pers_inv_k
+        const int band = w / ntiles, s0 = (w % ntiles) * TS, s1 = s0 + TS;
+        const long long g0 = (long long)band * pl.S + pl.stick[s0].x;
+        const long long g1 = (long long)band * pl.S + (s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S);
+        a0 = g0 & ~(EA - 1);
+        a1 = (g1 + EA - 1) & ~(EA - 1);
+        if (a1 > nall) a1 = nall & ~(EA - 1);
+    };
+    auto issue = [&](int w) {
+        long long a0, a1;
+        range(w, a0, a1);
+        const unsigned bytes = (unsigned)((a1 - a0) * (long long)sizeof(C));
+        mbar_expect_tx(&bar, bytes);
+        bulk_load(land, packed + a0, bytes, &bar);
+    };
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int w = blockIdx.x;
+    if (tid == 0 && w < total) issue(w);
+    unsigned par = 0;
+#pragma unroll 1
+    for (; w < total; w += gridDim.x) {
+        const int band = w / ntiles, s0 = (w % ntiles) * TS, s = s0 + sl;
+        const bool act = s < pl.nsticks;
+        const int4 st = pl.stick[act ? s : s0]; // {off, k3lo, len, .}
+        long long a0, a1;
+        range(w, a0, a1);
+        mbar_wait(&bar, par);
+        par ^= 1u;
+        const long long gs = (long long)band * pl.S + st.x;
+        const C *src = land + (gs - a0);
+        const int lim = (int)(a1 - gs);
+        auto fetch = [&](int idx) -> C {
+            if constexpr (EA == 1) return src[idx];
+            else return idx < lim ? src[idx] : __ldcs(packed + gs + idx);
+        };
+        C a[8], bq[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int ia = (t + 8 * j) - M - st.y, ib = (t + 8 * j) - st.y;
+            a[j] = (act && (unsigned)ia < (unsigned)st.z) ? fetch(ia) : czero<T>();
+            bq[j] = (act && (unsigned)ib < (unsigned)st.z) ? fetch(ib) : czero<T>();
+        }
+        const int ic = M - st.y;
+        const C cv = (act && t == 0 && (unsigned)ic < (unsigned)st.z) ? fetch(ic) : czero<T>();
+        // the previous tile's second half must have left the tile
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads(); // every thread holds its inputs: the landing zone may be refilled, the tile rewritten
+        if (tid == 0 && w + (int)gridDim.x < total) issue(w + (int)gridDim.x);
+        C *dst = A + (long long)band * a_band_stride + s0;
+        const unsigned rbytes = (unsigned)((pl.pitch - s0 < TS ? pl.pitch - s0 : TS) * (int)sizeof(C));
+        // rows z = 4 n' + e0 + (r & 1), n' = r >> 1, of the half in the tile
+        auto send_half = [&](int e0) {
+            for (int r = tid; r < 2 * M; r += NT)
+                bulk_store(dst + (long long)(4 * (r >> 1) + e0 + (r & 1)) * pl.pitch, tile + Z::lin(r, 0), rbytes);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        };
+        C u[8], y[1][8], y2[1][8];
+        r4_fold_inv<0, 0, T>(a, bq, cv, u, wt[0]);
+        sub_inv<F, T>(u, y, tws, ex, t);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) tile[Z::lin(2 * (t + 8 * q), sl)] = y[0][q];
+        r4_fold_inv<1, 0, T>(a, bq, cv, u, wt[1]);
+        sub_inv<F, T>(u, y, tws, ex, t);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) tile[Z::lin(2 * (t + 8 * q) + 1, sl)] = y[0][q];
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        send_half(0);
+        r4_fold_inv<2, 0, T>(a, bq, cv, u, wt[2]);
+        sub_inv<F, T>(u, y, tws, ex, t);
+        r4_fold_inv<3, 0, T>(a, bq, cv, u, wt[3]);
+        sub_inv<F, T>(u, y2, tws, ex, t);
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncthreads(); // the first half has left
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            tile[Z::lin(2 * (t + 8 * q), sl)] = y[0][q];
+            tile[Z::lin(2 * (t + 8 * q) + 1, sl)] = y2[0][q];
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        send_half(2);
+    }
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
 } // namespace fftb
