@@ -301,6 +301,16 @@ template <typename T> int launch_zr4_inv(const DevPlan &pl, const void *packed, 
 }
 template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
 {
+    if (pl.ry == 1) { // one plane of A (the 256 pattern's own plane kernels): persistent kernel
+        using ZP = ZPersR4<T, R4Z_NW>;
+        auto kp = zpass_r4_pers_fwd_k<T, R4Z_NW>;
+        const int ntiles = (pl.nsticks + ZP::TS - 1) / ZP::TS, total = ntiles * nb;
+        static int grid_cap = 0;
+        if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
+        if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
+        kp<<<total < grid_cap ? total : grid_cap, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
+        return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    }
     auto k = zpass_r4_fwd_k<T, R4Z_NW>;
     const size_t smem = ZR4<T, R4Z_NW>::smem_bytes;
     if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;

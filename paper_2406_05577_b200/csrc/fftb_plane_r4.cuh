@@ -700,9 +700,11 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
 }
 
 // ---------------------------------------------------------------------------------------------
-// z passes of the 256 pattern: one group of 8 lanes per stick, TS = 4 NW sticks per CTA, the same
-// tile transposition as the z-pass kernels of fftb_plane_fast.cuh (element (z, sl) in column
-// (sl + z/4) mod TS: the strided accesses z = 4 n' + e of the transforms are conflict-free).
+// forward z pass of the 256 pattern for plans whose forward plane kernel writes partial planes of A (ry > 1: generic
+// x/y patterns next to a 256 z axis), which it sums while it fills the tile: one group of 8 lanes per stick, TS = 4 NW
+// sticks per CTA, the same tile transposition as zpass_fast_fwd_k (element (z, sl) in column (sl + z/4) mod TS: the
+// strided accesses z = 4 n' + e of the transforms are conflict-free).  The inverse z pass and the forward one with a
+// single plane of A are the persistent kernels of fftb_zpass_pf.cuh.
 //   grid = (ceil(n_sticks / TS), bands)
 // ---------------------------------------------------------------------------------------------
 template <typename T, int NW> struct ZR4 {

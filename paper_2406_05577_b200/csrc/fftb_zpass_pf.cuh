@@ -389,4 +389,131 @@ zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
+// forward z pass of the 256 pattern (one plane of A): the rows of the residues e = 0, 1 and e = 2, 3 arrive in the half
+// tile one after the other, each requested as soon as every thread holds the values of the half before it
+template <typename T, int NW>
+__global__ void __launch_bounds__(NW * 32, 2)
+zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride,
+                    int ntiles, int total)
+{
+    using C = cx<T>;
+    using ZP = ZPersR4<T, NW>;
+    using F = typename ZP::F;
+    using Z = typename ZP::Z;
+    constexpr int M = ZP::M, P2 = F::P2, G = F::G, TS = ZP::TS, NT = NW * 32;
+    constexpr long long EA = ZP::EA;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *tile = reinterpret_cast<C *>(smem_raw);            // half tile: rows (n', e & 1)
+    C *land = tile + Z::TILE + NW * F::EXW;               // results of the tile's sticks in packed order
+    __shared__ __align__(8) unsigned long long bar;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int f = lane / P2, t = lane % P2;
+    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
+    const int sl = warp * G + f;
+    const C *tw = reinterpret_cast<const C *>(pl.tw3);
+    C tws[8], wt[4];
+#pragma unroll
+    for (int m = 1; m < 8; ++m) tws[m] = tw[(4 * t * m) & (ZP::N - 1)];
+    tws[0] = mk<T>((T)1, (T)0);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
+    const T scale = (T)pl.scale;
+
+    auto ncol_of = [&](int w) { const int s0 = (w % ntiles) * TS; return pl.pitch - s0 < TS ? pl.pitch - s0 : TS; };
+    // thread 0 announces the bytes of a half of tile w, then (after a CTA barrier) every thread asks for its rows
+    auto expect = [&](int w) { mbar_expect_tx(&bar, (unsigned)(2 * M * ncol_of(w) * (int)sizeof(C))); };
+    auto issue_half = [&](int w, int e0) {
+        const int band = w / ntiles, s0 = (w % ntiles) * TS;
+        const C *src = A + (long long)band * a_band_stride + s0;
+        const unsigned bytes = (unsigned)(ncol_of(w) * (int)sizeof(C));
+        for (int r = tid; r < 2 * M; r += NT)
+            bulk_load(tile + Z::lin(r, 0), src + (long long)(4 * (r >> 1) + e0 + (r & 1)) * pl.pitch, bytes, &bar);
+    };
+    if (tid == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int w = blockIdx.x;
+    if (w < total) {
+        if (tid == 0) expect(w);
+        __syncthreads();
+        issue_half(w, 0);
+    }
+    unsigned par = 0;
+#pragma unroll 1
+    for (; w < total; w += gridDim.x) {
+        const bool more = w + (int)gridDim.x < total;
+        const int band = w / ntiles, s0 = (w % ntiles) * TS, s = s0 + sl;
+        const bool act = s < pl.nsticks;
+        const int4 st = pl.stick[act ? s : s0];
+        const long long g0 = (long long)band * pl.S + pl.stick[s0].x;
+        const long long g1 = (long long)band * pl.S + (s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S);
+        const long long al = g0 & ~(EA - 1), b0 = (g0 + EA - 1) & ~(EA - 1), b1 = g1 & ~(EA - 1); // see zpass_pers_fwd_k
+        C y[1][8], y2[1][8], gq[8], fa[8], fb[8], fc;
+        // ---- residues e = 0, 1
+        mbar_wait(&bar, par);
+        par ^= 1u;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            y[0][q] = tile[Z::lin(2 * (t + 8 * q), sl)];
+            y2[0][q] = tile[Z::lin(2 * (t + 8 * q) + 1, sl)];
+        }
+        if (tid == 0) expect(w);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads(); // every thread holds its values: the other half of the rows may land
+        issue_half(w, 2);
+        sub_fwd<F, T>(y, gq, tws, ex, t);
+        r4_fold_fwd<0, 0, T>(gq, fa, fb, fc, wt[0]);
+        sub_fwd<F, T>(y2, gq, tws, ex, t);
+        r4_fold_fwd<1, 0, T>(gq, fa, fb, fc, wt[1]);
+        // ---- residues e = 2, 3
+        mbar_wait(&bar, par);
+        par ^= 1u;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            y[0][q] = tile[Z::lin(2 * (t + 8 * q), sl)];
+            y2[0][q] = tile[Z::lin(2 * (t + 8 * q) + 1, sl)];
+        }
+        // the previous tile's packed store must have read the landing zone before it is rewritten
+        if (tid == 0) {
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            if (more) expect(w + (int)gridDim.x);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (more) issue_half(w + (int)gridDim.x, 0);
+        sub_fwd<F, T>(y, gq, tws, ex, t);
+        r4_fold_fwd<2, 0, T>(gq, fa, fb, fc, wt[2]);
+        sub_fwd<F, T>(y2, gq, tws, ex, t);
+        r4_fold_fwd<3, 0, T>(gq, fa, fb, fc, wt[3]);
+        if (act) {
+            const long long gs = (long long)band * pl.S + st.x;
+            C *dst = land + (gs - al);
+            const int lo = (int)(b0 - gs), hi = (int)(b1 - gs); // stick elements [lo, hi) belong to the bulk store
+            auto put = [&](int idx, C v) {
+                v = mk<T>(v.x * scale, v.y * scale);
+                if constexpr (EA == 1) dst[idx] = v;
+                else if (idx >= lo && idx < hi) dst[idx] = v;
+                else packed[gs + idx] = v;
+            };
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int ia = (t + 8 * j) - M - st.y, ib = (t + 8 * j) - st.y;
+                if ((unsigned)ia < (unsigned)st.z) put(ia, fa[j]);
+                if ((unsigned)ib < (unsigned)st.z) put(ib, fb[j]);
+            }
+            const int ic = M - st.y;
+            if (t == 0 && (unsigned)ic < (unsigned)st.z) put(ic, fc);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (tid == 0 && b1 > b0) {
+            bulk_store(packed + b0, land + (b0 - al), (unsigned)((b1 - b0) * (long long)sizeof(C)));
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+    }
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+
 } // namespace fftb

@@ -433,8 +433,9 @@ def test_host_buffer_calls_pipelined(fb, oracle):
     assert _rel(h_o.numpy()[sample], ref) <= w.tol
 
 
-@pytest.mark.parametrize("n,a", [((64, 64, 64), (16, 16, 16)), ((128, 128, 128), (32, 32, 32)), ((96, 96, 192), (24, 24, 48))],
-                         ids=["64", "128", "96x96x192"])
+@pytest.mark.parametrize("n,a", [((64, 64, 64), (16, 16, 16)), ((128, 128, 128), (32, 32, 32)), ((96, 96, 192), (24, 24, 48)),
+                                 ((64, 64, 256), (16, 16, 64))],
+                         ids=["64", "128", "96x96x192", "64x64x256"])
 def test_complex64_odd_packed_ranges(fb, oracle, n, a):
     """complex64 z passes move the packed ranges of a tile by 16-byte bulk copies although a range may begin and end on
     an odd 8-byte element: S and nb odd, so ranges of both parities occur and the batch itself ends on an odd element;
