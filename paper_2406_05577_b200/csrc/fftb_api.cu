@@ -882,7 +882,17 @@ static int host_chunks(fftb_plan p, int nb)
     long long k = (long long)nb * p->desc.n[2] / 1024;
     if (k > 4) k = 4;
     if (k > nb) k = nb;
+    if (p->elem == 8 && k > nb / 2) k = nb / 2; // chunks start on even bands (host_chunk_start)
     return k < 1 ? 1 : (int)k;
+}
+// first band of chunk k of K: with 8-byte elements and an odd S a chunk must start on an even band, so that the
+// pointers handed to the device-pointer calls stay 16-byte aligned
+static int host_chunk_start(fftb_plan p, int nb, int k, int K)
+{
+    if (k >= K) return nb;
+    int b = (int)((long long)nb * k / K);
+    if (p->elem == 8) b &= ~1;
+    return b;
 }
 #define FFTB_CU(call) do { if ((call) != cudaSuccess) { p->sticky = FFTB_ECUDA; return FFTB_ECUDA; } } while (0)
 
@@ -904,7 +914,7 @@ int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb,
     FFTB_CU(cudaStreamWaitEvent(p->cs_in, p->hev_start, 0));
     int launches = 0;
     for (int k = 0; k < K; ++k) {
-        const int b0 = (int)((long long)nb * k / K), b1 = (int)((long long)nb * (k + 1) / K);
+        const int b0 = host_chunk_start(p, nb, k, K), b1 = host_chunk_start(p, nb, k + 1, K);
         FFTB_CU(cudaMemcpyAsync(stg + b0 * band, (const unsigned char *)h_packed + b0 * band, (size_t)(b1 - b0) * band,
                                 cudaMemcpyHostToDevice, p->cs_in));
         FFTB_CU(cudaEventRecord(p->hev_in[k], p->cs_in));
@@ -934,7 +944,7 @@ int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb,
     }
     int launches = 0;
     for (int k = 0; k < K; ++k) {
-        const int b0 = (int)((long long)nb * k / K), b1 = (int)((long long)nb * (k + 1) / K);
+        const int b0 = host_chunk_start(p, nb, k, K), b1 = host_chunk_start(p, nb, k + 1, K);
         rc = fftb_forward(p, (const unsigned char *)d_cuboid + b0 * cband, stg + b0 * band, b1 - b0, stream);
         if (rc) return rc;
         launches += p->launches;
@@ -970,7 +980,7 @@ int fftb_apply_vloc_host(fftb_plan p, const void *h_in, void *h_out, const void 
     FFTB_CU(cudaStreamWaitEvent(p->cs_in, p->hev_start, 0));
     int launches = 0;
     for (int k = 0; k < K; ++k) {
-        const int b0 = (int)((long long)nb * k / K), b1 = (int)((long long)nb * (k + 1) / K);
+        const int b0 = host_chunk_start(p, nb, k, K), b1 = host_chunk_start(p, nb, k + 1, K);
         FFTB_CU(cudaMemcpyAsync(stg + b0 * band, (const unsigned char *)h_in + b0 * band, (size_t)(b1 - b0) * band,
                                 cudaMemcpyHostToDevice, p->cs_in));
         FFTB_CU(cudaEventRecord(p->hev_in[k], p->cs_in));

@@ -37,6 +37,10 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
     constexpr long long EA = ZPers<T, F, NW>::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    // `packed` may be only 8-byte aligned (complex64 band chunks of the library's own calls): indices below count
+    // elements from the 16-byte boundary pk at or below it
+    const long long mis = (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
+    const C *pk = packed - mis;
     C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
     C *land = tile + Z::TILE + NW * F::EXW;               // packed values of the tile's sticks
     __shared__ __align__(8) unsigned long long bar;
@@ -56,7 +60,7 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
     // [a0, a1) (complex64: a range may begin and end on an odd element; the neighbours' values that come along are
     // not used).  The batch ends at nall: an odd last element is not covered (a1 < end of the range) and is read
     // straight from global.
-    const long long nall = (long long)(total / ntiles) * pl.S;
+    const long long nall = mis + (long long)(total / ntiles) * pl.S;
     struct Tile { int4 st; long long a0, a1; int band, s0; bool act; };
     auto describe = [&](int w) -> Tile {
         Tile d;
@@ -64,8 +68,8 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
         const int s = d.s0 + sl, s1 = d.s0 + TS;
         d.act = s < pl.nsticks;
         d.st = pl.stick[d.act ? s : d.s0]; // {off, k3lo, len, .}
-        const long long g0 = (long long)d.band * pl.S + pl.stick[d.s0].x;
-        const long long g1 = (long long)d.band * pl.S + (s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S);
+        const long long g0 = (mis + (long long)d.band * pl.S) + pl.stick[d.s0].x;
+        const long long g1 = (mis + (long long)d.band * pl.S) + (s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S);
         d.a0 = g0 & ~(EA - 1);
         d.a1 = (g1 + EA - 1) & ~(EA - 1);
         if (d.a1 > nall) d.a1 = nall & ~(EA - 1);
@@ -75,7 +79,7 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
     auto issue = [&](const Tile &d) {
         const unsigned bytes = (unsigned)((d.a1 - d.a0) * (long long)sizeof(C));
         mbar_expect_tx(&bar, bytes);
-        bulk_load(land, packed + d.a0, bytes, &bar);
+        if (bytes) bulk_load(land, pk + d.a0, bytes, &bar); // 0: a single odd last element of the batch, read directly
     };
     if (tid == 0) {
         mbar_init(&bar, 1);
@@ -96,12 +100,12 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
         const long long a0 = cur.a0, a1 = cur.a1;
         mbar_wait(&bar, par);
         par ^= 1u;
-        const long long gs = (long long)band * pl.S + st.x; // the stick's first element in the batch
+        const long long gs = (mis + (long long)band * pl.S) + st.x; // the stick's first element in the batch
         const C *src = land + (gs - a0);
         const int lim = (int)(a1 - gs);                      // elements of the stick from here on are not in the landing zone
         auto fetch = [&](int idx) -> C {
             if constexpr (EA == 1) return src[idx];
-            else return idx < lim ? src[idx] : __ldcs(packed + gs + idx);
+            else return idx < lim ? src[idx] : __ldcs(pk + gs + idx);
         };
         C x[P1], xs[P1];
 #pragma unroll
@@ -157,6 +161,10 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
     constexpr long long EA = ZPers<T, F, NW>::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    // `packed` may be only 8-byte aligned (complex64 band chunks of the library's own calls): indices below count
+    // elements from the 16-byte boundary pk at or below it
+    const long long mis = (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
+    C *pk = packed - mis;
     C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
     C *land = tile + Z::TILE + NW * F::EXW;               // results of the tile's sticks in packed order
     __shared__ __align__(8) unsigned long long bar;
@@ -202,8 +210,8 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
         // the tile's packed range [g0, g1) in elements of the whole batch (used after the transforms: loading the table
         // one tile ahead was measured 3% slower); its 16-byte aligned interior [b0, b1) leaves as one bulk store from the
         // landing zone (origin al), an odd first / last element (complex64) by a plain store
-        const long long g0 = (long long)band * pl.S + pl.stick[s0].x;
-        const long long g1 = (long long)band * pl.S + (s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S);
+        const long long g0 = (mis + (long long)band * pl.S) + pl.stick[s0].x;
+        const long long g1 = (mis + (long long)band * pl.S) + (s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S);
         const long long al = g0 & ~(EA - 1), b0 = (g0 + EA - 1) & ~(EA - 1), b1 = g1 & ~(EA - 1);
         mbar_wait(&bar, par);
         par ^= 1u;
@@ -227,14 +235,14 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
         sub_fwd<F, T>(y1, h1, tws, ex, t);
         post_fwd<F, 0, T>(h1, g);
         if (act) {
-            const long long gs = (long long)band * pl.S + st.x;
+            const long long gs = (mis + (long long)band * pl.S) + st.x;
             C *dst = land + (gs - al);
             const int lo = (int)(b0 - gs), hi = (int)(b1 - gs); // stick elements [lo, hi) belong to the bulk store
             auto put = [&](int idx, C v) {
                 v = mk<T>(v.x * scale, v.y * scale);
                 if constexpr (EA == 1) dst[idx] = v;
                 else if (idx >= lo && idx < hi) dst[idx] = v;
-                else packed[gs + idx] = v;
+                else pk[gs + idx] = v;
             };
             const int idb = M / 2 - st.y;
             if (t == 0 && (unsigned)idb < (unsigned)st.z) put(idb, csub(h0[P1 / 2], h1[P1 / 2]));
@@ -247,7 +255,7 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         if (tid == 0 && b1 > b0) {
-            bulk_store(packed + b0, land + (b0 - al), (unsigned)((b1 - b0) * (long long)sizeof(C)));
+            bulk_store(pk + b0, land + (b0 - al), (unsigned)((b1 - b0) * (long long)sizeof(C)));
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
     }
@@ -282,6 +290,10 @@ zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
     constexpr int M = ZP::M, P2 = F::P2, G = F::G, TS = ZP::TS, NT = NW * 32;
     constexpr long long EA = ZP::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    // `packed` may be only 8-byte aligned (complex64 band chunks of the library's own calls): indices below count
+    // elements from the 16-byte boundary pk at or below it
+    const long long mis = (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
+    const C *pk = packed - mis;
     C *tile = reinterpret_cast<C *>(smem_raw);            // half tile: rows (n', e & 1)
     C *land = tile + Z::TILE + NW * F::EXW;               // packed values of the tile's sticks
     __shared__ __align__(8) unsigned long long bar;
@@ -297,11 +309,11 @@ zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
 #pragma unroll
     for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
 
-    const long long nall = (long long)(total / ntiles) * pl.S;
+    const long long nall = mis + (long long)(total / ntiles) * pl.S;
     auto range = [&](int w, long long &a0, long long &a1) { // see zpass_pers_inv_k
         const int band = w / ntiles, s0 = (w % ntiles) * TS, s1 = s0 + TS;
-        const long long g0 = (long long)band * pl.S + pl.stick[s0].x;
-        const long long g1 = (long long)band * pl.S + (s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S);
+        const long long g0 = (mis + (long long)band * pl.S) + pl.stick[s0].x;
+        const long long g1 = (mis + (long long)band * pl.S) + (s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S);
         a0 = g0 & ~(EA - 1);
         a1 = (g1 + EA - 1) & ~(EA - 1);
         if (a1 > nall) a1 = nall & ~(EA - 1);
@@ -311,7 +323,7 @@ zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
         range(w, a0, a1);
         const unsigned bytes = (unsigned)((a1 - a0) * (long long)sizeof(C));
         mbar_expect_tx(&bar, bytes);
-        bulk_load(land, packed + a0, bytes, &bar);
+        if (bytes) bulk_load(land, pk + a0, bytes, &bar); // 0: a single odd last element of the batch, read directly
     };
     if (tid == 0) {
         mbar_init(&bar, 1);
@@ -330,12 +342,12 @@ zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
         range(w, a0, a1);
         mbar_wait(&bar, par);
         par ^= 1u;
-        const long long gs = (long long)band * pl.S + st.x;
+        const long long gs = (mis + (long long)band * pl.S) + st.x;
         const C *src = land + (gs - a0);
         const int lim = (int)(a1 - gs);
         auto fetch = [&](int idx) -> C {
             if constexpr (EA == 1) return src[idx];
-            else return idx < lim ? src[idx] : __ldcs(packed + gs + idx);
+            else return idx < lim ? src[idx] : __ldcs(pk + gs + idx);
         };
         C a[8], bq[8];
 #pragma unroll
@@ -403,6 +415,10 @@ zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
     constexpr int M = ZP::M, P2 = F::P2, G = F::G, TS = ZP::TS, NT = NW * 32;
     constexpr long long EA = ZP::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    // `packed` may be only 8-byte aligned (complex64 band chunks of the library's own calls): indices below count
+    // elements from the 16-byte boundary pk at or below it
+    const long long mis = (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
+    C *pk = packed - mis;
     C *tile = reinterpret_cast<C *>(smem_raw);            // half tile: rows (n', e & 1)
     C *land = tile + Z::TILE + NW * F::EXW;               // results of the tile's sticks in packed order
     __shared__ __align__(8) unsigned long long bar;
@@ -447,8 +463,8 @@ zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
         const int band = w / ntiles, s0 = (w % ntiles) * TS, s = s0 + sl;
         const bool act = s < pl.nsticks;
         const int4 st = pl.stick[act ? s : s0];
-        const long long g0 = (long long)band * pl.S + pl.stick[s0].x;
-        const long long g1 = (long long)band * pl.S + (s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S);
+        const long long g0 = (mis + (long long)band * pl.S) + pl.stick[s0].x;
+        const long long g1 = (mis + (long long)band * pl.S) + (s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S);
         const long long al = g0 & ~(EA - 1), b0 = (g0 + EA - 1) & ~(EA - 1), b1 = g1 & ~(EA - 1); // see zpass_pers_fwd_k
         C y[1][8], y2[1][8], gq[8], fa[8], fb[8], fc;
         // ---- residues e = 0, 1
@@ -488,14 +504,14 @@ zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
         sub_fwd<F, T>(y2, gq, tws, ex, t);
         r4_fold_fwd<3, 0, T>(gq, fa, fb, fc, wt[3]);
         if (act) {
-            const long long gs = (long long)band * pl.S + st.x;
+            const long long gs = (mis + (long long)band * pl.S) + st.x;
             C *dst = land + (gs - al);
             const int lo = (int)(b0 - gs), hi = (int)(b1 - gs); // stick elements [lo, hi) belong to the bulk store
             auto put = [&](int idx, C v) {
                 v = mk<T>(v.x * scale, v.y * scale);
                 if constexpr (EA == 1) dst[idx] = v;
                 else if (idx >= lo && idx < hi) dst[idx] = v;
-                else packed[gs + idx] = v;
+                else pk[gs + idx] = v;
             };
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
@@ -509,7 +525,7 @@ zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         if (tid == 0 && b1 > b0) {
-            bulk_store(packed + b0, land + (b0 - al), (unsigned)((b1 - b0) * (long long)sizeof(C)));
+            bulk_store(pk + b0, land + (b0 - al), (unsigned)((b1 - b0) * (long long)sizeof(C)));
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
     }

@@ -408,15 +408,17 @@ def test_device_calls_are_graph_capturable(fb):
     p.destroy()
 
 
-def test_host_buffer_calls_pipelined(fb, oracle):
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_host_buffer_calls_pipelined(fb, oracle, dtype):
     """Batches of 32 bands and more cross PCIe in chunks on the plan's copy streams, overlapped with the
-    transforms: same results as the device-pointer calls, complete when the caller's stream is."""
-    w = _small((64, 64, 64), (16, 16, 16), batch=43)
+    transforms: same results as the device-pointer calls, complete when the caller's stream is.  complex64: S is
+    odd, so the chunks must start on even bands to keep the packed pointers 16-byte aligned (43 * k / 4 is odd)."""
+    w = _small((64, 64, 64), (16, 16, 16), batch=43, dtype=dtype)
     p = _plan(fb, w, w.batch, host=True)
     k = p.points()
     c = wl.coefficients(w, *k)
     h_c = torch.from_numpy(c).pin_memory()
-    d_psi = torch.empty(p.cuboid_shape(w.batch), dtype=torch.complex128, device="cuda")
+    d_psi = torch.empty(p.cuboid_shape(w.batch), dtype=p.torch_complex, device="cuda")
     h_rt = torch.zeros_like(h_c).pin_memory()
     h_o = torch.zeros_like(h_c).pin_memory()
     v = wl.potential(w)
@@ -456,4 +458,21 @@ def test_complex64_odd_packed_ranges(fb, oracle, n, a):
     h = buf.cpu().numpy()
     assert (h[:guard] == np.complex64(777.0 - 555.0j)).all() and (h[-guard:] == np.complex64(777.0 - 555.0j)).all()
     assert _rel(h[guard:-guard].reshape(3, p.S), c) <= w.tol
+    p.destroy()
+
+
+def test_complex64_odd_band_chunks(fb, oracle, monkeypatch):
+    """A workspace of one band makes the library run band by band: with complex64 and an odd S every second chunk's
+    packed pointer is only 8-byte aligned, which the bulk copies of the z passes must cope with."""
+    monkeypatch.setenv("FFTB_WS_MB", "4")  # read by fftb_plan_create: 128^3 complex64 needs 3.3 MB of A per band
+    w = _small((128, 128, 128), (32, 32, 32), dtype="c64", batch=3)
+    p = _plan(fb, w, 3)
+    assert p.info["chunk_bands"] == 1 and p.S % 2 == 1
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    d_psi = p.inverse(torch.from_numpy(c).cuda())
+    rt = p.forward(d_psi)
+    torch.cuda.synchronize()
+    assert _rel(d_psi.cpu().numpy(), oracle.inverse(w.n, k, c)) <= w.tol
+    assert _rel(rt.cpu().numpy(), c) <= w.tol
     p.destroy()
