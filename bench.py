@@ -308,6 +308,40 @@ def run_ours(args, w):
     except Exception as exc:  # never fatal for the bench line
         graph_info = {"error": str(exc)[:200]}
 
+    # config 5's other arm (reading R11): the same packed data zero-padded to the full frequency cuboid
+    # and transformed UNPRUNED by the product's kernels through a FFTB_FLAG_DENSE plan: embed + inverse + forward + extract
+    dense_arm = None
+    if w.op == "inv_fwd_pruned_vs_dense" and world == 1 and not vloc:
+        try:
+            pd = fb.Plan(w.n, w.cutoff, batch=nb, dtype=w.dtype, scale="forward", dense=True).bind()
+            d_dense = torch.empty((nb, pd.S), dtype=plan.torch_complex, device="cuda")
+            d_back = torch.empty_like(d_dense)
+            d_psi_d = torch.empty(plan.cuboid_shape(nb), dtype=plan.torch_complex, device="cuda")
+            d_out_d = torch.empty_like(d_c)
+
+            def step_dense():
+                plan.dense_embed(pd, d_c, d_dense)
+                pd.inverse(d_dense, d_psi_d)
+                n = pd.last_launches()
+                pd.forward(d_psi_d, d_back)
+                n += pd.last_launches()
+                plan.dense_extract(pd, d_back, d_out_d)
+                return n + 2
+
+            ms_dense, _, _, l_dense = timed(step_dense, min(K, 5), 3)
+            step()
+            torch.cuda.synchronize()
+            rel_psi = float(torch.linalg.vector_norm(d_psi_d - d_psi) / torch.linalg.vector_norm(d_psi))
+            rel_c = float(torch.linalg.vector_norm(d_out_d - d_out) / torch.linalg.vector_norm(d_out))
+            dense_arm = {"ms_per_step": ms_dense, "value": transforms / (ms_dense * 1e-3), "unit": UNIT,
+                         "pruned_speedup": ms_dense / ms_step, "launches_per_step": l_dense // min(K, 5),
+                         "rel_l2_cuboid_dense_vs_pruned": rel_psi, "rel_l2_packed_dense_vs_pruned": rel_c,
+                         "what": "fftb_dense_embed + dense-plan fftb_inverse + fftb_forward + fftb_dense_extract on the same data"}
+            pd.destroy()
+            del d_dense, d_back, d_psi_d, d_out_d
+        except Exception as exc:  # never fatal for the bench line
+            dense_arm = {"error": str(exc)[:200]}
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu_baseline, _ = time_oracle(w, 2, 1)
@@ -330,6 +364,7 @@ def run_ours(args, w):
                               "nominal_tflops_5nlog2n": 2 * nb * nominal_flops_per_band_dir(w.n, info) / (ms_step * 1e-3) / 1e12},
             "kernel_ms_per_step": {kk: prof[kk][0] / K for kk in prof if prof[kk][1]},
             "cuda_graph": graph_info,
+            "dense_arm": dense_arm,
             "cpu_baseline": cpu_baseline,
         }
         print(json.dumps(line), flush=True)
