@@ -29,7 +29,9 @@
  *   apply_vloc c' = forward( V .* inverse(c) ), the cuboid never leaves the chip.
  *
  * Pointers named d_* are DEVICE pointers, h_* are HOST pointers; everything else is host.
- * All device pointers must be 16-byte aligned.  The caller owns every device buffer,
+ * Device pointers must be 16-byte aligned; complex128 CUBOID pointers must be 32-byte aligned (the
+ * kernels move two neighbouring x values as one 32-byte access); anything else is FFTB_EINVAL.
+ * The caller owns every device buffer,
  * including the table/workspace block handed to fftb_plan_bind; the plan owns host
  * memory only.  The execute calls enqueue work on `stream` (a cudaStream_t passed as
  * void*; NULL = the legacy default stream) and return without synchronising; they do not
@@ -91,17 +93,47 @@ typedef struct {
                              per band (the fast kernels accumulate the y residues themselves and write one) */
     int64_t chunk_bands_fwd;  /* bands per kernel group in fftb_forward */
     int64_t chunk_bands_vloc; /* bands per kernel group in fftb_apply_vloc */
+    int64_t ring_bands;   /* > 0: fftb_inverse and fftb_forward are ONE launch each that keeps the intermediate in a
+                             ring of this many band slots at workspace_offset (band b in slot b % ring_bands);
+                             0: separate z-pass and plane launches per band chunk, A[band][z][pitch] */
+    int64_t lead_bands;   /* how many bands the producers of the ring run ahead of its consumers */
+    /* layout of a ring slot (tile-major): stick s, plane z of the band sits at element
+     *   (s / ring_tile_sticks) * ring_tile_elems + (z / 2) * ring_pair_pitch + (z % 2) * ring_tile_sticks + s % ring_tile_sticks
+     * and a slot holds ceil(n_sticks / ring_tile_sticks) * ring_tile_elems elements */
+    int64_t ring_tile_sticks, ring_tile_elems, ring_pair_pitch;
 } fftb_plan_info;
+
+/* Optional tuning of a plan, for tests and measurements; everything 0 = the defaults fftb_plan_create uses. */
+enum fftb_tuning_flags {
+    FFTB_TUNE_GENERIC_Z = 1u,     /* z passes by the generic kernels even where a persistent TMA kernel exists */
+    FFTB_TUNE_GENERIC_PLANE = 2u, /* y/x passes by the generic plane kernel even where a persistent one exists */
+    FFTB_TUNE_FUSED = 4u,         /* fftb_inverse / fftb_forward as ONE cooperative launch each (z tiles and planes of the whole
+                                     batch, the intermediate in an L2-resident ring: 27% less DRAM traffic) where that launch
+                                     exists (128^3 grids); measured slower than the separate launches, hence opt-in */
+    FFTB_TUNE_NO_L2_HINTS = 8u    /* fused launches without L2 eviction priorities (ring evict_last, streams evict_first) */
+};
+typedef struct {
+    int64_t workspace_bytes; /* budget for the intermediate A inside the bind block (the plan rounds it to whole bands,
+                                at least one); 0 = default */
+    int32_t ring_bands;      /* band slots of the fused launches' ring; 0 = default (lead_bands + 4) */
+    int32_t lead_bands;      /* bands the producers run ahead; 0 = default (2) */
+    uint32_t flags;          /* fftb_tuning_flags */
+    uint32_t reserved;       /* must be 0 */
+} fftb_plan_tuning;
 
 /* Create a plan (host only, no CUDA call).  Builds the offset array -- the stick map -- from the
  * grid and the cut-off (Fig. 7), the per-k1 stick runs used by the y pass, and the
  * twiddle tables.
  * Predefined patterns (anything else: FFTB_EUNSUPPORTED):
- *   - N1 == N2, each of N1, N3 in {32, 64, 96, 128, 192, 256};
+ *   - N1 == N2, each of N1, N3 in {32, 64, 96, 128, 192, 256}, FFTB_C64 or FFTB_C128;
  *   - pruned plans: a_d <= N_d/4 on every axis (the paper's "cube of width twice the diameter of
  *     the sphere");
- *   - FFTB_C128 with N1 = 192 and dense FFTB_C128 beyond what fits one SM's shared memory. */
+ *   - dense plans (FFTB_FLAG_DENSE): FFTB_C128 only, N1 and N3 in {32, 64, 128, 256}. */
 int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc);
+
+/* The same with explicit tuning (tuning == NULL: fftb_plan_create).  FFTB_EINVAL for unknown flags or negative
+ * fields. */
+int fftb_plan_create_tuned(fftb_plan *out, const fftb_plan_desc *desc, const fftb_plan_tuning *tuning);
 
 /* Create a plan from an EXPLICIT stick map instead of a cut-off: the paper's general domain with an
  * offset array (PAPER.md:183-185: "x and y dense, only z compressed", :201 `offsets` argument), e.g. the
@@ -177,9 +209,10 @@ int fftb_plan_last_launches(fftb_plan p);
 
 /* Per-kernel timing for benchmarks.  fftb_plan_profile(p, 1) makes every later execute call record a
  * CUDA event pair around each kernel it launches (on the launching stream); fftb_plan_profile_read
- * waits for them, adds the elapsed milliseconds and launch counts per kernel kind into ms[5] and
- * count[5] -- 0 inverse z pass, 1 inverse plane, 2 forward plane, 3 forward z pass, 4 fused vloc
- * plane -- and clears the record.  fftb_plan_profile(p, 0) switches it off. */
+ * waits for them, adds the elapsed milliseconds and launch counts per kernel kind into ms[7] and
+ * count[7] -- 0 inverse z pass, 1 inverse plane, 2 forward plane, 3 forward z pass, 4 fused vloc
+ * plane, 5 fused inverse launch (z tiles + planes), 6 fused forward launch -- and clears the record.
+ * fftb_plan_profile(p, 0) switches it off. */
 int fftb_plan_profile(fftb_plan p, int enable);
 int fftb_plan_profile_read(fftb_plan p, double *ms, int64_t *count);
 

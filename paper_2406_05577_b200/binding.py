@@ -17,11 +17,12 @@ _LIBPATH = _HERE / "libfftb.so"
 FFTB_C64, FFTB_C128 = 0, 1
 FFTB_SCALE_NONE, FFTB_SCALE_FORWARD = 0, 1
 FFTB_FLAG_DENSE = 1
+FFTB_TUNE_GENERIC_Z, FFTB_TUNE_GENERIC_PLANE, FFTB_TUNE_FUSED, FFTB_TUNE_NO_L2_HINTS = 1, 2, 4, 8
 FFTB_OK, FFTB_EINVAL, FFTB_EUNSUPPORTED, FFTB_ENOMEM, FFTB_ECUDA, FFTB_ESTATE = 0, -1, -2, -3, -4, -5
 
 # every symbol include/fftb.h declares
 SYMBOLS = [
-    "fftb_plan_create", "fftb_plan_create_explicit", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
+    "fftb_plan_create", "fftb_plan_create_tuned", "fftb_plan_create_explicit", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
     "fftb_inverse", "fftb_forward", "fftb_apply_vloc",
     "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
     "fftb_dense_embed", "fftb_dense_extract", "fftb_packed_transpose",
@@ -37,7 +38,13 @@ class PlanDesc(ctypes.Structure):
 class PlanInfo(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int64) for k in (
         "n_points", "n_sticks", "n_xocc", "device_bytes", "device_bytes_host", "chunk_bands",
-        "min_bytes_per_band_dir", "workspace_offset", "pitch", "y_residues", "chunk_bands_fwd", "chunk_bands_vloc")]
+        "min_bytes_per_band_dir", "workspace_offset", "pitch", "y_residues", "chunk_bands_fwd", "chunk_bands_vloc",
+        "ring_bands", "lead_bands", "ring_tile_sticks", "ring_tile_elems", "ring_pair_pitch")]
+
+
+class PlanTuning(ctypes.Structure):
+    _fields_ = [("workspace_bytes", ctypes.c_int64), ("ring_bands", ctypes.c_int32), ("lead_bands", ctypes.c_int32),
+                ("flags", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
 
 
 class FftbError(RuntimeError):
@@ -59,6 +66,7 @@ def lib():
         L = ctypes.CDLL(str(_LIBPATH))
         vp, i32 = ctypes.c_void_p, ctypes.c_int
         L.fftb_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc)]
+        L.fftb_plan_create_tuned.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc), ctypes.POINTER(PlanTuning)]
         L.fftb_plan_create_explicit.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc), ctypes.c_int64, vp, vp, vp, vp]
         L.fftb_plan_info_get.argtypes = [vp, ctypes.POINTER(PlanInfo)]
         L.fftb_plan_get_map.argtypes = [vp, vp, vp, vp, vp, vp]
@@ -100,8 +108,9 @@ class Plan:
     """fftb_plan_create / bind / execute / destroy.  Tensors are torch CUDA tensors (or pinned host
     tensors for the *_host calls); shapes follow include/fftb.h: packed (nb, S), cuboid (nb, N3, N2, N1)."""
 
-    def __init__(self, n, cutoff=(0, 0, 0), batch=1, dtype="c128", scale="forward", dense=False, stick_map=None):
-        """stick_map = (k1, k2, k3lo, len) int arrays: fftb_plan_create_explicit instead of a cut-off."""
+    def __init__(self, n, cutoff=(0, 0, 0), batch=1, dtype="c128", scale="forward", dense=False, stick_map=None, tuning=None):
+        """stick_map = (k1, k2, k3lo, len) int arrays: fftb_plan_create_explicit instead of a cut-off.
+        tuning = dict(workspace_bytes=, ring_bands=, lead_bands=, flags=): fftb_plan_create_tuned."""
         d = PlanDesc()
         d.n[:] = [int(x) for x in n]
         d.cutoff[:] = [int(x) for x in cutoff]
@@ -110,7 +119,14 @@ class Plan:
         d.scale = FFTB_SCALE_FORWARD if scale == "forward" else FFTB_SCALE_NONE
         d.flags = FFTB_FLAG_DENSE if dense else 0
         self._h = ctypes.c_void_p()
-        if stick_map is None:
+        if stick_map is None and tuning is not None:
+            tu = PlanTuning()
+            tu.workspace_bytes = int(tuning.get("workspace_bytes", 0))
+            tu.ring_bands = int(tuning.get("ring_bands", 0))
+            tu.lead_bands = int(tuning.get("lead_bands", 0))
+            tu.flags = int(tuning.get("flags", 0))
+            _check(lib().fftb_plan_create_tuned(ctypes.byref(self._h), ctypes.byref(d), ctypes.byref(tu)), "fftb_plan_create_tuned")
+        elif stick_map is None:
             _check(lib().fftb_plan_create(ctypes.byref(self._h), ctypes.byref(d)), "fftb_plan_create")
         else:
             m = [np.ascontiguousarray(x, dtype=np.int32) for x in stick_map]
@@ -272,15 +288,15 @@ class Plan:
     def last_launches(self) -> int:
         return int(lib().fftb_plan_last_launches(self._h))
 
-    KERNEL_KINDS = ("zpass_inv", "plane_inv", "plane_fwd", "zpass_fwd", "plane_vloc")
+    KERNEL_KINDS = ("zpass_inv", "plane_inv", "plane_fwd", "zpass_fwd", "plane_vloc", "fused_inv", "fused_fwd")
 
     def profile(self, enable: bool):
         _check(lib().fftb_plan_profile(self._h, int(bool(enable))), "fftb_plan_profile")
 
     def profile_read(self):
         """-> {kernel kind: (total ms, launches)} since profiling was enabled / last read."""
-        ms = np.zeros(5, dtype=np.float64)
-        cnt = np.zeros(5, dtype=np.int64)
+        ms = np.zeros(len(self.KERNEL_KINDS), dtype=np.float64)
+        cnt = np.zeros(len(self.KERNEL_KINDS), dtype=np.int64)
         _check(lib().fftb_plan_profile_read(self._h, ms.ctypes.data_as(ctypes.c_void_p),
                                             cnt.ctypes.data_as(ctypes.c_void_p)), "fftb_plan_profile_read")
         return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(self.KERNEL_KINDS)}

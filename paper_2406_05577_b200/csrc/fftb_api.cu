@@ -11,12 +11,16 @@
 #include "fftb_plane_pf.cuh"
 #include "fftb_plane_r4.cuh"
 #include "fftb_zpass_pf.cuh"
+#include "fftb_fused.cuh"
 
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 
 using namespace fftb;
@@ -69,6 +73,64 @@ template <class AX, class AY> struct PlaneTune {
 
 constexpr int Z_LINES = 32, Z_NT = 256;
 
+// ------------------------------------------------------------------------------------------------
+// Launch-side state.  Nothing here depends on the calling thread or on a previous launch: the one piece of
+// per-kernel device state (the opt-in limit on dynamic shared memory) is raised ONCE per (kernel, device) to the
+// device's maximum under a mutex and never lowered, the occupancy of a (kernel, device, shared memory) triple is
+// cached in the same registry, and the SM count of the device a plan was bound on travels in its DevPlan.
+// ------------------------------------------------------------------------------------------------
+struct KernelState {
+    bool attr_set = false;
+    std::map<size_t, int> per_sm; // dynamic shared memory -> resident CTAs per SM
+};
+std::mutex g_reg_mu;
+std::map<std::pair<const void *, int>, KernelState> g_reg;
+
+int current_device()
+{
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return dev;
+}
+
+// makes kernel k launchable with `smem` bytes of dynamic shared memory on the current device; per_sm (optional)
+// receives the number of CTAs of `threads` threads that fit one SM
+int kernel_ready(const void *k, int threads, size_t smem, int *per_sm)
+{
+    const int dev = current_device();
+    std::lock_guard<std::mutex> lock(g_reg_mu);
+    KernelState &ks = g_reg[std::make_pair(k, dev)];
+    if (!ks.attr_set) {
+        int optin = 0;
+        cudaFuncAttributes fa;
+        if (cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) return FFTB_ECUDA;
+        if (cudaFuncGetAttributes(&fa, k) != cudaSuccess) return FFTB_ECUDA;
+        // static + dynamic shared memory of a block may not exceed the opt-in limit
+        const int dyn_max = optin - (int)fa.sharedSizeBytes;
+        if (dyn_max < 0 || cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max) != cudaSuccess) {
+            cudaGetLastError();
+            return FFTB_ECUDA;
+        }
+        ks.attr_set = true;
+    }
+    if (per_sm) {
+        auto it = ks.per_sm.find(smem);
+        if (it == ks.per_sm.end()) {
+            int occ = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, threads, smem) != cudaSuccess) return FFTB_ECUDA;
+            it = ks.per_sm.emplace(smem, occ).first;
+        }
+        *per_sm = it->second;
+        if (*per_sm < 1) return FFTB_EUNSUPPORTED;
+    }
+    return 0;
+}
+template <class K> int kernel_ready(K k, int threads, size_t smem, int *per_sm)
+{
+    return kernel_ready(reinterpret_cast<const void *>(k), threads, smem, per_sm);
+}
+int launch_status() { return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA; }
+
 struct ZLaunch {
     int (*inv)(const DevPlan &, const void *packed, void *A, long long stride, int nb, cudaStream_t);
     int (*fwd)(const DevPlan &, const void *A, void *packed, long long stride, int nb, cudaStream_t);
@@ -79,24 +141,33 @@ struct PlaneLaunch {
     int (*run[3])(const DevPlan &, const PlanTabs &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v,
                   long long sin, long long sout, int nb, cudaStream_t);
 };
+// one cooperative launch per direction (fftb_fused.cuh): the intermediate lives in a ring of `nslot` band slots
+struct FusedGeom { int ts, tile, rp; }; // sticks per z tile, elements of a tile's image, pitch of a row pair (ZFast)
+struct FusedLaunch {
+    FusedGeom geom;
+    int (*inv)(const DevPlan &, const PlanTabs &, const void *packed, void *ring, const CUtensorMap &ring_map, void *cuboid, long long stride,
+               int nb, int nslot, int lead, int hints, int *sync, cudaStream_t);
+    int (*fwd)(const DevPlan &, const PlanTabs &, const void *cuboid, void *ring, void *packed, long long stride, int nb, int nslot,
+               int lead, int hints, int *sync, cudaStream_t);
+};
 
 template <typename T, class AZ> int launch_zinv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
 {
     auto k = zpass_inv_k<T, AZ, Z_LINES, Z_NT>;
     const size_t smem = sizeof(cx<T>) * ((size_t)AZ::M * (Z_LINES | 1) + AZ::N);
-    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    if (int rc = kernel_ready(k, Z_NT, smem, nullptr)) return rc;
     dim3 grid((pl.nsticks + Z_LINES - 1) / Z_LINES, nb);
     k<<<grid, Z_NT, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    return launch_status();
 }
 template <typename T, class AZ> int launch_zfwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
 {
     auto k = zpass_fwd_k<T, AZ, Z_LINES, Z_NT>;
     const size_t smem = sizeof(cx<T>) * ((size_t)AZ::R * AZ::P2 * (AZ::P1 * (Z_LINES | 1) + 1) + AZ::N);
-    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    if (int rc = kernel_ready(k, Z_NT, smem, nullptr)) return rc;
     dim3 grid((pl.nsticks + Z_LINES - 1) / Z_LINES, nb);
     k<<<grid, Z_NT, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    return launch_status();
 }
 template <typename T, class AX, class AY, int MODE>
 int launch_plane(const DevPlan &pl, const PlanTabs &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
@@ -105,36 +176,16 @@ int launch_plane(const DevPlan &pl, const PlanTabs &, const void *Ain, void *Aou
     using TU = PlaneTune<AX, AY>;
     auto k = plane_k<T, AX, AY, TU::LX, TU::LY, TU::NT, MODE>;
     const size_t smem = PlaneSmem<T, AX, AY, TU::LX, TU::LY, TU::NT>::bytes;
-    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    if (int rc = kernel_ready(k, TU::NT, smem, nullptr)) return rc;
     dim3 grid(AY::R * pl.n3, nb);
     k<<<grid, TU::NT, smem, st>>>(pl, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    return launch_status();
 }
 
 // warp-synchronous persistent plane kernel (fftb_plane_fast.cuh): half-band power-of-two grids
 constexpr int FAST_NW = 4; // warps per CTA of the z-pass kernels (4 CTAs per SM)
 // warps per CTA of the plane kernel: a quarter of the x tasks of a plane
 template <int N> struct PlaneNW { static constexpr int value = N >= 128 ? 8 : (N == 96 ? 4 : 2); }; // must divide N / G; measured best
-
-static int g_sm_count = 0;
-static int current_device()
-{
-    int dev = 0;
-    cudaGetDevice(&dev);
-    return dev;
-}
-
-static int sm_count()
-{
-    if (!g_sm_count) {
-        int dev = 0, n = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
-            g_sm_count = n;
-        else
-            g_sm_count = 148;
-    }
-    return g_sm_count;
-}
 
 template <typename T, class F, int MODE>
 int launch_plane_fast(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *Aout, const void *cin, void *cout, const void *v, long long sin,
@@ -144,23 +195,13 @@ int launch_plane_fast(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, 
     auto k = plane_pf_k<T, F, NW, MODE>;
     const size_t smem = PlanePF<T, F, NW>::smem_bytes_mode(MODE, pl.pitch);
     if (smem > 227 * 1024) return FFTB_EUNSUPPORTED;
-    static int per_sm = 0;    // CTAs per SM of this instantiation
-    static size_t smem_set = 0;
-    static int dev_set = -1;  // attribute and occupancy are per device
-    const int dev = current_device();
-    if (!per_sm || smem != smem_set || dev != dev_set) {
-        smem_set = smem;
-        dev_set = dev;
-        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-        int occ = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, NW * 32, smem) != cudaSuccess || occ < 1) return FFTB_ECUDA;
-        per_sm = occ;
-    }
+    int per_sm = 0;
+    if (int rc = kernel_ready(k, NW * 32, smem, &per_sm)) return rc;
     const int nplanes = pl.n3 * nb;
-    int grid = sm_count() * per_sm;
+    int grid = pl.sms * per_sm;
     if (grid > nplanes) grid = nplanes;
     k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct, (const cx<T> *)Ain, (cx<T> *)Aout, (const cx<T> *)cin, (cx<T> *)cout, (const T *)v, sin, sout, nplanes);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    return launch_status();
 }
 template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
 {
@@ -175,17 +216,12 @@ int launch_plane_r4_inv(const DevPlan &pl, const PlanTabs &tabs, const void *Ain
     constexpr int NW = 8;
     auto k = plane_r4_inv_k<T, NW>;
     const size_t smem = PlaneR4<T, NW>::smem_bytes;
-    static int ready_dev = -1; // the attribute is per device: set again when the calling thread's device changes
-    const int dev = current_device();
-    if (ready_dev != dev) {
-        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-        ready_dev = dev;
-    }
+    if (int rc = kernel_ready(k, NW * 32, smem, nullptr)) return rc;
     const int nplanes = pl.n3 * nb;
-    int grid = sm_count();
+    int grid = pl.sms;
     if (grid > nplanes) grid = nplanes;
     k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)Ain, (cx<T> *)cout, sin, nplanes);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    return launch_status();
 }
 
 template <typename T>
@@ -195,17 +231,12 @@ int launch_plane_r4_vloc(const DevPlan &pl, const PlanTabs &tabs, const void *Ai
     constexpr int NW = 8;
     auto k = plane_r4_vloc_k<T, NW>;
     const size_t smem = PlaneR4<T, NW>::smem_bytes;
-    static int ready_dev = -1; // the attribute is per device: set again when the calling thread's device changes
-    const int dev = current_device();
-    if (ready_dev != dev) {
-        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-        ready_dev = dev;
-    }
+    if (int rc = kernel_ready(k, NW * 32, smem, nullptr)) return rc;
     const int nplanes = pl.n3 * nb;
-    int grid = sm_count();
+    int grid = pl.sms;
     if (grid > nplanes) grid = nplanes;
     k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)Ain, (cx<T> *)Aout, (const T *)v, sin, sout, nplanes);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    return launch_status();
 }
 
 template <typename T>
@@ -215,40 +246,34 @@ int launch_plane_r4_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *, v
     constexpr int NW = 8;
     auto k = plane_r4_fwd_k<T, NW>;
     const size_t smem = sizeof(cx<T>) * (size_t)PlaneR4<T, NW>::PB;
-    static int ready_dev = -1; // the attribute is per device: set again when the calling thread's device changes
-    const int dev = current_device();
-    if (ready_dev != dev) {
-        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
-        ready_dev = dev;
-    }
+    if (int rc = kernel_ready(k, NW * 32, smem, nullptr)) return rc;
     const int nplanes = pl.n3 * nb;
-    int grid = sm_count();
+    int grid = pl.sms;
     if (grid > nplanes) grid = nplanes;
     k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)cin, (cx<T> *)Aout, sout, nplanes);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    return launch_status();
 }
 
 bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)
 {
     if (dense) return false;
     if (dtype == FFTB_C128 && n == 128) { *out = make_plane_fast<double, 128, 8, 8>(); return true; }
-#ifndef FFTB_DEV
     if (dtype == FFTB_C128 && n == 64) { *out = make_plane_fast<double, 64, 8, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 128) { *out = make_plane_fast<float, 128, 8, 8>(); return true; }
     if (dtype == FFTB_C64 && n == 64) { *out = make_plane_fast<float, 64, 8, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 96) { *out = make_plane_fast<float, 96, 12, 4>(); return true; }   // 48 = 12 x 4
     if (dtype == FFTB_C128 && n == 96) { *out = make_plane_fast<double, 96, 12, 4>(); return true; }
-#endif
     return false;
 }
 
-// resident CTAs per SM of a persistent z-pass kernel (shared memory decides: 3 at N3 = 64, 128; 2 at 96)
-template <class K> static int zpers_grid(K kp, size_t smem, int total)
+// persistent z-pass kernels: grid = resident CTAs (shared memory decides: 3 per SM at N3 = 64, 128; 2 at 96), tiles strided over it
+template <class K> int zpers_launch_grid(K kp, int threads, size_t smem, const DevPlan &pl, int total, int *grid)
 {
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kp, FAST_NW * 32, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
-    const int cap = sm_count() * per_sm;
-    return total < cap ? total : cap;
+    if (int rc = kernel_ready(kp, threads, smem, &per_sm)) return rc;
+    const int cap = pl.sms * per_sm;
+    *grid = total < cap ? total : cap;
+    return 0;
 }
 
 template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
@@ -257,11 +282,10 @@ template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const voi
     const int ntiles = (pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), total = ntiles * nb;
     using ZP = ZPers<T, F, FAST_NW>;
     auto kp = zpass_pers_inv_k<T, F, FAST_NW>;
-    static int grid_cap = 0;
-    if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
-    if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
-    kp<<<total < grid_cap ? total : grid_cap, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    int grid = 0;
+    if (int rc = zpers_launch_grid(kp, FAST_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
+    kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
+    return launch_status();
 }
 template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
 {
@@ -269,17 +293,16 @@ template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const voi
     if (pl.ry == 1) { // one plane of A (fast plane kernels): persistent kernel
         using ZP = ZPers<T, F, FAST_NW>;
         auto kp = zpass_pers_fwd_k<T, F, FAST_NW>;
-        static int grid_cap = 0;
-        if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
-        if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
-        kp<<<total < grid_cap ? total : grid_cap, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
-        return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+        int grid = 0;
+        if (int rc = zpers_launch_grid(kp, FAST_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
+        kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
+        return launch_status();
     }
     auto k = zpass_fast_fwd_k<T, F, FAST_NW>; // partial planes of the generic plane kernel are summed here
     const size_t smem = ZFast<T, F, FAST_NW>::smem_bytes;
-    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    if (int rc = kernel_ready(k, FAST_NW * 32, smem, nullptr)) return rc;
     k<<<dim3(ntiles, nb), FAST_NW * 32, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    return launch_status();
 }
 template <typename T, int N, int P1, int P2> ZLaunch make_z_fast()
 {
@@ -293,11 +316,10 @@ template <typename T> int launch_zr4_inv(const DevPlan &pl, const void *packed, 
     using ZP = ZPersR4<T, R4Z_NW>;
     auto kp = zpass_r4_pers_inv_k<T, R4Z_NW>;
     const int ntiles = (pl.nsticks + ZP::TS - 1) / ZP::TS, total = ntiles * nb;
-    static int grid_cap = 0;
-    if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
-    if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
-    kp<<<total < grid_cap ? total : grid_cap, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    int grid = 0;
+    if (int rc = zpers_launch_grid(kp, R4Z_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
+    kp<<<grid, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
+    return launch_status();
 }
 template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
 {
@@ -305,18 +327,17 @@ template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void 
         using ZP = ZPersR4<T, R4Z_NW>;
         auto kp = zpass_r4_pers_fwd_k<T, R4Z_NW>;
         const int ntiles = (pl.nsticks + ZP::TS - 1) / ZP::TS, total = ntiles * nb;
-        static int grid_cap = 0;
-        if (cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZP::smem_bytes) != cudaSuccess) return FFTB_ECUDA;
-        if (!grid_cap) grid_cap = zpers_grid(kp, ZP::smem_bytes, 1 << 30);
-        kp<<<total < grid_cap ? total : grid_cap, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
-        return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+        int grid = 0;
+        if (int rc = zpers_launch_grid(kp, R4Z_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
+        kp<<<grid, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
+        return launch_status();
     }
     auto k = zpass_r4_fwd_k<T, R4Z_NW>;
     const size_t smem = ZR4<T, R4Z_NW>::smem_bytes;
-    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return FFTB_ECUDA;
+    if (int rc = kernel_ready(k, R4Z_NW * 32, smem, nullptr)) return rc;
     dim3 grid((pl.nsticks + ZR4<T, R4Z_NW>::TS - 1) / ZR4<T, R4Z_NW>::TS, nb);
     k<<<grid, R4Z_NW * 32, smem, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride);
-    return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA;
+    return launch_status();
 }
 
 bool find_z_fast(int dtype, int n, bool dense, ZLaunch *out)
@@ -325,14 +346,81 @@ bool find_z_fast(int dtype, int n, bool dense, ZLaunch *out)
     if (dtype == FFTB_C128 && n == 256) { *out = ZLaunch{&launch_zr4_inv<double>, &launch_zr4_fwd<double>}; return true; }
     if (dtype == FFTB_C64 && n == 256) { *out = ZLaunch{&launch_zr4_inv<float>, &launch_zr4_fwd<float>}; return true; }
     if (dtype == FFTB_C128 && n == 128) { *out = make_z_fast<double, 128, 8, 8>(); return true; }
-#ifndef FFTB_DEV
     if (dtype == FFTB_C128 && n == 64) { *out = make_z_fast<double, 64, 8, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 128) { *out = make_z_fast<float, 128, 8, 8>(); return true; }
     if (dtype == FFTB_C64 && n == 64) { *out = make_z_fast<float, 64, 8, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 96) { *out = make_z_fast<float, 96, 12, 4>(); return true; }
     if (dtype == FFTB_C128 && n == 96) { *out = make_z_fast<double, 96, 12, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 192) { *out = make_z_fast<float, 192, 24, 4>(); return true; }     // 96 = 24 x 4
-#endif
+    return false;
+}
+
+// ------------------------------------------------------------------------------------------------
+// fused launches (fftb_fused.cuh): cubic grids whose z axis uses the plane kernel's factorisation
+// ------------------------------------------------------------------------------------------------
+template <class K> int fused_grid(K k, int threads, size_t smem, const DevPlan &pl, int items, int *grid)
+{
+    int per_sm = 0;
+    if (int rc = kernel_ready(k, threads, smem, &per_sm)) return rc;
+    const int cap = pl.sms * per_sm; // every CTA of a cooperative launch is resident
+    *grid = items < cap ? items : cap;
+    return 0;
+}
+template <typename T, class F>
+int launch_fused_inv(const DevPlan &pl, const PlanTabs &tabs, const void *packed, void *ring, const CUtensorMap &ring_map, void *cuboid,
+                     long long stride, int nb, int nslot, int lead, int hints, int *sync, cudaStream_t st)
+{
+    constexpr int NW = PlaneNW<F::N>::value;
+    using FU = Fused<T, F, NW>;
+    auto k = fused_inv_k<T, F, NW>;
+    const int ntiles = (pl.nsticks + FU::Z::TS - 1) / FU::Z::TS;
+    const size_t smem = FU::smem_inv(ntiles);
+    if (smem > 227 * 1024) return FFTB_EUNSUPPORTED;
+    const int items = nb * (pl.n3 > ntiles ? pl.n3 : ntiles);
+    int grid = 0;
+    if (int rc = fused_grid(k, NW * 32, smem, pl, items, &grid)) return rc;
+    if (cudaMemsetAsync(sync, 0, 2 * sizeof(int) * (size_t)nb, st) != cudaSuccess) return FFTB_ECUDA;
+    const cx<T> *a_packed = (const cx<T> *)packed;
+    cx<T> *a_ring = (cx<T> *)ring, *a_cub = (cx<T> *)cuboid;
+    int *zdone = sync, *pdone = sync + nb;
+    void *args[] = {(void *)&pl, (void *)&tabs.ct, (void *)&a_packed, (void *)&a_ring, (void *)&ring_map, (void *)&a_cub, (void *)&stride,
+                    (void *)&nb, (void *)&nslot, (void *)&lead, (void *)&hints, (void *)&zdone, (void *)&pdone};
+    if (cudaLaunchCooperativeKernel((const void *)k, dim3(grid), dim3(NW * 32), args, smem, st) != cudaSuccess) return FFTB_ECUDA;
+    return launch_status();
+}
+template <typename T, class F>
+int launch_fused_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *cuboid, void *ring, void *packed, long long stride, int nb, int nslot,
+                     int lead, int hints, int *sync, cudaStream_t st)
+{
+    constexpr int NW = PlaneNW<F::N>::value;
+    using FU = Fused<T, F, NW>;
+    auto k = fused_fwd_k<T, F, NW>;
+    const size_t smem = FU::smem_fwd;
+    const int ntiles = (pl.nsticks + FU::Z::TS - 1) / FU::Z::TS;
+    const int items = nb * (pl.n3 > ntiles ? pl.n3 : ntiles);
+    int grid = 0;
+    if (int rc = fused_grid(k, NW * 32, smem, pl, items, &grid)) return rc;
+    if (cudaMemsetAsync(sync, 0, 2 * sizeof(int) * (size_t)nb, st) != cudaSuccess) return FFTB_ECUDA;
+    const cx<T> *a_cub = (const cx<T> *)cuboid;
+    cx<T> *a_ring = (cx<T> *)ring, *a_packed = (cx<T> *)packed;
+    int *pdone = sync, *zdone = sync + nb;
+    void *args[] = {(void *)&pl, (void *)&tabs.ct, (void *)&a_cub, (void *)&a_ring, (void *)&a_packed, (void *)&stride, (void *)&nb,
+                    (void *)&nslot, (void *)&lead, (void *)&hints, (void *)&pdone, (void *)&zdone};
+    if (cudaLaunchCooperativeKernel((const void *)k, dim3(grid), dim3(NW * 32), args, smem, st) != cudaSuccess) return FFTB_ECUDA;
+    return launch_status();
+}
+template <typename T, int N, int P1, int P2> FusedLaunch make_fused()
+{
+    using F = FastCfg<T, N, P1, P2>;
+    static_assert(Fused<T, F, PlaneNW<N>::value>::smem_fwd <= 227 * 1024, "fused forward kernel does not fit in shared memory");
+    using Z = typename Fused<T, F, PlaneNW<N>::value>::Z;
+    return FusedLaunch{FusedGeom{Z::TS, Z::TILE, Z::RP}, &launch_fused_inv<T, F>, &launch_fused_fwd<T, F>};
+}
+bool find_fused(int dtype, const int32_t n[3], bool dense, FusedLaunch *out)
+{
+    if (dense || n[0] != n[1] || n[0] != n[2]) return false;
+    if (dtype == FFTB_C128 && n[0] == 128) { *out = make_fused<double, 128, 8, 8>(); return true; }
+    if (dtype == FFTB_C64 && n[0] == 128) { *out = make_fused<float, 128, 8, 8>(); return true; }
     return false;
 }
 
@@ -355,18 +443,12 @@ bool find_z(int dtype, int n, bool dense, ZLaunch *out)
 {
 #define ZCASE(T, DT, N, D) \
     if (dtype == DT && n == N && dense == D) { *out = make_z<T, N, D>(); return true; }
-    ZCASE(double, FFTB_C128, 128, false)
-#ifdef FFTB_DEV256
-    ZCASE(double, FFTB_C128, 256, false)
-#endif
-#ifndef FFTB_DEV /* development builds (-DFFTB_DEV) instantiate the 128^3 complex128 kernels only */
     ZCASE(double, FFTB_C128, 32, false) ZCASE(double, FFTB_C128, 64, false) ZCASE(double, FFTB_C128, 96, false)
-    ZCASE(double, FFTB_C128, 192, false) ZCASE(double, FFTB_C128, 256, false)
+    ZCASE(double, FFTB_C128, 128, false) ZCASE(double, FFTB_C128, 192, false) ZCASE(double, FFTB_C128, 256, false)
     ZCASE(float, FFTB_C64, 32, false) ZCASE(float, FFTB_C64, 64, false) ZCASE(float, FFTB_C64, 96, false)
     ZCASE(float, FFTB_C64, 128, false) ZCASE(float, FFTB_C64, 192, false) ZCASE(float, FFTB_C64, 256, false)
     ZCASE(double, FFTB_C128, 32, true) ZCASE(double, FFTB_C128, 64, true) ZCASE(double, FFTB_C128, 128, true)
     ZCASE(double, FFTB_C128, 256, true)
-#endif
 #undef ZCASE
     return false;
 }
@@ -374,18 +456,12 @@ bool find_plane(int dtype, int n, bool dense, PlaneLaunch *out)
 {
 #define PCASE(T, DT, N, D) \
     if (dtype == DT && n == N && dense == D) { *out = make_plane<T, N, D>(); return true; }
-    PCASE(double, FFTB_C128, 128, false)
-#ifdef FFTB_DEV256
-    PCASE(double, FFTB_C128, 256, false)
-#endif
-#ifndef FFTB_DEV
     PCASE(double, FFTB_C128, 32, false) PCASE(double, FFTB_C128, 64, false) PCASE(double, FFTB_C128, 96, false)
-    PCASE(double, FFTB_C128, 192, false) PCASE(double, FFTB_C128, 256, false)
+    PCASE(double, FFTB_C128, 128, false) PCASE(double, FFTB_C128, 192, false) PCASE(double, FFTB_C128, 256, false)
     PCASE(float, FFTB_C64, 32, false) PCASE(float, FFTB_C64, 64, false) PCASE(float, FFTB_C64, 96, false)
     PCASE(float, FFTB_C64, 128, false) PCASE(float, FFTB_C64, 192, false) PCASE(float, FFTB_C64, 256, false)
     PCASE(double, FFTB_C128, 32, true) PCASE(double, FFTB_C128, 64, true) PCASE(double, FFTB_C128, 128, true)
     PCASE(double, FFTB_C128, 256, true)
-#endif
 #undef PCASE
     return false;
 }
@@ -424,8 +500,15 @@ struct fftb_plan_s {
     std::vector<unsigned char> h_tw[3];
     ZLaunch zl;
     PlaneLaunch plk;
+    FusedLaunch ful;
+    bool fused;          // fftb_inverse / fftb_forward are ONE cooperative launch each (fftb_fused.cuh)
+    int ring_bands, lead_bands; // the fused kernels' ring of intermediate band slots and the producers' lead
+    int l2_hints;        // fused kernels: evict_last on the ring, evict_first on the cuboid and packed streams
+    long long ring_slot; // elements of a ring slot: ntiles tile images (tile-major layout, fftb_fused.cuh)
+    int ring_ntiles;
+    CUtensorMap ring_map; // the ring as a 5-dimensional tensor (inverse plane items load a row out of every tile)
     // device block layout
-    size_t o_stick, o_col, o_perm, o_tw[3], o_ws, o_stage, bytes_min, bytes_stage;
+    size_t o_stick, o_col, o_perm, o_tw[3], o_sync, o_ws, o_stage, bytes_min, bytes_stage;
     long long a_inv_stride, a_fwd_stride; // elements per band of the intermediate (a_fwd_stride: vloc and generic forward)
     int chunk;                            // bands per kernel group (vloc: both intermediates live)
     int chunk_inv, chunk_fwd;             // inverse / forward alone
@@ -448,7 +531,7 @@ struct fftb_plan_s {
     size_t ev_used;
 };
 
-enum { K_ZINV = 0, K_PLANE_INV = 1, K_PLANE_FWD = 2, K_ZFWD = 3, K_PLANE_VLOC = 4, K_KINDS = 5 };
+enum { K_ZINV = 0, K_PLANE_INV = 1, K_PLANE_FWD = 2, K_ZFWD = 3, K_PLANE_VLOC = 4, K_FUSED_INV = 5, K_FUSED_FWD = 6, K_KINDS = 7 };
 
 static void prof_begin(fftb_plan p, int kind, cudaStream_t st)
 {
@@ -487,10 +570,13 @@ const char *fftb_strerror(int code)
 
 struct ExplicitMap { int64_t n; const int32_t *k1, *k2, *k3lo, *len; };
 
-static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const ExplicitMap *xm)
+static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const ExplicitMap *xm, const fftb_plan_tuning *tune)
 {
     if (!out || !desc) return FFTB_EINVAL;
     *out = nullptr;
+    const uint32_t tflags = tune ? tune->flags : 0u;
+    if (tflags & ~(uint32_t)(FFTB_TUNE_GENERIC_Z | FFTB_TUNE_GENERIC_PLANE | FFTB_TUNE_FUSED | FFTB_TUNE_NO_L2_HINTS)) return FFTB_EINVAL;
+    if (tune && (tune->workspace_bytes < 0 || tune->ring_bands < 0 || tune->lead_bands < 0)) return FFTB_EINVAL;
     const bool dense = (desc->flags & FFTB_FLAG_DENSE) != 0;
     if (xm && (dense || xm->n < 1 || xm->n > (int64_t)1 << 24 || !xm->k1 || !xm->k2 || !xm->k3lo || !xm->len)) return FFTB_EINVAL;
     if (desc->flags & ~(uint32_t)FFTB_FLAG_DENSE) return FFTB_EINVAL;
@@ -518,12 +604,13 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
     PlaneLaunch plk;
     bool fast_plane = false;
     if (!find_z(desc->dtype, desc->n[2], dense, &zl) || !find_plane(desc->dtype, desc->n[0], dense, &plk)) return FFTB_EUNSUPPORTED;
+    bool fast_z = false;
     {
-        const char *gen = getenv("FFTB_GENERIC_PLANE"); // debugging aid: keep the generic plane kernel
+        const bool gen_plane = (tflags & FFTB_TUNE_GENERIC_PLANE) != 0, gen_z = (tflags & FFTB_TUNE_GENERIC_Z) != 0;
         PlaneLaunch fast;
-        if (!(gen && gen[0] == '1') && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) { plk = fast; fast_plane = true; }
+        if (!gen_plane && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) { plk = fast; fast_plane = true; }
         // 256 pattern: persistent plane kernels of their own (four-way split, fftb_plane_r4.cuh)
-        if (!(gen && gen[0] == '1') && !dense && desc->n[0] == 256) {
+        if (!gen_plane && !dense && desc->n[0] == 256) {
             if (desc->dtype == FFTB_C128) {
                 plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
                 plk.run[MODE_FWD] = &launch_plane_r4_fwd<double>;
@@ -536,10 +623,11 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
             plk.ry = 1; // the forward and vloc kernels accumulate the four y residues into ONE plane of A themselves
             fast_plane = true; // persistent kernel: whole-batch launches (256 planes per band on 148 CTAs would waste half a wave)
         }
-        const char *genz = getenv("FFTB_GENERIC_Z");
         ZLaunch zfast;
-        if (!(genz && genz[0] == '1') && find_z_fast(desc->dtype, desc->n[2], dense, &zfast)) zl = zfast;
+        if (!gen_z && find_z_fast(desc->dtype, desc->n[2], dense, &zfast)) { zl = zfast; fast_z = true; }
     }
+    FusedLaunch ful = {{0, 0, 0}, nullptr, nullptr};
+    const bool fused = fast_plane && fast_z && (tflags & FFTB_TUNE_FUSED) && find_fused(desc->dtype, desc->n, dense, &ful);
     if (!dense && !xm)
         for (int d = 0; d < 3; ++d)
             if (4 * (long long)desc->cutoff[d] > desc->n[d]) return FFTB_EUNSUPPORTED; // half-band kernels only
@@ -559,6 +647,9 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         p->elem = desc->dtype == FFTB_C128 ? 16 : 8;
         p->zl = zl;
         p->plk = plk;
+        p->ful = ful;
+        p->fused = fused;
+        p->l2_hints = (tflags & FFTB_TUNE_NO_L2_HINTS) ? 0 : 1;
         p->ry = plk.ry;
         const int n1 = desc->n[0], n2 = desc->n[1], n3 = desc->n[2];
         p->C = (int64_t)n1 * n2 * n3;
@@ -662,7 +753,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         p->a_fwd_stride = (long long)p->ry * n3 * p->pitch;
         const size_t per_band = (size_t)(p->a_inv_stride + p->a_fwd_stride) * p->elem; // vloc needs both
         size_t budget = fast_plane ? (size_t)4 << 30 : (size_t)48 << 20;
-        if (const char *e = getenv("FFTB_WS_MB")) { long v = atol(e); if (v > 0) budget = (size_t)v << 20; }
+        if (tune && tune->workspace_bytes > 0) budget = (size_t)tune->workspace_bytes;
         auto chunk_of = [&](size_t bytes_per_band) {
             long long c = (long long)(budget / bytes_per_band);
             if (c < 1) c = 1;
@@ -677,11 +768,26 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         p->o_col = o; o = align_up(o + sizeof(int4) * p->h_col.size(), 256);
         for (int d = 0; d < 3; ++d) { p->o_tw[d] = o; o = align_up(o + p->h_tw[d].size(), 256); }
         p->o_perm = o; o = align_up(o + sizeof(int) * p->h_colperm.size(), 256);
+        p->o_sync = o; o = align_up(o + 2 * sizeof(int) * (size_t)desc->batch, 256); // per-band counters of the fused launches
         {
             size_t ws = (size_t)desc->batch * per_band;
             if (ws > budget) ws = budget;
             if (ws < per_band) ws = per_band;
+            // fused launches: a ring of band slots at the start of the workspace that stays in L2 (6 x 6.7 MB at 128^3
+            // complex128), producers 2 bands ahead of their consumers; nslot > lead >= 0 (fftb_fused.cuh)
+            p->ring_ntiles = fused ? (p->nsticks + ful.geom.ts - 1) / ful.geom.ts : 0;
+            p->ring_slot = fused ? (long long)p->ring_ntiles * ful.geom.tile : 0;
+            const size_t slot = fused ? (size_t)p->ring_slot * p->elem : (size_t)p->a_inv_stride * p->elem;
+            long long ring = tune && tune->ring_bands > 0 ? tune->ring_bands : 0, lead = tune && tune->lead_bands > 0 ? tune->lead_bands : 3;
+            if (ring == 0) ring = lead + 5;
+            if (ring > desc->batch) ring = desc->batch;
+            if (fused && ws < (size_t)ring * slot && (size_t)ring * slot <= budget) ws = (size_t)ring * slot; // tile-major slots are a little larger
+            if (fused && ws < slot) ws = slot;
+            if (ring > (long long)(ws / slot)) ring = (long long)(ws / slot);
+            if (lead > ring - 1) lead = ring - 1;
             p->o_ws = o; o = align_up(o + ws, 256);
+            p->ring_bands = (int)ring;
+            p->lead_bands = (int)lead;
         }
         p->bytes_min = o;
         p->o_stage = o; o = align_up(o + (size_t)desc->batch * (size_t)p->S * p->elem, 256);
@@ -701,13 +807,18 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
     return FFTB_OK;
 }
 
-int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc) { return plan_create_impl(out, desc, nullptr); }
+int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc) { return plan_create_impl(out, desc, nullptr, nullptr); }
+
+int fftb_plan_create_tuned(fftb_plan *out, const fftb_plan_desc *desc, const fftb_plan_tuning *tuning)
+{
+    return plan_create_impl(out, desc, nullptr, tuning);
+}
 
 int fftb_plan_create_explicit(fftb_plan *out, const fftb_plan_desc *desc, int64_t n_sticks, const int32_t *k1, const int32_t *k2,
                               const int32_t *k3lo, const int32_t *len)
 {
     const ExplicitMap xm = {n_sticks, k1, k2, k3lo, len};
-    return plan_create_impl(out, desc, &xm);
+    return plan_create_impl(out, desc, &xm, nullptr);
 }
 
 int fftb_plan_info_get(fftb_plan p, fftb_plan_info *info)
@@ -725,6 +836,11 @@ int fftb_plan_info_get(fftb_plan p, fftb_plan_info *info)
     info->workspace_offset = (int64_t)p->o_ws;
     info->pitch = p->pitch;
     info->y_residues = p->ry;
+    info->ring_bands = p->fused ? p->ring_bands : 0;
+    info->lead_bands = p->fused ? p->lead_bands : 0;
+    info->ring_tile_sticks = p->fused ? p->ful.geom.ts : 0;
+    info->ring_tile_elems = p->fused ? p->ful.geom.tile : 0;
+    info->ring_pair_pitch = p->fused ? p->ful.geom.rp : 0;
     return FFTB_OK;
 }
 
@@ -768,6 +884,14 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
         p->pipe_ok = true;
     }
     DevPlan &dv = p->dev;
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+            p->sticky = FFTB_ECUDA;
+            return FFTB_ECUDA;
+        }
+        dv.sms = sms;
+    }
     dv.n1 = p->desc.n[0]; dv.n2 = p->desc.n[1]; dv.n3 = p->desc.n[2];
     dv.nsticks = p->nsticks; dv.pitch = p->pitch; dv.nxocc = p->nxocc; dv.k1lo = p->k1lo; dv.ry = p->ry;
     dv.stick = (const int4 *)(m + p->o_stick);
@@ -777,16 +901,42 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
     dv.tw1 = m + p->o_tw[0]; dv.tw2 = m + p->o_tw[1]; dv.tw3 = m + p->o_tw[2];
     dv.S = p->S;
     dv.scale = p->desc.scale == FFTB_SCALE_FORWARD ? 1.0 / (double)p->C : 1.0;
+    if (p->fused) {
+        // the ring as a tensor of 8-byte units: TS elements of a row | row parity | row pair | tile | slot (fftb_fused.cuh)
+        const FusedGeom &ge = p->ful.geom;
+        const cuuint64_t unit = p->elem / 8;
+        const cuuint64_t dims[5] = {(cuuint64_t)ge.ts * unit, 2, (cuuint64_t)p->desc.n[2] / 2, (cuuint64_t)p->ring_ntiles, (cuuint64_t)p->ring_bands};
+        const cuuint64_t strides[4] = {(cuuint64_t)ge.ts * p->elem, (cuuint64_t)ge.rp * p->elem, (cuuint64_t)ge.tile * p->elem,
+                                       (cuuint64_t)p->ring_slot * p->elem};
+        const cuuint32_t box[5] = {(cuuint32_t)(ge.ts * unit), 1, 1, (cuuint32_t)p->ring_ntiles, 1};
+        const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+        typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                      const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                      CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+            qres != cudaDriverEntryPointSuccess || p->ring_ntiles > 256 ||
+            ((encode_fn)fn)(&p->ring_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, m + p->o_ws, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+            cudaGetLastError();
+            p->fused = false; // the separate launches need nothing of the kind
+        }
+    }
     return FFTB_OK;
 }
 
-static int check_exec(fftb_plan p, const void *a, const void *b, int nb)
+// packed arrays: 16-byte aligned; cuboids: 32-byte aligned for complex128 (the plane kernels move (x, x+1) pairs as
+// one 32-byte access), 16-byte aligned for complex64
+static int check_exec(fftb_plan p, const void *packed, const void *cuboid, int nb)
 {
-    if (!p || !a || !b) return FFTB_EINVAL;
+    if (!p || !packed || (!cuboid && nb >= 0)) return FFTB_EINVAL;
     if (p->sticky) return p->sticky;
     if (!p->d_mem) return FFTB_ESTATE;
-    if (nb < 1 || nb > p->desc.batch) return FFTB_EINVAL;
-    if (((uintptr_t)a | (uintptr_t)b) % 16) return FFTB_EINVAL;
+    const int n = nb < 0 ? -nb : nb; // nb < 0: no cuboid operand (apply_vloc checks its second packed array itself)
+    if (n < 1 || n > p->desc.batch) return FFTB_EINVAL;
+    if ((uintptr_t)packed % 16) return FFTB_EINVAL;
+    if (cuboid && (uintptr_t)cuboid % (p->elem == 16 ? 32 : 16)) return FFTB_EINVAL;
     return FFTB_OK;
 }
 
@@ -797,6 +947,15 @@ int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void
     cudaStream_t st = (cudaStream_t)stream;
     unsigned char *A = p->d_mem + p->o_ws;
     p->launches = 0;
+    if (p->fused) { // one cooperative launch: z tiles and planes of the whole batch, A in a ring of band slots (L2)
+        prof_begin(p, K_FUSED_INV, st);
+        rc = p->ful.inv(p->dev, p->tabs, d_packed, A, p->ring_map, d_cuboid, p->ring_slot, nb, p->ring_bands, p->lead_bands, p->l2_hints,
+                        (int *)(p->d_mem + p->o_sync), st);
+        prof_end(p, st);
+        if (rc) { p->sticky = rc; return rc; }
+        p->launches = 1;
+        return FFTB_OK;
+    }
     for (int b0 = 0; b0 < nb; b0 += p->chunk_inv) {
         const int nc = nb - b0 < p->chunk_inv ? nb - b0 : p->chunk_inv;
         const unsigned char *pk = (const unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
@@ -815,11 +974,20 @@ int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void
 
 int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void *stream)
 {
-    int rc = check_exec(p, d_cuboid, d_packed, nb);
+    int rc = check_exec(p, d_packed, d_cuboid, nb);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     unsigned char *A = p->d_mem + p->o_ws;
     p->launches = 0;
+    if (p->fused) {
+        prof_begin(p, K_FUSED_FWD, st);
+        rc = p->ful.fwd(p->dev, p->tabs, d_cuboid, A, d_packed, p->ring_slot, nb, p->ring_bands, p->lead_bands, p->l2_hints,
+                        (int *)(p->d_mem + p->o_sync), st);
+        prof_end(p, st);
+        if (rc) { p->sticky = rc; return rc; }
+        p->launches = 1;
+        return FFTB_OK;
+    }
     for (int b0 = 0; b0 < nb; b0 += p->chunk_fwd) {
         const int nc = nb - b0 < p->chunk_fwd ? nb - b0 : p->chunk_fwd;
         unsigned char *pk = (unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
@@ -838,8 +1006,9 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
 
 int fftb_apply_vloc(fftb_plan p, const void *d_in, void *d_out, const void *d_vloc, int nb, void *stream)
 {
-    int rc = check_exec(p, d_in, d_out, nb);
+    int rc = check_exec(p, d_in, nullptr, -nb);
     if (rc) return rc;
+    if (!d_out || (uintptr_t)d_out % 16) return FFTB_EINVAL;
     if (!d_vloc || (uintptr_t)d_vloc % 16) return FFTB_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     unsigned char *Ai = p->d_mem + p->o_ws;
@@ -1090,3 +1259,4 @@ int fftb_plan_destroy(fftb_plan p)
 }
 
 } // extern "C"
+

@@ -45,6 +45,7 @@ struct DevPlan {
     const void *tw1, *tw2, *tw3; // exp(+j 2 pi i / N_d), i < N_d, in the plan's precision
     long long S;       // points per band
     double scale;      // applied in zpass_fwd
+    int sms;           // host side only: SM count of the device the plan was bound on
 };
 
 template <int N_, int R_, int P1_, int P2_, bool HALF_> struct Axis {

@@ -65,7 +65,6 @@ def test_inverse_forward_vs_oracle(fb, oracle, w):
     assert all(np.array_equal(x, y) for x, y in zip(k, ko))
     c = wl.coefficients(w, *k)
     d_c = torch.from_numpy(c).cuda()
-    # stage check: A after the inverse z pass == oracle's z-only stage, read through the stick columns
     d_psi = p.inverse(d_c)
     torch.cuda.synchronize()
     psi_ref = oracle.inverse(w.n, ko, c)
@@ -187,7 +186,7 @@ def test_batch_chunking_and_partial_batches(fb, oracle):
         rt = p.forward(d_psi)
         torch.cuda.synchronize()
         assert _rel(rt.cpu().numpy(), c[:nb]) <= w.tol
-    assert p.last_launches() == 2 * -(-37 // p.info["chunk_bands_fwd"])  # the last call was a forward
+    assert p.info["ring_bands"] == 0 and p.last_launches() == 2 * -(-37 // p.info["chunk_bands_fwd"])  # the last call was a forward
     with pytest.raises(fb.FftbError):
         p.inverse(torch.zeros((38, p.S), dtype=torch.complex128, device="cuda"))
 
@@ -461,18 +460,19 @@ def test_complex64_odd_packed_ranges(fb, oracle, n, a):
     p.destroy()
 
 
-def test_complex64_odd_band_chunks(fb, oracle, monkeypatch):
-    """A workspace of one band makes the library run band by band: with complex64 and an odd S every second chunk's
-    packed pointer is only 8-byte aligned, which the bulk copies of the z passes must cope with."""
-    monkeypatch.setenv("FFTB_WS_MB", "4")  # read by fftb_plan_create: 128^3 complex64 needs 3.3 MB of A per band
+def test_complex64_odd_band_chunks(fb, oracle):
+    """A workspace budget of one band (fftb_plan_tuning.workspace_bytes) makes the library run band by band: with
+    complex64 and an odd S every second chunk's packed pointer is only 8-byte aligned, which the bulk copies of the z
+    passes must cope with."""
     w = _small((128, 128, 128), (32, 32, 32), dtype="c64", batch=3)
-    p = _plan(fb, w, 3)
-    assert p.info["chunk_bands"] == 1 and p.S % 2 == 1
+    p = fb.Plan(w.n, w.cutoff, batch=3, dtype="c64", tuning={"workspace_bytes": 4 << 20}).bind()
+    assert p.info["chunk_bands"] == 1 and p.S % 2 == 1 and p.info["ring_bands"] == 0
     k = p.points()
     c = wl.coefficients(w, *k)
     d_psi = p.inverse(torch.from_numpy(c).cuda())
     rt = p.forward(d_psi)
     torch.cuda.synchronize()
+    assert p.last_launches() == 6
     assert _rel(d_psi.cpu().numpy(), oracle.inverse(w.n, k, c)) <= w.tol
     assert _rel(rt.cpu().numpy(), c) <= w.tol
     p.destroy()

@@ -1,0 +1,333 @@
+"""GPU tests added in round 2: the fused launches (z tiles + planes in one cooperative kernel, the intermediate in an
+L2-resident ring), stage-level parity through the bind block, the tuning descriptor, band sharding on the CUDA path,
+two host threads driving two plans, and the alignment contract.  All comparisons with the oracle use north_star's
+bar (relative L2 1e-12 / 1e-5) unless a docstring derives another one."""
+import threading
+
+import numpy as np
+import pytest
+
+from paper_2406_05577_b200 import workloads as wl
+from paper_2406_05577_b200.sharding import band_range
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _rel(a, b):
+    a = np.asarray(a, dtype=np.complex128).ravel()
+    b = np.asarray(b, dtype=np.complex128).ravel()
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def fb():
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2406_05577_b200 import binding
+
+    binding.lib()
+    return binding
+
+
+def _w(n, a, dtype="c128", batch=3, dist="uniform", number=0):
+    return wl.Workload(number, "t", n, a, dtype, batch, dist, "inv_fwd")
+
+
+def _intermediate(p, bands):
+    """The intermediate A[b][z][stick] of the listed bands (an int = the first so many), read out of the caller-owned
+    bind block through the layout fftb_plan_info describes: A[band][z][pitch] for separate launches, tile-major ring
+    slots (band b in slot b % ring_bands) for the fused launches."""
+    bands = list(range(bands)) if isinstance(bands, int) else list(bands)
+    n3, pitch, ns = p.n[2], p.info["pitch"], p.info["n_sticks"]
+    elem = 16 if p.dtype == "c128" else 8
+    off = p.info["workspace_offset"]
+    out = []
+    if p.info["ring_bands"] == 0:
+        for b in bands:
+            raw = p.mem[off + b * n3 * pitch * elem:off + (b + 1) * n3 * pitch * elem]
+            out.append(raw.view(p.torch_complex).view(n3, pitch)[:, :ns].cpu().numpy())
+        return np.stack(out)
+    ts, te, rp, ring = p.info["ring_tile_sticks"], p.info["ring_tile_elems"], p.info["ring_pair_pitch"], p.info["ring_bands"]
+    slot = -(-ns // ts) * te
+    s, z = np.arange(ns)[None, :], np.arange(n3)[:, None]
+    idx = (s // ts) * te + (z // 2) * rp + (z % 2) * ts + s % ts
+    for b in bands:
+        sl = b % ring
+        raw = p.mem[off + sl * slot * elem:off + (sl + 1) * slot * elem].view(p.torch_complex).cpu().numpy()
+        out.append(raw[idx])
+    return np.stack(out)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# fused launches
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.timeout(300)
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("nb,ring,lead", [(1, 0, 0), (3, 0, 0), (7, 2, 1), (13, 3, 2), (40, 0, 0), (9, 1, 0)])
+def test_fused_launch_equals_separate_launches(fb, oracle, dtype, nb, ring, lead):
+    """fftb_inverse / fftb_forward as ONE cooperative launch (ring of band slots, per-band counters) do the same
+    arithmetic in the same order as the separate z-pass and plane launches: the outputs are bit-identical, for batches
+    smaller than, equal to and several times the ring, and for the smallest legal rings (slot reuse on every band)."""
+    w = _w((128, 128, 128), (32, 32, 32), dtype=dtype, batch=nb, dist="normal_decay", number=3)
+    pf = fb.Plan(w.n, w.cutoff, batch=nb, dtype=dtype, tuning={"flags": fb.FFTB_TUNE_FUSED, "ring_bands": ring, "lead_bands": lead}).bind()
+    pu = fb.Plan(w.n, w.cutoff, batch=nb, dtype=dtype).bind()
+    assert pf.info["ring_bands"] >= 1 and pu.info["ring_bands"] == 0
+    if ring:
+        assert pf.info["ring_bands"] == min(ring, nb) and pf.info["lead_bands"] <= max(pf.info["ring_bands"] - 1, 0)
+    k = pf.points()
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    psi_f, psi_u = pf.inverse(d_c), pu.inverse(d_c)
+    assert pf.last_launches() == 1 and pu.last_launches() == 2
+    torch.cuda.synchronize()
+    assert torch.equal(psi_f, psi_u)
+    g = torch.from_numpy(wl.cuboid(w, batch=min(nb, 3))).cuda()
+    g = g.repeat((nb + g.shape[0] - 1) // g.shape[0], 1, 1, 1)[:nb].contiguous()
+    g[nb - 1] *= 0.5  # the last band differs from its copies
+    f_f, f_u = pf.forward(g), pu.forward(g)
+    torch.cuda.synchronize()
+    assert torch.equal(f_f, f_u)
+    rt = pf.forward(psi_f)
+    torch.cuda.synchronize()
+    assert _rel(rt.cpu().numpy(), c) <= w.tol
+    sample = sorted({0, nb // 2, nb - 1})
+    assert _rel(psi_f[sample].cpu().numpy(), oracle.inverse(w.n, k, c[sample])) <= w.tol
+    pf.destroy(); pu.destroy()
+
+
+@pytest.mark.timeout(300)
+def test_fused_launch_repeatable(fb):
+    """The counters that order the items are cleared by every call: 20 back-to-back inverse + forward calls on one
+    plan, every result bit-identical to the first (a lost wake-up or a slot overwritten too early would show)."""
+    w = _w((128, 128, 128), (32, 32, 32), batch=24, dist="normal_decay", number=3)
+    p = fb.Plan(w.n, w.cutoff, batch=24, tuning={"flags": fb.FFTB_TUNE_FUSED, "ring_bands": 3, "lead_bands": 2}).bind()
+    assert p.info["ring_bands"] == 3
+    d_c = torch.from_numpy(wl.coefficients(w, *p.points())).cuda()
+    psi0 = p.inverse(d_c).clone()
+    rt0 = p.forward(psi0).clone()
+    for _ in range(20):
+        psi = p.inverse(d_c)
+        rt = p.forward(psi)
+        torch.cuda.synchronize()
+        assert torch.equal(psi, psi0) and torch.equal(rt, rt0)
+    p.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# stage-level parity: the intermediate A read back through fftb_plan_info.workspace_offset / pitch
+# ---------------------------------------------------------------------------------------------------------------
+STAGE = [((64, 64, 64), (16, 16, 16), "c128", {}), ((128, 128, 128), (32, 32, 32), "c128", {}),
+         ((128, 128, 128), (32, 32, 32), "c128", {"flags": 4}), ((128, 128, 128), (32, 32, 32), "c64", {"flags": 4}),
+         ((256, 256, 256), (64, 64, 64), "c128", {}),
+         ((96, 96, 192), (24, 24, 48), "c64", {}), ((32, 32, 32), (8, 8, 8), "c128", {})]
+
+
+@pytest.mark.parametrize("n,a,dtype,tuning", STAGE, ids=[f"{n[0]}x{n[2]}-{d}-{'fused' if t else 'default'}" for n, a, d, t in STAGE])
+def test_stage_parity_inverse_z_and_forward_xy(fb, oracle, n, a, dtype, tuning):
+    """After fftb_inverse the bind block holds A[b][z][stick] = the z-only stage of the oracle (its n_axes = 1 output)
+    at the stick's (k1 mod N1, k2 mod N2) column: every stick is an independent 1D transform, so the error is measured
+    PER STICK relative to that stick's own norm (a misplaced or mis-scaled stick cannot hide behind the others).
+    After fftb_forward it holds the x+y stage: for every z-plane the 2D transform of the plane at the stick columns,
+    which the oracle computes as its forward on an (N1, N2, 1) grid with the planes as batch."""
+    nb = 2
+    w = _w(n, a, dtype=dtype, batch=nb)
+    p = fb.Plan(n, a, batch=nb, dtype=dtype, scale="none", tuning=tuning or None).bind()
+    m = p.get_map()
+    k = p.points()
+    ns = p.info["n_sticks"]
+    c = wl.coefficients(w, *k)
+    p.inverse(torch.from_numpy(c).cuda())
+    torch.cuda.synchronize()
+    A = _intermediate(p, nb).astype(np.complex128)                                   # [b][z][s]
+    stage = oracle.inverse(n, k, c, n_axes=1)                                        # [b][i3][i2][i1], z transformed only
+    ref = stage[:, :, m["k2"] % n[1], m["k1"] % n[0]]                                # [b][z][s]
+    err = np.linalg.norm(A - ref, axis=1) / np.linalg.norm(ref, axis=1)               # per band and stick
+    assert err.max() <= w.tol, f"inverse z stage: stick {np.unravel_index(err.argmax(), err.shape)} rel {err.max():.3e}"
+    # forward: x+y stage
+    g = wl.cuboid(w, batch=nb)
+    p.forward(torch.from_numpy(g).cuda())
+    torch.cuda.synchronize()
+    assert p.info["y_residues"] == 1 or n[0] in (32, 192)
+    if p.info["y_residues"] == 1:
+        A = _intermediate(p, nb).astype(np.complex128)
+        k2d = (m["k1"], m["k2"], np.zeros(ns, np.int32))
+        ref = oracle.forward((n[0], n[1], 1), k2d, g.reshape(nb * n[2], 1, n[1], n[0]), 1.0).reshape(nb, n[2], ns)
+        assert _rel(A, ref) <= w.tol
+    p.destroy()
+
+
+@pytest.mark.timeout(600)
+@pytest.mark.parametrize("fused", [False, True], ids=["default", "fused"])
+def test_full_size_config3_stage_per_stick_and_generic_forward(fb, oracle, fused):
+    """Config 3 at full batch, in the launch configuration bench.py times (and in the opt-in fused one).  Its
+    1/(1+|k|^2) decay makes the whole-output L2 error blind to the high-|k| sticks, so (i) the intermediate of sampled
+    bands after the full-batch inverse is compared with the oracle's z-only stage STICK BY STICK; (ii) a full batch of
+    generic (not band-limited, seeded on the device) cuboids is transformed forward and two sampled bands are compared
+    with the oracle."""
+    w = wl.WORKLOADS[3]
+    p = fb.Plan(w.n, w.cutoff, batch=w.batch, dtype=w.dtype, tuning={"flags": fb.FFTB_TUNE_FUSED} if fused else None).bind()
+    ring = p.info["ring_bands"]
+    assert (ring >= 2) == fused
+    m, k = p.get_map(), p.points()
+    c = wl.coefficients(w, *k)
+    d_psi = p.inverse(torch.from_numpy(c).cuda())
+    torch.cuda.synchronize()
+    sample = [w.batch - 1, w.batch - ring] if fused else [0, 77, w.batch - 1]  # fused: the bands still in the ring
+    A = _intermediate(p, sample)
+    for got, b in zip(A, sample):
+        ref = oracle.inverse(w.n, k, c[b:b + 1], n_axes=1)[0][:, m["k2"] % w.n[1], m["k1"] % w.n[0]]
+        err = np.linalg.norm(got - ref, axis=0) / np.linalg.norm(ref, axis=0)
+        assert err.max() <= w.tol, f"band {b} stick {err.argmax()}: {err.max():.3e}"
+    del d_psi
+    gen = torch.Generator(device="cuda").manual_seed(3003)
+    g = torch.empty(p.cuboid_shape(w.batch), dtype=torch.complex128, device="cuda")
+    torch.view_as_real(g).uniform_(-1.0, 1.0, generator=gen)
+    f = p.forward(g)
+    torch.cuda.synchronize()
+    C = float(np.prod(w.n))
+    for b in (5, w.batch - 2):
+        ref = oracle.forward(w.n, k, g[b:b + 1].cpu().numpy(), 1.0 / C)
+        assert _rel(f[b:b + 1].cpu().numpy(), ref) <= w.tol
+    p.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# tuning descriptor (replaces the environment variables of round 1)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,a,dtype", [((64, 64, 64), (16, 16, 16), "c128"), ((128, 128, 128), (32, 32, 32), "c128"),
+                                       ((128, 128, 64), (32, 20, 16), "c64"), ((96, 96, 96), (24, 24, 24), "c64")])
+@pytest.mark.parametrize("flags", [1, 2, 3], ids=["generic_z", "generic_plane", "generic_both"])
+def test_generic_kernels_through_tuning_flags(fb, oracle, n, a, dtype, flags):
+    """FFTB_TUNE_GENERIC_Z / _PLANE route a plan through the generic kernels of fftb_kernels.cuh at sizes where a
+    persistent kernel exists: all four combinations of z pass and plane kernel agree with the oracle."""
+    w = _w(n, a, dtype=dtype, batch=3)
+    p = fb.Plan(n, a, batch=3, dtype=dtype, tuning={"flags": flags}).bind()
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    d_psi = p.inverse(d_c)
+    torch.cuda.synchronize()
+    assert _rel(d_psi.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol
+    g = wl.cuboid(w)
+    C = float(np.prod(n))
+    d_f = p.forward(torch.from_numpy(g).cuda())
+    v = wl.potential(w)
+    d_o = p.apply_vloc(d_c, torch.from_numpy(v).cuda())
+    torch.cuda.synchronize()
+    assert _rel(d_f.cpu().numpy(), oracle.forward(n, k, g, 1.0 / C)) <= w.tol
+    assert _rel(d_o.cpu().numpy(), oracle.apply_vloc(n, k, c, v, 1.0 / C)) <= w.tol
+    p.destroy()
+
+
+def test_tuning_is_validated(fb):
+    with pytest.raises(fb.FftbError) as e:
+        fb.Plan((64, 64, 64), (16, 16, 16), tuning={"flags": 16})
+    assert e.value.code == fb.FFTB_EINVAL
+    with pytest.raises(fb.FftbError) as e:
+        fb.Plan((64, 64, 64), (16, 16, 16), tuning={"ring_bands": -1})
+    assert e.value.code == fb.FFTB_EINVAL
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# alignment contract
+# ---------------------------------------------------------------------------------------------------------------
+def test_misaligned_pointers_are_refused(fb):
+    """complex128 cuboids are moved as 32-byte (x, x+1) pairs: a cuboid pointer at 16 mod 32 must come back as
+    FFTB_EINVAL instead of raising a misaligned-address fault in the kernel; packed pointers need 16 bytes."""
+    import ctypes
+
+    w = _w((64, 64, 64), (16, 16, 16), batch=1)
+    p = fb.Plan(w.n, w.cutoff, batch=1).bind()
+    L = fb.lib()
+    d_c = torch.zeros(p.S + 2, dtype=torch.complex128, device="cuda")
+    buf = torch.zeros(int(np.prod(w.n)) + 2, dtype=torch.complex128, device="cuda")
+    assert buf.data_ptr() % 32 == 0 and d_c.data_ptr() % 16 == 0
+    vp = ctypes.c_void_p
+    assert L.fftb_inverse(p._h, vp(d_c.data_ptr()), vp(buf.data_ptr() + 16), 1, None) == fb.FFTB_EINVAL
+    assert L.fftb_forward(p._h, vp(buf.data_ptr() + 16), vp(d_c.data_ptr()), 1, None) == fb.FFTB_EINVAL
+    assert L.fftb_inverse(p._h, vp(d_c.data_ptr() + 8), vp(buf.data_ptr()), 1, None) == fb.FFTB_EINVAL
+    assert L.fftb_inverse(p._h, vp(d_c.data_ptr() + 16), vp(buf.data_ptr() + 32), 1, None) == fb.FFTB_OK
+    torch.cuda.synchronize()
+    p.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# band sharding and host threads on the CUDA path
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,a,dtype,nb", [((128, 128, 128), (32, 32, 32), "c128", 11), ((64, 64, 64), (16, 16, 16), "c128", 9),
+                                          ((96, 96, 192), (24, 24, 48), "c64", 6)])
+def test_band_shards_are_bit_identical_to_the_unsharded_call(fb, oracle, n, a, dtype, nb):
+    """the batch is the only dimension split over GPUs.  Two shards
+    (sharding.band_range, world 2) run through two plans on two streams of one device: the concatenation equals the
+    unsharded fftb_inverse / fftb_apply_vloc result bit for bit, and the oracle within tolerance."""
+    w = _w(n, a, dtype=dtype, batch=nb)
+    whole = fb.Plan(n, a, batch=nb, dtype=dtype).bind()
+    k = whole.points()
+    c = wl.coefficients(w, *k)
+    v = wl.potential(w)
+    d_c, d_v = torch.from_numpy(c).cuda(), torch.from_numpy(v).cuda()
+    psi = whole.inverse(d_c)
+    hv = whole.apply_vloc(d_c, d_v)
+    torch.cuda.synchronize()
+    parts_psi, parts_hv, streams, plans = [], [], [], []
+    for r in range(2):
+        lo, hi = band_range(nb, 2, r)
+        pr = fb.Plan(n, a, batch=hi - lo, dtype=dtype).bind()
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            shard = d_c[lo:hi].contiguous()
+            parts_psi.append(pr.inverse(shard, stream=s))
+            parts_hv.append(pr.apply_vloc(shard, d_v, stream=s))
+        streams.append(s); plans.append(pr)
+    for s in streams:
+        s.synchronize()
+    assert torch.equal(torch.cat(parts_psi), psi) and torch.equal(torch.cat(parts_hv), hv)
+    sample = [0, nb - 1]
+    assert _rel(psi[sample].cpu().numpy(), oracle.inverse(n, k, c[sample])) <= w.tol
+    assert _rel(hv[sample].cpu().numpy(), oracle.apply_vloc(n, k, c[sample], v, 1.0 / float(np.prod(n)))) <= w.tol
+    for pr in plans + [whole]:
+        pr.destroy()
+
+
+@pytest.mark.timeout(300)
+def test_two_host_threads_two_plans(fb):
+    """Two host threads drive two plans of different pitch through the same kernel instantiations on two streams
+    (ctypes releases the GIL during the calls): the launch-side state is per plan or guarded, so every result equals
+    the one the same plan produced alone."""
+    specs = [((128, 128, 128), (32, 32, 32), 6), ((128, 128, 128), (20, 27, 13), 5), ((64, 64, 64), (16, 16, 16), 7), ((64, 64, 64), (9, 12, 16), 4)]
+    jobs = []
+    for i, (n, a, nb) in enumerate(specs):
+        w = _w(n, a, batch=nb)
+        p = fb.Plan(n, a, batch=nb, tuning={"flags": fb.FFTB_TUNE_FUSED} if i == 1 else None).bind()
+        d_c = torch.from_numpy(wl.coefficients(w, *p.points())).cuda()
+        d_v = torch.from_numpy(wl.potential(w)).cuda()
+        ref = (p.inverse(d_c).clone(), p.forward(p.inverse(d_c)).clone(), p.apply_vloc(d_c, d_v).clone())
+        jobs.append((p, d_c, d_v, ref))
+    torch.cuda.synchronize()
+    errors = []
+
+    def run(my):
+        try:
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                for _ in range(8):
+                    for p, d_c, d_v, ref in my:
+                        psi = p.inverse(d_c, stream=s)
+                        rt = p.forward(psi, stream=s)
+                        hv = p.apply_vloc(d_c, d_v, stream=s)
+                        s.synchronize()
+                        if not (torch.equal(psi, ref[0]) and torch.equal(rt, ref[1]) and torch.equal(hv, ref[2])):
+                            errors.append("mismatch")
+        except Exception as exc:  # noqa: BLE001
+            errors.append(repr(exc))
+
+    th = [threading.Thread(target=run, args=(jobs[0::2],)), threading.Thread(target=run, args=(jobs[1::2],))]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    assert not errors, errors[:3]
+    for p, *_ in jobs:
+        p.destroy()
