@@ -6,8 +6,9 @@
 One "step" = one pass of the whole hot path over one batch of synthetic input: for the default
 workload (BASELINE.json configs[2], "config 3": 128^3 grid, complex128, 128 bands, sphere radius 32)
 that is fftb_inverse followed by fftb_forward on all 128 bands, i.e. 256 band 3D-FFTs.
-Prints ONE JSON line on rank 0.  N > 1 shards BANDS over GPUs (every rank owns a full batch: weak
-scaling, no data-path collective).
+Prints ONE JSON line on rank 0.  N > 1 shards BANDS over GPUs, no data-path collective:
+--scaling weak (default) gives every rank a full batch of its own, --scaling strong splits the config's
+batch over the ranks with sharding.band_range.
 """
 from __future__ import annotations
 
@@ -31,8 +32,7 @@ METRIC = "band 3D-FFTs/sec (inv+fwd)"
 UNIT = "band-FFTs/s"
 NOMINAL_HBM_GBS = 8000.0     # BASELINE.json's "~8 TB/s" target denominator
 FALLBACK_HBM_GBS = 6650.0    # /opt/skills/guides/B200_PROFILING.md fallback
-FP64_PEAK_TFLOPS = 36.1      # probed on this pool's B200: 62 FMA/clk/SM @ 1965 MHz
-FP32_PEAK_TFLOPS = 65.9
+ALU_PROBE_RECORD = "profiles/r02_alu_probe.md"   # a recorded run of the probe bench.py repeats live (fftb_probe_fma)
 
 
 def measured_peaks():
@@ -136,6 +136,7 @@ def time_oracle(w, steps, warmup):
         oracle_step(w, k, c, v, orc)
     dt = (time.perf_counter() - t0) / steps
     return {"value": 2 * nb / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "what": "the plain oracle of oracle/ (per-axis DFT over the full padded cuboid, never tuned): a reported baseline, not a CPU FFT library",
             "sample": f"{nb} of {w.batch} bands of the workload per step (inverse+forward each), oracle as it stands, "
                       f"-O2 -fopenmp, {steps} steps after {warmup} warm-up"}, dt
 
@@ -183,7 +184,13 @@ def run_ours(args, w):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     fb.lib()  # fail loudly if libfftb.so is missing
 
-    nb = w.batch
+    from paper_2406_05577_b200.sharding import band_range, max_over_ranks
+
+    strong = args.scaling == "strong"
+    lo, hi = band_range(w.batch, world, rank) if strong else (0, w.batch)
+    nb = hi - lo
+    if nb < 1:
+        raise SystemExit(f"bench.py: --scaling strong needs at least one band per rank ({w.batch} bands, {world} ranks)")
     tflags = (fb.FFTB_TUNE_FUSED if args.fused else 0) | (fb.FFTB_TUNE_NO_L2_HINTS if args.no_l2_hints else 0)
     tuning = {"flags": tflags} if tflags else None
     if args.ring_bands or args.lead_bands:
@@ -192,8 +199,10 @@ def run_ours(args, w):
     info = plan.info
     elem = 16 if w.dtype == "c128" else 8
     k = plan.points()
-    # every rank owns its own batch of bands (band sharding); the seed differs per rank
-    c = wl.coefficients(w, *k, seed=1000 + w.number + 7919 * rank)
+    # weak: every rank owns its own batch of bands (the seed differs per rank); strong: every rank draws the config's
+    # batch and keeps its own contiguous band range (band sharding)
+    c = wl.coefficients(w, *k)[lo:hi] if strong else wl.coefficients(w, *k, batch=nb, seed=1000 + w.number + 7919 * rank)
+    c = np.ascontiguousarray(c)
     h_c = torch.from_numpy(c).pin_memory()
     h_out = torch.empty_like(h_c).pin_memory()
     d_c = h_c.cuda()
@@ -249,10 +258,7 @@ def run_ours(args, w):
         if profile:
             plan.profile(False)
         barrier()
-        if world > 1:
-            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(ms, device="cuda")  # the only collective: timing
         return ms / steps, clocks, prof, launches
 
     K, W = max(1, args.steps), max(3, args.warmup)
@@ -261,7 +267,7 @@ def run_ours(args, w):
     ms_prof, _, prof, _ = timed(step, K, 3, profile=True)
     ms_e2e, _, _, _ = timed(step_e2e, K, max(1, min(W, 3)))
 
-    transforms = 2 * nb * world
+    transforms = 2 * (w.batch if strong else nb * world)
     value = transforms / (ms_step * 1e-3)
     e2e_value = transforms / (ms_e2e * 1e-3)
     peak, peak_kind = measured_peaks()
@@ -287,11 +293,16 @@ def run_ours(args, w):
             traffic, traffic_source = ent[dom], tj.get("_source", {}).get(f"config{w.number}")
     except Exception:
         pass
-    if dom in ("fused_inv", "fused_fwd", "plane_inv", "plane_fwd"):
+    if dom in ("fused_inv", "fused_fwd", "plane_inv", "plane_fwd", "zpass_inv", "zpass_fwd"):
         # algorithmic bytes per launch: a fused launch does a whole direction, (S + C) elements
         # per band; a plane launch moves the cuboid side, C elements per band (its other operand, the
         # intermediate A, is not algorithmic traffic)
-        per_band = (info["n_points"] + C) * elem if dom.startswith("fused") else C * elem
+        if dom.startswith("fused"):
+            per_band = (info["n_points"] + C) * elem
+        elif dom.startswith("plane"):
+            per_band = C * elem
+        else:  # a z pass (only the launch-bound config 1 has one on top): packed sphere + the intermediate it writes or reads
+            per_band = (info["n_points"] + w.n[2] * info["n_sticks"]) * elem
         bytes_total = K * nb * per_band
         ach = bytes_total / (dom_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
@@ -300,10 +311,11 @@ def run_ours(args, w):
                 "bytes_per_launch": bytes_total / max(dom_n, 1)}
     else:
         fl = K * nb * 2 * nominal_flops_per_band_dir(w.n, info)
-        pk = FP64_PEAK_TFLOPS if w.dtype == "c128" else FP32_PEAK_TFLOPS
+        pk, pk_ms = fb.probe_fma(w.dtype)  # the plain FMA rate of this GPU, measured now
         ach = fl / (dom_ms * 1e-3) / 1e12
         roof = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
-                "peak_kind": "register-only FMA probe on this pool's B200 (DESIGN.md)", "traffic": traffic, "traffic_source": traffic_source,
+                "peak_kind": f"fftb_probe_fma, register-only FMA loop run live in this process ({pk_ms:.3f} ms; recorded run: {ALU_PROBE_RECORD})",
+                "traffic": traffic, "traffic_source": traffic_source,
                 "avg_launch_ms": dom_ms / max(dom_n, 1), "launches_timed": dom_n,
                 "note": "fused vloc never writes the cuboid; flops counted as 5 N log2 N per pruned line, y and x passes twice"}
 
@@ -367,9 +379,9 @@ def run_ours(args, w):
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
             "dtype": "f64" if w.dtype == "c128" else "f32", "data": "synthetic",
-            "config": config_dict(w, {"parallelism": f"band-sharded x{world}, no collective", "chunk_bands": info["chunk_bands"],
+            "config": config_dict(w, {"parallelism": f"band-sharded x{world}, no collective", "bands_per_gpu": nb, "chunk_bands": info["chunk_bands"],
                                       "ring_bands": info["ring_bands"], "lead_bands": info["lead_bands"]}),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e,
@@ -401,6 +413,9 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5 (default 3, the graded one)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = a full batch per GPU (default), strong = the config's batch split over the GPUs (sharding.band_range)")
+    ap.add_argument("--probe-alu", action="store_true", help="print the FP64 / FP32 FMA probe (fftb_probe_fma) as JSON and exit")
     ap.add_argument("--fused", action="store_true", help="one cooperative launch per direction (FFTB_TUNE_FUSED): the intermediate stays in L2")
     ap.add_argument("--no-l2-hints", action="store_true", help="fused launches without L2 eviction priorities (FFTB_TUNE_NO_L2_HINTS)")
     ap.add_argument("--ring-bands", type=int, default=0, help="fused launches: band slots of the ring (0 = library default)")
@@ -412,6 +427,18 @@ def main():
     if args.op != "config" and args.op != w.op:
         import dataclasses
         w = dataclasses.replace(w, op=args.op, name=f"{w.name} [--op {args.op}]")
+    if args.probe_alu:
+        import torch
+
+        from paper_2406_05577_b200 import binding as fb
+
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        out = {"gpu": torch.cuda.get_device_name(), "sms": torch.cuda.get_device_properties(0).multi_processor_count}
+        for dt in ("c128", "c64"):
+            tf, ms = fb.probe_fma(dt)
+            out["fp64" if dt == "c128" else "fp32"] = {"tflops": tf, "ms": ms}
+        print(json.dumps(out), flush=True)
+        return
     if args.impl == "reference":
         run_reference(args, w)
     else:

@@ -207,6 +207,13 @@ int fftb_packed_transpose(fftb_plan p, const void *d_in, void *d_out, int nb, in
 /* Number of kernels the last execute call on this plan launched (for launch accounting). */
 int fftb_plan_last_launches(fftb_plan p);
 
+/* Device probe for benchmarks: the FMA rate of the plain FP64 (FFTB_C128) or FP32 (FFTB_C64) pipe of the current
+ * device in TFLOP/s (2 flops per FMA), from a register-only loop on all SMs; *ms (may be NULL) receives the best of
+ * five runs.  Unlike the execute calls this one allocates a scratch array, runs on the legacy default stream and WAITS
+ * for the result.  It is the denominator of the "alu" roofline of the fused local-potential workloads
+ * ("FP64 pipe utilisation ... over the probed peak"). */
+int fftb_probe_fma(int dtype, double *tflops, double *ms);
+
 /* Per-kernel timing for benchmarks.  fftb_plan_profile(p, 1) makes every later execute call record a
  * CUDA event pair around each kernel it launches (on the launching stream); fftb_plan_profile_read
  * waits for them, adds the elapsed milliseconds and launch counts per kernel kind into ms[7] and

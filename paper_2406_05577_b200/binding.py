@@ -26,7 +26,7 @@ SYMBOLS = [
     "fftb_inverse", "fftb_forward", "fftb_apply_vloc",
     "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
     "fftb_dense_embed", "fftb_dense_extract", "fftb_packed_transpose",
-    "fftb_plan_last_launches", "fftb_plan_profile", "fftb_plan_profile_read", "fftb_plan_destroy", "fftb_strerror",
+    "fftb_probe_fma", "fftb_plan_last_launches", "fftb_plan_profile", "fftb_plan_profile_read", "fftb_plan_destroy", "fftb_strerror",
 ]
 
 
@@ -78,6 +78,7 @@ def lib():
         for name in ("fftb_dense_embed", "fftb_dense_extract"):
             getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
         L.fftb_packed_transpose.argtypes = [vp, vp, vp, i32, i32, vp]
+        L.fftb_probe_fma.argtypes = [i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
         L.fftb_plan_last_launches.argtypes = [vp]
         L.fftb_plan_profile.argtypes = [vp, i32]
         L.fftb_plan_profile_read.argtypes = [vp, vp, vp]
@@ -90,6 +91,13 @@ def lib():
 
 def strerror(code: int) -> str:
     return lib().fftb_strerror(code).decode()
+
+
+def probe_fma(dtype="c128"):
+    """-> (TFLOP/s, ms) of the register-only FMA probe on the current device (fftb_probe_fma)."""
+    tf, ms = ctypes.c_double(), ctypes.c_double()
+    _check(lib().fftb_probe_fma(FFTB_C128 if dtype == "c128" else FFTB_C64, ctypes.byref(tf), ctypes.byref(ms)), "fftb_probe_fma")
+    return tf.value, ms.value
 
 
 def _check(rc, what):

@@ -12,6 +12,7 @@
 #include "fftb_plane_r4.cuh"
 #include "fftb_zpass_pf.cuh"
 #include "fftb_fused.cuh"
+#include "fftb_probe.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -1218,6 +1219,15 @@ int fftb_packed_transpose(fftb_plan p, const void *d_in, void *d_out, int nb, in
 }
 
 int fftb_plan_last_launches(fftb_plan p) { return p ? p->launches : FFTB_EINVAL; }
+
+int fftb_probe_fma(int dtype, double *tflops, double *ms)
+{
+    if (!tflops || (dtype != FFTB_C64 && dtype != FFTB_C128)) return FFTB_EINVAL;
+    const double v = dtype == FFTB_C128 ? probe_fma_tflops<double>(ms) : probe_fma_tflops<float>(ms);
+    if (v < 0.0) return FFTB_ECUDA;
+    *tflops = v;
+    return FFTB_OK;
+}
 
 
 int fftb_plan_profile(fftb_plan p, int enable)

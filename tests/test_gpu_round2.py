@@ -277,7 +277,7 @@ def test_band_shards_are_bit_identical_to_the_unsharded_call(fb, oracle, n, a, d
         s = torch.cuda.Stream()
         s.wait_stream(torch.cuda.current_stream())
         with torch.cuda.stream(s):
-            shard = d_c[lo:hi].contiguous()
+            shard = d_c[lo:hi].clone()  # a fresh allocation: a complex64 slice that starts on an odd band is only 8-byte aligned
             parts_psi.append(pr.inverse(shard, stream=s))
             parts_hv.append(pr.apply_vloc(shard, d_v, stream=s))
         streams.append(s); plans.append(pr)
