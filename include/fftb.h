@@ -225,6 +225,51 @@ int fftb_plan_profile_read(fftb_plan p, double *ms, int64_t *count);
 
 int fftb_plan_destroy(fftb_plan p);
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * Slab-distributed transform: ONE transform spread over `world` GPUs the way
+ * the paper's plane-wave variant does it on a 1D grid.  Rank r owns
+ *   - the sticks of a contiguous range of occupied k1 columns (ranges balanced by stick count), i.e. the contiguous
+ *     part [packed_lo[r], packed_lo[r+1]) of every band of the packed array, and
+ *   - the z-planes [z_lo[r], z_lo[r+1]) of the cuboid (contiguous slabs of N3).
+ * inverse: z pass on the own sticks -> exchange (only pruned stick data travels) -> y/x passes on the own planes;
+ * forward: the mirror image.  The library does every step but the transport: `*_begin` leaves the blocks for the
+ * peers either in `d_send` (layout [peer][band][row][column], peer blocks in rank order; hand it to an NCCL all-to-all
+ * with the counts of fftb_slab_plan_counts) or, when `d_peer` is given, directly in the peers' intermediates through
+ * peer-mapped pointers (d_peer[i] = what fftb_slab_plan_exchange_ptr returns on rank i; then the pack kernel IS the
+ * exchange and d_send / d_recv are not used).  `*_end` consumes `d_recv` ([peer][band][row][column]) or, with
+ * d_recv == NULL, the intermediate the peers have written.  The caller orders begin -> transport -> end (stream order on
+ * one GPU; a barrier or events between ranks).  Same conventions, scale, alignment and error codes as above;
+ * FFTB_EUNSUPPORTED additionally for world > 16, fewer occupied k1 columns or z-planes than ranks, FFTB_FLAG_DENSE, or a
+ * pattern whose forward plane kernel writes partial planes. */
+typedef struct fftb_slab_plan_s *fftb_slab_plan;
+
+typedef struct {
+    int64_t n_points_local;  /* packed points of this rank per band: packed_lo[rank+1] - packed_lo[rank] */
+    int64_t n_sticks_local;
+    int64_t planes_local;    /* z-planes of this rank's slab */
+    int64_t device_bytes;    /* smallest block fftb_slab_plan_bind accepts */
+    int64_t n_points, n_sticks; /* of the whole transform */
+} fftb_slab_info;
+
+/* host only; every rank calls it with the same desc and world and gets the same partition */
+int fftb_slab_plan_create(fftb_slab_plan *out, const fftb_plan_desc *desc, int world, int rank);
+int fftb_slab_plan_info_get(fftb_slab_plan p, fftb_slab_info *info);
+/* the partition: stick_lo, packed_lo and z_lo have world + 1 entries each (any may be NULL) */
+int fftb_slab_plan_counts(fftb_slab_plan p, int64_t *stick_lo, int64_t *packed_lo, int64_t *z_lo);
+int fftb_slab_plan_bind(fftb_slab_plan p, void *d_mem, size_t bytes, void *stream);
+/* device pointer (inside the bind block) peers write to in the direct mode: which = 0 the intermediate the INVERSE
+ * exchange fills (all sticks x own planes), 1 the one the FORWARD exchange fills (own sticks x all planes) */
+int fftb_slab_plan_exchange_ptr(fftb_slab_plan p, int which, void **d_ptr);
+
+/* d_packed_local [nb][n_points_local]; d_cuboid_slab [nb][planes_local][N2][N1]; d_peer: host array of `world` device
+ * pointers or NULL; d_send / d_recv: device buffers of the sizes the counts imply, or NULL in the direct mode */
+int fftb_slab_inverse_begin(fftb_slab_plan p, const void *d_packed_local, void *const *d_peer, void *d_send, int nb, void *stream);
+int fftb_slab_inverse_end(fftb_slab_plan p, const void *d_recv, void *d_cuboid_slab, int nb, void *stream);
+int fftb_slab_forward_begin(fftb_slab_plan p, const void *d_cuboid_slab, void *const *d_peer, void *d_send, int nb, void *stream);
+int fftb_slab_forward_end(fftb_slab_plan p, const void *d_recv, void *d_packed_local, int nb, void *stream);
+int fftb_slab_plan_destroy(fftb_slab_plan p);
+
+
 const char *fftb_strerror(int code);
 
 #ifdef __cplusplus

@@ -26,7 +26,9 @@ SYMBOLS = [
     "fftb_inverse", "fftb_forward", "fftb_apply_vloc",
     "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
     "fftb_dense_embed", "fftb_dense_extract", "fftb_packed_transpose",
-    "fftb_probe_fma", "fftb_plan_last_launches", "fftb_plan_profile", "fftb_plan_profile_read", "fftb_plan_destroy", "fftb_strerror",
+    "fftb_probe_fma", "fftb_plan_last_launches",
+    "fftb_slab_plan_create", "fftb_slab_plan_info_get", "fftb_slab_plan_counts", "fftb_slab_plan_bind", "fftb_slab_plan_exchange_ptr",
+    "fftb_slab_inverse_begin", "fftb_slab_inverse_end", "fftb_slab_forward_begin", "fftb_slab_forward_end", "fftb_slab_plan_destroy", "fftb_plan_profile", "fftb_plan_profile_read", "fftb_plan_destroy", "fftb_strerror",
 ]
 
 

@@ -13,6 +13,7 @@
 #include "fftb_zpass_pf.cuh"
 #include "fftb_fused.cuh"
 #include "fftb_probe.cuh"
+#include "fftb_slab.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -1264,6 +1265,281 @@ int fftb_plan_destroy(fftb_plan p)
         cudaEventDestroy(p->hev_done);
         for (int i = 0; i < 8; ++i) { cudaEventDestroy(p->hev_in[i]); cudaEventDestroy(p->hev_out[i]); }
     }
+    delete p;
+    return FFTB_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// slab-distributed transform (include/fftb.h; fftb_slab.cuh): two ordinary plans -- the z passes on the own sticks
+// (an explicit stick map, the whole z axis) and the plane passes on all sticks (run on the own z slab only) -- and
+// the row-copy kernel between them
+// ------------------------------------------------------------------------------------------------
+struct fftb_slab_plan_s {
+    int world, rank, batch, n3;
+    size_t elem;
+    fftb_plan zp, pp;
+    std::vector<int64_t> stick_lo, packed_lo, z_lo; // world + 1 entries each
+    size_t o_z, o_p, bytes;
+    bool bound;
+};
+
+static int slab_pitch(int64_t nsticks) { return (int)((nsticks + 15) / 16 * 16); }
+
+static int slab_copy(fftb_slab_plan p, const SlabSegs &sg, const void *src, int max_rows, int nb, cudaStream_t st)
+{
+    int rb = max_rows < 64 ? max_rows : 64;
+    if (rb < 1) rb = 1;
+    dim3 grid(rb, nb, sg.n);
+    if (p->elem == 16) slab_rows_k<double2><<<grid, 256, 0, st>>>(sg, (const double2 *)src);
+    else slab_rows_k<float2><<<grid, 256, 0, st>>>(sg, (const float2 *)src);
+    return cudaGetLastError() == cudaSuccess ? FFTB_OK : FFTB_ECUDA;
+}
+
+int fftb_slab_plan_create(fftb_slab_plan *out, const fftb_plan_desc *desc, int world, int rank)
+{
+    if (!out || !desc) return FFTB_EINVAL;
+    *out = nullptr;
+    if (world < 1 || rank < 0 || rank >= world) return FFTB_EINVAL;
+    if (world > SLAB_MAXR || (desc->flags & FFTB_FLAG_DENSE)) return FFTB_EUNSUPPORTED;
+    fftb_plan pp = nullptr;
+    int rc = plan_create_impl(&pp, desc, nullptr, nullptr);
+    if (rc) return rc;
+    fftb_slab_plan_s *p = new (std::nothrow) fftb_slab_plan_s();
+    if (!p) { fftb_plan_destroy(pp); return FFTB_ENOMEM; }
+    p->world = world; p->rank = rank; p->batch = desc->batch; p->n3 = desc->n[2]; p->elem = pp->elem;
+    p->pp = pp; p->zp = nullptr; p->bound = false;
+    if (pp->nxocc < world || desc->n[2] < world || pp->ry != 1) { fftb_slab_plan_destroy(p); return FFTB_EUNSUPPORTED; }
+    // sticks: contiguous ranges of occupied k1 columns, cut where the running stick count passes r * n_sticks / world
+    p->stick_lo.assign(world + 1, 0);
+    {
+        int col = 0;
+        for (int r = 1; r < world; ++r) {
+            const int64_t target = (int64_t)r * pp->nsticks / world;
+            int c = col + 1; // at least one column per rank
+            while (c < pp->nxocc - (world - r) && pp->h_col[c].x < target) ++c;
+            col = c;
+            p->stick_lo[r] = pp->h_col[c].x;
+        }
+        p->stick_lo[world] = pp->nsticks;
+    }
+    p->packed_lo.resize(world + 1);
+    p->z_lo.resize(world + 1);
+    for (int r = 0; r <= world; ++r) {
+        p->packed_lo[r] = pp->off[(size_t)p->stick_lo[r]];
+        p->z_lo[r] = (int64_t)r * desc->n[2] / world;
+    }
+    // the own sticks as an explicit map (the whole z axis, the band count of the description)
+    const int64_t s0 = p->stick_lo[rank], s1 = p->stick_lo[rank + 1];
+    const ExplicitMap xm = {s1 - s0, pp->k1.data() + s0, pp->k2.data() + s0, pp->k3lo.data() + s0, pp->len.data() + s0};
+    fftb_plan_desc dz = *desc;
+    for (int d = 0; d < 3; ++d) dz.cutoff[d] = 0;
+    rc = plan_create_impl(&p->zp, &dz, &xm, nullptr);
+    if (!rc && (p->zp->ry != 1 || p->zp->chunk_inv < desc->batch || p->zp->chunk_fwd < desc->batch || pp->chunk_inv < desc->batch ||
+                pp->chunk_fwd < desc->batch))
+        rc = FFTB_EUNSUPPORTED; // the whole batch goes through the intermediates in one piece
+    if (rc) { fftb_slab_plan_destroy(p); return rc; }
+    p->o_z = 0;
+    p->o_p = align_up(p->zp->bytes_min, 256);
+    p->bytes = p->o_p + align_up(pp->bytes_min, 256);
+    *out = p;
+    return FFTB_OK;
+}
+
+int fftb_slab_plan_info_get(fftb_slab_plan p, fftb_slab_info *info)
+{
+    if (!p || !info) return FFTB_EINVAL;
+    info->n_points_local = p->packed_lo[p->rank + 1] - p->packed_lo[p->rank];
+    info->n_sticks_local = p->stick_lo[p->rank + 1] - p->stick_lo[p->rank];
+    info->planes_local = p->z_lo[p->rank + 1] - p->z_lo[p->rank];
+    info->device_bytes = (int64_t)p->bytes;
+    info->n_points = p->pp->S;
+    info->n_sticks = p->pp->nsticks;
+    return FFTB_OK;
+}
+
+int fftb_slab_plan_counts(fftb_slab_plan p, int64_t *stick_lo, int64_t *packed_lo, int64_t *z_lo)
+{
+    if (!p) return FFTB_EINVAL;
+    const size_t n = (size_t)p->world + 1;
+    if (stick_lo) memcpy(stick_lo, p->stick_lo.data(), n * sizeof(int64_t));
+    if (packed_lo) memcpy(packed_lo, p->packed_lo.data(), n * sizeof(int64_t));
+    if (z_lo) memcpy(z_lo, p->z_lo.data(), n * sizeof(int64_t));
+    return FFTB_OK;
+}
+
+int fftb_slab_plan_bind(fftb_slab_plan p, void *d_mem, size_t bytes, void *stream)
+{
+    if (!p || !d_mem) return FFTB_EINVAL;
+    if ((uintptr_t)d_mem % 256) return FFTB_EINVAL;
+    if (bytes < p->bytes) return FFTB_ENOMEM;
+    unsigned char *m = (unsigned char *)d_mem;
+    int rc = fftb_plan_bind(p->zp, m + p->o_z, p->o_p - p->o_z, stream);
+    if (!rc) rc = fftb_plan_bind(p->pp, m + p->o_p, p->bytes - p->o_p, stream);
+    p->bound = rc == FFTB_OK;
+    return rc;
+}
+
+int fftb_slab_plan_exchange_ptr(fftb_slab_plan p, int which, void **d_ptr)
+{
+    if (!p || !d_ptr || (which != 0 && which != 1)) return FFTB_EINVAL;
+    if (!p->bound) return FFTB_ESTATE;
+    *d_ptr = which == 0 ? (void *)(p->pp->d_mem + p->pp->o_ws) : (void *)(p->zp->d_mem + p->zp->o_ws);
+    return FFTB_OK;
+}
+
+static int slab_check(fftb_slab_plan p, const void *a, const void *b, bool need_b, int nb)
+{
+    if (!p || !a || (need_b && !b)) return FFTB_EINVAL;
+    if (!p->bound) return FFTB_ESTATE;
+    if (p->zp->sticky) return p->zp->sticky;
+    if (p->pp->sticky) return p->pp->sticky;
+    if (nb < 1 || nb > p->batch) return FFTB_EINVAL;
+    if ((uintptr_t)a % 16 || (need_b && (uintptr_t)b % 16)) return FFTB_EINVAL;
+    return FFTB_OK;
+}
+
+// segments of an exchange.  to_planes: rows = z-planes of the slab owner, columns = sticks of the stick owner (inverse);
+// otherwise the forward direction.  send: this rank is the source of the rows (pack side), else the unpack side.
+int fftb_slab_inverse_begin(fftb_slab_plan p, const void *d_packed_local, void *const *d_peer, void *d_send, int nb, void *stream)
+{
+    int rc = slab_check(p, d_packed_local, d_send, d_peer == nullptr, nb);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    fftb_plan zp = p->zp;
+    unsigned char *A = zp->d_mem + zp->o_ws;
+    rc = zp->zl.inv(zp->dev, d_packed_local, A, zp->a_inv_stride, nb, st);
+    if (rc) { zp->sticky = rc; return rc; }
+    const int r = p->rank, R = p->world;
+    const long long n_r = p->stick_lo[r + 1] - p->stick_lo[r], pitch_r = zp->pitch, pitch = p->pp->pitch;
+    SlabSegs sg;
+    sg.n = R;
+    long long off = 0;
+    int max_rows = 1;
+    for (int d = 0; d < R; ++d) {
+        const long long slab_d = p->z_lo[d + 1] - p->z_lo[d];
+        SlabSeg &g = sg.s[d];
+        g.rows = (int)slab_d; g.cols = (int)n_r; g.peer = d;
+        g.src_off = p->z_lo[d] * pitch_r; g.src_sb = (long long)p->n3 * pitch_r; g.src_sr = pitch_r;
+        if (d_peer) { // straight into peer d's intermediate A[band][own plane][all sticks]
+            if (!d_peer[d]) return FFTB_EINVAL;
+            sg.dst[d] = d_peer[d];
+            g.dst_off = p->stick_lo[r]; g.dst_sb = slab_d * pitch; g.dst_sr = pitch;
+        } else {      // staging buffer [peer][band][row][column]
+            sg.dst[d] = d_send;
+            g.dst_off = off; g.dst_sb = slab_d * n_r; g.dst_sr = n_r;
+            off += (long long)nb * slab_d * n_r;
+        }
+        if (g.rows > max_rows) max_rows = g.rows;
+    }
+    return slab_copy(p, sg, A, max_rows, nb, st);
+}
+
+int fftb_slab_inverse_end(fftb_slab_plan p, const void *d_recv, void *d_cuboid_slab, int nb, void *stream)
+{
+    int rc = slab_check(p, d_cuboid_slab, nullptr, false, nb);
+    if (rc) return rc;
+    if ((uintptr_t)d_cuboid_slab % (p->elem == 16 ? 32 : 16) || (d_recv && (uintptr_t)d_recv % 16)) return FFTB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    fftb_plan pp = p->pp;
+    unsigned char *A = pp->d_mem + pp->o_ws;
+    const int r = p->rank, R = p->world;
+    const long long slab_r = p->z_lo[r + 1] - p->z_lo[r], pitch = pp->pitch;
+    if (d_recv) { // [peer][band][own plane][the peer's sticks] -> A[band][own plane][all sticks]
+        SlabSegs sg;
+        sg.n = R;
+        long long off = 0;
+        for (int s = 0; s < R; ++s) {
+            const long long n_s = p->stick_lo[s + 1] - p->stick_lo[s];
+            SlabSeg &g = sg.s[s];
+            g.rows = (int)slab_r; g.cols = (int)n_s; g.peer = s;
+            g.src_off = off; g.src_sb = slab_r * n_s; g.src_sr = n_s;
+            sg.dst[s] = A;
+            g.dst_off = p->stick_lo[s]; g.dst_sb = slab_r * pitch; g.dst_sr = pitch;
+            off += (long long)nb * slab_r * n_s;
+        }
+        rc = slab_copy(p, sg, d_recv, (int)slab_r, nb, st);
+        if (rc) return rc;
+    }
+    DevPlan dv = pp->dev;
+    dv.n3 = (int)slab_r; // the plane kernels walk the planes of the slab only
+    rc = pp->plk.run[MODE_INV](dv, pp->tabs, A, nullptr, nullptr, d_cuboid_slab, nullptr, slab_r * pitch, 0, nb, st);
+    if (rc) pp->sticky = rc;
+    return rc;
+}
+
+int fftb_slab_forward_begin(fftb_slab_plan p, const void *d_cuboid_slab, void *const *d_peer, void *d_send, int nb, void *stream)
+{
+    int rc = slab_check(p, d_cuboid_slab, d_send, d_peer == nullptr, nb);
+    if (rc) return rc;
+    if ((uintptr_t)d_cuboid_slab % (p->elem == 16 ? 32 : 16)) return FFTB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    fftb_plan pp = p->pp;
+    unsigned char *A = pp->d_mem + pp->o_ws;
+    const int r = p->rank, R = p->world;
+    const long long slab_r = p->z_lo[r + 1] - p->z_lo[r], pitch = pp->pitch;
+    DevPlan dv = pp->dev;
+    dv.n3 = (int)slab_r;
+    rc = pp->plk.run[MODE_FWD](dv, pp->tabs, nullptr, A, d_cuboid_slab, nullptr, nullptr, 0, slab_r * pitch, nb, st);
+    if (rc) { pp->sticky = rc; return rc; }
+    SlabSegs sg;
+    sg.n = R;
+    long long off = 0;
+    for (int d = 0; d < R; ++d) {
+        const long long n_d = p->stick_lo[d + 1] - p->stick_lo[d], pitch_d = slab_pitch(n_d);
+        SlabSeg &g = sg.s[d];
+        g.rows = (int)slab_r; g.cols = (int)n_d; g.peer = d;
+        g.src_off = p->stick_lo[d]; g.src_sb = slab_r * pitch; g.src_sr = pitch;
+        if (d_peer) { // straight into peer d's intermediate A[band][all planes][own sticks]
+            if (!d_peer[d]) return FFTB_EINVAL;
+            sg.dst[d] = d_peer[d];
+            g.dst_off = p->z_lo[r] * pitch_d; g.dst_sb = (long long)p->n3 * pitch_d; g.dst_sr = pitch_d;
+        } else {
+            sg.dst[d] = d_send;
+            g.dst_off = off; g.dst_sb = slab_r * n_d; g.dst_sr = n_d;
+            off += (long long)nb * slab_r * n_d;
+        }
+    }
+    return slab_copy(p, sg, A, (int)slab_r, nb, st);
+}
+
+int fftb_slab_forward_end(fftb_slab_plan p, const void *d_recv, void *d_packed_local, int nb, void *stream)
+{
+    int rc = slab_check(p, d_packed_local, nullptr, false, nb);
+    if (rc) return rc;
+    if (d_recv && (uintptr_t)d_recv % 16) return FFTB_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    fftb_plan zp = p->zp;
+    unsigned char *A = zp->d_mem + zp->o_ws;
+    const int r = p->rank, R = p->world;
+    const long long n_r = p->stick_lo[r + 1] - p->stick_lo[r], pitch_r = zp->pitch;
+    if (d_recv) { // [peer][band][the peer's planes][own sticks] -> A[band][all planes][own sticks]
+        SlabSegs sg;
+        sg.n = R;
+        long long off = 0;
+        int max_rows = 1;
+        for (int s = 0; s < R; ++s) {
+            const long long slab_s = p->z_lo[s + 1] - p->z_lo[s];
+            SlabSeg &g = sg.s[s];
+            g.rows = (int)slab_s; g.cols = (int)n_r; g.peer = s;
+            g.src_off = off; g.src_sb = slab_s * n_r; g.src_sr = n_r;
+            sg.dst[s] = A;
+            g.dst_off = p->z_lo[s] * pitch_r; g.dst_sb = (long long)p->n3 * pitch_r; g.dst_sr = pitch_r;
+            off += (long long)nb * slab_s * n_r;
+            if (g.rows > max_rows) max_rows = g.rows;
+        }
+        rc = slab_copy(p, sg, d_recv, max_rows, nb, st);
+        if (rc) return rc;
+    }
+    rc = zp->zl.fwd(zp->dev, A, d_packed_local, zp->a_fwd_stride, nb, st);
+    if (rc) zp->sticky = rc;
+    return rc;
+}
+
+int fftb_slab_plan_destroy(fftb_slab_plan p)
+{
+    if (!p) return FFTB_EINVAL;
+    if (p->zp) fftb_plan_destroy(p->zp);
+    if (p->pp) fftb_plan_destroy(p->pp);
     delete p;
     return FFTB_OK;
 }
