@@ -195,14 +195,15 @@ def run_ours(args, w):
     tuning = {"flags": tflags} if tflags else None
     if args.ring_bands or args.lead_bands:
         tuning = dict(tuning or {}, ring_bands=args.ring_bands, lead_bands=args.lead_bands)
-    plan = fb.Plan(w.n, w.cutoff, batch=nb, dtype=w.dtype, scale="forward", tuning=tuning).bind(host_staging=True)
+    bfast = args.layout == "batch_fastest"
+    plan = fb.Plan(w.n, w.cutoff, batch=nb, dtype=w.dtype, scale="forward", tuning=tuning, batch_fastest=bfast).bind(host_staging=True)
     info = plan.info
     elem = 16 if w.dtype == "c128" else 8
     k = plan.points()
     # weak: every rank owns its own batch of bands (the seed differs per rank); strong: every rank draws the config's
     # batch and keeps its own contiguous band range (band sharding)
     c = wl.coefficients(w, *k)[lo:hi] if strong else wl.coefficients(w, *k, batch=nb, seed=1000 + w.number + 7919 * rank)
-    c = np.ascontiguousarray(c)
+    c = np.ascontiguousarray(c.T if bfast else c)  # batch-fastest: [S][nb], the paper's Fig. 8 layout
     h_c = torch.from_numpy(c).pin_memory()
     h_out = torch.empty_like(h_c).pin_memory()
     d_c = h_c.cuda()
@@ -382,7 +383,8 @@ def run_ours(args, w):
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
             "dtype": "f64" if w.dtype == "c128" else "f32", "data": "synthetic",
             "config": config_dict(w, {"parallelism": f"band-sharded x{world}, no collective", "bands_per_gpu": nb, "chunk_bands": info["chunk_bands"],
-                                      "ring_bands": info["ring_bands"], "lead_bands": info["lead_bands"]}),
+                                      "ring_bands": info["ring_bands"], "lead_bands": info["lead_bands"],
+                                      "packed_layout": "[S][nb] batch-fastest" if bfast else "[nb][S] band-slowest"}),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h_c.numel() * elem), "d2h_bytes_per_step": int(h_out.numel() * elem),
@@ -415,6 +417,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = a full batch per GPU (default), strong = the config's batch split over the GPUs (sharding.band_range)")
+    ap.add_argument("--layout", default="band_slowest", choices=["band_slowest", "batch_fastest"],
+                    help="layout of the packed arrays: [nb][S] (default, north_star) or [S][nb] (FFTB_FLAG_BATCH_FASTEST, PAPER.md:219-221)")
     ap.add_argument("--probe-alu", action="store_true", help="print the FP64 / FP32 FMA probe (fftb_probe_fma) as JSON and exit")
     ap.add_argument("--fused", action="store_true", help="one cooperative launch per direction (FFTB_TUNE_FUSED): the intermediate stays in L2")
     ap.add_argument("--no-l2-hints", action="store_true", help="fused launches without L2 eviction priorities (FFTB_TUNE_NO_L2_HINTS)")

@@ -64,9 +64,15 @@ enum fftb_status {
 enum fftb_dtype { FFTB_C64 = 0, FFTB_C128 = 1 };               /* element type of packed and cuboid */
 enum fftb_scale { FFTB_SCALE_NONE = 0, FFTB_SCALE_FORWARD = 1 }; /* 1/(N1 N2 N3) applied in forward */
 enum fftb_flags {
-    FFTB_FLAG_DENSE = 1u /* no pruning: every (k1,k2) is a full-length stick, S = C, `cutoff` ignored.
-                            This is the "pad the sphere to the cube, transform the entire cube" route of
-                            PAPER.md:110-112, run by the same kernels (BASELINE config 5). */
+    FFTB_FLAG_DENSE = 1u, /* no pruning: every (k1,k2) is a full-length stick, S = C, `cutoff` ignored.
+                             This is the "pad the sphere to the cube, transform the entire cube" route of
+                             PAPER.md:110-112, run by the same kernels (BASELINE config 5). */
+    FFTB_FLAG_BATCH_FASTEST = 2u /* the PACKED arrays of every execute call are batch-fastest, [S][nb] (element [point][band],
+                             nb = the bands of that call): the layout of the paper's own example, Fig. 8 "b x y z"
+                             (PAPER.md:219-221).  The transposition is folded into the z passes (their tile loads and
+                             stores), no extra pass over the packed arrays; the cuboid stays [nb][N3][N2][N1].  Only for
+                             N3 in {64, 96, 128, 192 (FFTB_C64)} with N1 in {64, 96, 128, 256}: FFTB_EUNSUPPORTED
+                             otherwise; not together with FFTB_FLAG_DENSE (FFTB_EINVAL). */
 };
 
 typedef struct {

@@ -17,6 +17,7 @@ _LIBPATH = _HERE / "libfftb.so"
 FFTB_C64, FFTB_C128 = 0, 1
 FFTB_SCALE_NONE, FFTB_SCALE_FORWARD = 0, 1
 FFTB_FLAG_DENSE = 1
+FFTB_FLAG_BATCH_FASTEST = 2
 FFTB_TUNE_GENERIC_Z, FFTB_TUNE_GENERIC_PLANE, FFTB_TUNE_FUSED, FFTB_TUNE_NO_L2_HINTS = 1, 2, 4, 8
 FFTB_OK, FFTB_EINVAL, FFTB_EUNSUPPORTED, FFTB_ENOMEM, FFTB_ECUDA, FFTB_ESTATE = 0, -1, -2, -3, -4, -5
 
@@ -118,7 +119,8 @@ class Plan:
     """fftb_plan_create / bind / execute / destroy.  Tensors are torch CUDA tensors (or pinned host
     tensors for the *_host calls); shapes follow include/fftb.h: packed (nb, S), cuboid (nb, N3, N2, N1)."""
 
-    def __init__(self, n, cutoff=(0, 0, 0), batch=1, dtype="c128", scale="forward", dense=False, stick_map=None, tuning=None):
+    def __init__(self, n, cutoff=(0, 0, 0), batch=1, dtype="c128", scale="forward", dense=False, stick_map=None, tuning=None,
+                 batch_fastest=False):
         """stick_map = (k1, k2, k3lo, len) int arrays: fftb_plan_create_explicit instead of a cut-off.
         tuning = dict(workspace_bytes=, ring_bands=, lead_bands=, flags=): fftb_plan_create_tuned."""
         d = PlanDesc()
@@ -127,7 +129,8 @@ class Plan:
         d.batch = int(batch)
         d.dtype = FFTB_C128 if dtype == "c128" else FFTB_C64
         d.scale = FFTB_SCALE_FORWARD if scale == "forward" else FFTB_SCALE_NONE
-        d.flags = FFTB_FLAG_DENSE if dense else 0
+        d.flags = (FFTB_FLAG_DENSE if dense else 0) | (FFTB_FLAG_BATCH_FASTEST if batch_fastest else 0)
+        self.batch_fastest = bool(batch_fastest)
         self._h = ctypes.c_void_p()
         if stick_map is None and tuning is not None:
             tu = PlanTuning()
@@ -201,14 +204,21 @@ class Plan:
     def cuboid_shape(self, nb):
         return (nb, self.n[2], self.n[1], self.n[0])
 
+    def packed_shape(self, nb):
+        """(nb, S), or (S, nb) for a FFTB_FLAG_BATCH_FASTEST plan"""
+        return (self.S, nb) if self.batch_fastest else (nb, self.S)
+
+    def _nb(self, packed):
+        return packed.shape[1] if self.batch_fastest else packed.shape[0]
+
     # ---- execute
     def inverse(self, packed, cuboid=None, stream=None):
         import torch
 
-        nb = packed.shape[0]
+        nb = self._nb(packed)
         if cuboid is None:
             cuboid = torch.empty(self.cuboid_shape(nb), dtype=self.torch_complex, device=packed.device)
-        _check(lib().fftb_inverse(self._h, self._chk(packed, (nb, self.S)), self._chk(cuboid, self.cuboid_shape(nb)),
+        _check(lib().fftb_inverse(self._h, self._chk(packed, self.packed_shape(nb)), self._chk(cuboid, self.cuboid_shape(nb)),
                                   nb, _stream_ptr(stream)), "fftb_inverse")
         return cuboid
 
@@ -217,38 +227,38 @@ class Plan:
 
         nb = cuboid.shape[0]
         if packed is None:
-            packed = torch.empty((nb, self.S), dtype=self.torch_complex, device=cuboid.device)
-        _check(lib().fftb_forward(self._h, self._chk(cuboid, self.cuboid_shape(nb)), self._chk(packed, (nb, self.S)),
+            packed = torch.empty(self.packed_shape(nb), dtype=self.torch_complex, device=cuboid.device)
+        _check(lib().fftb_forward(self._h, self._chk(cuboid, self.cuboid_shape(nb)), self._chk(packed, self.packed_shape(nb)),
                                   nb, _stream_ptr(stream)), "fftb_forward")
         return packed
 
     def apply_vloc(self, packed_in, vloc, packed_out=None, stream=None):
         import torch
 
-        nb = packed_in.shape[0]
+        nb = self._nb(packed_in)
         if packed_out is None:
             packed_out = torch.empty_like(packed_in)
-        _check(lib().fftb_apply_vloc(self._h, self._chk(packed_in, (nb, self.S)), self._chk(packed_out, (nb, self.S)),
+        _check(lib().fftb_apply_vloc(self._h, self._chk(packed_in, self.packed_shape(nb)), self._chk(packed_out, self.packed_shape(nb)),
                                      self._chk(vloc, (self.n[2], self.n[1], self.n[0]), dtype=self.torch_real),
                                      nb, _stream_ptr(stream)), "fftb_apply_vloc")
         return packed_out
 
     def inverse_host(self, h_packed, cuboid, stream=None):
-        nb = h_packed.shape[0]
-        _check(lib().fftb_inverse_host(self._h, self._chk(h_packed, (nb, self.S), cuda=False),
+        nb = self._nb(h_packed)
+        _check(lib().fftb_inverse_host(self._h, self._chk(h_packed, self.packed_shape(nb), cuda=False),
                                        self._chk(cuboid, self.cuboid_shape(nb)), nb, _stream_ptr(stream)), "fftb_inverse_host")
         return cuboid
 
     def forward_host(self, cuboid, h_packed, stream=None):
         nb = cuboid.shape[0]
         _check(lib().fftb_forward_host(self._h, self._chk(cuboid, self.cuboid_shape(nb)),
-                                       self._chk(h_packed, (nb, self.S), cuda=False), nb, _stream_ptr(stream)), "fftb_forward_host")
+                                       self._chk(h_packed, self.packed_shape(nb), cuda=False), nb, _stream_ptr(stream)), "fftb_forward_host")
         return h_packed
 
     def apply_vloc_host(self, h_in, h_out, vloc, stream=None):
-        nb = h_in.shape[0]
-        _check(lib().fftb_apply_vloc_host(self._h, self._chk(h_in, (nb, self.S), cuda=False),
-                                          self._chk(h_out, (nb, self.S), cuda=False),
+        nb = self._nb(h_in)
+        _check(lib().fftb_apply_vloc_host(self._h, self._chk(h_in, self.packed_shape(nb), cuda=False),
+                                          self._chk(h_out, self.packed_shape(nb), cuda=False),
                                           self._chk(vloc, (self.n[2], self.n[1], self.n[0]), dtype=self.torch_real),
                                           nb, _stream_ptr(stream)), "fftb_apply_vloc_host")
         return h_out

@@ -134,8 +134,10 @@ template <class K> int kernel_ready(K k, int threads, size_t smem, int *per_sm)
 int launch_status() { return cudaGetLastError() == cudaSuccess ? 0 : FFTB_ECUDA; }
 
 struct ZLaunch {
-    int (*inv)(const DevPlan &, const void *packed, void *A, long long stride, int nb, cudaStream_t);
-    int (*fwd)(const DevPlan &, const void *A, void *packed, long long stride, int nb, cudaStream_t);
+    // pk_pitch: 0 = packed [band][point]; > 0 = batch-fastest packed [point][pk_pitch bands] (persistent TMA z kernels only)
+    int (*inv)(const DevPlan &, const void *packed, void *A, long long stride, int nb, long long pk_pitch, cudaStream_t);
+    int (*fwd)(const DevPlan &, const void *A, void *packed, long long stride, int nb, long long pk_pitch, cudaStream_t);
+    bool batch_fastest; // the launchers accept pk_pitch > 0
 };
 struct PlanTabs { ColTab ct; ColTab4 ct4; }; // column tables passed by value to the fast kernels
 struct PlaneLaunch {
@@ -153,8 +155,9 @@ struct FusedLaunch {
                int lead, int hints, int *sync, cudaStream_t);
 };
 
-template <typename T, class AZ> int launch_zinv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
+template <typename T, class AZ> int launch_zinv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, long long pk_pitch, cudaStream_t st)
 {
+    if (pk_pitch) return FFTB_EUNSUPPORTED;
     auto k = zpass_inv_k<T, AZ, Z_LINES, Z_NT>;
     const size_t smem = sizeof(cx<T>) * ((size_t)AZ::M * (Z_LINES | 1) + AZ::N);
     if (int rc = kernel_ready(k, Z_NT, smem, nullptr)) return rc;
@@ -162,8 +165,9 @@ template <typename T, class AZ> int launch_zinv(const DevPlan &pl, const void *p
     k<<<grid, Z_NT, smem, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride);
     return launch_status();
 }
-template <typename T, class AZ> int launch_zfwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
+template <typename T, class AZ> int launch_zfwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, long long pk_pitch, cudaStream_t st)
 {
+    if (pk_pitch) return FFTB_EUNSUPPORTED;
     auto k = zpass_fwd_k<T, AZ, Z_LINES, Z_NT>;
     const size_t smem = sizeof(cx<T>) * ((size_t)AZ::R * AZ::P2 * (AZ::P1 * (Z_LINES | 1) + 1) + AZ::N);
     if (int rc = kernel_ready(k, Z_NT, smem, nullptr)) return rc;
@@ -278,28 +282,29 @@ template <class K> int zpers_launch_grid(K kp, int threads, size_t smem, const D
     return 0;
 }
 
-template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
+template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, long long pk_pitch, cudaStream_t st)
 {
-    // persistent kernel, global memory moved by the TMA engine only
+    // persistent kernel, global memory moved by the TMA engine only (batch-fastest packed arrays: per-element cp.async)
     const int ntiles = (pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), total = ntiles * nb;
     using ZP = ZPers<T, F, FAST_NW>;
-    auto kp = zpass_pers_inv_k<T, F, FAST_NW>;
+    auto kp = pk_pitch ? zpass_pers_inv_k<T, F, FAST_NW, true> : zpass_pers_inv_k<T, F, FAST_NW, false>;
     int grid = 0;
     if (int rc = zpers_launch_grid(kp, FAST_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
-    kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
+    kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total, pk_pitch);
     return launch_status();
 }
-template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
+template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, long long pk_pitch, cudaStream_t st)
 {
     const int ntiles = (pl.nsticks + F::G * FAST_NW - 1) / (F::G * FAST_NW), total = ntiles * nb;
     if (pl.ry == 1) { // one plane of A (fast plane kernels): persistent kernel
         using ZP = ZPers<T, F, FAST_NW>;
-        auto kp = zpass_pers_fwd_k<T, F, FAST_NW>;
+        auto kp = pk_pitch ? zpass_pers_fwd_k<T, F, FAST_NW, true> : zpass_pers_fwd_k<T, F, FAST_NW, false>;
         int grid = 0;
         if (int rc = zpers_launch_grid(kp, FAST_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
-        kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
+        kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total, pk_pitch);
         return launch_status();
     }
+    if (pk_pitch) return FFTB_EUNSUPPORTED;
     auto k = zpass_fast_fwd_k<T, F, FAST_NW>; // partial planes of the generic plane kernel are summed here
     const size_t smem = ZFast<T, F, FAST_NW>::smem_bytes;
     if (int rc = kernel_ready(k, FAST_NW * 32, smem, nullptr)) return rc;
@@ -309,12 +314,13 @@ template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const voi
 template <typename T, int N, int P1, int P2> ZLaunch make_z_fast()
 {
     using F = FastCfg<T, N, P1, P2>;
-    return ZLaunch{&launch_zfast_inv<T, F>, &launch_zfast_fwd<T, F>};
+    return ZLaunch{&launch_zfast_inv<T, F>, &launch_zfast_fwd<T, F>, true};
 }
 // z passes of the 256 pattern (fftb_plane_r4.cuh)
 constexpr int R4Z_NW = 4;
-template <typename T> int launch_zr4_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, cudaStream_t st)
+template <typename T> int launch_zr4_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, long long pk_pitch, cudaStream_t st)
 {
+    if (pk_pitch) return FFTB_EUNSUPPORTED;
     using ZP = ZPersR4<T, R4Z_NW>;
     auto kp = zpass_r4_pers_inv_k<T, R4Z_NW>;
     const int ntiles = (pl.nsticks + ZP::TS - 1) / ZP::TS, total = ntiles * nb;
@@ -323,8 +329,9 @@ template <typename T> int launch_zr4_inv(const DevPlan &pl, const void *packed, 
     kp<<<grid, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
     return launch_status();
 }
-template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, cudaStream_t st)
+template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, long long pk_pitch, cudaStream_t st)
 {
+    if (pk_pitch) return FFTB_EUNSUPPORTED;
     if (pl.ry == 1) { // one plane of A (the 256 pattern's own plane kernels): persistent kernel
         using ZP = ZPersR4<T, R4Z_NW>;
         auto kp = zpass_r4_pers_fwd_k<T, R4Z_NW>;
@@ -345,8 +352,8 @@ template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void 
 bool find_z_fast(int dtype, int n, bool dense, ZLaunch *out)
 {
     if (dense) return false;
-    if (dtype == FFTB_C128 && n == 256) { *out = ZLaunch{&launch_zr4_inv<double>, &launch_zr4_fwd<double>}; return true; }
-    if (dtype == FFTB_C64 && n == 256) { *out = ZLaunch{&launch_zr4_inv<float>, &launch_zr4_fwd<float>}; return true; }
+    if (dtype == FFTB_C128 && n == 256) { *out = ZLaunch{&launch_zr4_inv<double>, &launch_zr4_fwd<double>, false}; return true; }
+    if (dtype == FFTB_C64 && n == 256) { *out = ZLaunch{&launch_zr4_inv<float>, &launch_zr4_fwd<float>, false}; return true; }
     if (dtype == FFTB_C128 && n == 128) { *out = make_z_fast<double, 128, 8, 8>(); return true; }
     if (dtype == FFTB_C128 && n == 64) { *out = make_z_fast<double, 64, 8, 4>(); return true; }
     if (dtype == FFTB_C64 && n == 128) { *out = make_z_fast<float, 128, 8, 8>(); return true; }
@@ -429,7 +436,7 @@ bool find_fused(int dtype, const int32_t n[3], bool dense, FusedLaunch *out)
 template <typename T, int N, bool DENSE> ZLaunch make_z()
 {
     using AZ = typename ZX<N, DENSE>::type;
-    return ZLaunch{&launch_zinv<T, AZ>, &launch_zfwd<T, AZ>};
+    return ZLaunch{&launch_zinv<T, AZ>, &launch_zfwd<T, AZ>, false};
 }
 template <typename T, int N, bool DENSE> PlaneLaunch make_plane()
 {
@@ -504,6 +511,7 @@ struct fftb_plan_s {
     PlaneLaunch plk;
     FusedLaunch ful;
     bool fused;          // fftb_inverse / fftb_forward are ONE cooperative launch each (fftb_fused.cuh)
+    bool bf;             // packed arrays are batch-fastest: [point][band], nb bands per point in a call with nb bands
     int ring_bands, lead_bands; // the fused kernels' ring of intermediate band slots and the producers' lead
     int l2_hints;        // fused kernels: evict_last on the ring, evict_first on the cuboid and packed streams
     long long ring_slot; // elements of a ring slot: ntiles tile images (tile-major layout, fftb_fused.cuh)
@@ -581,7 +589,9 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
     if (tune && (tune->workspace_bytes < 0 || tune->ring_bands < 0 || tune->lead_bands < 0)) return FFTB_EINVAL;
     const bool dense = (desc->flags & FFTB_FLAG_DENSE) != 0;
     if (xm && (dense || xm->n < 1 || xm->n > (int64_t)1 << 24 || !xm->k1 || !xm->k2 || !xm->k3lo || !xm->len)) return FFTB_EINVAL;
-    if (desc->flags & ~(uint32_t)FFTB_FLAG_DENSE) return FFTB_EINVAL;
+    if (desc->flags & ~(uint32_t)(FFTB_FLAG_DENSE | FFTB_FLAG_BATCH_FASTEST)) return FFTB_EINVAL;
+    const bool bf = (desc->flags & FFTB_FLAG_BATCH_FASTEST) != 0;
+    if (bf && dense) return FFTB_EINVAL;
     if (desc->dtype != FFTB_C64 && desc->dtype != FFTB_C128) return FFTB_EINVAL;
     if (desc->scale != FFTB_SCALE_NONE && desc->scale != FFTB_SCALE_FORWARD) return FFTB_EINVAL;
     if (desc->batch < 1) return FFTB_EINVAL;
@@ -628,8 +638,10 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         ZLaunch zfast;
         if (!gen_z && find_z_fast(desc->dtype, desc->n[2], dense, &zfast)) { zl = zfast; fast_z = true; }
     }
+    // batch-fastest packed arrays: the transposition is folded into the persistent z passes, which must then exist
+    if (bf && !(zl.batch_fastest && plk.ry == 1)) return FFTB_EUNSUPPORTED;
     FusedLaunch ful = {{0, 0, 0}, nullptr, nullptr};
-    const bool fused = fast_plane && fast_z && (tflags & FFTB_TUNE_FUSED) && find_fused(desc->dtype, desc->n, dense, &ful);
+    const bool fused = !bf && fast_plane && fast_z && (tflags & FFTB_TUNE_FUSED) && find_fused(desc->dtype, desc->n, dense, &ful);
     if (!dense && !xm)
         for (int d = 0; d < 3; ++d)
             if (4 * (long long)desc->cutoff[d] > desc->n[d]) return FFTB_EUNSUPPORTED; // half-band kernels only
@@ -651,6 +663,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         p->plk = plk;
         p->ful = ful;
         p->fused = fused;
+        p->bf = bf;
         p->l2_hints = (tflags & FFTB_TUNE_NO_L2_HINTS) ? 0 : 1;
         p->ry = plk.ry;
         const int n1 = desc->n[0], n2 = desc->n[1], n3 = desc->n[2];
@@ -960,10 +973,10 @@ int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void
     }
     for (int b0 = 0; b0 < nb; b0 += p->chunk_inv) {
         const int nc = nb - b0 < p->chunk_inv ? nb - b0 : p->chunk_inv;
-        const unsigned char *pk = (const unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
+        const unsigned char *pk = (const unsigned char *)d_packed + (p->bf ? (size_t)b0 : (size_t)b0 * p->S) * p->elem;
         unsigned char *cb = (unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
         prof_begin(p, K_ZINV, st);
-        rc = p->zl.inv(p->dev, pk, A, p->a_inv_stride, nc, st);
+        rc = p->zl.inv(p->dev, pk, A, p->a_inv_stride, nc, p->bf ? nb : 0, st);
         prof_end(p, st);
         prof_begin(p, K_PLANE_INV, st);
         if (!rc) rc = p->plk.run[MODE_INV](p->dev, p->tabs, A, nullptr, nullptr, cb, nullptr, p->a_inv_stride, 0, nc, st);
@@ -992,13 +1005,13 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
     }
     for (int b0 = 0; b0 < nb; b0 += p->chunk_fwd) {
         const int nc = nb - b0 < p->chunk_fwd ? nb - b0 : p->chunk_fwd;
-        unsigned char *pk = (unsigned char *)d_packed + (size_t)b0 * p->S * p->elem;
+        unsigned char *pk = (unsigned char *)d_packed + (p->bf ? (size_t)b0 : (size_t)b0 * p->S) * p->elem;
         const unsigned char *cb = (const unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
         prof_begin(p, K_PLANE_FWD, st);
         rc = p->plk.run[MODE_FWD](p->dev, p->tabs, nullptr, A, cb, nullptr, nullptr, 0, p->a_fwd_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_ZFWD, st);
-        if (!rc) rc = p->zl.fwd(p->dev, A, pk, p->a_fwd_stride, nc, st);
+        if (!rc) rc = p->zl.fwd(p->dev, A, pk, p->a_fwd_stride, nc, p->bf ? nb : 0, st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
         p->launches += 2;
@@ -1018,16 +1031,16 @@ int fftb_apply_vloc(fftb_plan p, const void *d_in, void *d_out, const void *d_vl
     p->launches = 0;
     for (int b0 = 0; b0 < nb; b0 += p->chunk) {
         const int nc = nb - b0 < p->chunk ? nb - b0 : p->chunk;
-        const unsigned char *pi = (const unsigned char *)d_in + (size_t)b0 * p->S * p->elem;
-        unsigned char *po = (unsigned char *)d_out + (size_t)b0 * p->S * p->elem;
+        const unsigned char *pi = (const unsigned char *)d_in + (p->bf ? (size_t)b0 : (size_t)b0 * p->S) * p->elem;
+        unsigned char *po = (unsigned char *)d_out + (p->bf ? (size_t)b0 : (size_t)b0 * p->S) * p->elem;
         prof_begin(p, K_ZINV, st);
-        rc = p->zl.inv(p->dev, pi, Ai, p->a_inv_stride, nc, st);
+        rc = p->zl.inv(p->dev, pi, Ai, p->a_inv_stride, nc, p->bf ? nb : 0, st);
         prof_end(p, st);
         prof_begin(p, K_PLANE_VLOC, st);
         if (!rc) rc = p->plk.run[MODE_VLOC](p->dev, p->tabs, Ai, Af, nullptr, nullptr, d_vloc, p->a_inv_stride, p->a_fwd_stride, nc, st);
         prof_end(p, st);
         prof_begin(p, K_ZFWD, st);
-        if (!rc) rc = p->zl.fwd(p->dev, Af, po, p->a_fwd_stride, nc, st);
+        if (!rc) rc = p->zl.fwd(p->dev, Af, po, p->a_fwd_stride, nc, p->bf ? nb : 0, st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
         p->launches += 3;
@@ -1049,7 +1062,7 @@ static int check_host(fftb_plan p, int nb)
 static int host_chunks(fftb_plan p, int nb)
 {
     // at least 1024 z-planes per chunk keep the persistent kernels efficient; at most 4 chunks
-    if (!p->pipe_ok) return 1;
+    if (!p->pipe_ok || p->bf) return 1; // a band chunk of a batch-fastest array is no contiguous piece of host memory
     long long k = (long long)nb * p->desc.n[2] / 1024;
     if (k > 4) k = 4;
     if (k > nb) k = nb;
@@ -1300,7 +1313,7 @@ int fftb_slab_plan_create(fftb_slab_plan *out, const fftb_plan_desc *desc, int w
     if (!out || !desc) return FFTB_EINVAL;
     *out = nullptr;
     if (world < 1 || rank < 0 || rank >= world) return FFTB_EINVAL;
-    if (world > SLAB_MAXR || (desc->flags & FFTB_FLAG_DENSE)) return FFTB_EUNSUPPORTED;
+    if (world > SLAB_MAXR || desc->flags) return FFTB_EUNSUPPORTED;
     fftb_plan pp = nullptr;
     int rc = plan_create_impl(&pp, desc, nullptr, nullptr);
     if (rc) return rc;
@@ -1407,7 +1420,7 @@ int fftb_slab_inverse_begin(fftb_slab_plan p, const void *d_packed_local, void *
     cudaStream_t st = (cudaStream_t)stream;
     fftb_plan zp = p->zp;
     unsigned char *A = zp->d_mem + zp->o_ws;
-    rc = zp->zl.inv(zp->dev, d_packed_local, A, zp->a_inv_stride, nb, st);
+    rc = zp->zl.inv(zp->dev, d_packed_local, A, zp->a_inv_stride, nb, 0, st);
     if (rc) { zp->sticky = rc; return rc; }
     const int r = p->rank, R = p->world;
     const long long n_r = p->stick_lo[r + 1] - p->stick_lo[r], pitch_r = zp->pitch, pitch = p->pp->pitch;
@@ -1530,7 +1543,7 @@ int fftb_slab_forward_end(fftb_slab_plan p, const void *d_recv, void *d_packed_l
         rc = slab_copy(p, sg, d_recv, max_rows, nb, st);
         if (rc) return rc;
     }
-    rc = zp->zl.fwd(zp->dev, A, d_packed_local, zp->a_fwd_stride, nb, st);
+    rc = zp->zl.fwd(zp->dev, A, d_packed_local, zp->a_fwd_stride, nb, 0, st);
     if (rc) zp->sticky = rc;
     return rc;
 }

@@ -27,19 +27,41 @@ template <typename T, class F, int NW> struct ZPers {
     static constexpr int CTAS_PER_SM = F::P1 > 16 ? 2 : 3;
 };
 
-template <typename T, class F, int NW>
+// Batch-fastest packed arrays (BF; Fig. 8 "b x y z": the band index is the fastest one, element
+// [point][band] with `pk_pitch` bands per point): the packed range of a tile is no contiguous run of memory any more but
+// one element out of every row of pk_pitch.  The kernels stay as they are except for the two places that touch the packed
+// array: the landing zone is filled by per-element asynchronous copies (cp.async, completion counted on the same
+// mbarrier) and emptied by per-element stores, and the tiles are walked band-fastest (w = tile * bands + band), so that
+// the CTAs that run side by side read and write neighbouring elements of the same rows while those are in L2.  The
+// transposition [point][band] <-> [band][point] is thereby folded into the z pass; no separate copy of the packed
+// arrays is needed (fftb_packed_transpose remains for callers that want one).
+__device__ __forceinline__ void cp_async_elem(double2 *sdst, const double2 *gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(smem_u32(sdst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_elem(float2 *sdst, const float2 *gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(sdst)), "l"(gsrc) : "memory");
+}
+// the mbarrier gets this thread's arrival once all of its earlier cp.async copies have landed
+__device__ __forceinline__ void cp_async_arrive(unsigned long long *bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+template <typename T, class F, int NW, bool BF>
 __global__ void __launch_bounds__(NW * 32, ZPers<T, F, NW>::CTAS_PER_SM)
 zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride,
-                 int ntiles, int total)
+                 int ntiles, int total, long long pk_pitch)
 {
     using C = cx<T>;
     using Z = ZFast<T, F, NW>;
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
-    constexpr long long EA = ZPers<T, F, NW>::EA;
+    constexpr long long EA = BF ? 1 : ZPers<T, F, NW>::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     // `packed` may be only 8-byte aligned (complex64 band chunks of the library's own calls): indices below count
     // elements from the 16-byte boundary pk at or below it
-    const long long mis = (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
+    const long long mis = BF ? 0 : (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
     const C *pk = packed - mis;
     C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
     C *land = tile + Z::TILE + NW * F::EXW;               // packed values of the tile's sticks
@@ -54,41 +76,51 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
     for (int m = 1; m < P1; ++m) tws[m] = tw[modn<N>(2 * t * m)];
     tws[0] = mk<T>((T)1, (T)0);
     const C g = tw[t];
+    const int nbands = total / ntiles;
 
     // Descriptor of tile w, loaded one iteration before it is used (the stick table is in global memory): this
     // lane's stick and the packed range of the tile in elements of the whole batch, widened to 16-byte boundaries
     // [a0, a1) (complex64: a range may begin and end on an odd element; the neighbours' values that come along are
     // not used).  The batch ends at nall: an odd last element is not covered (a1 < end of the range) and is read
-    // straight from global.
-    const long long nall = mis + (long long)(total / ntiles) * pl.S;
+    // straight from global.  BF: the range counts points of one band, [a0, a1) = the tile's points exactly.
+    const long long nall = mis + (long long)nbands * pl.S;
     struct Tile { int4 st; long long a0, a1; int band, s0; bool act; };
     auto describe = [&](int w) -> Tile {
         Tile d;
-        d.band = w / ntiles, d.s0 = (w % ntiles) * TS;
+        if constexpr (BF) d.band = w % nbands, d.s0 = (w / nbands) * TS;
+        else d.band = w / ntiles, d.s0 = (w % ntiles) * TS;
         const int s = d.s0 + sl, s1 = d.s0 + TS;
         d.act = s < pl.nsticks;
         d.st = pl.stick[d.act ? s : d.s0]; // {off, k3lo, len, .}
-        const long long g0 = (mis + (long long)d.band * pl.S) + pl.stick[d.s0].x;
-        const long long g1 = (mis + (long long)d.band * pl.S) + (s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S);
+        const long long base = BF ? 0 : mis + (long long)d.band * pl.S;
+        const long long g0 = base + pl.stick[d.s0].x;
+        const long long g1 = base + (s1 < pl.nsticks ? (long long)pl.stick[s1].x : pl.S);
         d.a0 = g0 & ~(EA - 1);
         d.a1 = (g1 + EA - 1) & ~(EA - 1);
-        if (d.a1 > nall) d.a1 = nall & ~(EA - 1);
+        if (!BF && d.a1 > nall) d.a1 = nall & ~(EA - 1);
         return d;
     };
-    // thread 0: ask for the packed range of a tile
+    // ask for the packed range of a tile: thread 0 with one bulk copy, or (BF) every thread with its share of elements
     auto issue = [&](const Tile &d) {
-        const unsigned bytes = (unsigned)((d.a1 - d.a0) * (long long)sizeof(C));
-        mbar_expect_tx(&bar, bytes);
-        if (bytes) bulk_load(land, pk + d.a0, bytes, &bar); // 0: a single odd last element of the batch, read directly
+        if constexpr (BF) {
+            const C *src = packed + d.a0 * pk_pitch + d.band;
+            const int n = (int)(d.a1 - d.a0);
+            for (int i = tid; i < n; i += NT) cp_async_elem(land + i, src + (long long)i * pk_pitch);
+            cp_async_arrive(&bar);
+        } else if (tid == 0) {
+            const unsigned bytes = (unsigned)((d.a1 - d.a0) * (long long)sizeof(C));
+            mbar_expect_tx(&bar, bytes);
+            if (bytes) bulk_load(land, pk + d.a0, bytes, &bar); // 0: a single odd last element of the batch, read directly
+        }
     };
     if (tid == 0) {
-        mbar_init(&bar, 1);
+        mbar_init(&bar, BF ? NT : 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     int w = blockIdx.x;
     Tile cur = describe(w < total ? w : 0), nxt = cur;
-    if (tid == 0 && w < total) issue(cur);
+    if (w < total) issue(cur);
     unsigned par = 0;
 #pragma unroll 1
     for (; w < total; w += gridDim.x) {
@@ -100,7 +132,7 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
         const long long a0 = cur.a0, a1 = cur.a1;
         mbar_wait(&bar, par);
         par ^= 1u;
-        const long long gs = (mis + (long long)band * pl.S) + st.x; // the stick's first element in the batch
+        const long long gs = (BF ? 0 : mis + (long long)band * pl.S) + st.x; // the stick's first element
         const C *src = land + (gs - a0);
         const int lim = (int)(a1 - gs);                      // elements of the stick from here on are not in the landing zone
         auto fetch = [&](int idx) -> C {
@@ -119,7 +151,7 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads(); // every thread holds its inputs: the landing zone may be refilled, the tile rewritten
-        if (tid == 0 && more) issue(nxt);
+        if (more) issue(nxt);
 #pragma unroll
         for (int jj = 0; jj < P1; ++jj) xs[jj] = x[jj];
         xs[P1 / 2] = cadd(xs[P1 / 2], bv);
@@ -149,21 +181,21 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
 
 // Forward (F5 z-DFT keeping the stick's k3, scale, F6 pack): the N rows A[z][s0 .. s0 + TS) of the next tile are
 // requested as bulk loads as soon as every thread holds its tile values; the results of a tile are collected in the
-// landing zone in packed order and leave as ONE bulk store (the packed range of TS consecutive sticks is contiguous).
-// Only for one plane of A (ry == 1).
-template <typename T, class F, int NW>
+// landing zone in packed order and leave as ONE bulk store (the packed range of TS consecutive sticks is contiguous),
+// or (BF) as per-element stores into the batch-fastest array.  Only for one plane of A (ry == 1).
+template <typename T, class F, int NW, bool BF>
 __global__ void __launch_bounds__(NW * 32, ZPers<T, F, NW>::CTAS_PER_SM)
 zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride,
-                 int ntiles, int total)
+                 int ntiles, int total, long long pk_pitch)
 {
     using C = cx<T>;
     using Z = ZFast<T, F, NW>;
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
-    constexpr long long EA = ZPers<T, F, NW>::EA;
+    constexpr long long EA = BF ? 1 : ZPers<T, F, NW>::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     // `packed` may be only 8-byte aligned (complex64 band chunks of the library's own calls): indices below count
     // elements from the 16-byte boundary pk at or below it
-    const long long mis = (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
+    const long long mis = BF ? 0 : (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
     C *pk = packed - mis;
     C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
     C *land = tile + Z::TILE + NW * F::EXW;               // results of the tile's sticks in packed order
@@ -179,12 +211,15 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
     tws[0] = mk<T>((T)1, (T)0);
     const C g = tw[t];
     const T scale = (T)pl.scale;
+    const int nbands = total / ntiles;
+    auto band_of = [&](int w) { return BF ? w % nbands : w / ntiles; };
+    auto s0_of = [&](int w) { return (BF ? w / nbands : w % ntiles) * TS; };
 
     auto ncol_of = [&](int s0) { return pl.pitch - s0 < TS ? pl.pitch - s0 : TS; };
     // thread 0 announces the bytes of tile w, then (after a CTA barrier) every thread asks for its rows
-    auto expect = [&](int w) { mbar_expect_tx(&bar, (unsigned)(N * ncol_of((w % ntiles) * TS) * (int)sizeof(C))); };
+    auto expect = [&](int w) { mbar_expect_tx(&bar, (unsigned)(N * ncol_of(s0_of(w)) * (int)sizeof(C))); };
     auto issue_rows = [&](int w) {
-        const int band = w / ntiles, s0 = (w % ntiles) * TS;
+        const int band = band_of(w), s0 = s0_of(w);
         const C *src = A + (long long)band * a_band_stride + s0;
         const unsigned bytes = (unsigned)(ncol_of(s0) * (int)sizeof(C));
         for (int z = tid; z < N; z += NT) bulk_load(tile + Z::lin(z, 0), src + (long long)z * pl.pitch, bytes, &bar);
@@ -204,14 +239,15 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
 #pragma unroll 1
     for (; w < total; w += gridDim.x) {
         const bool more = w + (int)gridDim.x < total;
-        const int band = w / ntiles, s0 = (w % ntiles) * TS, s = s0 + sl;
+        const int band = band_of(w), s0 = s0_of(w), s = s0 + sl;
         const bool act = s < pl.nsticks;
         const int4 st = pl.stick[act ? s : s0];
         // the tile's packed range [g0, g1) in elements of the whole batch (used after the transforms: loading the table
         // one tile ahead was measured 3% slower); its 16-byte aligned interior [b0, b1) leaves as one bulk store from the
-        // landing zone (origin al), an odd first / last element (complex64) by a plain store
-        const long long g0 = (mis + (long long)band * pl.S) + pl.stick[s0].x;
-        const long long g1 = (mis + (long long)band * pl.S) + (s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S);
+        // landing zone (origin al), an odd first / last element (complex64) by a plain store.  BF: points of one band.
+        const long long base = BF ? 0 : mis + (long long)band * pl.S;
+        const long long g0 = base + pl.stick[s0].x;
+        const long long g1 = base + (s0 + TS < pl.nsticks ? (long long)pl.stick[s0 + TS].x : pl.S);
         const long long al = g0 & ~(EA - 1), b0 = (g0 + EA - 1) & ~(EA - 1), b1 = g1 & ~(EA - 1);
         mbar_wait(&bar, par);
         par ^= 1u;
@@ -225,7 +261,7 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
             }
         // the previous tile's packed store must have read the landing zone before it is rewritten
         if (tid == 0) {
-            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            if constexpr (!BF) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
             if (more) expect(w + (int)gridDim.x);
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -235,7 +271,7 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
         sub_fwd<F, T>(y1, h1, tws, ex, t);
         post_fwd<F, 0, T>(h1, g);
         if (act) {
-            const long long gs = (mis + (long long)band * pl.S) + st.x;
+            const long long gs = base + st.x;
             C *dst = land + (gs - al);
             const int lo = (int)(b0 - gs), hi = (int)(b1 - gs); // stick elements [lo, hi) belong to the bulk store
             auto put = [&](int idx, C v) {
@@ -254,7 +290,13 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
-        if (tid == 0 && b1 > b0) {
+        if constexpr (BF) {
+            // the tile's points, one element out of every row of the batch-fastest array (the next write to the landing
+            // zone comes after the next CTA barrier, which this thread only reaches once its loop is done)
+            C *out = packed + g0 * pk_pitch + band;
+            const int n = (int)(g1 - g0);
+            for (int i = tid; i < n; i += NT) out[(long long)i * pk_pitch] = land[i];
+        } else if (tid == 0 && b1 > b0) {
             bulk_store(pk + b0, land + (b0 - al), (unsigned)((b1 - b0) * (long long)sizeof(C)));
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }

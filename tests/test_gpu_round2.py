@@ -331,3 +331,73 @@ def test_two_host_threads_two_plans(fb):
     assert not errors, errors[:3]
     for p, *_ in jobs:
         p.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# batch-fastest packed arrays (Fig. 8 "b x y z")
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,a,dtype,nb", [((64, 64, 64), (16, 16, 16), "c128", 7), ((128, 128, 128), (32, 32, 32), "c128", 5),
+                                          ((96, 96, 192), (24, 24, 48), "c64", 6), ((128, 128, 64), (32, 20, 16), "c64", 37),
+                                          ((96, 96, 96), (24, 24, 24), "c128", 1), ((256, 256, 128), (40, 64, 32), "c128", 2)])
+def test_batch_fastest_plans_vs_oracle(fb, oracle, n, a, dtype, nb):
+    """FFTB_FLAG_BATCH_FASTEST: the packed arrays of every call are [S][nb] (band index fastest); the z passes read and
+    write them directly.  Inverse, forward of a generic cuboid and the fused local potential against the oracle's
+    results TRANSPOSED, and bit for bit against the band-slowest plan (the arithmetic is the same, only the addresses
+    of the packed elements differ).  The input must survive and nothing outside [0, S nb) may be written."""
+    w = _w(n, a, dtype=dtype, batch=nb)
+    pf = fb.Plan(n, a, batch=nb, dtype=dtype, batch_fastest=True).bind()
+    ps = fb.Plan(n, a, batch=nb, dtype=dtype).bind()
+    k = ps.points()
+    c = wl.coefficients(w, *k)                                       # [nb][S]
+    d_c = torch.from_numpy(c).cuda()
+    d_ct = torch.from_numpy(np.ascontiguousarray(c.T)).cuda()         # [S][nb]
+    psi = pf.inverse(d_ct)
+    torch.cuda.synchronize()
+    assert torch.equal(psi, ps.inverse(d_c)) and torch.equal(d_ct.cpu(), torch.from_numpy(np.ascontiguousarray(c.T)))
+    sample = [0, nb - 1]
+    if n[0] <= 128:
+        assert _rel(psi[sample].cpu().numpy(), oracle.inverse(n, k, c[sample])) <= w.tol
+    g = wl.cuboid(w)
+    d_g = torch.from_numpy(g).cuda()
+    guard = 4
+    buf = torch.full((guard + pf.S * nb + guard,), 777.0 - 555.0j, dtype=pf.torch_complex, device="cuda")
+    out = buf[guard:guard + pf.S * nb].view(pf.S, nb)
+    pf.forward(d_g, out)
+    torch.cuda.synchronize()
+    h = buf.cpu().numpy()
+    assert (h[:guard] == h[0]).all() and (h[-guard:] == h[0]).all() and h[0] == np.asarray(777.0 - 555.0j, dtype=h.dtype)
+    assert torch.equal(out.t().contiguous(), ps.forward(d_g))
+    C = float(np.prod(n))
+    if n[0] <= 128:
+        assert _rel(out.t()[sample].cpu().numpy(), oracle.forward(n, k, g[sample], 1.0 / C)) <= w.tol
+    v = wl.potential(w)
+    d_v = torch.from_numpy(v).cuda()
+    hv = pf.apply_vloc(d_ct, d_v)
+    torch.cuda.synchronize()
+    assert tuple(hv.shape) == (pf.S, nb) and torch.equal(hv.t().contiguous(), ps.apply_vloc(d_c, d_v))
+    if n[0] <= 128:
+        assert _rel(hv.t()[sample].cpu().numpy(), oracle.apply_vloc(n, k, c[sample], v, 1.0 / C)) <= w.tol
+    pf.destroy(); ps.destroy()
+
+
+def test_batch_fastest_band_chunks_and_host_calls(fb, oracle):
+    """A workspace of two bands makes the library walk a batch-fastest array chunk by chunk (column ranges of [S][nb]),
+    and the *_host calls move such an array in one piece."""
+    n, a, nb = (64, 64, 64), (16, 16, 16), 7
+    w = _w(n, a, batch=nb)
+    p = fb.Plan(n, a, batch=nb, batch_fastest=True, tuning={"workspace_bytes": 2 * 64 * 800 * 16 * 2}).bind(host_staging=True)
+    assert p.info["chunk_bands"] < nb
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    ct = np.ascontiguousarray(c.T)
+    psi = p.inverse(torch.from_numpy(ct).cuda())
+    rt = p.forward(psi)
+    torch.cuda.synchronize()
+    assert _rel(psi.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol and _rel(rt.cpu().numpy(), ct) <= w.tol
+    h_in = torch.from_numpy(ct).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    v = wl.potential(w)
+    p.apply_vloc_host(h_in, h_out, torch.from_numpy(v).cuda())
+    torch.cuda.synchronize()
+    assert _rel(h_out.numpy().T, oracle.apply_vloc(n, k, c, v, 1.0 / float(np.prod(n)))) <= w.tol
+    p.destroy()

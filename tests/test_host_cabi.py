@@ -84,7 +84,11 @@ def test_error_paths():
     assert _create_rc((0, 32, 32), (8, 8, 8)) == fb.FFTB_EINVAL
     assert _create_rc((32, 32, 32), (8, 8, 8), batch=0) == fb.FFTB_EINVAL
     assert _create_rc((32, 32, 32), (8, 8, 8), dtype=7) == fb.FFTB_EINVAL
-    assert _create_rc((32, 32, 32), (8, 8, 8), flags=2) == fb.FFTB_EINVAL
+    assert _create_rc((32, 32, 32), (8, 8, 8), flags=4) == fb.FFTB_EINVAL
+    assert _create_rc((64, 64, 64), (16, 16, 16), flags=3) == fb.FFTB_EINVAL       # dense and batch-fastest together
+    assert _create_rc((64, 64, 64), (16, 16, 16), flags=2) == fb.FFTB_OK
+    assert _create_rc((32, 32, 32), (8, 8, 8), flags=2) == fb.FFTB_EUNSUPPORTED   # no persistent z pass to fold the transposition into
+    assert _create_rc((256, 256, 256), (64, 64, 64), flags=2) == fb.FFTB_EUNSUPPORTED
     # outside the predefined patterns
     assert _create_rc((40, 40, 40), (8, 8, 8)) == fb.FFTB_EUNSUPPORTED
     assert _create_rc((32, 64, 32), (8, 8, 8)) == fb.FFTB_EUNSUPPORTED
