@@ -130,11 +130,14 @@ typedef struct {
 /* Create a plan (host only, no CUDA call).  Builds the offset array -- the stick map -- from the
  * grid and the cut-off (Fig. 7), the per-k1 stick runs used by the y pass, and the
  * twiddle tables.
- * Predefined patterns (anything else: FFTB_EUNSUPPORTED):
- *   - N1 == N2, each of N1, N3 in {32, 64, 96, 128, 192, 256}, FFTB_C64 or FFTB_C128;
- *   - pruned plans: a_d <= N_d/4 on every axis (the paper's "cube of width twice the diameter of
- *     the sphere");
- *   - dense plans (FFTB_FLAG_DENSE): FFTB_C128 only, N1 and N3 in {32, 64, 128, 256}. */
+ * Predefined patterns (anything else: FFTB_EUNSUPPORTED), FFTB_C64 or FFTB_C128 unless stated:
+ *   - N3 in {32, 64, 96, 128, 192, 256}; N1 == N2 in the same set, or (N1, N2) one of (32, 64), (64, 32), (64, 128),
+ *     (128, 64);
+ *   - pruned plans with a_d <= N_d/4 on every axis (the paper's "cube of width twice the diameter of the sphere",
+ *     PAPER.md:110): half-band kernels, persistent TMA kernels where they exist (N1 == N2 in {64, 96, 128, 256});
+ *   - pruned plans with N_d/4 < a_d < N_d/2 on some axis: full-band axis patterns, FFTB_C128 only, N1 == N2 and N3 in
+ *     {32, 64, 128, 256};
+ *   - dense plans (FFTB_FLAG_DENSE): FFTB_C128 only, N1 == N2 and N3 in {32, 64, 128, 256}. */
 int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc);
 
 /* The same with explicit tuning (tuning == NULL: fftb_plan_create).  FFTB_EINVAL for unknown flags or negative
@@ -147,9 +150,9 @@ int fftb_plan_create_tuned(fftb_plan *out, const fftb_plan_desc *desc, const fft
  * k3lo[s] .. k3lo[s]+len[s]-1 of column (k1[s], k2[s]); `desc->cutoff` is ignored, FFTB_FLAG_DENSE is not
  * allowed.  The arrays (host, n_sticks entries each) are copied.
  *   FFTB_EINVAL        a point outside [-N_d/2, N_d/2), len < 1, sticks not strictly ascending in (k1, k2)
- *   FFTB_EUNSUPPORTED  outside the predefined patterns of fftb_plan_create, or: a frequency beyond
- *                      |k_d| <= N_d/4 (half-band kernels), a hole in the occupied k1 range, or a k1 whose
- *                      k2 values are not one contiguous run. */
+ *   FFTB_EUNSUPPORTED  outside the predefined patterns of fftb_plan_create (a frequency beyond |k_d| <= N_d/4 makes
+ *                      it a full-band plan: FFTB_C128 only), a hole in the occupied k1 range, or a k1 whose k2
+ *                      values are not one contiguous run. */
 int fftb_plan_create_explicit(fftb_plan *out, const fftb_plan_desc *desc, int64_t n_sticks, const int32_t *k1,
                               const int32_t *k2, const int32_t *k3lo, const int32_t *len);
 

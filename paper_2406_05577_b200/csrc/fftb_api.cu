@@ -448,6 +448,25 @@ template <typename T, int N, bool DENSE> PlaneLaunch make_plane()
                        {&launch_plane<T, AX, AY, MODE_INV>, &launch_plane<T, AX, AY, MODE_FWD>, &launch_plane<T, AX, AY, MODE_VLOC>}};
 }
 
+// rectangular x/y grids (N1 != N2): the generic plane kernel with one axis pattern per axis
+template <typename T, int NX, int NY> PlaneLaunch make_plane_xy()
+{
+    using AX = typename ZX<NX, false>::type;
+    using AY = typename YA<NY, false>::type;
+    static_assert(PlaneSmem<T, AX, AY, PlaneTune<AX, AY>::LX, PlaneTune<AX, AY>::LY, PlaneTune<AX, AY>::NT>::bytes <= 227 * 1024,
+                  "plane does not fit in shared memory");
+    return PlaneLaunch{AY::R,
+                       {&launch_plane<T, AX, AY, MODE_INV>, &launch_plane<T, AX, AY, MODE_FWD>, &launch_plane<T, AX, AY, MODE_VLOC>}};
+}
+bool find_plane_xy(int dtype, int nx, int ny, PlaneLaunch *out)
+{
+#define XYCASE(NX, NY) \
+    if (nx == NX && ny == NY) { *out = dtype == FFTB_C128 ? make_plane_xy<double, NX, NY>() : make_plane_xy<float, NX, NY>(); return true; }
+    XYCASE(32, 64) XYCASE(64, 32) XYCASE(64, 128) XYCASE(128, 64)
+#undef XYCASE
+    return false;
+}
+
 bool find_z(int dtype, int n, bool dense, ZLaunch *out)
 {
 #define ZCASE(T, DT, N, D) \
@@ -610,19 +629,34 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
             if (s > 0 && !(xm->k1[s - 1] < xm->k1[s] || (xm->k1[s - 1] == xm->k1[s] && xm->k2[s - 1] < xm->k2[s]))) return FFTB_EINVAL;
         }
     }
-    // predefined patterns
-    if (desc->n[0] != desc->n[1]) return FFTB_EUNSUPPORTED;
+    // predefined patterns.  A cut-off (or explicit map) that reaches beyond N_d/4 on some axis is no half-band problem any
+    // more: such plans run on the full-band axis patterns of the dense plans (generic kernels, complex128), with their
+    // pruned stick map.  N1 != N2: generic plane kernel, a few predefined pairs.
+    bool wide = false;
+    if (!dense && !xm)
+        for (int d = 0; d < 3; ++d) wide = wide || 4 * (long long)desc->cutoff[d] > desc->n[d];
+    if (xm)
+        for (int64_t s = 0; s < xm->n; ++s) {
+            const long long lo = xm->k3lo[s], hi = lo + xm->len[s] - 1;
+            wide = wide || 4 * llabs((long long)xm->k1[s]) > desc->n[0] || 4 * llabs((long long)xm->k2[s]) > desc->n[1] || 4 * lo < -desc->n[2] ||
+                   4 * hi > desc->n[2];
+        }
+    const bool full_band = dense || wide, rect = desc->n[0] != desc->n[1];
+    if (bf && wide) return FFTB_EUNSUPPORTED;
     ZLaunch zl;
     PlaneLaunch plk;
     bool fast_plane = false;
-    if (!find_z(desc->dtype, desc->n[2], dense, &zl) || !find_plane(desc->dtype, desc->n[0], dense, &plk)) return FFTB_EUNSUPPORTED;
+    if (!find_z(desc->dtype, desc->n[2], full_band, &zl)) return FFTB_EUNSUPPORTED;
+    if (rect ? (full_band || !find_plane_xy(desc->dtype, desc->n[0], desc->n[1], &plk)) : !find_plane(desc->dtype, desc->n[0], full_band, &plk))
+        return FFTB_EUNSUPPORTED;
+    const bool dense_cfg = full_band || rect; // no persistent kernels for these
     bool fast_z = false;
     {
         const bool gen_plane = (tflags & FFTB_TUNE_GENERIC_PLANE) != 0, gen_z = (tflags & FFTB_TUNE_GENERIC_Z) != 0;
         PlaneLaunch fast;
-        if (!gen_plane && find_plane_fast(desc->dtype, desc->n[0], dense, &fast)) { plk = fast; fast_plane = true; }
+        if (!gen_plane && find_plane_fast(desc->dtype, desc->n[0], dense_cfg, &fast)) { plk = fast; fast_plane = true; }
         // 256 pattern: persistent plane kernels of their own (four-way split, fftb_plane_r4.cuh)
-        if (!gen_plane && !dense && desc->n[0] == 256) {
+        if (!gen_plane && !dense_cfg && desc->n[0] == 256) {
             if (desc->dtype == FFTB_C128) {
                 plk.run[MODE_INV] = &launch_plane_r4_inv<double>;
                 plk.run[MODE_FWD] = &launch_plane_r4_fwd<double>;
@@ -636,23 +670,12 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
             fast_plane = true; // persistent kernel: whole-batch launches (256 planes per band on 148 CTAs would waste half a wave)
         }
         ZLaunch zfast;
-        if (!gen_z && find_z_fast(desc->dtype, desc->n[2], dense, &zfast)) { zl = zfast; fast_z = true; }
+        if (!gen_z && find_z_fast(desc->dtype, desc->n[2], full_band, &zfast)) { zl = zfast; fast_z = true; }
     }
     // batch-fastest packed arrays: the transposition is folded into the persistent z passes, which must then exist
     if (bf && !(zl.batch_fastest && plk.ry == 1)) return FFTB_EUNSUPPORTED;
     FusedLaunch ful = {{0, 0, 0}, nullptr, nullptr};
     const bool fused = !bf && fast_plane && fast_z && (tflags & FFTB_TUNE_FUSED) && find_fused(desc->dtype, desc->n, dense, &ful);
-    if (!dense && !xm)
-        for (int d = 0; d < 3; ++d)
-            if (4 * (long long)desc->cutoff[d] > desc->n[d]) return FFTB_EUNSUPPORTED; // half-band kernels only
-    if (xm) { // half-band kernels only: every frequency within [-N_d/4, N_d/4]
-        for (int64_t s = 0; s < xm->n; ++s) {
-            const long long lo = xm->k3lo[s], hi = lo + xm->len[s] - 1;
-            if (4 * llabs((long long)xm->k1[s]) > desc->n[0] || 4 * llabs((long long)xm->k2[s]) > desc->n[1]) return FFTB_EUNSUPPORTED;
-            if (4 * lo < -desc->n[2] || 4 * hi > desc->n[2]) return FFTB_EUNSUPPORTED;
-        }
-    }
-
     fftb_plan_s *p = new (std::nothrow) fftb_plan_s();
     if (!p) return FFTB_ENOMEM;
     try {

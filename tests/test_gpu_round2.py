@@ -401,3 +401,39 @@ def test_batch_fastest_band_chunks_and_host_calls(fb, oracle):
     torch.cuda.synchronize()
     assert _rel(h_out.numpy().T, oracle.apply_vloc(n, k, c, v, 1.0 / float(np.prod(n)))) <= w.tol
     p.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# wider predefined patterns: N1 != N2 and cut-offs beyond N/4
+# ---------------------------------------------------------------------------------------------------------------
+WIDER = [((32, 64, 32), (8, 16, 8), "c128"), ((64, 32, 96), (16, 8, 24), "c64"), ((64, 128, 96), (16, 32, 24), "c128"),
+         ((128, 64, 256), (32, 16, 64), "c64"), ((128, 64, 64), (20, 7, 16), "c128"),
+         ((32, 32, 32), (12, 8, 8), "c128"), ((64, 64, 64), (24, 31, 20), "c128"), ((128, 128, 64), (40, 50, 31), "c128"),
+         ((64, 64, 128), (16, 16, 60), "c128")]
+
+
+@pytest.mark.parametrize("n,a,dtype", WIDER, ids=[f"{n[0]}x{n[1]}x{n[2]}-a{a[0]}.{a[1]}.{a[2]}-{d}" for n, a, d in WIDER])
+def test_rectangular_grids_and_wide_cutoffs_vs_oracle(fb, oracle, n, a, dtype):
+    """Grids with N1 != N2 (generic plane kernel, one axis pattern per axis) and cut-offs with N/4 < a < N/2 on some axis
+    (full-band axis patterns with the pruned stick map): map bit-exact, inverse / forward / local potential vs the oracle."""
+    nb = 3
+    w = _w(n, a, dtype=dtype, batch=nb)
+    p = fb.Plan(n, a, batch=nb, dtype=dtype).bind()
+    k = p.points()
+    assert all(np.array_equal(x, y) for x, y in zip(k, oracle.enum_points(n, a)))
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    d_psi = p.inverse(d_c)
+    torch.cuda.synchronize()
+    assert _rel(d_psi.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol
+    g = wl.cuboid(w)
+    C = float(np.prod(n))
+    d_f = p.forward(torch.from_numpy(g).cuda())
+    v = wl.potential(w)
+    d_o = p.apply_vloc(d_c, torch.from_numpy(v).cuda())
+    rt = p.forward(d_psi)
+    torch.cuda.synchronize()
+    assert _rel(d_f.cpu().numpy(), oracle.forward(n, k, g, 1.0 / C)) <= w.tol
+    assert _rel(d_o.cpu().numpy(), oracle.apply_vloc(n, k, c, v, 1.0 / C)) <= w.tol
+    assert _rel(rt.cpu().numpy(), c) <= w.tol
+    p.destroy()

@@ -91,8 +91,11 @@ def test_error_paths():
     assert _create_rc((256, 256, 256), (64, 64, 64), flags=2) == fb.FFTB_EUNSUPPORTED
     # outside the predefined patterns
     assert _create_rc((40, 40, 40), (8, 8, 8)) == fb.FFTB_EUNSUPPORTED
-    assert _create_rc((32, 64, 32), (8, 8, 8)) == fb.FFTB_EUNSUPPORTED
-    assert _create_rc((32, 32, 32), (12, 8, 8)) == fb.FFTB_EUNSUPPORTED   # a > N/4: not a half-band plan
+    assert _create_rc((32, 64, 32), (8, 8, 8)) == fb.FFTB_OK              # N1 != N2: one of the predefined pairs
+    assert _create_rc((96, 64, 32), (8, 8, 8)) == fb.FFTB_EUNSUPPORTED    # ... this one is not
+    assert _create_rc((32, 32, 32), (12, 8, 8)) == fb.FFTB_OK             # a > N/4: full-band axis patterns (complex128)
+    assert _create_rc((32, 32, 32), (12, 8, 8), dtype=fb.FFTB_C64) == fb.FFTB_EUNSUPPORTED
+    assert _create_rc((96, 96, 96), (30, 8, 8)) == fb.FFTB_EUNSUPPORTED   # no full-band pattern of length 96
     assert L.fftb_plan_create(None, None) == fb.FFTB_EINVAL
     assert L.fftb_plan_destroy(None) == fb.FFTB_EINVAL
     assert L.fftb_plan_info_get(None, None) == fb.FFTB_EINVAL
@@ -161,8 +164,9 @@ def test_explicit_stick_map_round_trip_and_errors():
         fb.Plan(n, stick_map=(k1, k2, far, ln))
     assert e.value.code == fb.FFTB_EINVAL
     wide = ln.copy(); wide[0] = 17 - lo[0] + 1
-    with pytest.raises(fb.FftbError) as e:      # beyond the half band |k| <= N/4
-        fb.Plan(n, stick_map=(k1, k2, lo, wide))
+    fb.Plan(n, stick_map=(k1, k2, lo, wide)).destroy()   # beyond the half band |k| <= N/4: full-band patterns, complex128
+    with pytest.raises(fb.FftbError) as e:
+        fb.Plan(n, stick_map=(k1, k2, lo, wide), dtype="c64")
     assert e.value.code == fb.FFTB_EUNSUPPORTED
     hole = np.ones(k1.size, bool); hole[np.flatnonzero(k1 == k1[k1.size // 2])[1]] = False
     with pytest.raises(fb.FftbError) as e:      # a k2 run with a hole
