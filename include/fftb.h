@@ -89,8 +89,8 @@ typedef struct {
     int64_t n_sticks;     /* occupied (k1,k2) columns */
     int64_t n_xocc;       /* distinct k1 with at least one stick */
     int64_t device_bytes; /* smallest block fftb_plan_bind accepts (tables + workspace) */
-    int64_t device_bytes_host; /* block size that also holds the staging area of the *_host calls
-                                  (batch * S elements more) */
+    int64_t device_bytes_host; /* block size that also holds the two staging areas of the *_host calls
+                                  (2 * batch * S elements more) */
     int64_t chunk_bands;  /* bands per kernel group in fftb_inverse (the workspace holds this many) */
     int64_t min_bytes_per_band_dir; /* algorithmic bytes of one band, one direction: (S + C) * elem */
     int64_t workspace_offset; /* byte offset of the plane-major intermediate A inside the bind block */
@@ -185,12 +185,14 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
 int fftb_apply_vloc(fftb_plan p, const void *d_packed_in, void *d_packed_out, const void *d_vloc, int nb,
                     void *stream);
 
-/* The same three operations with the PACKED arrays in host memory (pinned memory makes the copies
- * asynchronous): the library copies them through the staging area inside the bind block, cuboid and vloc
- * stay device pointers.  Large batches cross PCIe in band chunks on two copy streams owned by the plan
- * (created in fftb_plan_bind), overlapped with the transforms of the neighbouring chunks; the calls stay
- * ordered on `stream`: work queued on it earlier is finished before the first copy, work queued later
- * sees the complete result. */
+/* The same three operations with the PACKED arrays in host memory (pinned memory makes the copies asynchronous): the
+ * library copies them through two staging areas inside the bind block (one per direction), cuboid and vloc stay device
+ * pointers.  Large batches cross PCIe in band chunks on two copy streams owned by the plan (created in fftb_plan_bind),
+ * overlapped with the transforms of the neighbouring chunks, and the host-to-device copies of a call may run while the
+ * device-to-host copies of the previous call are still under way (both directions of the link at once).  Ordering:
+ *   - a call's OUTPUT is complete in host memory when `stream` reaches the end of the call (work queued later sees it);
+ *   - a call's host INPUT is read by copies that are ordered after the previous call's kernels, not after other work
+ *     queued on `stream`: its contents must be final when the call is made. */
 int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb, void *stream);
 int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb, void *stream);
 int fftb_apply_vloc_host(fftb_plan p, const void *h_packed_in, void *h_packed_out, const void *d_vloc, int nb,

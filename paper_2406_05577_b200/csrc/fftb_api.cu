@@ -537,7 +537,7 @@ struct fftb_plan_s {
     int ring_ntiles;
     CUtensorMap ring_map; // the ring as a 5-dimensional tensor (inverse plane items load a row out of every tile)
     // device block layout
-    size_t o_stick, o_col, o_perm, o_tw[3], o_sync, o_ws, o_stage, bytes_min, bytes_stage;
+    size_t o_stick, o_col, o_perm, o_tw[3], o_sync, o_ws, o_stage, o_stage_out, bytes_min, bytes_stage;
     long long a_inv_stride, a_fwd_stride; // elements per band of the intermediate (a_fwd_stride: vloc and generic forward)
     int chunk;                            // bands per kernel group (vloc: both intermediates live)
     int chunk_inv, chunk_fwd;             // inverse / forward alone
@@ -547,7 +547,8 @@ struct fftb_plan_s {
     // *_host calls: the packed arrays cross PCIe in HOST_PIPE band chunks on two private copy streams, so
     // that a chunk's copy runs while its neighbours are transformed (created once in fftb_plan_bind)
     cudaStream_t cs_in, cs_out;
-    cudaEvent_t hev_start, hev_done, hev_in[8], hev_out[8];
+    cudaEvent_t hev_in_free, hev_done, hev_in[8], hev_out[8];
+    bool in_free_recorded; // hev_in_free has been recorded at least once
     bool pipe_ok;
     DevPlan dev;
     PlanTabs tabs; // the column table again, as a by-value kernel parameter of the fast plane kernels
@@ -828,11 +829,15 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
             p->lead_bands = (int)lead;
         }
         p->bytes_min = o;
+        // two staging areas of the *_host calls: packed arrays arriving from the host and leaving for it (separate, so that
+        // the next call's host-to-device copies run while this call's device-to-host copies are still under way)
         p->o_stage = o; o = align_up(o + (size_t)desc->batch * (size_t)p->S * p->elem, 256);
+        p->o_stage_out = o; o = align_up(o + (size_t)desc->batch * (size_t)p->S * p->elem, 256);
         p->bytes_stage = o;
         p->d_mem = nullptr;
         p->staging = false;
         p->pipe_ok = false;
+        p->in_free_recorded = false;
         p->sticky = 0;
         p->launches = 0;
         p->prof = false;
@@ -913,7 +918,7 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
     if (p->staging && !p->pipe_ok) {
         bool ok = cudaStreamCreateWithFlags(&p->cs_in, cudaStreamNonBlocking) == cudaSuccess &&
                   cudaStreamCreateWithFlags(&p->cs_out, cudaStreamNonBlocking) == cudaSuccess &&
-                  cudaEventCreateWithFlags(&p->hev_start, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&p->hev_in_free, cudaEventDisableTiming) == cudaSuccess &&
                   cudaEventCreateWithFlags(&p->hev_done, cudaEventDisableTiming) == cudaSuccess;
         for (int i = 0; i < 8 && ok; ++i)
             ok = cudaEventCreateWithFlags(&p->hev_in[i], cudaEventDisableTiming) == cudaSuccess &&
@@ -1103,6 +1108,22 @@ static int host_chunk_start(fftb_plan p, int nb, int k, int K)
 }
 #define FFTB_CU(call) do { if ((call) != cudaSuccess) { p->sticky = FFTB_ECUDA; return FFTB_ECUDA; } } while (0)
 
+// The incoming staging area may be refilled once the kernels of the previous call that read it are done (not: once
+// everything queued on the caller's stream is done -- that would put this call's host-to-device copies behind the
+// previous call's device-to-host copies, and PCIe would never carry both directions at once).
+static int host_in_begin(fftb_plan p)
+{
+    if (p->in_free_recorded) FFTB_CU(cudaStreamWaitEvent(p->cs_in, p->hev_in_free, 0));
+    return FFTB_OK;
+}
+static int host_in_end(fftb_plan p, cudaStream_t st)
+{
+    if (!p->pipe_ok) return FFTB_OK;
+    FFTB_CU(cudaEventRecord(p->hev_in_free, st));
+    p->in_free_recorded = true;
+    return FFTB_OK;
+}
+
 int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb, void *stream)
 {
     int rc = check_host(p, nb);
@@ -1114,11 +1135,10 @@ int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb,
     const size_t band = (size_t)p->S * p->elem, cband = (size_t)p->C * p->elem;
     if (K == 1) {
         FFTB_CU(cudaMemcpyAsync(stg, h_packed, (size_t)nb * band, cudaMemcpyHostToDevice, st));
-        return fftb_inverse(p, stg, d_cuboid, nb, stream);
+        rc = fftb_inverse(p, stg, d_cuboid, nb, stream);
+        return rc ? rc : host_in_end(p, st);
     }
-    // the copies start after everything already queued on the caller's stream (it may still read the staging area)
-    FFTB_CU(cudaEventRecord(p->hev_start, st));
-    FFTB_CU(cudaStreamWaitEvent(p->cs_in, p->hev_start, 0));
+    if ((rc = host_in_begin(p))) return rc;
     int launches = 0;
     for (int k = 0; k < K; ++k) {
         const int b0 = host_chunk_start(p, nb, k, K), b1 = host_chunk_start(p, nb, k + 1, K);
@@ -1131,7 +1151,7 @@ int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb,
         launches += p->launches;
     }
     p->launches = launches;
-    return FFTB_OK;
+    return host_in_end(p, st);
 }
 
 int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb, void *stream)
@@ -1140,7 +1160,7 @@ int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb,
     if (rc) return rc;
     if (!h_packed || !d_cuboid) return FFTB_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned char *stg = p->d_mem + p->o_stage;
+    unsigned char *stg = p->d_mem + p->o_stage_out;
     const int K = host_chunks(p, nb);
     const size_t band = (size_t)p->S * p->elem, cband = (size_t)p->C * p->elem;
     if (K == 1) {
@@ -1160,7 +1180,8 @@ int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb,
         FFTB_CU(cudaMemcpyAsync((unsigned char *)h_packed + b0 * band, stg + b0 * band, (size_t)(b1 - b0) * band,
                                 cudaMemcpyDeviceToHost, p->cs_out));
     }
-    // the call completes, in the caller's stream order, when the last chunk is in host memory
+    // the call completes, in the caller's stream order, when the last chunk is in host memory (this also keeps the
+    // outgoing staging area from being rewritten too early)
     FFTB_CU(cudaEventRecord(p->hev_done, p->cs_out));
     FFTB_CU(cudaStreamWaitEvent(st, p->hev_done, 0));
     p->launches = launches;
@@ -1173,18 +1194,17 @@ int fftb_apply_vloc_host(fftb_plan p, const void *h_in, void *h_out, const void 
     if (rc) return rc;
     if (!h_in || !h_out) return FFTB_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned char *stg = p->d_mem + p->o_stage;
+    unsigned char *stg = p->d_mem + p->o_stage, *sto = p->d_mem + p->o_stage_out;
     const int K = host_chunks(p, nb);
     const size_t band = (size_t)p->S * p->elem;
     if (K == 1) {
         FFTB_CU(cudaMemcpyAsync(stg, h_in, (size_t)nb * band, cudaMemcpyHostToDevice, st));
-        rc = fftb_apply_vloc(p, stg, stg, d_vloc, nb, stream);
+        rc = fftb_apply_vloc(p, stg, sto, d_vloc, nb, stream);
         if (rc) return rc;
-        FFTB_CU(cudaMemcpyAsync(h_out, stg, (size_t)nb * band, cudaMemcpyDeviceToHost, st));
-        return FFTB_OK;
+        FFTB_CU(cudaMemcpyAsync(h_out, sto, (size_t)nb * band, cudaMemcpyDeviceToHost, st));
+        return host_in_end(p, st);
     }
-    FFTB_CU(cudaEventRecord(p->hev_start, st));
-    FFTB_CU(cudaStreamWaitEvent(p->cs_in, p->hev_start, 0));
+    if ((rc = host_in_begin(p))) return rc;
     int launches = 0;
     for (int k = 0; k < K; ++k) {
         const int b0 = host_chunk_start(p, nb, k, K), b1 = host_chunk_start(p, nb, k + 1, K);
@@ -1192,14 +1212,15 @@ int fftb_apply_vloc_host(fftb_plan p, const void *h_in, void *h_out, const void 
                                 cudaMemcpyHostToDevice, p->cs_in));
         FFTB_CU(cudaEventRecord(p->hev_in[k], p->cs_in));
         FFTB_CU(cudaStreamWaitEvent(st, p->hev_in[k], 0));
-        rc = fftb_apply_vloc(p, stg + b0 * band, stg + b0 * band, d_vloc, b1 - b0, stream);
+        rc = fftb_apply_vloc(p, stg + b0 * band, sto + b0 * band, d_vloc, b1 - b0, stream);
         if (rc) return rc;
         launches += p->launches;
         FFTB_CU(cudaEventRecord(p->hev_out[k], st));
         FFTB_CU(cudaStreamWaitEvent(p->cs_out, p->hev_out[k], 0));
-        FFTB_CU(cudaMemcpyAsync((unsigned char *)h_out + b0 * band, stg + b0 * band, (size_t)(b1 - b0) * band,
+        FFTB_CU(cudaMemcpyAsync((unsigned char *)h_out + b0 * band, sto + b0 * band, (size_t)(b1 - b0) * band,
                                 cudaMemcpyDeviceToHost, p->cs_out));
     }
+    if ((rc = host_in_end(p, st))) return rc;
     FFTB_CU(cudaEventRecord(p->hev_done, p->cs_out));
     FFTB_CU(cudaStreamWaitEvent(st, p->hev_done, 0));
     p->launches = launches;
@@ -1297,7 +1318,7 @@ int fftb_plan_destroy(fftb_plan p)
     if (p->pipe_ok) {
         cudaStreamDestroy(p->cs_in);
         cudaStreamDestroy(p->cs_out);
-        cudaEventDestroy(p->hev_start);
+        cudaEventDestroy(p->hev_in_free);
         cudaEventDestroy(p->hev_done);
         for (int i = 0; i < 8; ++i) { cudaEventDestroy(p->hev_in[i]); cudaEventDestroy(p->hev_out[i]); }
     }
