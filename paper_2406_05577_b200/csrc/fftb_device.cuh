@@ -180,4 +180,45 @@ __device__ __forceinline__ void ld_pair(const float2 *p, float2 &a, float2 &b)
     b = make_float2(v.z, v.w);
 }
 
+// ---- L2 eviction priorities (createpolicy + .L2::cache_hint) ------------------------------------------------------
+// L2 eviction priority of a global access (createpolicy): the ring of intermediate rows is kept (evict_last) while
+// the cuboid and packed streams pass through (evict_first)
+__device__ __forceinline__ unsigned long long l2_policy(int kind) // 0 normal, 1 evict_first, 2 evict_last
+{
+    unsigned long long p;
+    if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    else if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void st_pair_hint(double2 *p, double2 a, double2 b, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v4.f64 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_pair_hint(float2 *p, float2 a, float2 b, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_hint(double2 *p, double2 a, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(a.x), "d"(a.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_hint(float2 *p, float2 a, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(a.x), "f"(a.y), "l"(pol) : "memory");
+}
+
+__device__ __forceinline__ double2 ld_hint(const double2 *p, unsigned long long pol)
+{
+    double2 v;
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float2 ld_hint(const float2 *p, unsigned long long pol)
+{
+    float2 v;
+    asm volatile("ld.global.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+
 } // namespace fftb

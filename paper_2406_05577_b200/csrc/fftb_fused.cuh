@@ -60,16 +60,6 @@ __device__ __forceinline__ void spin_until_ge(const int *p, int target)
 {
     while (ld_relaxed_gpu(p) < target) __nanosleep(32);
 }
-// L2 eviction priority of a global access (createpolicy): the ring of intermediate rows is kept (evict_last) while
-// the cuboid and packed streams pass through (evict_first)
-__device__ __forceinline__ unsigned long long l2_policy(int kind) // 0 normal, 1 evict_first, 2 evict_last
-{
-    unsigned long long p;
-    if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    else if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
 __device__ __forceinline__ void bulk_load_hint(void *sdst, const void *gsrc, unsigned bytes, unsigned long long *bar, unsigned long long pol)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(smem_u32(sdst)),
@@ -90,23 +80,6 @@ __device__ __forceinline__ void bulk_store_hint(void *gdst, const void *ssrc, un
                  "r"((unsigned)__cvta_generic_to_shared(ssrc)), "r"(bytes), "l"(pol)
                  : "memory");
 }
-__device__ __forceinline__ void st_pair_hint(double2 *p, double2 a, double2 b, unsigned long long pol)
-{
-    asm volatile("st.global.L2::cache_hint.v4.f64 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void st_pair_hint(float2 *p, float2 a, float2 b, unsigned long long pol)
-{
-    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void st_hint(double2 *p, double2 a, unsigned long long pol)
-{
-    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(a.x), "d"(a.y), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void st_hint(float2 *p, float2 a, unsigned long long pol)
-{
-    asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(a.x), "f"(a.y), "l"(pol) : "memory");
-}
-
 constexpr int fused_max(int a, int b) { return a > b ? a : b; }
 constexpr int fused_even(int x) { return (x + 1) & ~1; }
 

@@ -289,6 +289,8 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     constexpr int N = R4::N, M = R4::M, P2 = F::P2, G = F::G, YP = R4::YP;
     constexpr int XT = R4::NXT / NW;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    // the plane of A this kernel accumulates its four y residues into is read and rewritten within microseconds: keep it in L2
+    const unsigned long long pol_keep = l2_policy(2);
     C *pbuf = reinterpret_cast<C *>(smem_raw);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
@@ -378,10 +380,10 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
-                        oa[j] = (act && (unsigned)ia < (unsigned)co.y) ? __ldcg(d + ia) : czero<T>();
-                        ob[j] = (act && (unsigned)ib < (unsigned)co.y) ? __ldcg(d + ib) : czero<T>();
+                        oa[j] = (act && (unsigned)ia < (unsigned)co.y) ? ld_hint(d + ia, pol_keep) : czero<T>();
+                        ob[j] = (act && (unsigned)ib < (unsigned)co.y) ? ld_hint(d + ib, pol_keep) : czero<T>();
                     }
-                    if (hc) oc = __ldcg(d + ic);
+                    if (hc) oc = ld_hint(d + ic, pol_keep);
                 }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
@@ -391,10 +393,10 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
-                        if ((unsigned)ia < (unsigned)co.y) d[ia] = R > 0 ? cadd(oa[j], pa[j]) : pa[j];
-                        if ((unsigned)ib < (unsigned)co.y) d[ib] = R > 0 ? cadd(ob[j], pb[j]) : pb[j];
+                        if ((unsigned)ia < (unsigned)co.y) st_hint(d + ia, R > 0 ? cadd(oa[j], pa[j]) : pa[j], pol_keep);
+                        if ((unsigned)ib < (unsigned)co.y) st_hint(d + ib, R > 0 ? cadd(ob[j], pb[j]) : pb[j], pol_keep);
                     }
-                    if (hc) d[ic] = R > 0 ? cadd(oc, pcv) : pcv;
+                    if (hc) st_hint(d + ic, R > 0 ? cadd(oc, pcv) : pcv, pol_keep);
                 }
             }
             // single-stick columns: one warp per column, dot product with conj(W^{k2 y}) over the quarter's lines
@@ -408,7 +410,7 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
                     acc.x += __shfl_xor_sync(0xffffffffu, acc.x, sft);
                     acc.y += __shfl_xor_sync(0xffffffffu, acc.y, sft);
                 }
-                if (lane == 0) dst[co.x] = R > 0 ? cadd(__ldcg(dst + co.x), acc) : acc;
+                if (lane == 0) st_hint(dst + co.x, R > 0 ? cadd(ld_hint(dst + co.x, pol_keep), acc) : acc, pol_keep);
             }
         };
 #pragma unroll 1
@@ -450,6 +452,8 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
     constexpr int N = R4::N, M = R4::M, P2 = F::P2, G = F::G, YP = R4::YP, ZCOL = R4::ZCOL;
     constexpr int XT = R4::NXT / NW;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    // the plane of A this kernel accumulates its four y residues into is read and rewritten within microseconds: keep it in L2
+    const unsigned long long pol_keep = l2_policy(2);
     C *pbuf = reinterpret_cast<C *>(smem_raw);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
@@ -637,10 +641,10 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
-                        oa[j] = (c.act && (unsigned)ia < (unsigned)c.co.y) ? __ldcg(d + ia) : czero<T>();
-                        ob[j] = (c.act && (unsigned)ib < (unsigned)c.co.y) ? __ldcg(d + ib) : czero<T>();
+                        oa[j] = (c.act && (unsigned)ia < (unsigned)c.co.y) ? ld_hint(d + ia, pol_keep) : czero<T>();
+                        ob[j] = (c.act && (unsigned)ib < (unsigned)c.co.y) ? ld_hint(d + ib, pol_keep) : czero<T>();
                     }
-                    if (hc) oc = __ldcg(d + ic);
+                    if (hc) oc = ld_hint(d + ic, pol_keep);
                 }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
@@ -650,10 +654,10 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
-                        if ((unsigned)ia < (unsigned)c.co.y) d[ia] = R > 0 ? cadd(oa[j], pa[j]) : pa[j];
-                        if ((unsigned)ib < (unsigned)c.co.y) d[ib] = R > 0 ? cadd(ob[j], pb[j]) : pb[j];
+                        if ((unsigned)ia < (unsigned)c.co.y) st_hint(d + ia, R > 0 ? cadd(oa[j], pa[j]) : pa[j], pol_keep);
+                        if ((unsigned)ib < (unsigned)c.co.y) st_hint(d + ib, R > 0 ? cadd(ob[j], pb[j]) : pb[j], pol_keep);
                     }
-                    if (hc) d[ic] = R > 0 ? cadd(oc, pcv) : pcv;
+                    if (hc) st_hint(d + ic, R > 0 ? cadd(oc, pcv) : pcv, pol_keep);
                 }
             }
             for (int k = warp; k < n_one; k += NW) {
@@ -666,7 +670,7 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
                     acc.x += __shfl_xor_sync(0xffffffffu, acc.x, sft);
                     acc.y += __shfl_xor_sync(0xffffffffu, acc.y, sft);
                 }
-                if (lane == 0) dst[co.x] = R > 0 ? cadd(__ldcg(dst + co.x), acc) : acc;
+                if (lane == 0) st_hint(dst + co.x, R > 0 ? cadd(ld_hint(dst + co.x, pol_keep), acc) : acc, pol_keep);
             }
         };
         using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>;
