@@ -32,7 +32,7 @@ METRIC = "band 3D-FFTs/sec (inv+fwd)"
 UNIT = "band-FFTs/s"
 NOMINAL_HBM_GBS = 8000.0     # BASELINE.json's "~8 TB/s" target denominator
 FALLBACK_HBM_GBS = 6650.0    # /opt/skills/guides/B200_PROFILING.md fallback
-ALU_PROBE_RECORD = "profiles/r02_alu_probe.md"   # a recorded run of the probe bench.py repeats live (fftb_probe_fma)
+ALU_PROBE_RECORD = "profiles/r02_device_probes.md"   # a recorded run of the probe bench.py repeats live (fftb_probe_fma)
 
 
 def measured_peaks():
@@ -419,7 +419,7 @@ def main():
                     help="N > 1: weak = a full batch per GPU (default), strong = the config's batch split over the GPUs (sharding.band_range)")
     ap.add_argument("--layout", default="band_slowest", choices=["band_slowest", "batch_fastest"],
                     help="layout of the packed arrays: [nb][S] (default, north_star) or [S][nb] (FFTB_FLAG_BATCH_FASTEST, PAPER.md:219-221)")
-    ap.add_argument("--probe-alu", action="store_true", help="print the FP64 / FP32 FMA probe (fftb_probe_fma) as JSON and exit")
+    ap.add_argument("--probe-alu", action="store_true", help="print the device probes (FP64 / FP32 FMA rate, store port of an SM) as JSON and exit")
     ap.add_argument("--fused", action="store_true", help="one cooperative launch per direction (FFTB_TUNE_FUSED): the intermediate stays in L2")
     ap.add_argument("--no-l2-hints", action="store_true", help="fused launches without L2 eviction priorities (FFTB_TUNE_NO_L2_HINTS)")
     ap.add_argument("--ring-bands", type=int, default=0, help="fused launches: band slots of the ring (0 = library default)")
@@ -441,6 +441,7 @@ def main():
         for dt in ("c128", "c64"):
             tf, ms = fb.probe_fma(dt)
             out["fp64" if dt == "c128" else "fp32"] = {"tflops": tf, "ms": ms}
+        out["store_port"] = {str(n): dict(zip(("bytes_per_clk_per_sm", "gbs"), fb.probe_store_port(n))) for n in (1, 8, 37, 74, out["sms"])}
         print(json.dumps(out), flush=True)
         return
     if args.impl == "reference":

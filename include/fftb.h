@@ -121,7 +121,7 @@ enum fftb_tuning_flags {
 typedef struct {
     int64_t workspace_bytes; /* budget for the intermediate A inside the bind block (the plan rounds it to whole bands,
                                 at least one); 0 = default */
-    int32_t ring_bands;      /* band slots of the fused launches' ring; 0 = default (lead_bands + 4) */
+    int32_t ring_bands;      /* band slots of the fused launches' ring; 0 = default (lead_bands + 2) */
     int32_t lead_bands;      /* bands the producers run ahead; 0 = default (2) */
     uint32_t flags;          /* fftb_tuning_flags */
     uint32_t reserved;       /* must be 0 */
@@ -224,6 +224,11 @@ int fftb_plan_last_launches(fftb_plan p);
  * for the result.  It is the denominator of the "alu" roofline of the fused local-potential workloads
  * ("FP64 pipe utilisation ... over the probed peak"). */
 int fftb_probe_fma(int dtype, double *tflops, double *ms);
+/* The same kind of probe for the global-store port of an SM: `n_sms` CTAs (one per SM) stream 32-byte stores; returns the
+ * bytes per clock ONE SM sustained (issue-side clocks) and the aggregate GB/s (may be NULL).  Allocates 32 MB per CTA,
+ * legacy default stream, waits.  On B200 an SM stores 32 B/clk however few SMs take part, which bounds the x phase of
+ * the inverse plane kernels. */
+int fftb_probe_store_port(int n_sms, double *bytes_per_clk_per_sm, double *gbs);
 
 /* Per-kernel timing for benchmarks.  fftb_plan_profile(p, 1) makes every later execute call record a
  * CUDA event pair around each kernel it launches (on the launching stream); fftb_plan_profile_read

@@ -27,7 +27,7 @@ SYMBOLS = [
     "fftb_inverse", "fftb_forward", "fftb_apply_vloc",
     "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
     "fftb_dense_embed", "fftb_dense_extract", "fftb_packed_transpose",
-    "fftb_probe_fma", "fftb_plan_last_launches",
+    "fftb_probe_fma", "fftb_probe_store_port", "fftb_plan_last_launches",
     "fftb_slab_plan_create", "fftb_slab_plan_info_get", "fftb_slab_plan_counts", "fftb_slab_plan_bind", "fftb_slab_plan_exchange_ptr",
     "fftb_slab_inverse_begin", "fftb_slab_inverse_end", "fftb_slab_forward_begin", "fftb_slab_forward_end", "fftb_slab_plan_destroy", "fftb_plan_profile", "fftb_plan_profile_read", "fftb_plan_destroy", "fftb_strerror",
 ]
@@ -82,6 +82,7 @@ def lib():
             getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
         L.fftb_packed_transpose.argtypes = [vp, vp, vp, i32, i32, vp]
         L.fftb_probe_fma.argtypes = [i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+        L.fftb_probe_store_port.argtypes = [i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
         L.fftb_plan_last_launches.argtypes = [vp]
         L.fftb_plan_profile.argtypes = [vp, i32]
         L.fftb_plan_profile_read.argtypes = [vp, vp, vp]
@@ -101,6 +102,13 @@ def probe_fma(dtype="c128"):
     tf, ms = ctypes.c_double(), ctypes.c_double()
     _check(lib().fftb_probe_fma(FFTB_C128 if dtype == "c128" else FFTB_C64, ctypes.byref(tf), ctypes.byref(ms)), "fftb_probe_fma")
     return tf.value, ms.value
+
+
+def probe_store_port(n_sms):
+    """-> (bytes per clock per SM, aggregate GB/s) of n_sms SMs streaming 32-byte stores (fftb_probe_store_port)."""
+    v, g = ctypes.c_double(), ctypes.c_double()
+    _check(lib().fftb_probe_store_port(int(n_sms), ctypes.byref(v), ctypes.byref(g)), "fftb_probe_store_port")
+    return v.value, g.value
 
 
 def _check(rc, what):

@@ -812,13 +812,13 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
             size_t ws = (size_t)desc->batch * per_band;
             if (ws > budget) ws = budget;
             if (ws < per_band) ws = per_band;
-            // fused launches: a ring of band slots at the start of the workspace that stays in L2 (6 x 6.7 MB at 128^3
+            // fused launches: a ring of band slots at the start of the workspace that stays in L2 (4 x 6.7 MB at 128^3
             // complex128), producers 2 bands ahead of their consumers; nslot > lead >= 0 (fftb_fused.cuh)
             p->ring_ntiles = fused ? (p->nsticks + ful.geom.ts - 1) / ful.geom.ts : 0;
             p->ring_slot = fused ? (long long)p->ring_ntiles * ful.geom.tile : 0;
             const size_t slot = fused ? (size_t)p->ring_slot * p->elem : (size_t)p->a_inv_stride * p->elem;
-            long long ring = tune && tune->ring_bands > 0 ? tune->ring_bands : 0, lead = tune && tune->lead_bands > 0 ? tune->lead_bands : 3;
-            if (ring == 0) ring = lead + 5;
+            long long ring = tune && tune->ring_bands > 0 ? tune->ring_bands : 0, lead = tune && tune->lead_bands > 0 ? tune->lead_bands : 2;
+            if (ring == 0) ring = lead + 2; // measured (profiles/r02_fused_ring_sweep.md): the smaller the ring, the less of it leaks to DRAM
             if (ring > desc->batch) ring = desc->batch;
             if (fused && ws < (size_t)ring * slot && (size_t)ring * slot <= budget) ws = (size_t)ring * slot; // tile-major slots are a little larger
             if (fused && ws < slot) ws = slot;
@@ -1277,6 +1277,15 @@ int fftb_packed_transpose(fftb_plan p, const void *d_in, void *d_out, int nb, in
 }
 
 int fftb_plan_last_launches(fftb_plan p) { return p ? p->launches : FFTB_EINVAL; }
+
+int fftb_probe_store_port(int n_sms, double *bytes_per_clk_per_sm, double *gbs)
+{
+    if (!bytes_per_clk_per_sm || n_sms < 1 || n_sms > 1024) return FFTB_EINVAL;
+    const double v = probe_store_port(n_sms, gbs);
+    if (v < 0.0) return FFTB_ECUDA;
+    *bytes_per_clk_per_sm = v;
+    return FFTB_OK;
+}
 
 int fftb_probe_fma(int dtype, double *tflops, double *ms)
 {

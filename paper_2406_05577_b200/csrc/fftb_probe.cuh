@@ -58,4 +58,59 @@ template <typename T> double probe_fma_tflops(double *ms_out)
     return 2.0 * fma / (best * 1e-3) / 1e12;
 }
 
+// ---- store port: how many bytes per clock ONE SM can push to global memory -------------------------------------------
+// The inverse plane kernels issue a z-plane's 262 KB of cuboid stores within their x phase; this probe shows the rate an
+// SM cannot exceed however few SMs are storing (32 B/clk on B200), which is what bounds that phase.
+__global__ void __launch_bounds__(256, 1) probe_store_k(double2 *out, long long per_cta_elems, int iters, long long *clk)
+{
+    double2 *base = out + (long long)blockIdx.x * per_cta_elems;
+    const int tid = threadIdx.x;
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+        // every warp writes 1 KB per instruction (32 lanes x 32 B), 16 instructions back to back like an x task
+        double2 *p = base + ((long long)it * 256 * 16 + tid) * 2;
+#pragma unroll
+        for (int u = 0; u < 16; ++u)
+            asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p + (long long)u * 512), "d"(1.0), "d"(2.0), "d"(3.0), "d"((double)it) : "memory");
+    }
+    __syncthreads();
+    if (tid == 0) clk[blockIdx.x] = clock64() - t0;
+}
+
+// n_ctas CTAs (one per SM) stream 32 MB each; returns bytes per clock per SM (issue-side clocks), aggregate GB/s in *gbs
+inline double probe_store_port(int n_ctas, double *gbs)
+{
+    constexpr int ITERS = 256;
+    const long long per_cta = (long long)ITERS * 256 * 16 * 2;
+    double2 *out = nullptr;
+    long long *clk = nullptr;
+    if (n_ctas < 1 || cudaMalloc(&out, sizeof(double2) * (size_t)per_cta * n_ctas) != cudaSuccess) return -1.0;
+    if (cudaMalloc(&clk, sizeof(long long) * (size_t)n_ctas) != cudaSuccess) { cudaFree(out); return -1.0; }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    probe_store_k<<<n_ctas, 256>>>(out, per_cta, 8, clk); // warm-up
+    cudaEventRecord(e0, 0);
+    probe_store_k<<<n_ctas, 256>>>(out, per_cta, ITERS, clk);
+    cudaEventRecord(e1, 0);
+    double res = -1.0;
+    if (cudaEventSynchronize(e1) == cudaSuccess && cudaGetLastError() == cudaSuccess) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        long long *h = new long long[n_ctas];
+        cudaMemcpy(h, clk, sizeof(long long) * (size_t)n_ctas, cudaMemcpyDeviceToHost);
+        double avg = 0.0;
+        for (int i = 0; i < n_ctas; ++i) avg += (double)h[i];
+        delete[] h;
+        const double bytes = (double)per_cta * 16.0;
+        res = bytes / (avg / n_ctas);
+        if (gbs) *gbs = bytes * n_ctas / (ms * 1e-3) / 1e9;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    cudaFree(clk);
+    return res;
+}
+
 } // namespace fftb
