@@ -58,7 +58,9 @@ enum fftb_status {
     FFTB_EUNSUPPORTED = -2, /* a description outside the predefined patterns (see fftb_plan_create) */
     FFTB_ENOMEM = -3,       /* host allocation failed, or the bind block is too small */
     FFTB_ECUDA = -4,        /* a CUDA call or launch failed; sticky until the plan is destroyed */
-    FFTB_ESTATE = -5        /* execute before fftb_plan_bind, or mismatched plans */
+    FFTB_ESTATE = -5,       /* execute before fftb_plan_bind, or mismatched plans */
+    FFTB_ETOOBIG = -6       /* fftb_inverse_static only: the plan's tables plus one band of its intermediate do not fit in
+                               the library's static scratch array (FFTB_STATIC_SCRATCH_BYTES) */
 };
 
 enum fftb_dtype { FFTB_C64 = 0, FFTB_C128 = 1 };               /* element type of packed and cuboid */
@@ -176,6 +178,26 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream);
 /* inverse: d_packed [nb][S] -> d_cuboid [nb][N3][N2][N1].  unpack + pruned z pass on the sticks,
  * y pass on the occupied x columns only, x pass last (Fig. 3, 112: staged padding). */
 int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void *stream);
+
+/* inverse for callers that cannot allocate device memory at all (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the SAME kernels as fftb_inverse (the separate z-pass and plane launches), but the
+ * plan's tables and the intermediate A live in ONE array of FFTB_STATIC_SCRATCH_BYTES that the library itself holds in
+ * device memory (a file-scope `static __device__` array: every GPU that loads the library keeps these 16 MiB until the
+ * process exits).  The plan needs no fftb_plan_bind and no bind block (a bound plan's block is not touched); the caller
+ * passes only the input and the output, same layouts, alignment and nb range as fftb_inverse.  The call makes no
+ * cudaMalloc / cudaFree and calls no allocating routine: it copies the plan's tables (host memory the plan owns; some
+ * tens of KB) into the array on `stream`, then enqueues the kernels for as many bands at a time as the rest of the array
+ * holds.  Results are bit-identical to fftb_inverse.
+ *   FFTB_ETOOBIG  tables + ONE band of the intermediate (N3 * pitch elements) exceed FFTB_STATIC_SCRATCH_BYTES; e.g.
+ *                 128^3 complex128 at radius 32 needs 6.4 MiB and fits (two bands at a time), 256^3 at radius 64 needs
+ *                 50 MiB and is refused.  Nothing is enqueued.
+ *   FFTB_EINVAL / FFTB_ECUDA as for fftb_inverse; a failure here does not make the plan sticky.
+ * Every call on a device SHARES the one array, and the array keeps the last call's contents: each call rewrites the
+ * tables and every element of A it later reads, so nothing has to start at zero, but two calls that overlap on the GPU
+ * (different streams without an event between them, or two host threads on different streams) race on it -- keep
+ * them on one stream or order them yourself.  The plan itself is only read. */
+#define FFTB_STATIC_SCRATCH_BYTES (16u * 1024u * 1024u)
+int fftb_inverse_static(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void *stream);
 
 /* forward: d_cuboid -> d_packed, the mirror image; applies the plan's scale. */
 int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void *stream);

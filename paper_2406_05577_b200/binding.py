@@ -19,12 +19,13 @@ FFTB_SCALE_NONE, FFTB_SCALE_FORWARD = 0, 1
 FFTB_FLAG_DENSE = 1
 FFTB_FLAG_BATCH_FASTEST = 2
 FFTB_TUNE_GENERIC_Z, FFTB_TUNE_GENERIC_PLANE, FFTB_TUNE_FUSED, FFTB_TUNE_NO_L2_HINTS = 1, 2, 4, 8
-FFTB_OK, FFTB_EINVAL, FFTB_EUNSUPPORTED, FFTB_ENOMEM, FFTB_ECUDA, FFTB_ESTATE = 0, -1, -2, -3, -4, -5
+FFTB_OK, FFTB_EINVAL, FFTB_EUNSUPPORTED, FFTB_ENOMEM, FFTB_ECUDA, FFTB_ESTATE, FFTB_ETOOBIG = 0, -1, -2, -3, -4, -5, -6
+FFTB_STATIC_SCRATCH_BYTES = 16 * 1024 * 1024  # the library-held device array fftb_inverse_static works in
 
 # every symbol include/fftb.h declares
 SYMBOLS = [
     "fftb_plan_create", "fftb_plan_create_tuned", "fftb_plan_create_explicit", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
-    "fftb_inverse", "fftb_forward", "fftb_apply_vloc",
+    "fftb_inverse", "fftb_inverse_static", "fftb_forward", "fftb_apply_vloc",
     "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
     "fftb_dense_embed", "fftb_dense_extract", "fftb_packed_transpose",
     "fftb_probe_fma", "fftb_probe_store_port", "fftb_plan_last_launches",
@@ -74,7 +75,7 @@ def lib():
         L.fftb_plan_info_get.argtypes = [vp, ctypes.POINTER(PlanInfo)]
         L.fftb_plan_get_map.argtypes = [vp, vp, vp, vp, vp, vp]
         L.fftb_plan_bind.argtypes = [vp, vp, ctypes.c_size_t, vp]
-        for name in ("fftb_inverse", "fftb_forward", "fftb_inverse_host", "fftb_forward_host"):
+        for name in ("fftb_inverse", "fftb_inverse_static", "fftb_forward", "fftb_inverse_host", "fftb_forward_host"):
             getattr(L, name).argtypes = [vp, vp, vp, i32, vp]
         for name in ("fftb_apply_vloc", "fftb_apply_vloc_host"):
             getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
@@ -228,6 +229,14 @@ class Plan:
             cuboid = torch.empty(self.cuboid_shape(nb), dtype=self.torch_complex, device=packed.device)
         _check(lib().fftb_inverse(self._h, self._chk(packed, self.packed_shape(nb)), self._chk(cuboid, self.cuboid_shape(nb)),
                                   nb, _stream_ptr(stream)), "fftb_inverse")
+        return cuboid
+
+    def inverse_static(self, packed, cuboid, stream=None):
+        """fftb_inverse_static: no bind block; tables and intermediate in the library's static device array.  The caller
+        passes the output too (this call allocates nothing)."""
+        nb = self._nb(packed)
+        _check(lib().fftb_inverse_static(self._h, self._chk(packed, self.packed_shape(nb)), self._chk(cuboid, self.cuboid_shape(nb)),
+                                         nb, _stream_ptr(stream)), "fftb_inverse_static")
         return cuboid
 
     def forward(self, cuboid, packed=None, stream=None):

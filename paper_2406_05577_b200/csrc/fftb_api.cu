@@ -594,6 +594,7 @@ const char *fftb_strerror(int code)
     case FFTB_ENOMEM: return "out of memory / bind block too small";
     case FFTB_ECUDA: return "CUDA error";
     case FFTB_ESTATE: return "plan not bound / mismatched plans";
+    case FFTB_ETOOBIG: return "transform too large for the static scratch array (FFTB_STATIC_SCRATCH_BYTES)";
     default: return "unknown fftb status";
     }
 }
@@ -1332,6 +1333,89 @@ int fftb_plan_destroy(fftb_plan p)
         for (int i = 0; i < 8; ++i) { cudaEventDestroy(p->hev_in[i]); cudaEventDestroy(p->hev_out[i]); }
     }
     delete p;
+    return FFTB_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// fftb_inverse_static (include/fftb.h): the inverse transform for callers that may not allocate device memory.  The
+// scratch the two kernels of a band chunk share -- the plane-major intermediate A -- and the plan's tables live in a
+// file-scope device array instead of a caller-owned bind block.
+//
+// In HOST code the name g_static_scratch is only a stand-in for the symbol: it is not a device address, and a kernel
+// handed `g_static_scratch` itself would fault (or, where the GPU can reach host memory, silently use the wrong memory).
+// Its device address is looked up once per device with cudaGetSymbolAddress (that device current), kept in a small
+// table under a mutex, and THAT pointer goes to the kernels.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_scratch[FFTB_STATIC_SCRATCH_BYTES];
+
+struct StaticScratch { unsigned char *ptr; int sms; };
+static std::mutex g_static_mu;
+static std::map<int, StaticScratch> g_static_dev; // device ordinal -> device address of g_static_scratch, SM count
+
+static int static_scratch_current_device(StaticScratch *out)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return FFTB_ECUDA; }
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    auto it = g_static_dev.find(dev);
+    if (it == g_static_dev.end()) {
+        StaticScratch s = {nullptr, 0};
+        if (cudaGetSymbolAddress((void **)&s.ptr, g_static_scratch) != cudaSuccess || !s.ptr || (uintptr_t)s.ptr % 256) {
+            cudaGetLastError();
+            return FFTB_ECUDA;
+        }
+        if (cudaDeviceGetAttribute(&s.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || s.sms < 1) {
+            cudaGetLastError();
+            return FFTB_ECUDA;
+        }
+        it = g_static_dev.emplace(dev, s).first;
+    }
+    *out = it->second;
+    return 0;
+}
+
+int fftb_inverse_static(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void *stream)
+{
+    if (!p || !d_packed || !d_cuboid) return FFTB_EINVAL;
+    if (nb < 1 || nb > p->desc.batch) return FFTB_EINVAL;
+    if ((uintptr_t)d_packed % 16 || (uintptr_t)d_cuboid % (p->elem == 16 ? 32 : 16)) return FFTB_EINVAL;
+    // layout inside the array: the tables at the offsets they have in a bind block (all before o_sync), then A
+    const size_t o_a = p->o_sync, band = (size_t)p->a_inv_stride * p->elem;
+    if (o_a + band > (size_t)FFTB_STATIC_SCRATCH_BYTES) return FFTB_ETOOBIG;
+    StaticScratch sc;
+    if (int rc = static_scratch_current_device(&sc)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char *m = sc.ptr;
+    // the array keeps whatever the last call (of any plan) left: rewrite the tables, every time.  A needs no clearing: the
+    // z pass of a chunk writes every (z, stick) element the plane kernel of that chunk reads.
+    cudaError_t e = cudaMemcpyAsync(m + p->o_stick, p->h_stick.data(), sizeof(int4) * p->h_stick.size(), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(m + p->o_col, p->h_col.data(), sizeof(int4) * p->h_col.size(), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(m + p->o_perm, p->h_colperm.data(), sizeof(int) * p->h_colperm.size(), cudaMemcpyHostToDevice, st);
+    for (int d = 0; d < 3 && e == cudaSuccess; ++d)
+        e = cudaMemcpyAsync(m + p->o_tw[d], p->h_tw[d].data(), p->h_tw[d].size(), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return FFTB_ECUDA; }
+    DevPlan dv;
+    dv.n1 = p->desc.n[0]; dv.n2 = p->desc.n[1]; dv.n3 = p->desc.n[2];
+    dv.nsticks = p->nsticks; dv.pitch = p->pitch; dv.nxocc = p->nxocc; dv.k1lo = p->k1lo; dv.ry = p->ry;
+    dv.stick = (const int4 *)(m + p->o_stick);
+    dv.col = (const int4 *)(m + p->o_col);
+    dv.colperm = (const int *)(m + p->o_perm);
+    dv.n_multi = p->n_multi;
+    dv.tw1 = m + p->o_tw[0]; dv.tw2 = m + p->o_tw[1]; dv.tw3 = m + p->o_tw[2];
+    dv.S = p->S;
+    dv.scale = p->desc.scale == FFTB_SCALE_FORWARD ? 1.0 / (double)p->C : 1.0;
+    dv.sms = sc.sms;
+    unsigned char *A = m + o_a;
+    long long chunk = (long long)(((size_t)FFTB_STATIC_SCRATCH_BYTES - o_a) / band);
+    if (chunk > nb) chunk = nb;
+    for (int b0 = 0; b0 < nb; b0 += (int)chunk) {
+        const int nc = nb - b0 < (int)chunk ? nb - b0 : (int)chunk;
+        const unsigned char *pk = (const unsigned char *)d_packed + (p->bf ? (size_t)b0 : (size_t)b0 * p->S) * p->elem;
+        unsigned char *cb = (unsigned char *)d_cuboid + (size_t)b0 * p->C * p->elem;
+        int rc = p->zl.inv(dv, pk, A, p->a_inv_stride, nc, p->bf ? nb : 0, st);
+        if (!rc) rc = p->plk.run[MODE_INV](dv, p->tabs, A, nullptr, nullptr, cb, nullptr, p->a_inv_stride, 0, nc, st);
+        if (rc) return rc;
+    }
     return FFTB_OK;
 }
 
