@@ -193,8 +193,8 @@ def run_ours(args, w):
         raise SystemExit(f"bench.py: --scaling strong needs at least one band per rank ({w.batch} bands, {world} ranks)")
     tflags = (fb.FFTB_TUNE_FUSED if args.fused else 0) | (fb.FFTB_TUNE_NO_L2_HINTS if args.no_l2_hints else 0)
     tuning = {"flags": tflags} if tflags else None
-    if args.ring_bands or args.lead_bands:
-        tuning = dict(tuning or {}, ring_bands=args.ring_bands, lead_bands=args.lead_bands)
+    if args.ring_bands or args.lead_bands or args.z_ctas:
+        tuning = dict(tuning or {}, ring_bands=args.ring_bands, lead_bands=args.lead_bands, z_ctas=args.z_ctas)
     bfast = args.layout == "batch_fastest"
     plan = fb.Plan(w.n, w.cutoff, batch=nb, dtype=w.dtype, scale="forward", tuning=tuning, batch_fastest=bfast).bind(host_staging=True)
     info = plan.info
@@ -424,6 +424,7 @@ def main():
     ap.add_argument("--no-l2-hints", action="store_true", help="fused launches without L2 eviction priorities (FFTB_TUNE_NO_L2_HINTS)")
     ap.add_argument("--ring-bands", type=int, default=0, help="fused launches: band slots of the ring (0 = library default)")
     ap.add_argument("--lead-bands", type=int, default=0, help="fused launches: bands the producers run ahead (0 = library default)")
+    ap.add_argument("--z-ctas", type=int, default=0, help="fused launches: spatial split, this many CTAs take the z tiles only (0 = merged walk)")
     ap.add_argument("--op", default="config", choices=["config", "inv_fwd", "vloc"],
                     help="operation of the step: the config's own (default), or the same grid and batch with the other one")
     args = ap.parse_args()

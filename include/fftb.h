@@ -126,7 +126,9 @@ typedef struct {
     int32_t ring_bands;      /* band slots of the fused launches' ring; 0 = default (lead_bands + 2) */
     int32_t lead_bands;      /* bands the producers run ahead; 0 = default (2) */
     uint32_t flags;          /* fftb_tuning_flags */
-    uint32_t reserved;       /* must be 0 */
+    uint32_t z_ctas;         /* fused launches: > 0 = spatial split, this many CTAs take the z tiles only and the others the
+                                planes only (ignored if the launch has no more CTAs than that); 0 = every CTA walks both
+                                lists merged (default); > 1024: FFTB_EINVAL */
 } fftb_plan_tuning;
 
 /* Create a plan (host only, no CUDA call).  Builds the offset array -- the stick map -- from the

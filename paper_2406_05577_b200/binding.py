@@ -48,7 +48,7 @@ class PlanInfo(ctypes.Structure):
 
 class PlanTuning(ctypes.Structure):
     _fields_ = [("workspace_bytes", ctypes.c_int64), ("ring_bands", ctypes.c_int32), ("lead_bands", ctypes.c_int32),
-                ("flags", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
+                ("flags", ctypes.c_uint32), ("z_ctas", ctypes.c_uint32)]
 
 
 class FftbError(RuntimeError):
@@ -131,7 +131,7 @@ class Plan:
     def __init__(self, n, cutoff=(0, 0, 0), batch=1, dtype="c128", scale="forward", dense=False, stick_map=None, tuning=None,
                  batch_fastest=False):
         """stick_map = (k1, k2, k3lo, len) int arrays: fftb_plan_create_explicit instead of a cut-off.
-        tuning = dict(workspace_bytes=, ring_bands=, lead_bands=, flags=): fftb_plan_create_tuned."""
+        tuning = dict(workspace_bytes=, ring_bands=, lead_bands=, flags=, z_ctas=): fftb_plan_create_tuned."""
         d = PlanDesc()
         d.n[:] = [int(x) for x in n]
         d.cutoff[:] = [int(x) for x in cutoff]
@@ -147,6 +147,7 @@ class Plan:
             tu.ring_bands = int(tuning.get("ring_bands", 0))
             tu.lead_bands = int(tuning.get("lead_bands", 0))
             tu.flags = int(tuning.get("flags", 0))
+            tu.z_ctas = int(tuning.get("z_ctas", 0))
             _check(lib().fftb_plan_create_tuned(ctypes.byref(self._h), ctypes.byref(d), ctypes.byref(tu)), "fftb_plan_create_tuned")
         elif stick_map is None:
             _check(lib().fftb_plan_create(ctypes.byref(self._h), ctypes.byref(d)), "fftb_plan_create")

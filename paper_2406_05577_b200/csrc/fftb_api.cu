@@ -150,9 +150,9 @@ struct FusedGeom { int ts, tile, rp; }; // sticks per z tile, elements of a tile
 struct FusedLaunch {
     FusedGeom geom;
     int (*inv)(const DevPlan &, const PlanTabs &, const void *packed, void *ring, const CUtensorMap &ring_map, void *cuboid, long long stride,
-               int nb, int nslot, int lead, int hints, int *sync, cudaStream_t);
+               int nb, int nslot, int lead, int nz, int hints, int *sync, cudaStream_t);
     int (*fwd)(const DevPlan &, const PlanTabs &, const void *cuboid, void *ring, void *packed, long long stride, int nb, int nslot,
-               int lead, int hints, int *sync, cudaStream_t);
+               int lead, int nz, int hints, int *sync, cudaStream_t);
 };
 
 template <typename T, class AZ> int launch_zinv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, long long pk_pitch, cudaStream_t st)
@@ -377,7 +377,7 @@ template <class K> int fused_grid(K k, int threads, size_t smem, const DevPlan &
 }
 template <typename T, class F>
 int launch_fused_inv(const DevPlan &pl, const PlanTabs &tabs, const void *packed, void *ring, const CUtensorMap &ring_map, void *cuboid,
-                     long long stride, int nb, int nslot, int lead, int hints, int *sync, cudaStream_t st)
+                     long long stride, int nb, int nslot, int lead, int nz, int hints, int *sync, cudaStream_t st)
 {
     constexpr int NW = PlaneNW<F::N>::value;
     using FU = Fused<T, F, NW>;
@@ -388,18 +388,19 @@ int launch_fused_inv(const DevPlan &pl, const PlanTabs &tabs, const void *packed
     const int items = nb * (pl.n3 > ntiles ? pl.n3 : ntiles);
     int grid = 0;
     if (int rc = fused_grid(k, NW * 32, smem, pl, items, &grid)) return rc;
+    if (nz >= grid) nz = 0; // spatial split needs CTAs of both roles: fall back to the merged walk
     if (cudaMemsetAsync(sync, 0, 2 * sizeof(int) * (size_t)nb, st) != cudaSuccess) return FFTB_ECUDA;
     const cx<T> *a_packed = (const cx<T> *)packed;
     cx<T> *a_ring = (cx<T> *)ring, *a_cub = (cx<T> *)cuboid;
     int *zdone = sync, *pdone = sync + nb;
     void *args[] = {(void *)&pl, (void *)&tabs.ct, (void *)&a_packed, (void *)&a_ring, (void *)&ring_map, (void *)&a_cub, (void *)&stride,
-                    (void *)&nb, (void *)&nslot, (void *)&lead, (void *)&hints, (void *)&zdone, (void *)&pdone};
+                    (void *)&nb, (void *)&nslot, (void *)&lead, (void *)&nz, (void *)&hints, (void *)&zdone, (void *)&pdone};
     if (cudaLaunchCooperativeKernel((const void *)k, dim3(grid), dim3(NW * 32), args, smem, st) != cudaSuccess) return FFTB_ECUDA;
     return launch_status();
 }
 template <typename T, class F>
 int launch_fused_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *cuboid, void *ring, void *packed, long long stride, int nb, int nslot,
-                     int lead, int hints, int *sync, cudaStream_t st)
+                     int lead, int nz, int hints, int *sync, cudaStream_t st)
 {
     constexpr int NW = PlaneNW<F::N>::value;
     using FU = Fused<T, F, NW>;
@@ -409,12 +410,13 @@ int launch_fused_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *cuboid
     const int items = nb * (pl.n3 > ntiles ? pl.n3 : ntiles);
     int grid = 0;
     if (int rc = fused_grid(k, NW * 32, smem, pl, items, &grid)) return rc;
+    if (nz >= grid) nz = 0;
     if (cudaMemsetAsync(sync, 0, 2 * sizeof(int) * (size_t)nb, st) != cudaSuccess) return FFTB_ECUDA;
     const cx<T> *a_cub = (const cx<T> *)cuboid;
     cx<T> *a_ring = (cx<T> *)ring, *a_packed = (cx<T> *)packed;
     int *pdone = sync, *zdone = sync + nb;
     void *args[] = {(void *)&pl, (void *)&tabs.ct, (void *)&a_cub, (void *)&a_ring, (void *)&a_packed, (void *)&stride, (void *)&nb,
-                    (void *)&nslot, (void *)&lead, (void *)&hints, (void *)&pdone, (void *)&zdone};
+                    (void *)&nslot, (void *)&lead, (void *)&nz, (void *)&hints, (void *)&pdone, (void *)&zdone};
     if (cudaLaunchCooperativeKernel((const void *)k, dim3(grid), dim3(NW * 32), args, smem, st) != cudaSuccess) return FFTB_ECUDA;
     return launch_status();
 }
@@ -533,6 +535,7 @@ struct fftb_plan_s {
     bool bf;             // packed arrays are batch-fastest: [point][band], nb bands per point in a call with nb bands
     int ring_bands, lead_bands; // the fused kernels' ring of intermediate band slots and the producers' lead
     int l2_hints;        // fused kernels: evict_last on the ring, evict_first on the cuboid and packed streams
+    int z_ctas;          // fused kernels: > 0 = spatial split, this many CTAs walk the z tiles only (fftb_fused.cuh)
     long long ring_slot; // elements of a ring slot: ntiles tile images (tile-major layout, fftb_fused.cuh)
     int ring_ntiles;
     CUtensorMap ring_map; // the ring as a 5-dimensional tensor (inverse plane items load a row out of every tile)
@@ -607,7 +610,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
     *out = nullptr;
     const uint32_t tflags = tune ? tune->flags : 0u;
     if (tflags & ~(uint32_t)(FFTB_TUNE_GENERIC_Z | FFTB_TUNE_GENERIC_PLANE | FFTB_TUNE_FUSED | FFTB_TUNE_NO_L2_HINTS)) return FFTB_EINVAL;
-    if (tune && (tune->workspace_bytes < 0 || tune->ring_bands < 0 || tune->lead_bands < 0)) return FFTB_EINVAL;
+    if (tune && (tune->workspace_bytes < 0 || tune->ring_bands < 0 || tune->lead_bands < 0 || tune->z_ctas > 1024)) return FFTB_EINVAL;
     const bool dense = (desc->flags & FFTB_FLAG_DENSE) != 0;
     if (xm && (dense || xm->n < 1 || xm->n > (int64_t)1 << 24 || !xm->k1 || !xm->k2 || !xm->k3lo || !xm->len)) return FFTB_EINVAL;
     if (desc->flags & ~(uint32_t)(FFTB_FLAG_DENSE | FFTB_FLAG_BATCH_FASTEST)) return FFTB_EINVAL;
@@ -690,6 +693,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         p->fused = fused;
         p->bf = bf;
         p->l2_hints = (tflags & FFTB_TUNE_NO_L2_HINTS) ? 0 : 1;
+        p->z_ctas = tune ? (int)tune->z_ctas : 0;
         p->ry = plk.ry;
         const int n1 = desc->n[0], n2 = desc->n[1], n3 = desc->n[2];
         p->C = (int64_t)n1 * n2 * n3;
@@ -993,7 +997,7 @@ int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void
     p->launches = 0;
     if (p->fused) { // one cooperative launch: z tiles and planes of the whole batch, A in a ring of band slots (L2)
         prof_begin(p, K_FUSED_INV, st);
-        rc = p->ful.inv(p->dev, p->tabs, d_packed, A, p->ring_map, d_cuboid, p->ring_slot, nb, p->ring_bands, p->lead_bands, p->l2_hints,
+        rc = p->ful.inv(p->dev, p->tabs, d_packed, A, p->ring_map, d_cuboid, p->ring_slot, nb, p->ring_bands, p->lead_bands, p->z_ctas, p->l2_hints,
                         (int *)(p->d_mem + p->o_sync), st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
@@ -1025,7 +1029,7 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
     p->launches = 0;
     if (p->fused) {
         prof_begin(p, K_FUSED_FWD, st);
-        rc = p->ful.fwd(p->dev, p->tabs, d_cuboid, A, d_packed, p->ring_slot, nb, p->ring_bands, p->lead_bands, p->l2_hints,
+        rc = p->ful.fwd(p->dev, p->tabs, d_cuboid, A, d_packed, p->ring_slot, nb, p->ring_bands, p->lead_bands, p->z_ctas, p->l2_hints,
                         (int *)(p->d_mem + p->o_sync), st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }

@@ -19,6 +19,9 @@
 // key order, and a CTA publishes everything it has finished before it blocks: the unfinished item with the globally
 // smallest key can always run, so the schedule cannot deadlock.  With lead >= 2 bands the producers run far enough
 // ahead that a consumer practically never waits.
+// Variant (kernel argument nz > 0, fftb_plan_tuning.z_ctas): a SPATIAL split -- CTAs 0 .. nz-1 walk the z tiles only,
+// the others the planes only, each list still in band order, so the same argument holds; the z CTAs then run as far
+// ahead as the ring allows (nslot bands) and `lead` plays no part.
 //
 // Ring layout.  The TMA engine of an SM takes a bulk copy about every 19 cycles (measured), so a z tile that leaves as
 // one copy per z row (128 of them) would keep the CTA waiting for 2 500 cycles.  A ring slot is therefore TILE-MAJOR:
@@ -109,7 +112,7 @@ template <typename T, class F, int NW>
 __global__ void __launch_bounds__(NW * 32, 1)
 fused_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct, const cx<T> *__restrict__ packed,
             cx<T> *__restrict__ ring, const __grid_constant__ CUtensorMap ring_map, cx<T> *__restrict__ cub_out, long long slot_stride,
-            int nb, int nslot, int lead, int hints, int *__restrict__ zdone, int *__restrict__ pdone)
+            int nb, int nslot, int lead, int nz, int hints, int *__restrict__ zdone, int *__restrict__ pdone)
 {
     using C = cx<T>;
     using FU = Fused<T, F, NW>;
@@ -263,9 +266,12 @@ fused_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab c
     auto publish_z = [&](int band) { red_relaxed_gpu(zdone + band); };
 
     // this CTA's next tile (band zb, tile zj) and next plane (band pb, plane pz); both lists advance by GD items
+    // nz > 0 (spatial split): the first nz CTAs take the z tiles only, the others the planes only
     const int GD = (int)gridDim.x, bid = (int)blockIdx.x;
-    int zb = bid / ntiles, zj = bid % ntiles, pb = bid / n3, pz = bid % n3;
-    const int dzb = GD / ntiles, dzj = GD % ntiles, dpb = GD / n3, dpz = GD % n3;
+    const bool zrole = nz > 0 && bid < nz, prole = nz > 0 && bid >= nz;
+    const int zs = nz > 0 ? nz : GD, pi = prole ? bid - nz : bid, ps = nz > 0 ? GD - nz : GD;
+    int zb = prole ? nb : bid / ntiles, zj = bid % ntiles, pb = zrole ? nb : pi / n3, pz = pi % n3;
+    const int dzb = zs / ntiles, dzj = zs % ntiles, dpb = ps / n3, dpz = ps % n3;
     bool run_z = false;
     auto peek = [&]() -> int { // 0 none, 1 z tile, 2 plane
         const bool hz = zb < nb, hp = pb < nb;
@@ -442,7 +448,7 @@ template <typename T, class F, int NW>
 __global__ void __launch_bounds__(NW * 32, 1)
 fused_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct, const cx<T> *__restrict__ cub_in,
             cx<T> *__restrict__ ring, cx<T> *__restrict__ packed, long long slot_stride, int nb, int nslot, int lead,
-            int hints, int *__restrict__ pdone, int *__restrict__ zdone)
+            int nz, int hints, int *__restrict__ pdone, int *__restrict__ zdone)
 {
     using C = cx<T>;
     using FU = Fused<T, F, NW>;
@@ -598,9 +604,12 @@ fused_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab c
     };
 
     // this CTA's next tile (band zb, tile zj) and next plane (band pb, plane pz); both lists advance by GD items
+    // nz > 0 (spatial split): the first nz CTAs take the z tiles only, the others the planes only
     const int GD = (int)gridDim.x, bid = (int)blockIdx.x;
-    int zb = bid / ntiles, zj = bid % ntiles, pb = bid / n3, pz = bid % n3;
-    const int dzb = GD / ntiles, dzj = GD % ntiles, dpb = GD / n3, dpz = GD % n3;
+    const bool zrole = nz > 0 && bid < nz, prole = nz > 0 && bid >= nz;
+    const int zs = nz > 0 ? nz : GD, pi = prole ? bid - nz : bid, ps = nz > 0 ? GD - nz : GD;
+    int zb = prole ? nb : bid / ntiles, zj = bid % ntiles, pb = zrole ? nb : pi / n3, pz = pi % n3;
+    const int dzb = zs / ntiles, dzj = zs % ntiles, dpb = ps / n3, dpz = ps % n3;
     auto peek = [&]() -> int { // 0 none, 1 z tile, 2 plane
         const bool hz = zb < nb, hp = pb < nb;
         if (!hz) return hp ? 2 : 0;

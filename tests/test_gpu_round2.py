@@ -64,13 +64,17 @@ def _intermediate(p, bands):
 # ---------------------------------------------------------------------------------------------------------------
 @pytest.mark.timeout(300)
 @pytest.mark.parametrize("dtype", ["c128", "c64"])
-@pytest.mark.parametrize("nb,ring,lead", [(1, 0, 0), (3, 0, 0), (7, 2, 1), (13, 3, 2), (40, 0, 0), (9, 1, 0)])
-def test_fused_launch_equals_separate_launches(fb, oracle, dtype, nb, ring, lead):
+@pytest.mark.parametrize("nb,ring,lead,zc", [(1, 0, 0, 0), (3, 0, 0, 0), (7, 2, 1, 0), (13, 3, 2, 0), (40, 0, 0, 0), (9, 1, 0, 0),
+                                             (1, 0, 0, 20), (13, 3, 2, 24), (40, 0, 0, 16), (9, 1, 0, 40), (6, 2, 1, 147), (6, 2, 1, 1000)])
+def test_fused_launch_equals_separate_launches(fb, oracle, dtype, nb, ring, lead, zc):
     """fftb_inverse / fftb_forward as ONE cooperative launch (ring of band slots, per-band counters) do the same
     arithmetic in the same order as the separate z-pass and plane launches: the outputs are bit-identical, for batches
-    smaller than, equal to and several times the ring, and for the smallest legal rings (slot reuse on every band)."""
+    smaller than, equal to and several times the ring, and for the smallest legal rings (slot reuse on every band).
+    zc > 0: the spatial split (zc CTAs walk the z tiles only, the others the planes only; one plane CTA left at 147, and
+    a value beyond the grid falls back to the merged walk)."""
     w = _w((128, 128, 128), (32, 32, 32), dtype=dtype, batch=nb, dist="normal_decay", number=3)
-    pf = fb.Plan(w.n, w.cutoff, batch=nb, dtype=dtype, tuning={"flags": fb.FFTB_TUNE_FUSED, "ring_bands": ring, "lead_bands": lead}).bind()
+    pf = fb.Plan(w.n, w.cutoff, batch=nb, dtype=dtype,
+                 tuning={"flags": fb.FFTB_TUNE_FUSED, "ring_bands": ring, "lead_bands": lead, "z_ctas": zc}).bind()
     pu = fb.Plan(w.n, w.cutoff, batch=nb, dtype=dtype).bind()
     assert pf.info["ring_bands"] >= 1 and pu.info["ring_bands"] == 0
     if ring:
@@ -226,6 +230,9 @@ def test_tuning_is_validated(fb):
     assert e.value.code == fb.FFTB_EINVAL
     with pytest.raises(fb.FftbError) as e:
         fb.Plan((64, 64, 64), (16, 16, 16), tuning={"ring_bands": -1})
+    assert e.value.code == fb.FFTB_EINVAL
+    with pytest.raises(fb.FftbError) as e:
+        fb.Plan((64, 64, 64), (16, 16, 16), tuning={"z_ctas": 1025})
     assert e.value.code == fb.FFTB_EINVAL
 
 
