@@ -368,6 +368,16 @@ def run_ours(args, w):
                          "pruned_speedup": ms_dense / ms_step, "launches_per_step": l_dense // min(K, 5),
                          "rel_l2_cuboid_dense_vs_pruned": rel_psi, "rel_l2_packed_dense_vs_pruned": rel_c,
                          "what": "fftb_dense_embed + dense-plan fftb_inverse + fftb_forward + fftb_dense_extract on the same data"}
+            # per-kernel times of the dense plan (second, profiled pass): the plane kinds hold a y pass and an x pass each
+            pd.profile(True)
+            for _ in range(3):
+                step_dense()
+            torch.cuda.synchronize()
+            dprof = pd.profile_read()
+            pd.profile(False)
+            dense_arm["kernel_ms_per_step"] = {kk: dprof[kk][0] / 3 for kk in dprof if dprof[kk][1]}
+            cube = float(np.prod(w.n)) * elem * nb
+            dense_arm["cube_passes_gbs"] = 12 * cube / 1e9 / (sum(dense_arm["kernel_ms_per_step"].values()) * 1e-3)  # 6 passes, read + write each
             pd.destroy()
             del d_dense, d_back, d_psi_d, d_out_d
         except Exception as exc:  # never fatal for the bench line

@@ -139,9 +139,11 @@ typedef struct {
  *     (128, 64);
  *   - pruned plans with a_d <= N_d/4 on every axis (the paper's "cube of width twice the diameter of the sphere",
  *     PAPER.md:110): half-band kernels, persistent TMA kernels where they exist (N1 == N2 in {64, 96, 128, 256});
- *   - pruned plans with N_d/4 < a_d < N_d/2 on some axis: full-band axis patterns, FFTB_C128 only, N1 == N2 and N3 in
+ *   - pruned plans with N_d/4 < a_d < N_d/2 on some axis: full-band axis patterns (generic kernels), N1 == N2 and N3 in
  *     {32, 64, 128, 256};
- *   - dense plans (FFTB_FLAG_DENSE): FFTB_C128 only, N1 == N2 and N3 in {32, 64, 128, 256}. */
+ *   - dense plans (FFTB_FLAG_DENSE): N1 == N2 and N3 in {32, 64, 128, 256}; the cubes 64^3, 128^3 and 256^3 run three
+ *     line passes per direction on the transform core of the persistent kernels (fftb_dense.cuh), the others the
+ *     generic kernels. */
 int fftb_plan_create(fftb_plan *out, const fftb_plan_desc *desc);
 
 /* The same with explicit tuning (tuning == NULL: fftb_plan_create).  FFTB_EINVAL for unknown flags or negative
@@ -155,7 +157,7 @@ int fftb_plan_create_tuned(fftb_plan *out, const fftb_plan_desc *desc, const fft
  * allowed.  The arrays (host, n_sticks entries each) are copied.
  *   FFTB_EINVAL        a point outside [-N_d/2, N_d/2), len < 1, sticks not strictly ascending in (k1, k2)
  *   FFTB_EUNSUPPORTED  outside the predefined patterns of fftb_plan_create (a frequency beyond |k_d| <= N_d/4 makes
- *                      it a full-band plan: FFTB_C128 only), a hole in the occupied k1 range, or a k1 whose k2
+ *                      it a full-band plan), a hole in the occupied k1 range, or a k1 whose k2
  *                      values are not one contiguous run. */
 int fftb_plan_create_explicit(fftb_plan *out, const fftb_plan_desc *desc, int64_t n_sticks, const int32_t *k1,
                               const int32_t *k2, const int32_t *k3lo, const int32_t *len);

@@ -12,6 +12,7 @@
 #include "fftb_plane_r4.cuh"
 #include "fftb_zpass_pf.cuh"
 #include "fftb_fused.cuh"
+#include "fftb_dense.cuh"
 #include "fftb_probe.cuh"
 #include "fftb_slab.cuh"
 
@@ -144,6 +145,7 @@ struct PlaneLaunch {
     int ry;
     int (*run[3])(const DevPlan &, const PlanTabs &, const void *Ain, void *Aout, const void *cin, void *cout, const void *v,
                   long long sin, long long sout, int nb, cudaStream_t);
+    int nkern[3] = {1, 1, 1}; // kernels one run launches (the dense arm's plane stage is a y pass and an x pass)
 };
 // one cooperative launch per direction (fftb_fused.cuh): the intermediate lives in a ring of `nslot` band slots
 struct FusedGeom { int ts, tile, rp; }; // sticks per z tile, elements of a tile's image, pitch of a row pair (ZFast)
@@ -435,6 +437,96 @@ bool find_fused(int dtype, const int32_t n[3], bool dense, FusedLaunch *out)
     return false;
 }
 
+// ------------------------------------------------------------------------------------------------
+// dense arm (fftb_dense.cuh): three line passes per direction on the warp-synchronous core, cubic grids
+// ------------------------------------------------------------------------------------------------
+constexpr int DENSE_NW = 4;
+template <typename T, class F, int MODE, bool PAIR>
+int launch_dense_axis(const void *in, void *out, const DenseGeom &ge, const void *tw, const void *v, double scale, int nb, cudaStream_t st)
+{
+    auto k = dense_axis_k<T, F, DENSE_NW, MODE, PAIR>;
+    const size_t smem = sizeof(cx<T>) * (size_t)DENSE_NW * F::EXW;
+    if (int rc = kernel_ready(k, DENSE_NW * 32, smem, nullptr)) return rc;
+    constexpr int per_cta = DENSE_NW * F::G;
+    dim3 grid((ge.lines + per_cta - 1) / per_cta, nb);
+    k<<<grid, DENSE_NW * 32, smem, st>>>((const cx<T> *)in, (cx<T> *)out, ge, (const cx<T> *)tw, (const T *)v, (T)scale);
+    return launch_status();
+}
+// the passes as strides; A[z][k1][k2] with row pitch pl.pitch = N1 N2 (the dense stick map: stick s = k1 N2 + k2)
+inline DenseGeom dense_geom_z(const DevPlan &pl, long long a_stride, bool inverse)
+{
+    // packed [stick][k3] <-> A[z][stick]
+    DenseGeom p2a = {0, pl.n3, 1, 0, 1, pl.pitch, pl.S, a_stride, pl.nsticks, pl.nsticks};
+    DenseGeom a2p = {0, 1, pl.pitch, 0, pl.n3, 1, a_stride, pl.S, pl.nsticks, pl.nsticks};
+    return inverse ? p2a : a2p;
+}
+inline DenseGeom dense_geom_y(const DevPlan &pl, long long a_stride)
+{
+    // in place on A: line (z, k1) is contiguous in k2 / y
+    return DenseGeom{pl.pitch, pl.n2, 1, pl.pitch, pl.n2, 1, a_stride, a_stride, pl.n1, pl.n3 * pl.n1};
+}
+inline DenseGeom dense_geom_x(const DevPlan &pl, long long a_in, long long a_out, int side) // 0: A -> cuboid, 1: cuboid -> A, 2: A -> A
+{
+    const long long C = (long long)pl.n1 * pl.n2 * pl.n3, row = pl.n1, plane = (long long)pl.n1 * pl.n2;
+    DenseGeom g;
+    g.nv = pl.n2;
+    g.lines = pl.n3 * pl.n2;
+    if (side == 1) { g.in_u = plane; g.in_v = row; g.in_i = 1; g.in_band = C; }
+    else { g.in_u = pl.pitch; g.in_v = 1; g.in_i = pl.n2; g.in_band = a_in; }
+    if (side == 0) { g.out_u = plane; g.out_v = row; g.out_i = 1; g.out_band = C; }
+    else { g.out_u = pl.pitch; g.out_v = 1; g.out_i = pl.n2; g.out_band = a_out; }
+    return g;
+}
+template <typename T, class F> int launch_dense_zinv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, long long pk_pitch, cudaStream_t st)
+{
+    if (pk_pitch) return FFTB_EUNSUPPORTED;
+    return launch_dense_axis<T, F, DENSE_INV, false>(packed, A, dense_geom_z(pl, stride, true), pl.tw3, nullptr, 1.0, nb, st);
+}
+template <typename T, class F> int launch_dense_zfwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, long long pk_pitch, cudaStream_t st)
+{
+    if (pk_pitch) return FFTB_EUNSUPPORTED;
+    return launch_dense_axis<T, F, DENSE_FWD, false>(A, packed, dense_geom_z(pl, stride, false), pl.tw3, nullptr, pl.scale, nb, st);
+}
+template <typename T, class F>
+int launch_dense_plane_inv(const DevPlan &pl, const PlanTabs &, const void *Ain, void *, const void *, void *cout, const void *, long long sin, long long,
+                           int nb, cudaStream_t st)
+{
+    void *A = const_cast<void *>(Ain); // the workspace: the y pass works on it in place
+    if (int rc = launch_dense_axis<T, F, DENSE_INV, true>(A, A, dense_geom_y(pl, sin), pl.tw2, nullptr, 1.0, nb, st)) return rc;
+    return launch_dense_axis<T, F, DENSE_INV, true>(A, cout, dense_geom_x(pl, sin, 0, 0), pl.tw1, nullptr, 1.0, nb, st);
+}
+template <typename T, class F>
+int launch_dense_plane_fwd(const DevPlan &pl, const PlanTabs &, const void *, void *Aout, const void *cin, void *, const void *, long long, long long sout,
+                           int nb, cudaStream_t st)
+{
+    if (int rc = launch_dense_axis<T, F, DENSE_FWD, true>(cin, Aout, dense_geom_x(pl, 0, sout, 1), pl.tw1, nullptr, 1.0, nb, st)) return rc;
+    return launch_dense_axis<T, F, DENSE_FWD, true>(Aout, Aout, dense_geom_y(pl, sout), pl.tw2, nullptr, 1.0, nb, st);
+}
+template <typename T, class F>
+int launch_dense_plane_vloc(const DevPlan &pl, const PlanTabs &, const void *Ain, void *Aout, const void *, void *, const void *v, long long sin,
+                            long long sout, int nb, cudaStream_t st)
+{
+    void *A = const_cast<void *>(Ain);
+    if (int rc = launch_dense_axis<T, F, DENSE_INV, true>(A, A, dense_geom_y(pl, sin), pl.tw2, nullptr, 1.0, nb, st)) return rc;
+    if (int rc = launch_dense_axis<T, F, DENSE_VLOC, true>(A, Aout, dense_geom_x(pl, sin, sout, 2), pl.tw1, v, 1.0, nb, st)) return rc;
+    return launch_dense_axis<T, F, DENSE_FWD, true>(Aout, Aout, dense_geom_y(pl, sout), pl.tw2, nullptr, 1.0, nb, st);
+}
+template <typename T, int N, int P1, int P2> void make_dense_fast(ZLaunch *zl, PlaneLaunch *plk)
+{
+    using F = FastCfg<T, N, P1, P2>;
+    *zl = ZLaunch{&launch_dense_zinv<T, F>, &launch_dense_zfwd<T, F>, false};
+    *plk = PlaneLaunch{1, {&launch_dense_plane_inv<T, F>, &launch_dense_plane_fwd<T, F>, &launch_dense_plane_vloc<T, F>}, {2, 2, 3}};
+}
+bool find_dense_fast(int dtype, const int32_t n[3], ZLaunch *zl, PlaneLaunch *plk)
+{
+    if (n[0] != n[1] || n[0] != n[2]) return false;
+#define DCASE(N, P1, P2) \
+    if (n[0] == N) { if (dtype == FFTB_C128) make_dense_fast<double, N, P1, P2>(zl, plk); else make_dense_fast<float, N, P1, P2>(zl, plk); return true; }
+    DCASE(64, 8, 4) DCASE(128, 8, 8) DCASE(256, 16, 8)
+#undef DCASE
+    return false;
+}
+
 template <typename T, int N, bool DENSE> ZLaunch make_z()
 {
     using AZ = typename ZX<N, DENSE>::type;
@@ -479,6 +571,7 @@ bool find_z(int dtype, int n, bool dense, ZLaunch *out)
     ZCASE(float, FFTB_C64, 128, false) ZCASE(float, FFTB_C64, 192, false) ZCASE(float, FFTB_C64, 256, false)
     ZCASE(double, FFTB_C128, 32, true) ZCASE(double, FFTB_C128, 64, true) ZCASE(double, FFTB_C128, 128, true)
     ZCASE(double, FFTB_C128, 256, true)
+    ZCASE(float, FFTB_C64, 32, true) ZCASE(float, FFTB_C64, 64, true) ZCASE(float, FFTB_C64, 128, true) ZCASE(float, FFTB_C64, 256, true)
 #undef ZCASE
     return false;
 }
@@ -492,6 +585,7 @@ bool find_plane(int dtype, int n, bool dense, PlaneLaunch *out)
     PCASE(float, FFTB_C64, 128, false) PCASE(float, FFTB_C64, 192, false) PCASE(float, FFTB_C64, 256, false)
     PCASE(double, FFTB_C128, 32, true) PCASE(double, FFTB_C128, 64, true) PCASE(double, FFTB_C128, 128, true)
     PCASE(double, FFTB_C128, 256, true)
+    PCASE(float, FFTB_C64, 32, true) PCASE(float, FFTB_C64, 64, true) PCASE(float, FFTB_C64, 128, true) PCASE(float, FFTB_C64, 256, true)
 #undef PCASE
     return false;
 }
@@ -651,9 +745,14 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
     ZLaunch zl;
     PlaneLaunch plk;
     bool fast_plane = false;
-    if (!find_z(desc->dtype, desc->n[2], full_band, &zl)) return FFTB_EUNSUPPORTED;
-    if (rect ? (full_band || !find_plane_xy(desc->dtype, desc->n[0], desc->n[1], &plk)) : !find_plane(desc->dtype, desc->n[0], full_band, &plk))
-        return FFTB_EUNSUPPORTED;
+    // dense cubes of 64, 128, 256 points: the line-pass kernel of fftb_dense.cuh (whole-batch launches)
+    const bool dense_fast = dense && !(tflags & (FFTB_TUNE_GENERIC_Z | FFTB_TUNE_GENERIC_PLANE)) && find_dense_fast(desc->dtype, desc->n, &zl, &plk);
+    if (dense_fast) fast_plane = true;
+    else {
+        if (!find_z(desc->dtype, desc->n[2], full_band, &zl)) return FFTB_EUNSUPPORTED;
+        if (rect ? (full_band || !find_plane_xy(desc->dtype, desc->n[0], desc->n[1], &plk)) : !find_plane(desc->dtype, desc->n[0], full_band, &plk))
+            return FFTB_EUNSUPPORTED;
+    }
     const bool dense_cfg = full_band || rect; // no persistent kernels for these
     bool fast_z = false;
     {
@@ -1015,7 +1114,7 @@ int fftb_inverse(fftb_plan p, const void *d_packed, void *d_cuboid, int nb, void
         if (!rc) rc = p->plk.run[MODE_INV](p->dev, p->tabs, A, nullptr, nullptr, cb, nullptr, p->a_inv_stride, 0, nc, st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
-        p->launches += 2;
+        p->launches += 1 + p->plk.nkern[MODE_INV];
     }
     return FFTB_OK;
 }
@@ -1047,7 +1146,7 @@ int fftb_forward(fftb_plan p, const void *d_cuboid, void *d_packed, int nb, void
         if (!rc) rc = p->zl.fwd(p->dev, A, pk, p->a_fwd_stride, nc, p->bf ? nb : 0, st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
-        p->launches += 2;
+        p->launches += 1 + p->plk.nkern[MODE_FWD];
     }
     return FFTB_OK;
 }
@@ -1076,7 +1175,7 @@ int fftb_apply_vloc(fftb_plan p, const void *d_in, void *d_out, const void *d_vl
         if (!rc) rc = p->zl.fwd(p->dev, Af, po, p->a_fwd_stride, nc, p->bf ? nb : 0, st);
         prof_end(p, st);
         if (rc) { p->sticky = rc; return rc; }
-        p->launches += 3;
+        p->launches += 2 + p->plk.nkern[MODE_VLOC];
     }
     return FFTB_OK;
 }

@@ -215,12 +215,13 @@ def test_host_buffer_calls(fb, oracle):
         p2.inverse_host(h_c, d_psi)
 
 
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
 @pytest.mark.parametrize("n,a", [((32, 32, 32), (8, 8, 8)), ((64, 64, 64), (16, 16, 16)), ((128, 128, 128), (32, 32, 32)),
                                  ((256, 256, 256), (64, 64, 64))])
-def test_pruned_vs_dense(fb, oracle, n, a):
+def test_pruned_vs_dense(fb, oracle, n, a, dtype):
     """BASELINE config 5: the same data zero-padded to the full cuboid and transformed unpruned by
     the product's kernels gives the same result as the pruned path."""
-    w = _small(n, a, batch=1 if n[0] >= 128 else 2)
+    w = _small(n, a, dtype=dtype, batch=1 if n[0] >= 128 else 2)
     pp = _plan(fb, w, w.batch)
     pd = _plan(fb, w, w.batch, dense=True)
     k = pp.points()
@@ -231,7 +232,7 @@ def test_pruned_vs_dense(fb, oracle, n, a):
     psi_d = pd.inverse(d_dense_in)
     torch.cuda.synchronize()
     # embedding is a pure scatter: bit-exact against the oracle-side definition
-    cube = np.zeros((w.batch,) + tuple(n), np.complex128)  # [b][k1+N1/2][k2+N2/2][k3+N3/2]
+    cube = np.zeros((w.batch,) + tuple(n), w.complex_dtype)  # [b][k1+N1/2][k2+N2/2][k3+N3/2]
     cube[:, k[0] + n[0] // 2, k[1] + n[1] // 2, k[2] + n[2] // 2] = c
     assert np.array_equal(d_dense_in.cpu().numpy().reshape(cube.shape), cube)
     assert _rel(psi_d.cpu().numpy(), psi_p.cpu().numpy()) <= w.tol

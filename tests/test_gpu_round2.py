@@ -416,7 +416,8 @@ def test_batch_fastest_band_chunks_and_host_calls(fb, oracle):
 WIDER = [((32, 64, 32), (8, 16, 8), "c128"), ((64, 32, 96), (16, 8, 24), "c64"), ((64, 128, 96), (16, 32, 24), "c128"),
          ((128, 64, 256), (32, 16, 64), "c64"), ((128, 64, 64), (20, 7, 16), "c128"),
          ((32, 32, 32), (12, 8, 8), "c128"), ((64, 64, 64), (24, 31, 20), "c128"), ((128, 128, 64), (40, 50, 31), "c128"),
-         ((64, 64, 128), (16, 16, 60), "c128")]
+         ((64, 64, 128), (16, 16, 60), "c128"), ((32, 32, 32), (12, 8, 8), "c64"), ((64, 64, 256), (24, 31, 100), "c64"),
+         ((128, 128, 64), (40, 50, 31), "c64")]
 
 
 @pytest.mark.parametrize("n,a,dtype", WIDER, ids=[f"{n[0]}x{n[1]}x{n[2]}-a{a[0]}.{a[1]}.{a[2]}-{d}" for n, a, d in WIDER])
@@ -443,4 +444,60 @@ def test_rectangular_grids_and_wide_cutoffs_vs_oracle(fb, oracle, n, a, dtype):
     assert _rel(d_f.cpu().numpy(), oracle.forward(n, k, g, 1.0 / C)) <= w.tol
     assert _rel(d_o.cpu().numpy(), oracle.apply_vloc(n, k, c, v, 1.0 / C)) <= w.tol
     assert _rel(rt.cpu().numpy(), c) <= w.tol
+    p.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# dense arm on the line-pass kernel (fftb_dense.cuh), both precisions
+# ---------------------------------------------------------------------------------------------------------------
+DENSE = [((64, 64, 64), "c128", {}), ((64, 64, 64), "c64", {}), ((128, 128, 128), "c128", {}), ((128, 128, 128), "c64", {}),
+         ((256, 256, 256), "c128", {}), ((256, 256, 256), "c64", {}),
+         ((32, 32, 32), "c64", {}), ((32, 32, 64), "c64", {}), ((64, 64, 64), "c64", {"flags": 3}), ((64, 64, 64), "c128", {"flags": 3})]
+
+
+@pytest.mark.timeout(600)
+@pytest.mark.parametrize("n,dtype,tuning", DENSE, ids=[f"{n[0]}x{n[2]}-{d}-{'generic' if t else 'default'}" for n, d, t in DENSE])
+def test_dense_arm_vs_oracle(fb, oracle, n, dtype, tuning):
+    """FFTB_FLAG_DENSE plans (every point of the cube is a coefficient) against the oracle, whose
+    transform is dense anyway: inverse of random coefficients, forward of a generic cuboid, the fused local-potential
+    apply, and the round trip.  Cubes of 64, 128, 256 points run the line-pass kernel (three passes per direction, the
+    first radix-2 split with data in both halves), the others and `flags = generic` the generic kernels.  256^3: the
+    oracle's defining sums at sampled outputs (its full transform of 16.7 M points per band takes too long here)."""
+    big = n[0] >= 256
+    nb = 1 if big else 2
+    w = _w(n, (0, 0, 0), dtype=dtype, batch=nb, number=5)
+    p = fb.Plan(n, batch=nb, dtype=dtype, dense=True, tuning=tuning or None).bind()
+    assert p.S == n[0] * n[1] * n[2] and p.info["y_residues"] == (1 if not tuning and n[0] == n[2] and n[0] >= 64 else p.info["y_residues"])
+    k = p.points()
+    c = wl.coefficients(w, *k)
+    g = wl.cuboid(w, batch=nb)
+    v = wl.potential(w)
+    C = float(np.prod(n))
+    d_c, d_g, d_v = torch.from_numpy(c).cuda(), torch.from_numpy(g).cuda(), torch.from_numpy(v).cuda()
+    d_psi = p.inverse(d_c)
+    assert p.last_launches() == (3 if not tuning and n[0] == n[2] and n[0] >= 64 else p.last_launches())
+    d_f = p.forward(d_g)
+    d_o = p.apply_vloc(d_c, d_v)
+    d_rt = p.forward(d_psi)
+    torch.cuda.synchronize()
+    assert torch.equal(d_c.cpu(), torch.from_numpy(c)) and torch.equal(d_g.cpu(), torch.from_numpy(g))
+    assert _rel(d_rt.cpu().numpy(), c) <= w.tol
+    if not big:
+        assert _rel(d_psi.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol
+        assert _rel(d_f.cpu().numpy(), oracle.forward(n, k, g, 1.0 / C)) <= w.tol
+        assert _rel(d_o.cpu().numpy(), oracle.apply_vloc(n, k, c, v, 1.0 / C)) <= w.tol
+    else:
+        rng = np.random.default_rng(7)
+        idx = np.concatenate([[0, 1, int(C) - 1, n[0] * n[1], n[0]], rng.integers(0, int(C), size=11)]).astype(np.int64)
+        want = oracle.brute_inverse_at(n, k, c, idx)
+        got = d_psi.cpu().numpy().reshape(nb, -1)[:, idx]
+        scale = np.linalg.norm(d_psi.cpu().numpy().ravel()) / np.sqrt(C)   # rms magnitude of an output
+        assert np.max(np.abs(got - want)) <= w.tol * scale * np.sqrt(np.log2(C))
+        wantf = oracle.brute_forward_at(n, k, g, idx, 1.0 / C)
+        gotf = d_f.cpu().numpy()[:, idx]
+        scalef = np.linalg.norm(d_f.cpu().numpy().ravel()) / np.sqrt(C)
+        assert np.max(np.abs(gotf - wantf)) <= w.tol * scalef * np.sqrt(np.log2(C))
+        # the local-potential apply against its own two halves (each checked above)
+        chk = p.forward((d_psi * d_v.unsqueeze(0)).contiguous())
+        assert _rel(d_o.cpu().numpy(), chk.cpu().numpy()) <= w.tol
     p.destroy()

@@ -93,8 +93,10 @@ def test_error_paths():
     assert _create_rc((40, 40, 40), (8, 8, 8)) == fb.FFTB_EUNSUPPORTED
     assert _create_rc((32, 64, 32), (8, 8, 8)) == fb.FFTB_OK              # N1 != N2: one of the predefined pairs
     assert _create_rc((96, 64, 32), (8, 8, 8)) == fb.FFTB_EUNSUPPORTED    # ... this one is not
-    assert _create_rc((32, 32, 32), (12, 8, 8)) == fb.FFTB_OK             # a > N/4: full-band axis patterns (complex128)
-    assert _create_rc((32, 32, 32), (12, 8, 8), dtype=fb.FFTB_C64) == fb.FFTB_EUNSUPPORTED
+    assert _create_rc((32, 32, 32), (12, 8, 8)) == fb.FFTB_OK             # a > N/4: full-band axis patterns
+    assert _create_rc((32, 32, 32), (12, 8, 8), dtype=fb.FFTB_C64) == fb.FFTB_OK
+    assert _create_rc((64, 64, 64), (0, 0, 0), dtype=fb.FFTB_C64, flags=1) == fb.FFTB_OK    # dense, either precision
+    assert _create_rc((32, 32, 64), (0, 0, 0), dtype=fb.FFTB_C64, flags=1) == fb.FFTB_OK
     assert _create_rc((96, 96, 96), (30, 8, 8)) == fb.FFTB_EUNSUPPORTED   # no full-band pattern of length 96
     assert L.fftb_plan_create(None, None) == fb.FFTB_EINVAL
     assert L.fftb_plan_destroy(None) == fb.FFTB_EINVAL
@@ -164,10 +166,8 @@ def test_explicit_stick_map_round_trip_and_errors():
         fb.Plan(n, stick_map=(k1, k2, far, ln))
     assert e.value.code == fb.FFTB_EINVAL
     wide = ln.copy(); wide[0] = 17 - lo[0] + 1
-    fb.Plan(n, stick_map=(k1, k2, lo, wide)).destroy()   # beyond the half band |k| <= N/4: full-band patterns, complex128
-    with pytest.raises(fb.FftbError) as e:
-        fb.Plan(n, stick_map=(k1, k2, lo, wide), dtype="c64")
-    assert e.value.code == fb.FFTB_EUNSUPPORTED
+    fb.Plan(n, stick_map=(k1, k2, lo, wide)).destroy()   # beyond the half band |k| <= N/4: full-band patterns, either precision
+    fb.Plan(n, stick_map=(k1, k2, lo, wide), dtype="c64").destroy()
     hole = np.ones(k1.size, bool); hole[np.flatnonzero(k1 == k1[k1.size // 2])[1]] = False
     with pytest.raises(fb.FftbError) as e:      # a k2 run with a hole
         fb.Plan(n, stick_map=(k1[hole], k2[hole], lo[hole], ln[hole]))
