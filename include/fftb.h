@@ -154,13 +154,19 @@ int fftb_plan_create_tuned(fftb_plan *out, const fftb_plan_desc *desc, const fft
  * offset array (PAPER.md:183-185: "x and y dense, only z compressed", :201 `offsets` argument), e.g. the
  * g-vector list of a plane-wave code whose sphere is shifted by a k-point.  Stick s is the k3 run
  * k3lo[s] .. k3lo[s]+len[s]-1 of column (k1[s], k2[s]); `desc->cutoff` is ignored, FFTB_FLAG_DENSE is not
- * allowed.  The arrays (host, n_sticks entries each) are copied.
+ * allowed.  The arrays (host, n_sticks entries each) are copied.  The map may have HOLES -- k1 values without a stick inside
+ * the occupied k1 range, k2 values without a stick inside a column's k2 run (the g-vector list of a cell whose sphere is cut by
+ * a second criterion): the plan fills them with zero-length sticks of its own, which the caller never sees (get_map and
+ * info.n_sticks report the map as given; the intermediate's pitch counts them).
  *   FFTB_EINVAL        a point outside [-N_d/2, N_d/2), len < 1, sticks not strictly ascending in (k1, k2)
  *   FFTB_EUNSUPPORTED  outside the predefined patterns of fftb_plan_create (a frequency beyond |k_d| <= N_d/4 makes
- *                      it a full-band plan), a hole in the occupied k1 range, or a k1 whose k2
- *                      values are not one contiguous run. */
+ *                      it a full-band plan). */
 int fftb_plan_create_explicit(fftb_plan *out, const fftb_plan_desc *desc, int64_t n_sticks, const int32_t *k1,
                               const int32_t *k2, const int32_t *k3lo, const int32_t *len);
+
+/* The same with explicit tuning (tuning == NULL: fftb_plan_create_explicit). */
+int fftb_plan_create_explicit_tuned(fftb_plan *out, const fftb_plan_desc *desc, int64_t n_sticks, const int32_t *k1,
+                                    const int32_t *k2, const int32_t *k3lo, const int32_t *len, const fftb_plan_tuning *tuning);
 
 int fftb_plan_info_get(fftb_plan p, fftb_plan_info *info);
 

@@ -24,7 +24,7 @@ FFTB_STATIC_SCRATCH_BYTES = 16 * 1024 * 1024  # the library-held device array ff
 
 # every symbol include/fftb.h declares
 SYMBOLS = [
-    "fftb_plan_create", "fftb_plan_create_tuned", "fftb_plan_create_explicit", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
+    "fftb_plan_create", "fftb_plan_create_tuned", "fftb_plan_create_explicit", "fftb_plan_create_explicit_tuned", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
     "fftb_inverse", "fftb_inverse_static", "fftb_forward", "fftb_apply_vloc",
     "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
     "fftb_dense_embed", "fftb_dense_extract", "fftb_packed_transpose",
@@ -72,6 +72,8 @@ def lib():
         L.fftb_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc)]
         L.fftb_plan_create_tuned.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc), ctypes.POINTER(PlanTuning)]
         L.fftb_plan_create_explicit.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc), ctypes.c_int64, vp, vp, vp, vp]
+        L.fftb_plan_create_explicit_tuned.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDesc), ctypes.c_int64, vp, vp, vp, vp,
+                                                      ctypes.POINTER(PlanTuning)]
         L.fftb_plan_info_get.argtypes = [vp, ctypes.POINTER(PlanInfo)]
         L.fftb_plan_get_map.argtypes = [vp, vp, vp, vp, vp, vp]
         L.fftb_plan_bind.argtypes = [vp, vp, ctypes.c_size_t, vp]
@@ -141,21 +143,28 @@ class Plan:
         d.flags = (FFTB_FLAG_DENSE if dense else 0) | (FFTB_FLAG_BATCH_FASTEST if batch_fastest else 0)
         self.batch_fastest = bool(batch_fastest)
         self._h = ctypes.c_void_p()
-        if stick_map is None and tuning is not None:
+        tu = None
+        if tuning is not None:
             tu = PlanTuning()
             tu.workspace_bytes = int(tuning.get("workspace_bytes", 0))
             tu.ring_bands = int(tuning.get("ring_bands", 0))
             tu.lead_bands = int(tuning.get("lead_bands", 0))
             tu.flags = int(tuning.get("flags", 0))
             tu.z_ctas = int(tuning.get("z_ctas", 0))
+        if stick_map is None and tu is not None:
             _check(lib().fftb_plan_create_tuned(ctypes.byref(self._h), ctypes.byref(d), ctypes.byref(tu)), "fftb_plan_create_tuned")
         elif stick_map is None:
             _check(lib().fftb_plan_create(ctypes.byref(self._h), ctypes.byref(d)), "fftb_plan_create")
         else:
             m = [np.ascontiguousarray(x, dtype=np.int32) for x in stick_map]
             assert len(m) == 4 and all(x.shape == m[0].shape and x.ndim == 1 for x in m)
-            _check(lib().fftb_plan_create_explicit(ctypes.byref(self._h), ctypes.byref(d), ctypes.c_int64(m[0].size),
-                                                   *[x.ctypes.data_as(ctypes.c_void_p) for x in m]), "fftb_plan_create_explicit")
+            ptrs = [x.ctypes.data_as(ctypes.c_void_p) for x in m]
+            if tu is None:
+                _check(lib().fftb_plan_create_explicit(ctypes.byref(self._h), ctypes.byref(d), ctypes.c_int64(m[0].size), *ptrs),
+                       "fftb_plan_create_explicit")
+            else:
+                _check(lib().fftb_plan_create_explicit_tuned(ctypes.byref(self._h), ctypes.byref(d), ctypes.c_int64(m[0].size), *ptrs,
+                                                             ctypes.byref(tu)), "fftb_plan_create_explicit_tuned")
         self.n = tuple(int(x) for x in n)
         self.batch = int(batch)
         self.dtype = dtype

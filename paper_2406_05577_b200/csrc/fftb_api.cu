@@ -616,6 +616,7 @@ struct fftb_plan_s {
     size_t elem;
     int64_t S, C;
     int nsticks, nxocc, pitch, k1lo, ry;
+    int nphantom; // zero-length sticks the builder put into the holes of an explicit map (counted in nsticks, hidden from the caller)
     std::vector<int32_t> k1, k2, k3lo, len;
     std::vector<int64_t> off;
     std::vector<int4> h_stick, h_col;
@@ -800,11 +801,19 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         // ---- stick map: k1 major, k2 minor, both ascending over signed values (reading R5); either
         // generated from the cut-off (Eq. 9) or given explicitly
         std::vector<int32_t> ck1, ck2, clo, cln;
+        p->nphantom = 0;
         if (xm) {
-            ck1.assign(xm->k1, xm->k1 + xm->n);
-            ck2.assign(xm->k2, xm->k2 + xm->n);
-            clo.assign(xm->k3lo, xm->k3lo + xm->n);
-            cln.assign(xm->len, xm->len + xm->n);
+            // The kernels need (R6) one contiguous range of occupied k1 and one contiguous k2 run per k1.  A map with holes
+            // gets them filled with zero-length PHANTOM sticks (a missing k1 column: one phantom at k2 = 0): no packed
+            // point, a zero column of the intermediate in the inverse, a column nobody reads in the forward direction.
+            for (int64_t s = 0; s < xm->n; ++s) {
+                if (s > 0 && xm->k1[s] == xm->k1[s - 1])
+                    for (int q2 = xm->k2[s - 1] + 1; q2 < xm->k2[s]; ++q2) { ck1.push_back(xm->k1[s]); ck2.push_back(q2); clo.push_back(0); cln.push_back(0); }
+                else if (s > 0)
+                    for (int q1 = xm->k1[s - 1] + 1; q1 < xm->k1[s]; ++q1) { ck1.push_back(q1); ck2.push_back(0); clo.push_back(0); cln.push_back(0); }
+                ck1.push_back(xm->k1[s]); ck2.push_back(xm->k2[s]); clo.push_back(xm->k3lo[s]); cln.push_back(xm->len[s]);
+            }
+            p->nphantom = (int)((int64_t)ck1.size() - xm->n);
             a[0] = a[1] = a[2] = 0;
         } else {
             const int k1a = dense ? -(n1 / 2) : -a[0], k1b = dense ? (n1 + 1) / 2 - 1 : a[0];
@@ -968,11 +977,18 @@ int fftb_plan_create_explicit(fftb_plan *out, const fftb_plan_desc *desc, int64_
     return plan_create_impl(out, desc, &xm, nullptr);
 }
 
+int fftb_plan_create_explicit_tuned(fftb_plan *out, const fftb_plan_desc *desc, int64_t n_sticks, const int32_t *k1, const int32_t *k2,
+                                    const int32_t *k3lo, const int32_t *len, const fftb_plan_tuning *tuning)
+{
+    const ExplicitMap xm = {n_sticks, k1, k2, k3lo, len};
+    return plan_create_impl(out, desc, &xm, tuning);
+}
+
 int fftb_plan_info_get(fftb_plan p, fftb_plan_info *info)
 {
     if (!p || !info) return FFTB_EINVAL;
     info->n_points = p->S;
-    info->n_sticks = p->nsticks;
+    info->n_sticks = p->nsticks - p->nphantom;
     info->n_xocc = p->nxocc;
     info->device_bytes = (int64_t)p->bytes_min;
     info->device_bytes_host = (int64_t)p->bytes_stage;
@@ -995,6 +1011,20 @@ int fftb_plan_get_map(fftb_plan p, int32_t *k1, int32_t *k2, int32_t *k3lo, int3
 {
     if (!p) return FFTB_EINVAL;
     const size_t n = (size_t)p->nsticks;
+    if (p->nphantom) { // the caller's map: the phantom sticks that fill its holes are left out
+        size_t o = 0;
+        for (size_t s = 0; s < n; ++s) {
+            if (p->len[s] == 0) continue;
+            if (k1) k1[o] = p->k1[s];
+            if (k2) k2[o] = p->k2[s];
+            if (k3lo) k3lo[o] = p->k3lo[s];
+            if (len) len[o] = p->len[s];
+            if (off) off[o] = p->off[s];
+            ++o;
+        }
+        if (off) off[o] = p->off[n];
+        return FFTB_OK;
+    }
     if (k1) memcpy(k1, p->k1.data(), n * sizeof(int32_t));
     if (k2) memcpy(k2, p->k2.data(), n * sizeof(int32_t));
     if (k3lo) memcpy(k3lo, p->k3lo.data(), n * sizeof(int32_t));

@@ -501,3 +501,67 @@ def test_dense_arm_vs_oracle(fb, oracle, n, dtype, tuning):
         chk = p.forward((d_psi * d_v.unsqueeze(0)).contiguous())
         assert _rel(d_o.cpu().numpy(), chk.cpu().numpy()) <= w.tol
     p.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# explicit stick maps with holes (the offsets array describes any set of z-sticks)
+# ---------------------------------------------------------------------------------------------------------------
+HOLES = [((64, 64, 64), 13, (1, -2, 3), "c128", {}), ((128, 128, 128), 27, (-3, 4, 2), "c128", {}), ((128, 128, 128), 27, (-3, 4, 2), "c64", {}),
+         ((256, 256, 64), 14, (1, -1, 1), "c128", {}), ((32, 32, 96), 6, (1, 1, -9), "c64", {}), ((64, 64, 64), 25, (1, 0, -2), "c128", {}),
+         ((128, 128, 128), 27, (-3, 4, 2), "c128", {"flags": 4}), ((64, 64, 64), 13, (1, -2, 3), "c128", {"flags": 3})]
+
+
+@pytest.mark.timeout(300)
+@pytest.mark.parametrize("n,radius,centre,dtype,tuning", HOLES,
+                         ids=[f"{n[0]}x{n[2]}-r{r}-{d}-{t.get('flags', 0)}" for n, r, c, d, t in HOLES])
+def test_explicit_map_with_holes_vs_oracle(fb, oracle, n, radius, centre, dtype, tuning):
+    """A k-point-shifted ball with randomly shortened sticks, out of which the test then removes sticks: single sticks
+    and runs of 1 - 40 sticks inside k2 runs, the first stick after a column start, and whole k1 columns (two of them
+    neighbours).  The plan fills the holes with zero-length sticks of its own; the caller sees its own map, the packed
+    array has no element for them, and inverse / forward / local potential match the oracle's plain definition on the
+    point list the TEST expands from the map.  Persistent TMA kernels (64, 128, 256 half-band), generic kernels (32;
+    radius 25 on 64: full-band), the fused launch (flags 4)."""
+    from test_host_cabi import _shifted_ball_map
+
+    full = _shifted_ball_map(n, radius, centre, trim_seed=11)
+    k1f, k2f = full[0], full[1]
+    rng = np.random.default_rng(radius)
+    keep = np.ones(k1f.size, bool)
+    cols = np.unique(k1f)
+    for c1 in (cols[2], cols[3], cols[len(cols) // 2]):                      # whole k1 columns, two of them neighbours
+        keep[k1f == c1] = False
+    for c1 in cols[5:-2:3]:                                                  # holes inside k2 runs
+        idx = np.flatnonzero(k1f == c1)
+        if idx.size >= 5:
+            a = int(rng.integers(1, idx.size - 2))
+            b = min(idx.size - 1, a + int(rng.integers(1, 41)))
+            keep[idx[a:b]] = False
+    sm = tuple(x[keep] for x in full)
+    assert sm[0].size < k1f.size - 10
+    nb = 3
+    p = fb.Plan(n, batch=nb, dtype=dtype, stick_map=sm, tuning=tuning or None).bind()
+    if tuning.get("flags") == 4:
+        assert p.info["ring_bands"] >= 1
+    m = p.get_map()
+    for key, ref in zip(("k1", "k2", "k3lo", "len"), sm):
+        assert np.array_equal(m[key], ref), key
+    rep = np.repeat(np.arange(sm[0].size), sm[3])
+    off = np.concatenate([[0], np.cumsum(sm[3])])[:-1]
+    k = (sm[0][rep], sm[1][rep], (sm[2][rep] + (np.arange(rep.size) - off[rep])).astype(np.int32))
+    assert p.S == rep.size and all(np.array_equal(x, y) for x, y in zip(p.points(), k))
+    w = _w(n, (0, 0, 0), dtype=dtype, batch=nb)
+    c = wl.coefficients(w, *k)
+    g = wl.cuboid(w)
+    v = wl.potential(w)
+    C = float(np.prod(n))
+    d_c = torch.from_numpy(c).cuda()
+    d_psi = p.inverse(d_c)
+    d_f = p.forward(torch.from_numpy(g).cuda())
+    d_o = p.apply_vloc(d_c, torch.from_numpy(v).cuda())
+    d_rt = p.forward(d_psi)
+    torch.cuda.synchronize()
+    assert _rel(d_psi.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol
+    assert _rel(d_f.cpu().numpy(), oracle.forward(n, k, g, 1.0 / C)) <= w.tol
+    assert _rel(d_o.cpu().numpy(), oracle.apply_vloc(n, k, c, v, 1.0 / C)) <= w.tol
+    assert _rel(d_rt.cpu().numpy(), c) <= w.tol
+    p.destroy()

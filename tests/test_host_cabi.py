@@ -168,10 +168,19 @@ def test_explicit_stick_map_round_trip_and_errors():
     wide = ln.copy(); wide[0] = 17 - lo[0] + 1
     fb.Plan(n, stick_map=(k1, k2, lo, wide)).destroy()   # beyond the half band |k| <= N/4: full-band patterns, either precision
     fb.Plan(n, stick_map=(k1, k2, lo, wide), dtype="c64").destroy()
-    hole = np.ones(k1.size, bool); hole[np.flatnonzero(k1 == k1[k1.size // 2])[1]] = False
-    with pytest.raises(fb.FftbError) as e:      # a k2 run with a hole
-        fb.Plan(n, stick_map=(k1[hole], k2[hole], lo[hole], ln[hole]))
-    assert e.value.code == fb.FFTB_EUNSUPPORTED
+    # holes (a missing stick inside a k2 run, a missing k1 column): accepted, filled by the plan with zero-length sticks
+    # of its own that the caller never sees -- the map read back is the map given
+    hole = np.ones(k1.size, bool)
+    hole[np.flatnonzero(k1 == k1[k1.size // 2])[1]] = False
+    hole[k1 == k1[0] + 2] = False
+    hm = (k1[hole], k2[hole], lo[hole], ln[hole])
+    ph = fb.Plan(n, batch=2, stick_map=hm)
+    mh = ph.get_map()
+    for key, ref in zip(("k1", "k2", "k3lo", "len"), hm):
+        assert np.array_equal(mh[key], ref), key
+    assert np.array_equal(mh["off"], np.concatenate([[0], np.cumsum(hm[3])]))
+    assert ph.S == int(hm[3].sum()) and ph.info["n_sticks"] == hm[0].size and ph.info["pitch"] >= hm[0].size + 2
+    ph.destroy()
     with pytest.raises(fb.FftbError) as e:      # dense + explicit
         fb.Plan(n, stick_map=sm, dense=True)
     assert e.value.code == fb.FFTB_EINVAL
