@@ -247,12 +247,11 @@ int launch_plane_r4_vloc(const DevPlan &pl, const PlanTabs &tabs, const void *Ai
     return launch_status();
 }
 
-template <typename T>
-int launch_plane_r4_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *, void *Aout, const void *cin, void *, const void *, long long,
-                        long long sout, int nb, cudaStream_t st)
+template <typename T, bool TM>
+int launch_plane_r4_fwd_tm(const DevPlan &pl, const PlanTabs &tabs, const void *cin, void *Aout, long long sout, int nb, cudaStream_t st)
 {
     constexpr int NW = 8;
-    auto k = plane_r4_fwd_k<T, NW>;
+    auto k = plane_r4_fwd_k<T, NW, TM>;
     const size_t smem = sizeof(cx<T>) * (size_t)PlaneR4<T, NW>::PB;
     if (int rc = kernel_ready(k, NW * 32, smem, nullptr)) return rc;
     const int nplanes = pl.n3 * nb;
@@ -260,6 +259,19 @@ int launch_plane_r4_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *, v
     if (grid > nplanes) grid = nplanes;
     k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)cin, (cx<T> *)Aout, sout, nplanes);
     return launch_status();
+}
+// the sums over the y residues live in tensor memory if every warp's y tasks fit its columns (fftb_plane_r4.cuh)
+template <typename T> bool r4_sums_fit_tmem(const DevPlan &pl)
+{
+    using R4 = PlaneR4<T, 8>;
+    return ycol_tasks<typename R4::F>(pl.n_multi) <= R4::TMT * 8;
+}
+template <typename T>
+int launch_plane_r4_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *, void *Aout, const void *cin, void *, const void *, long long,
+                        long long sout, int nb, cudaStream_t st)
+{
+    return r4_sums_fit_tmem<T>(pl) ? launch_plane_r4_fwd_tm<T, true>(pl, tabs, cin, Aout, sout, nb, st)
+                                   : launch_plane_r4_fwd_tm<T, false>(pl, tabs, cin, Aout, sout, nb, st);
 }
 
 bool find_plane_fast(int dtype, int n, bool dense, PlaneLaunch *out)

@@ -20,6 +20,7 @@
 // plane_r4_fwd_k below is the adjoint chain, plane_r4_vloc_k the fused local-potential apply.
 #pragma once
 #include "fftb_plane_pf.cuh"
+#include "fftb_tmem.cuh"
 
 namespace fftb {
 
@@ -39,7 +40,100 @@ template <typename T, int NW> struct PlaneR4 {
     static constexpr int NXT = M / F::G;          // x tasks per quarter (G lines each)
     static_assert(NXT % NW == 0, "x tasks must divide evenly over the warps");
     static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)PB + (size_t)NW * ZONE);
+    // y tasks (G columns each) per quarter: at most ycol_tasks(NCOL), dealt round-robin over the warps
+    static constexpr int MAXT = (((NCOL + 7) / 8 * 8 + F::G - 1) / F::G + NW - 1) / NW;
+    // y tasks per warp whose partial sums fit the warp's share of tensor memory (two warps per lane quarter: 256 columns)
+    static constexpr int TMT = 256 / tmem_cols16<T>();
 };
+
+// The y tasks of a warp are the same for every plane and quarter: which column each lane group works on and, for the
+// kernels that read the row of A, which bulk copies bring the task's stick runs into the warp's landing zone.  Looked up
+// ONCE per kernel and kept in shared memory -- inside the plane loop a task then costs one shared-memory load instead
+// of two dependent look-ups in the column tables, a warp reduction and up to G copy instructions (measured on config 5:
+// 740 of the 2 400 cycles of an inverse y task).
+template <typename T, int NW> struct R4Tasks {
+    using R4 = PlaneR4<T, NW>;
+    static constexpr int G = R4::F::G;
+    int4 desc[NW][R4::MAXT][G]; // {x, stick count (0: no column), k2lo, column}; x = first value of the column in the landing
+                                // zone (r4_tasks_zone) or first stick of the column in the row of A (r4_tasks_rows)
+    int4 copy[NW][R4::MAXT][G]; // bulk copies of the task: {row offset, bytes (0: none), zone offset, 0}
+    int total[NW][R4::MAXT];    // bytes of all copies of the task
+};
+template <typename T, int NW>
+__device__ __forceinline__ void r4_tasks_rows(R4Tasks<T, NW> &ts, const DevPlan &pl, const ColTab4 &ct, int warp, int lane, int ytasks_w)
+{
+    using F = typename PlaneR4<T, NW>::F;
+    for (int k = 0; k < ytasks_w; ++k) {
+        if (lane < F::G) {
+            const int ci = ycol_index<F>(warp + k * NW, lane);
+            int4 d = make_int4(0, 0, 0, 0);
+            if (ci < pl.n_multi) {
+                const int col = ct.perm[ci];
+                const int4 co = ct.col[col];
+                d = make_int4(co.x, co.y, co.z, col);
+            }
+            ts.desc[warp][k][lane] = d;
+        }
+    }
+    __syncwarp();
+}
+// If the G columns of a task are neighbours in k1 (complex128: ycol_index is the identity) their stick runs are ONE
+// contiguous range of the row -- the sticks are ordered by (k1, k2) -- and arrive as one copy, unless single-stick
+// columns of an explicit map lie in between and make the range longer than the zone; otherwise one copy per column
+// (complex64: 16-byte units, so a run is widened to even element indices; the row's pitch is even).
+template <typename T, int NW>
+__device__ __forceinline__ void r4_tasks_zone(R4Tasks<T, NW> &ts, const DevPlan &pl, const ColTab4 &ct, int warp, int lane, int ytasks_w)
+{
+    using R4 = PlaneR4<T, NW>;
+    using F = typename R4::F;
+    constexpr int G = F::G, EA = 16 / (int)sizeof(cx<T>);
+    constexpr int GWy = F::LW / F::P2 < 1 ? 1 : F::LW / F::P2, Dy = F::P2 / GWy;
+    constexpr bool NEIGHBOURS = (GWy <= 1 || Dy <= 1);
+    for (int k = 0; k < ytasks_w; ++k) {
+        int4 d = make_int4(0, 0, 0, 0), cp = make_int4(0, 0, 0, 0);
+        int x1 = 0;
+        if (lane < G) {
+            const int ci = ycol_index<F>(warp + k * NW, lane);
+            if (ci < pl.n_multi) {
+                const int col = ct.perm[ci];
+                const int4 co = ct.col[col];
+                d = make_int4(co.x, co.y, co.z, col);
+                x1 = co.x + co.y;
+            }
+        }
+        // lane 0's column is the first of the task (it always exists); the largest end closes the range
+        const int first = __shfl_sync(0xffffffffu, d.x, 0);
+        int last = x1;
+#pragma unroll
+        for (int sft = 1; sft < G; sft <<= 1) last = max(last, __shfl_xor_sync(0xffffffffu, last, sft));
+        const int a0 = first & ~(EA - 1), a1 = (last + EA - 1) & ~(EA - 1);
+        if (NEIGHBOURS && a1 - a0 <= R4::ZONE) {
+            if (lane == 0) cp = make_int4(a0, (a1 - a0) * (int)sizeof(cx<T>), 0, 0);
+            d.x = d.y > 0 ? d.x - a0 : 0;
+        } else if (lane < G && d.y > 0) {
+            const int sh = d.x & (EA - 1);
+            cp = make_int4(d.x - sh, ((d.y + sh + EA - 1) & ~(EA - 1)) * (int)sizeof(cx<T>), lane * R4::ZCOL, 0);
+            d.x = lane * R4::ZCOL + sh;
+        }
+        int total = cp.y;
+#pragma unroll
+        for (int sft = 1; sft < G; sft <<= 1) total += __shfl_xor_sync(0xffffffffu, total, sft);
+        if (lane < G) { ts.desc[warp][k][lane] = d; ts.copy[warp][k][lane] = cp; }
+        if (lane == 0) ts.total[warp][k] = total;
+    }
+    __syncwarp();
+}
+// TMA: the stick runs of this warp's y task k of the plane whose row of A is `row` -> the warp's landing zone
+template <typename T, int NW>
+__device__ __forceinline__ void r4_zone_issue(const R4Tasks<T, NW> &ts, const cx<T> *row, cx<T> *zone, unsigned long long *bar, int warp, int lane, int k)
+{
+    if (lane == 0) mbar_expect_tx(bar, (unsigned)ts.total[warp][k]);
+    __syncwarp();
+    if (lane < R4Tasks<T, NW>::G) {
+        const int4 cp = ts.copy[warp][k][lane];
+        if (cp.y > 0) bulk_load(zone + cp.z, row + cp.x, (unsigned)cp.y, bar);
+    }
+}
 
 // u_e of one lane: slots s = t + 8 j; a = x[s - 64], b = x[s], c = x[+64] (lane 0, slot 0 only, else 0)
 template <int E, int J, typename T>
@@ -85,40 +179,10 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int ytasks_w = ntask_y > warp ? (ntask_y - warp + NW - 1) / NW : 0; // y tasks of this warp per quarter
 
-    struct YCol { bool act; int col; int4 co; };
-    auto ycol = [&](int task) -> YCol {
-        YCol c;
-        const int ci = ycol_index<F>(task, f);
-        c.act = ci < pl.n_multi;
-        c.col = ct.perm[c.act ? ci : 0];
-        c.co = ct.col[c.col];
-        return c;
-    };
-    // TMA: the stick runs of the G columns of y task `task` of plane (b, z) -> this warp's landing zone
-    auto zone_issue = [&](int b, int z, int task) {
-        const C *row = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
-        int bytes = 0;
-        int4 co = make_int4(0, 0, 0, 0);
-        if (lane < G) {
-            const int ci = ycol_index<F>(task, lane);
-            if (ci < pl.n_multi) {
-                co = ct.col[ct.perm[ci]];
-                // bulk copies move 16-byte multiples from 16-byte aligned addresses: for 8-byte elements the run is
-                // widened to even element indices (the row's pitch is even, so the widened run stays inside the row)
-                const int sh = sizeof(C) == 8 ? (co.x & 1) : 0;
-                co.x -= sh;
-                co.y += sh;
-                if (sizeof(C) == 8) co.y = (co.y + 1) & ~1;
-                bytes = co.y * (int)sizeof(C);
-            }
-        }
-        int total = bytes;
-#pragma unroll
-        for (int sft = 1; sft < G; sft <<= 1) total += __shfl_xor_sync(0xffffffffu, total, sft);
-        if (lane == 0) mbar_expect_tx(&bar_zone[warp], (unsigned)total);
-        __syncwarp();
-        if (bytes > 0) bulk_load(zone + lane * ZCOL, row + co.x, (unsigned)bytes, &bar_zone[warp]);
-    };
+    __shared__ R4Tasks<T, NW> ts;
+    r4_tasks_zone<T, NW>(ts, pl, ct, warp, lane, ytasks_w);
+    auto zone_issue = [&](const C *row, int k) { r4_zone_issue<T, NW>(ts, row, zone, &bar_zone[warp], warp, lane, k); };
+    auto row_of = [&](int b, int z) { return Ain + (long long)b * a_in_stride + (long long)z * pl.pitch; };
 
     if (tid == 0) {
         for (int w = 0; w < NW; ++w) mbar_init(&bar_zone[w], 1);
@@ -127,13 +191,13 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     __syncthreads();
     int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;
     const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;
-    if (kplanes > 0 && ytasks_w > 0) zone_issue(b, z, warp);
+    if (kplanes > 0 && ytasks_w > 0) zone_issue(row_of(b, z), 0);
 
 #pragma unroll 1
     for (int i = 0; i < kplanes; ++i) {
         const int zc = z + dz, zn = zc >= pl.n3 ? zc - pl.n3 : zc, bn = b + db + (zc >= pl.n3 ? 1 : 0); // next plane
         const bool more = i + 1 < kplanes;
-        const C *row = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
+        const C *row = row_of(b, z);
         // ================================================== Y_R: columns -> pbuf (lines y = 4 y' + R)
         auto yphase = [&](auto rc) {
             constexpr int R = decltype(rc)::value;
@@ -147,31 +211,31 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             }
 #pragma unroll 1
             for (int k = 0; k < ytasks_w; ++k) {
-                const int task = warp + k * NW;
-                const YCol c = ycol(task);
+                const int4 d = ts.desc[warp][k][f]; // {first value in the zone, stick count, k2lo, column}
+                const bool act = d.y > 0;
                 mbar_wait(&bar_zone[warp], zone_par);
                 zone_par ^= 1u;
-                const C *src = zone + f * ZCOL + (sizeof(C) == 8 ? (c.co.x & 1) : 0); // see zone_issue
+                const C *src = zone + d.x;
                 C a[8], bq[8], u[8], y[1][8];
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
-                    const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
-                    a[j] = (c.act && (unsigned)ia < (unsigned)c.co.y) ? src[ia] : czero<T>();
-                    bq[j] = (c.act && (unsigned)ib < (unsigned)c.co.y) ? src[ib] : czero<T>();
+                    const int ia = (t + 8 * j) - M - d.z, ib = (t + 8 * j) - d.z;
+                    a[j] = ((unsigned)ia < (unsigned)d.y) ? src[ia] : czero<T>();
+                    bq[j] = ((unsigned)ib < (unsigned)d.y) ? src[ib] : czero<T>();
                 }
-                const int ic = M - c.co.z;
-                const C cv = (c.act && t == 0 && (unsigned)ic < (unsigned)c.co.y) ? src[ic] : czero<T>();
+                const int ic = M - d.z;
+                const C cv = (t == 0 && (unsigned)ic < (unsigned)d.y) ? src[ic] : czero<T>();
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp(); // every lane has its values: the landing zone may be refilled
                 // next y task of this warp: same quarter, next quarter (same row again), or the next plane
-                if (k + 1 < ytasks_w) zone_issue(b, z, task + NW);
-                else if (R < 3) zone_issue(b, z, warp);
-                else if (more) zone_issue(bn, zn, warp);
+                if (k + 1 < ytasks_w) zone_issue(row, k + 1);
+                else if (R < 3) zone_issue(row, 0);
+                else if (more) zone_issue(row_of(bn, zn), 0);
                 r4_fold_inv<R, 0, T>(a, bq, cv, u, wt[R]);
-                C *pc = pbuf + c.col * YP;
-                sub_inv<F, T>(u, y, tws, ExSkew<T, P2, 1>{pc, c.act}, t); // exchanged in place in the column
+                C *pc = pbuf + d.w * YP;
+                sub_inv<F, T>(u, y, tws, ExSkew<T, P2, 1>{pc, act}, t); // exchanged in place in the column
                 __syncwarp();
-                if (c.act) {
+                if (act) {
 #pragma unroll
                     for (int q = 0; q < 8; ++q) pc[t + 8 * q] = y[0][q];
                 }
@@ -273,12 +337,17 @@ __device__ __forceinline__ void r4_part_fwd(const cx<T> (&gq)[8], cx<T> (&pa)[8]
 // forward plane kernel of the 256 pattern: the adjoint chain, quarter by quarter.
 //     X_r: each of the 64 lines y = 4 y' + r: (x, x+1) pairs loaded in two batches (e = 0,1 and e = 2,3),
 //          four length-64 transforms, F[k1] accumulated over e -> the occupied k1 columns of pbuf    | barrier
-//     Y_r: every column: length-64 transform over y', the part of residue r of F[k2] is ADDED to the one
-//          plane A[b][z][.] (r = 0 stores; the same lane wrote the same addresses one quarter earlier)  | barrier
+//     Y_r: every column: length-64 transform over y', the part of residue r of F[k2] is ADDED to the parts of the
+//          residues before it; residue 3 stores the sum into the one plane A[b][z][.]                    | barrier
+// Where the running sums live (TM): the same thread handles the same columns in every quarter, so it parks its 16 values
+// per y task in TENSOR MEMORY (tcgen05.st / tcgen05.ld, fftb_tmem.cuh: 256 columns per warp, two warps per lane
+// quarter) -- A is written once and never read.  !TM (a warp has more y tasks than its columns hold: complex128 maps
+// with more than 128 multi-stick columns): read-modify-write of the plane of A through L2, as in round 1.  Measured on
+// config 5: 0.833 -> 0.670 ms per launch, bit-identical results (the sums are formed in the same order).
 // The quarter-plane buffer leaves no room for a TMA landing zone of G = 4 lines of 4 KB per warp, so
 // the cuboid lines are loaded straight into registers here.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NW>
+template <typename T, int NW, bool TM>
 __global__ void __launch_bounds__(NW * 32, 1)
 plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab4 ct, const cx<T> *__restrict__ cub_in,
                cx<T> *__restrict__ Aout, long long a_out_stride, int nplanes)
@@ -308,6 +377,16 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;
     const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;
+    const int ytasks_w = ntask_y > warp ? (ntask_y - warp + NW - 1) / NW : 0; // y tasks of this warp per quarter
+    __shared__ R4Tasks<T, NW> ts;
+    __shared__ unsigned tm_slot;
+    r4_tasks_rows<T, NW>(ts, pl, ct, warp, lane, ytasks_w);
+    unsigned tm_warp = 0; // this warp's columns of tensor memory: lanes 32 (warp % 4) .., columns 256 (warp / 4) ..
+    if constexpr (TM) {
+        if (warp == 0) tmem_alloc(&tm_slot, 512);
+        tmem_publish();
+        tm_warp = tm_slot + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * 256);
+    }
 
     // the lines of an x task are loaded into registers when the task starts; one task earlier they are
     // requested into L2 (measured: 0.92 -> 0.90 ms on config 5; gathering the (x, x + 1) pairs of a batch
@@ -362,34 +441,61 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
         // ================================================== Y_R: columns -> partial plane R of A
         auto yphase = [&](auto rc) {
             constexpr int R = decltype(rc)::value;
-            // One plane of A: residue 0 stores, residues 1..3 add to what the SAME lane stored one quarter ago
-            // (still in L2; the loads are issued before the transform whose result they are added to).
             C *dst = Aout + (long long)b * a_out_stride + (long long)z * pl.pitch;
 #pragma unroll 1
-            for (int task = warp; task < ntask_y; task += NW) {
-                const int ci = ycol_index<F>(task, f);
-                const bool act = ci < pl.n_multi;
-                const int col = ct.perm[act ? ci : 0];
-                const int4 co = ct.col[col];
-                C *pc = pbuf + col * YP;
+            for (int k = 0; k < ytasks_w; ++k) {
+                const int4 co = ts.desc[warp][k][f]; // {first stick, stick count (0: no column), k2lo, column}
+                const bool act = co.y > 0;
+                C *pc = pbuf + co.w * YP;
                 C *d = dst + co.x;
                 const int ic = M - co.z;
-                const bool hc = act && t == 0 && (unsigned)ic < (unsigned)co.y;
-                C y[1][8], gq[8], pa[8], pb[8], pcv, oa[8], ob[8], oc = czero<T>();
-                if constexpr (R > 0) {
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
-                        oa[j] = (act && (unsigned)ia < (unsigned)co.y) ? ld_hint(d + ia, pol_keep) : czero<T>();
-                        ob[j] = (act && (unsigned)ib < (unsigned)co.y) ? ld_hint(d + ib, pol_keep) : czero<T>();
+                const bool hc = t == 0 && (unsigned)ic < (unsigned)co.y; // the +N/4 alias: one column at most, through L2
+                C y[1][8], gq[8], pa[8], pb[8], pcv, oc = czero<T>();
+                if constexpr (TM) {
+                    const unsigned taddr = tm_warp + (unsigned)(k * tmem_cols16<T>());
+                    typename TmemWords<T>::type old;
+                    if constexpr (R > 0) {
+                        tmem_get16_issue(taddr, old); // lands while the column is transformed
+                        if (hc) oc = ld_hint(d + ic, pol_keep);
                     }
-                    if (hc) oc = ld_hint(d + ic, pol_keep);
-                }
 #pragma unroll
-                for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
-                sub_fwd<F, T>(y, gq, tws, ExSkew<T, P2, 1>{pc, act}, t); // exchanged in place in the column
-                r4_part_fwd<R, 0, T>(gq, pa, pb, pcv, wt[R]);
-                if (act) {
+                    for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
+                    sub_fwd<F, T>(y, gq, tws, ExSkew<T, P2, 1>{pc, act}, t); // exchanged in place in the column
+                    r4_part_fwd<R, 0, T>(gq, pa, pb, pcv, wt[R]);
+                    if constexpr (R > 0) {
+                        tmem_wait_ld();
+                        tmem_add16(old, pa, pb);
+                    }
+                    if constexpr (R < 3) {
+                        tmem_put16(taddr, pa, pb);
+                        tmem_wait_st();
+                        if (hc) st_hint(d + ic, R > 0 ? cadd(oc, pcv) : pcv, pol_keep);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
+                            if ((unsigned)ia < (unsigned)co.y) d[ia] = pa[j];
+                            if ((unsigned)ib < (unsigned)co.y) d[ib] = pb[j];
+                        }
+                        if (hc) d[ic] = cadd(oc, pcv);
+                    }
+                } else {
+                    // residue 0 stores, residues 1..3 add to what the SAME lane stored one quarter ago (still in L2; the loads
+                    // are issued before the transform whose result they are added to)
+                    C oa[8], ob[8];
+                    if constexpr (R > 0) {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
+                            oa[j] = ((unsigned)ia < (unsigned)co.y) ? ld_hint(d + ia, pol_keep) : czero<T>();
+                            ob[j] = ((unsigned)ib < (unsigned)co.y) ? ld_hint(d + ib, pol_keep) : czero<T>();
+                        }
+                        if (hc) oc = ld_hint(d + ic, pol_keep);
+                    }
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
+                    sub_fwd<F, T>(y, gq, tws, ExSkew<T, P2, 1>{pc, act}, t); // exchanged in place in the column
+                    r4_part_fwd<R, 0, T>(gq, pa, pb, pcv, wt[R]);
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
@@ -426,6 +532,10 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             __syncthreads();
         }
         z = zn; b = bn;
+    }
+    if constexpr (TM) {
+        tmem_publish(); // every warp is done with its columns
+        if (warp == 0) tmem_dealloc(tm_slot, 512);
     }
 }
 
