@@ -216,13 +216,17 @@ template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
     using F = FastCfg<T, N, P1, P2>;
     return PlaneLaunch{1, {&launch_plane_fast<T, F, MODE_INV>, &launch_plane_fast<T, F, MODE_FWD>, &launch_plane_fast<T, F, MODE_VLOC>}};
 }
-// inverse plane kernel of the 256 pattern (fftb_plane_r4.cuh)
-template <typename T>
-int launch_plane_r4_inv(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *, const void *, void *cout, const void *, long long sin,
-                        long long, int nb, cudaStream_t st)
+// the 256 pattern parks per-thread values of the y tasks in tensor memory if every warp's y tasks fit its columns (fftb_plane_r4.cuh)
+template <typename T> bool r4_tasks_fit_tmem(const DevPlan &pl)
+{
+    using R4 = PlaneR4<T, 8>;
+    return ycol_tasks<typename R4::F>(pl.n_multi) <= R4::TMT * 8;
+}
+template <typename T, bool TM>
+int launch_plane_r4_inv_tm(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *cout, long long sin, int nb, cudaStream_t st)
 {
     constexpr int NW = 8;
-    auto k = plane_r4_inv_k<T, NW>;
+    auto k = plane_r4_inv_k<T, NW, TM>;
     const size_t smem = PlaneR4<T, NW>::smem_bytes;
     if (int rc = kernel_ready(k, NW * 32, smem, nullptr)) return rc;
     const int nplanes = pl.n3 * nb;
@@ -230,6 +234,14 @@ int launch_plane_r4_inv(const DevPlan &pl, const PlanTabs &tabs, const void *Ain
     if (grid > nplanes) grid = nplanes;
     k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)Ain, (cx<T> *)cout, sin, nplanes);
     return launch_status();
+}
+// inverse plane kernel of the 256 pattern (fftb_plane_r4.cuh)
+template <typename T>
+int launch_plane_r4_inv(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *, const void *, void *cout, const void *, long long sin,
+                        long long, int nb, cudaStream_t st)
+{
+    return r4_tasks_fit_tmem<T>(pl) ? launch_plane_r4_inv_tm<T, true>(pl, tabs, Ain, cout, sin, nb, st)
+                                    : launch_plane_r4_inv_tm<T, false>(pl, tabs, Ain, cout, sin, nb, st);
 }
 
 template <typename T>
@@ -260,17 +272,11 @@ int launch_plane_r4_fwd_tm(const DevPlan &pl, const PlanTabs &tabs, const void *
     k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)cin, (cx<T> *)Aout, sout, nplanes);
     return launch_status();
 }
-// the sums over the y residues live in tensor memory if every warp's y tasks fit its columns (fftb_plane_r4.cuh)
-template <typename T> bool r4_sums_fit_tmem(const DevPlan &pl)
-{
-    using R4 = PlaneR4<T, 8>;
-    return ycol_tasks<typename R4::F>(pl.n_multi) <= R4::TMT * 8;
-}
 template <typename T>
 int launch_plane_r4_fwd(const DevPlan &pl, const PlanTabs &tabs, const void *, void *Aout, const void *cin, void *, const void *, long long,
                         long long sout, int nb, cudaStream_t st)
 {
-    return r4_sums_fit_tmem<T>(pl) ? launch_plane_r4_fwd_tm<T, true>(pl, tabs, cin, Aout, sout, nb, st)
+    return r4_tasks_fit_tmem<T>(pl) ? launch_plane_r4_fwd_tm<T, true>(pl, tabs, cin, Aout, sout, nb, st)
                                    : launch_plane_r4_fwd_tm<T, false>(pl, tabs, cin, Aout, sout, nb, st);
 }
 

@@ -56,7 +56,7 @@ template <typename T, int NW> struct R4Tasks {
     static constexpr int G = R4::F::G;
     int4 desc[NW][R4::MAXT][G]; // {x, stick count (0: no column), k2lo, column}; x = first value of the column in the landing
                                 // zone (r4_tasks_zone) or first stick of the column in the row of A (r4_tasks_rows)
-    int4 copy[NW][R4::MAXT][G]; // bulk copies of the task: {row offset, bytes (0: none), zone offset, 0}
+    int4 copy[NW][R4::MAXT][G]; // bulk copies of the task: {row offset, bytes (0: none), zone offset, .}; .w = first stick of lane group G's column in the row
     int total[NW][R4::MAXT];    // bytes of all copies of the task
 };
 template <typename T, int NW>
@@ -91,7 +91,7 @@ __device__ __forceinline__ void r4_tasks_zone(R4Tasks<T, NW> &ts, const DevPlan 
     constexpr bool NEIGHBOURS = (GWy <= 1 || Dy <= 1);
     for (int k = 0; k < ytasks_w; ++k) {
         int4 d = make_int4(0, 0, 0, 0), cp = make_int4(0, 0, 0, 0);
-        int x1 = 0;
+        int x1 = 0, col_first = 0;
         if (lane < G) {
             const int ci = ycol_index<F>(warp + k * NW, lane);
             if (ci < pl.n_multi) {
@@ -99,6 +99,7 @@ __device__ __forceinline__ void r4_tasks_zone(R4Tasks<T, NW> &ts, const DevPlan 
                 const int4 co = ct.col[col];
                 d = make_int4(co.x, co.y, co.z, col);
                 x1 = co.x + co.y;
+                col_first = co.x;
             }
         }
         // lane 0's column is the first of the task (it always exists); the largest end closes the range
@@ -118,7 +119,7 @@ __device__ __forceinline__ void r4_tasks_zone(R4Tasks<T, NW> &ts, const DevPlan 
         int total = cp.y;
 #pragma unroll
         for (int sft = 1; sft < G; sft <<= 1) total += __shfl_xor_sync(0xffffffffu, total, sft);
-        if (lane < G) { ts.desc[warp][k][lane] = d; ts.copy[warp][k][lane] = cp; }
+        if (lane < G) { cp.w = col_first; ts.desc[warp][k][lane] = d; ts.copy[warp][k][lane] = cp; }
         if (lane == 0) ts.total[warp][k] = total;
     }
     __syncwarp();
@@ -148,7 +149,7 @@ __device__ __forceinline__ void r4_fold_inv(const cx<T> (&a)[8], const cx<T> (&b
     }
 }
 
-template <typename T, int NW>
+template <typename T, int NW, bool TM>
 __global__ void __launch_bounds__(NW * 32, 1)
 plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab4 ct, const cx<T> *__restrict__ Ain,
                cx<T> *__restrict__ cub_out, long long a_in_stride, int nplanes)
@@ -184,11 +185,22 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     auto zone_issue = [&](const C *row, int k) { r4_zone_issue<T, NW>(ts, row, zone, &bar_zone[warp], warp, lane, k); };
     auto row_of = [&](int b, int z) { return Ain + (long long)b * a_in_stride + (long long)z * pl.pitch; };
 
+    // TM: a thread's 16 inputs per y task are the same in all four quarters: quarter 0 takes them from the landing zone and
+    // parks them in tensor memory, the quarters 1..3 fetch them from there (no bulk copy, no landing-zone reads; the row of
+    // A is read once per plane instead of four times).  !TM: a warp has more y tasks than its columns of tensor memory hold.
+    __shared__ unsigned tm_slot;
+    unsigned tm_warp = 0; // this warp's columns of tensor memory: lanes 32 (warp % 4) .., columns 256 (warp / 4) ..
     if (tid == 0) {
         for (int w = 0; w < NW; ++w) mbar_init(&bar_zone[w], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncthreads();
+    if constexpr (TM) {
+        if (warp == 0) tmem_alloc(&tm_slot, 512);
+        tmem_publish();
+        tm_warp = tm_slot + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * 256);
+    } else {
+        __syncthreads();
+    }
     int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;
     const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;
     if (kplanes > 0 && ytasks_w > 0) zone_issue(row_of(b, z), 0);
@@ -213,24 +225,41 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             for (int k = 0; k < ytasks_w; ++k) {
                 const int4 d = ts.desc[warp][k][f]; // {first value in the zone, stick count, k2lo, column}
                 const bool act = d.y > 0;
-                mbar_wait(&bar_zone[warp], zone_par);
-                zone_par ^= 1u;
-                const C *src = zone + d.x;
-                C a[8], bq[8], u[8], y[1][8];
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const int ia = (t + 8 * j) - M - d.z, ib = (t + 8 * j) - d.z;
-                    a[j] = ((unsigned)ia < (unsigned)d.y) ? src[ia] : czero<T>();
-                    bq[j] = ((unsigned)ib < (unsigned)d.y) ? src[ib] : czero<T>();
-                }
                 const int ic = M - d.z;
-                const C cv = (t == 0 && (unsigned)ic < (unsigned)d.y) ? src[ic] : czero<T>();
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                __syncwarp(); // every lane has its values: the landing zone may be refilled
-                // next y task of this warp: same quarter, next quarter (same row again), or the next plane
-                if (k + 1 < ytasks_w) zone_issue(row, k + 1);
-                else if (R < 3) zone_issue(row, 0);
-                else if (more) zone_issue(row_of(bn, zn), 0);
+                const bool hc = t == 0 && (unsigned)ic < (unsigned)d.y; // the +N/4 alias: one column at most
+                C a[8], bq[8], u[8], y[1][8], cv;
+                if constexpr (TM && R > 0) {
+                    typename TmemWords<T>::type wds;
+                    tmem_get16_issue(tm_warp + (unsigned)(k * tmem_cols16<T>()), wds);
+                    cv = hc ? __ldcg(row + ts.copy[warp][k][f].w + ic) : czero<T>();
+                    tmem_wait_ld();
+                    tmem_unpack16(wds, a, bq);
+                } else {
+                    mbar_wait(&bar_zone[warp], zone_par);
+                    zone_par ^= 1u;
+                    const C *src = zone + d.x;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int ia = (t + 8 * j) - M - d.z, ib = (t + 8 * j) - d.z;
+                        a[j] = ((unsigned)ia < (unsigned)d.y) ? src[ia] : czero<T>();
+                        bq[j] = ((unsigned)ib < (unsigned)d.y) ? src[ib] : czero<T>();
+                    }
+                    cv = hc ? src[ic] : czero<T>();
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    __syncwarp(); // every lane has its values: the landing zone may be refilled
+                    if constexpr (TM) {
+                        // the zone is used in quarter 0 only: the next task of this plane, or the first one of the next plane
+                        if (k + 1 < ytasks_w) zone_issue(row, k + 1);
+                        else if (more) zone_issue(row_of(bn, zn), 0);
+                        tmem_put16(tm_warp + (unsigned)(k * tmem_cols16<T>()), a, bq);
+                        tmem_wait_st();
+                    } else {
+                        // next y task of this warp: same quarter, next quarter (same row again), or the next plane
+                        if (k + 1 < ytasks_w) zone_issue(row, k + 1);
+                        else if (R < 3) zone_issue(row, 0);
+                        else if (more) zone_issue(row_of(bn, zn), 0);
+                    }
+                }
                 r4_fold_inv<R, 0, T>(a, bq, cv, u, wt[R]);
                 C *pc = pbuf + d.w * YP;
                 sub_inv<F, T>(u, y, tws, ExSkew<T, P2, 1>{pc, act}, t); // exchanged in place in the column
@@ -295,6 +324,10 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             __syncthreads();
         }
         z = zn; b = bn;
+    }
+    if constexpr (TM) {
+        tmem_publish(); // every warp is done with its columns
+        if (warp == 0) tmem_dealloc(tm_slot, 512);
     }
 }
 

@@ -91,6 +91,22 @@ __device__ __forceinline__ void tmem_add16(const TmemWords64 &o, float2 (&a)[8],
         b[i].x += __uint_as_float(o.w[16 + 2 * i]); b[i].y += __uint_as_float(o.w[16 + 2 * i + 1]);
     }
 }
+__device__ __forceinline__ void tmem_unpack16(const TmemWords128 &o, double2 (&a)[8], double2 (&b)[8])
+{
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        a[i].x = __hiloint2double((int)o.w[4 * i + 1], (int)o.w[4 * i]); a[i].y = __hiloint2double((int)o.w[4 * i + 3], (int)o.w[4 * i + 2]);
+        b[i].x = __hiloint2double((int)o.w[32 + 4 * i + 1], (int)o.w[32 + 4 * i]); b[i].y = __hiloint2double((int)o.w[32 + 4 * i + 3], (int)o.w[32 + 4 * i + 2]);
+    }
+}
+__device__ __forceinline__ void tmem_unpack16(const TmemWords64 &o, float2 (&a)[8], float2 (&b)[8])
+{
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        a[i].x = __uint_as_float(o.w[2 * i]); a[i].y = __uint_as_float(o.w[2 * i + 1]);
+        b[i].x = __uint_as_float(o.w[16 + 2 * i]); b[i].y = __uint_as_float(o.w[16 + 2 * i + 1]);
+    }
+}
 template <typename T> __host__ __device__ constexpr int tmem_cols16() { return 16 * (int)sizeof(cx<T>) / 4; } // columns taken by 16 values
 
 } // namespace fftb
