@@ -244,12 +244,12 @@ int launch_plane_r4_inv(const DevPlan &pl, const PlanTabs &tabs, const void *Ain
                                     : launch_plane_r4_inv_tm<T, false>(pl, tabs, Ain, cout, sin, nb, st);
 }
 
-template <typename T>
-int launch_plane_r4_vloc(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *Aout, const void *, void *, const void *v, long long sin,
-                         long long sout, int nb, cudaStream_t st)
+template <typename T, bool TM>
+int launch_plane_r4_vloc_tm(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *Aout, const void *v, long long sin, long long sout, int nb,
+                            cudaStream_t st)
 {
     constexpr int NW = 8;
-    auto k = plane_r4_vloc_k<T, NW>;
+    auto k = plane_r4_vloc_k<T, NW, TM>;
     const size_t smem = PlaneR4<T, NW>::smem_bytes;
     if (int rc = kernel_ready(k, NW * 32, smem, nullptr)) return rc;
     const int nplanes = pl.n3 * nb;
@@ -257,6 +257,13 @@ int launch_plane_r4_vloc(const DevPlan &pl, const PlanTabs &tabs, const void *Ai
     if (grid > nplanes) grid = nplanes;
     k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)Ain, (cx<T> *)Aout, (const T *)v, sin, sout, nplanes);
     return launch_status();
+}
+template <typename T>
+int launch_plane_r4_vloc(const DevPlan &pl, const PlanTabs &tabs, const void *Ain, void *Aout, const void *, void *, const void *v, long long sin,
+                         long long sout, int nb, cudaStream_t st)
+{
+    return r4_tasks_fit_tmem<T>(pl) ? launch_plane_r4_vloc_tm<T, true>(pl, tabs, Ain, Aout, v, sin, sout, nb, st)
+                                    : launch_plane_r4_vloc_tm<T, false>(pl, tabs, Ain, Aout, v, sin, sout, nb, st);
 }
 
 template <typename T, bool TM>

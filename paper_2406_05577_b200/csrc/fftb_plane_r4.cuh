@@ -56,7 +56,7 @@ template <typename T, int NW> struct R4Tasks {
     static constexpr int G = R4::F::G;
     int4 desc[NW][R4::MAXT][G]; // {x, stick count (0: no column), k2lo, column}; x = first value of the column in the landing
                                 // zone (r4_tasks_zone) or first stick of the column in the row of A (r4_tasks_rows)
-    int4 copy[NW][R4::MAXT][G]; // bulk copies of the task: {row offset, bytes (0: none), zone offset, .}; .w = first stick of lane group G's column in the row
+    int4 copy[NW][R4::MAXT][G]; // bulk copies of the task: {row offset, bytes (0: none), zone offset, .}; .w = first stick of this lane group's column in the row of A
     int total[NW][R4::MAXT];    // bytes of all copies of the task
 };
 template <typename T, int NW>
@@ -584,7 +584,7 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
 // The cuboid is never written (I6').  The landing zone is scratch during X_r, so the first y task of
 // a quarter is requested after X_{r-1} and lands during Y_fwd_{r-1}.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NW>
+template <typename T, int NW, bool TM>
 __global__ void __launch_bounds__(NW * 32, 1)
 plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab4 ct, const cx<T> *__restrict__ Ain,
                 cx<T> *__restrict__ Aout, const T *__restrict__ vloc, long long a_in_stride, long long a_out_stride, int nplanes)
@@ -617,52 +617,34 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
     const int kplanes = nplanes > (int)blockIdx.x ? (nplanes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int ytasks_w = ntask_y > warp ? (ntask_y - warp + NW - 1) / NW : 0;
 
-    struct YCol { bool act; int col; int4 co; };
-    auto ycol = [&](int task) -> YCol {
-        YCol c;
-        const int ci = ycol_index<F>(task, f);
-        c.act = ci < pl.n_multi;
-        c.col = ct.perm[c.act ? ci : 0];
-        c.co = ct.col[c.col];
-        return c;
-    };
-    auto zone_issue = [&](int b, int z, int task) {
-        const C *row = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
-        int bytes = 0;
-        int4 co = make_int4(0, 0, 0, 0);
-        if (lane < G) {
-            const int ci = ycol_index<F>(task, lane);
-            if (ci < pl.n_multi) {
-                co = ct.col[ct.perm[ci]];
-                const int sh = sizeof(C) == 8 ? (co.x & 1) : 0; // see plane_r4_inv_k
-                co.x -= sh;
-                co.y += sh;
-                if (sizeof(C) == 8) co.y = (co.y + 1) & ~1;
-                bytes = co.y * (int)sizeof(C);
-            }
-        }
-        int total = bytes;
-#pragma unroll
-        for (int sft = 1; sft < G; sft <<= 1) total += __shfl_xor_sync(0xffffffffu, total, sft);
-        if (lane == 0) mbar_expect_tx(&bar_zone[warp], (unsigned)total);
-        __syncwarp();
-        if (bytes > 0) bulk_load(zone + lane * ZCOL, row + co.x, (unsigned)bytes, &bar_zone[warp]);
-    };
+    __shared__ R4Tasks<T, NW> ts; // y-task descriptors of the warps, built once
+    r4_tasks_zone<T, NW>(ts, pl, ct, warp, lane, ytasks_w);
+    auto zone_issue = [&](const C *row, int k) { r4_zone_issue<T, NW>(ts, row, zone, &bar_zone[warp], warp, lane, k); };
+    auto row_of = [&](int b, int z) { return Ain + (long long)b * a_in_stride + (long long)z * pl.pitch; };
+    // TM: the running sums of the forward y passes live in tensor memory, as in plane_r4_fwd_k
+    __shared__ unsigned tm_slot;
+    unsigned tm_warp = 0;
 
     if (tid == 0) {
         for (int w = 0; w < NW; ++w) mbar_init(&bar_zone[w], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncthreads();
+    if constexpr (TM) {
+        if (warp == 0) tmem_alloc(&tm_slot, 512);
+        tmem_publish();
+        tm_warp = tm_slot + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * 256);
+    } else {
+        __syncthreads();
+    }
     int z = blockIdx.x % pl.n3, b = blockIdx.x / pl.n3;
     const int dz = gridDim.x % pl.n3, db = gridDim.x / pl.n3;
-    if (kplanes > 0 && ytasks_w > 0) zone_issue(b, z, warp);
+    if (kplanes > 0 && ytasks_w > 0) zone_issue(row_of(b, z), 0);
 
 #pragma unroll 1
     for (int i = 0; i < kplanes; ++i) {
         const int zc = z + dz, zn = zc >= pl.n3 ? zc - pl.n3 : zc, bn = b + db + (zc >= pl.n3 ? 1 : 0);
         const bool more = i + 1 < kplanes;
-        const C *row = Ain + (long long)b * a_in_stride + (long long)z * pl.pitch;
+        const C *row = row_of(b, z);
         C *dst = Aout + (long long)b * a_out_stride + (long long)z * pl.pitch;
         // ================================================== Y_inv_R: columns -> pbuf
         auto yinv = [&](auto rc) {
@@ -677,28 +659,28 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
             }
 #pragma unroll 1
             for (int k = 0; k < ytasks_w; ++k) {
-                const int task = warp + k * NW;
-                const YCol c = ycol(task);
+                const int4 d = ts.desc[warp][k][f]; // {first value in the zone, stick count, k2lo, column}
+                const bool act = d.y > 0;
                 mbar_wait(&bar_zone[warp], zone_par);
                 zone_par ^= 1u;
-                const C *src = zone + f * ZCOL + (sizeof(C) == 8 ? (c.co.x & 1) : 0);
+                const C *src = zone + d.x;
                 C a[8], bq[8], u[8], y[1][8];
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
-                    const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
-                    a[j] = (c.act && (unsigned)ia < (unsigned)c.co.y) ? src[ia] : czero<T>();
-                    bq[j] = (c.act && (unsigned)ib < (unsigned)c.co.y) ? src[ib] : czero<T>();
+                    const int ia = (t + 8 * j) - M - d.z, ib = (t + 8 * j) - d.z;
+                    a[j] = ((unsigned)ia < (unsigned)d.y) ? src[ia] : czero<T>();
+                    bq[j] = ((unsigned)ib < (unsigned)d.y) ? src[ib] : czero<T>();
                 }
-                const int ic = M - c.co.z;
-                const C cv = (c.act && t == 0 && (unsigned)ic < (unsigned)c.co.y) ? src[ic] : czero<T>();
+                const int ic = M - d.z;
+                const C cv = (t == 0 && (unsigned)ic < (unsigned)d.y) ? src[ic] : czero<T>();
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
-                if (k + 1 < ytasks_w) zone_issue(b, z, task + NW); // within the y phase the zone is a landing zone only
+                if (k + 1 < ytasks_w) zone_issue(row, k + 1); // within the y phase the zone is a landing zone only
                 r4_fold_inv<R, 0, T>(a, bq, cv, u, wt[R]);
-                C *pc = pbuf + c.col * YP;
-                sub_inv<F, T>(u, y, tws, ExSkew<T, P2, 1>{pc, c.act}, t);
+                C *pc = pbuf + d.w * YP;
+                sub_inv<F, T>(u, y, tws, ExSkew<T, P2, 1>{pc, act}, t);
                 __syncwarp();
-                if (c.act) {
+                if (act) {
 #pragma unroll
                     for (int q = 0; q < 8; ++q) pc[t + 8 * q] = y[0][q];
                 }
@@ -773,32 +755,63 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
         auto yfwd = [&](auto rc) {
             constexpr int R = decltype(rc)::value;
 #pragma unroll 1
-            for (int task = warp; task < ntask_y; task += NW) {
-                const YCol c = ycol(task);
-                C *pc = pbuf + c.col * YP;
-                C *d = dst + c.co.x;
-                const int ic = M - c.co.z;
-                const bool hc = c.act && t == 0 && (unsigned)ic < (unsigned)c.co.y;
-                C y[1][8], gq[8], pa[8], pb[8], pcv, oa[8], ob[8], oc = czero<T>();
-                if constexpr (R > 0) {
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
-                        oa[j] = (c.act && (unsigned)ia < (unsigned)c.co.y) ? ld_hint(d + ia, pol_keep) : czero<T>();
-                        ob[j] = (c.act && (unsigned)ib < (unsigned)c.co.y) ? ld_hint(d + ib, pol_keep) : czero<T>();
+            for (int k = 0; k < ytasks_w; ++k) {
+                const int4 dk = ts.desc[warp][k][f]; // {., stick count (0: no column), k2lo, column}
+                const int4 co = make_int4(ts.copy[warp][k][f].w, dk.y, dk.z, dk.w); // .x = first stick of the column in the row of A
+                const bool act = co.y > 0;
+                C *pc = pbuf + co.w * YP;
+                C *d = dst + co.x;
+                const int ic = M - co.z;
+                const bool hc = t == 0 && (unsigned)ic < (unsigned)co.y; // the +N/4 alias: one column at most, through L2
+                C y[1][8], gq[8], pa[8], pb[8], pcv, oc = czero<T>();
+                if constexpr (TM) {
+                    const unsigned taddr = tm_warp + (unsigned)(k * tmem_cols16<T>());
+                    typename TmemWords<T>::type old;
+                    if constexpr (R > 0) {
+                        tmem_get16_issue(taddr, old); // lands while the column is transformed
+                        if (hc) oc = ld_hint(d + ic, pol_keep);
                     }
-                    if (hc) oc = ld_hint(d + ic, pol_keep);
-                }
 #pragma unroll
-                for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
-                sub_fwd<F, T>(y, gq, tws, ExSkew<T, P2, 1>{pc, c.act}, t);
-                r4_part_fwd<R, 0, T>(gq, pa, pb, pcv, wt[R]);
-                if (c.act) {
+                    for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
+                    sub_fwd<F, T>(y, gq, tws, ExSkew<T, P2, 1>{pc, act}, t);
+                    r4_part_fwd<R, 0, T>(gq, pa, pb, pcv, wt[R]);
+                    if constexpr (R > 0) {
+                        tmem_wait_ld();
+                        tmem_add16(old, pa, pb);
+                    }
+                    if constexpr (R < 3) {
+                        tmem_put16(taddr, pa, pb);
+                        tmem_wait_st();
+                        if (hc) st_hint(d + ic, R > 0 ? cadd(oc, pcv) : pcv, pol_keep);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
+                            if ((unsigned)ia < (unsigned)co.y) d[ia] = pa[j];
+                            if ((unsigned)ib < (unsigned)co.y) d[ib] = pb[j];
+                        }
+                        if (hc) d[ic] = cadd(oc, pcv);
+                    }
+                } else {
+                    C oa[8], ob[8];
+                    if constexpr (R > 0) {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
+                            oa[j] = ((unsigned)ia < (unsigned)co.y) ? ld_hint(d + ia, pol_keep) : czero<T>();
+                            ob[j] = ((unsigned)ib < (unsigned)co.y) ? ld_hint(d + ib, pol_keep) : czero<T>();
+                        }
+                        if (hc) oc = ld_hint(d + ic, pol_keep);
+                    }
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) y[0][q] = pc[t + 8 * q];
+                    sub_fwd<F, T>(y, gq, tws, ExSkew<T, P2, 1>{pc, act}, t);
+                    r4_part_fwd<R, 0, T>(gq, pa, pb, pcv, wt[R]);
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
-                        const int ia = (t + 8 * j) - M - c.co.z, ib = (t + 8 * j) - c.co.z;
-                        if ((unsigned)ia < (unsigned)c.co.y) st_hint(d + ia, R > 0 ? cadd(oa[j], pa[j]) : pa[j], pol_keep);
-                        if ((unsigned)ib < (unsigned)c.co.y) st_hint(d + ib, R > 0 ? cadd(ob[j], pb[j]) : pb[j], pol_keep);
+                        const int ia = (t + 8 * j) - M - co.z, ib = (t + 8 * j) - co.z;
+                        if ((unsigned)ia < (unsigned)co.y) st_hint(d + ia, R > 0 ? cadd(oa[j], pa[j]) : pa[j], pol_keep);
+                        if ((unsigned)ib < (unsigned)co.y) st_hint(d + ib, R > 0 ? cadd(ob[j], pb[j]) : pb[j], pol_keep);
                     }
                     if (hc) st_hint(d + ic, R > 0 ? cadd(oc, pcv) : pcv, pol_keep);
                 }
@@ -831,8 +844,8 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
             __syncthreads();
             // the zone is a landing zone again: the first y task of the next quarter (or plane) lands during Y_fwd_r
             if (ytasks_w > 0) {
-                if (r < 3) zone_issue(b, z, warp);
-                else if (more) zone_issue(bn, zn, warp);
+                if (r < 3) zone_issue(row, 0);
+                else if (more) zone_issue(row_of(bn, zn), 0);
             }
             switch (r) {
             case 0: yfwd(I0{}); break;
@@ -843,6 +856,10 @@ plane_r4_vloc_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColT
             // no barrier: the next Y_inv touches the same columns from the same warp
         }
         z = zn; b = bn;
+    }
+    if constexpr (TM) {
+        tmem_publish(); // every warp is done with its columns
+        if (warp == 0) tmem_dealloc(tm_slot, 512);
     }
 }
 

@@ -346,6 +346,61 @@ def test_explicit_map_many_single_stick_columns_256(fb, oracle):
     p.destroy()
 
 
+def _explicit_256_case(fb, oracle, sm, n, dtype, nb):
+    p = fb.Plan(n, batch=nb, dtype=dtype, stick_map=sm).bind()
+    k = p.points()
+    w = wl.Workload(0, "explicit", n, (0, 0, 0), dtype, nb, "uniform", "inv_fwd")
+    c = wl.coefficients(w, *k)
+    d_c = torch.from_numpy(c).cuda()
+    d_psi = p.inverse(d_c)
+    torch.cuda.synchronize()
+    assert _rel(d_psi.cpu().numpy(), oracle.inverse(n, k, c)) <= w.tol
+    C = float(np.prod(n))
+    g = wl.cuboid(w)
+    d_f = p.forward(torch.from_numpy(g).cuda())
+    v = wl.potential(w)
+    d_o = p.apply_vloc(d_c, torch.from_numpy(v).cuda())
+    torch.cuda.synchronize()
+    assert _rel(d_f.cpu().numpy(), oracle.forward(n, k, g, 1.0 / C)) <= w.tol
+    assert _rel(d_o.cpu().numpy(), oracle.apply_vloc(n, k, c, v, 1.0 / C)) <= w.tol
+    p.destroy()
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_explicit_map_129_multi_stick_columns_256(fb, oracle, dtype):
+    """All 129 k1 columns of a 256 x 256 grid hold several sticks: 33 y tasks, one more than the warps' columns of tensor
+    memory hold in complex128 -- the plane kernels of the 256 pattern then take their variants without tensor memory
+    (running sums of the forward y passes through L2, inputs of the inverse y passes through the landing zone)."""
+    n = (256, 256, 32)
+    k1, k2, k3lo, ln = [], [], [], []
+    for a in range(-64, 65):
+        half = 1 + (a % 3) if abs(a) < 60 else 64 - abs(a) + 1  # 3, 5 or 7 sticks; the edge columns up to 11
+        for b in range(-half, half + 1):
+            k1.append(a); k2.append(b); k3lo.append(-2 - (a + b) % 3); ln.append(4 + (a * b) % 3)
+    sm = tuple(np.asarray(x, dtype=np.int32) for x in (k1, k2, k3lo, ln))
+    _explicit_256_case(fb, oracle, sm, n, dtype, 2)
+
+
+def test_explicit_map_singles_between_multi_stick_columns_256(fb, oracle):
+    """Single-stick columns BETWEEN multi-stick columns of a 256 x 256 grid, and a column reaching |k2| = 64: the stick
+    runs of a y task's four columns are then one contiguous range of the row of A only together with the single sticks
+    that lie in between (the inverse plane kernel's one bulk copy per task covers them), and the +N/4 alias of the y axis
+    travels through L2 next to the sums in tensor memory."""
+    n = (256, 256, 32)
+    k1, k2, k3lo, ln = [], [], [], []
+    for a in range(-40, 41):
+        if a % 3 == 1:
+            run = [a % 5 - 2]
+        elif a == 0:
+            run = range(-64, 65)
+        else:
+            run = range(-(abs(a) % 29) - 1, (abs(a) % 31) + 2)
+        for b in run:
+            k1.append(a); k2.append(b); k3lo.append(-3 + (a - b) % 2); ln.append(3 + (a * a + b) % 4)
+    sm = tuple(np.asarray(x, dtype=np.int32) for x in (k1, k2, k3lo, ln))
+    _explicit_256_case(fb, oracle, sm, n, "c128", 3)
+
+
 @pytest.mark.parametrize("dtype,nb", [("c128", 37), ("c64", 64), ("c128", 1)])
 def test_batch_fastest_packed_layout(fb, oracle, dtype, nb):
     """PAPER.md:219-221 (Fig. 8, "b x y z"): coefficients held with the band index fastest go through
