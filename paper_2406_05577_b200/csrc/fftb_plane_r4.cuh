@@ -21,6 +21,7 @@
 #pragma once
 #include "fftb_plane_pf.cuh"
 #include "fftb_tmem.cuh"
+#include <cuda.h>
 
 namespace fftb {
 
@@ -44,6 +45,9 @@ template <typename T, int NW> struct PlaneR4 {
     static constexpr int MAXT = (((NCOL + 7) / 8 * 8 + F::G - 1) / F::G + NW - 1) / NW;
     // y tasks per warp whose partial sums fit the warp's share of tensor memory (two warps per lane quarter: 256 columns)
     static constexpr int TMT = 256 / tmem_cols16<T>();
+    // forward kernel: elements of a warp's landing zone (G lines x 64 (x, x+1) pairs) and its dynamic shared memory
+    static constexpr int LZE = F::G * M * 2;
+    static constexpr size_t smem_bytes_fwd = sizeof(cx<T>) * ((size_t)PB + (size_t)NW * LZE) + 128;
 };
 
 // The y tasks of a warp are the same for every plane and quarter: which column each lane group works on and, for the
@@ -331,6 +335,15 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     }
 }
 
+// one half (h = 0: e = 0, 1; h = 1: e = 2, 3) of the (x, x+1) pairs of the G lines y = 4 (ylg mod 64 ..+G) + r of a plane:
+// coordinates of the cuboid tensor of plane_r4_fwd_k (built by the launcher): {0, h, 0, r, ylg}, ylg = (band n3 + z) 64 + y / 4
+__device__ __forceinline__ void r4_lines_box_load(void *sdst, const void *tmap, int half, int r, int ylg, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(smem_u32(sdst)),
+                 "l"(tmap), "r"(0), "r"(half), "r"(0), "r"(r), "r"(ylg), "r"(smem_u32(bar))
+                 : "memory");
+}
+
 // adjoint of r4_fold_inv: accumulate F[k] = sum_e conj(W^{e k}) G_e[k mod 64] for k = s - 64 (fa), s (fb), +64 (fc)
 template <int E, int J, typename T>
 __device__ __forceinline__ void r4_fold_fwd(const cx<T> (&gq)[8], cx<T> (&fa)[8], cx<T> (&fb)[8], cx<T> &fc, cx<T> wte)
@@ -377,12 +390,17 @@ __device__ __forceinline__ void r4_part_fwd(const cx<T> (&gq)[8], cx<T> (&pa)[8]
 // quarter) -- A is written once and never read.  !TM (a warp has more y tasks than its columns hold: complex128 maps
 // with more than 128 multi-stick columns): read-modify-write of the plane of A through L2, as in round 1.  Measured on
 // config 5: 0.833 -> 0.670 ms per launch, bit-identical results (the sums are formed in the same order).
-// The quarter-plane buffer leaves no room for a TMA landing zone of G = 4 lines of 4 KB per warp, so
-// the cuboid lines are loaded straight into registers here.
+// The quarter-plane buffer leaves no room for a landing zone of G = 4 whole lines (4 KB each) per warp, but a sub-transform
+// pair e = 0, 1 (or 2, 3) needs only every other (x, x+1) pair of a line: the cuboid is described to the TMA engine as a
+// 5-dimensional tensor (4 doubles | half | n' | y mod 4 | y / 4 over all planes and bands), and ONE tensor copy gathers a
+// half of the pairs of a task's four lines -- 32-byte pieces 64 bytes apart -- into 8 KB of shared memory, dense
+// [line][n'][pair].  The second half of a task lands while its first two transforms run, the first half of the next
+// task during the last two: no warp waits for a register load any more (round 1-2: two batches of 32-byte loads into
+// registers, `long_scoreboard` the kernel's largest stall; 0.659 -> 0.595 ms on config 5, bit-identical).
 // ---------------------------------------------------------------------------------------------
 template <typename T, int NW, bool TM>
 __global__ void __launch_bounds__(NW * 32, 1)
-plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab4 ct, const cx<T> *__restrict__ cub_in,
+plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab4 ct, const __grid_constant__ CUtensorMap cmap,
                cx<T> *__restrict__ Aout, long long a_out_stride, int nplanes)
 {
     using C = cx<T>;
@@ -394,6 +412,13 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     // the plane of A this kernel accumulates its four y residues into is read and rewritten within microseconds: keep it in L2
     const unsigned long long pol_keep = l2_policy(2);
     C *pbuf = reinterpret_cast<C *>(smem_raw);
+    // landing zone of this warp: one half (e = 0, 1 or e = 2, 3) of the (x, x+1) pairs of the G lines of an x task, dense
+    // [line][n'][pair]; a tensor copy's destination must be 128-byte aligned
+    unsigned char *lz_raw = smem_raw + sizeof(C) * (size_t)R4::PB;
+    lz_raw += (128u - (smem_u32(lz_raw) & 127u)) & 127u;
+    C *lzone = reinterpret_cast<C *>(lz_raw) + (size_t)(threadIdx.x >> 5) * R4::LZE;
+    __shared__ __align__(8) unsigned long long bar_lz[NW];
+    unsigned lz_par = 0;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
     const C *tw = reinterpret_cast<const C *>(pl.tw1);
@@ -414,6 +439,11 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     __shared__ R4Tasks<T, NW> ts;
     __shared__ unsigned tm_slot;
     r4_tasks_rows<T, NW>(ts, pl, ct, warp, lane, ytasks_w);
+    if (tid == 0) {
+        for (int w = 0; w < NW; ++w) mbar_init(&bar_lz[w], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if constexpr (!TM) __syncthreads();
     unsigned tm_warp = 0; // this warp's columns of tensor memory: lanes 32 (warp % 4) .., columns 256 (warp / 4) ..
     if constexpr (TM) {
         if (warp == 0) tmem_alloc(&tm_slot, 512);
@@ -421,16 +451,32 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
         tm_warp = tm_slot + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * 256);
     }
 
-    // the lines of an x task are loaded into registers when the task starts; one task earlier they are
-    // requested into L2 (measured: 0.92 -> 0.90 ms on config 5; gathering the (x, x + 1) pairs of a batch
-    // into a landing zone with 16-byte cp.async copies instead was measured at 1.20 ms)
-    auto lines_prefetch = [&](int b, int z, int r, int v) {
-        if (lane < G) {
-            const int yl = (warp + v * NW) * G + lane;
-            bulk_prefetch_l2(cub_in + (((long long)b * pl.n3 + z) * N + (4 * yl + r)) * N, (unsigned)(N * sizeof(C)));
+    // box of (plane (bb, zz), quarter rr, x task vv of this warp, half hh) -> this warp's landing zone
+    auto box_issue = [&](int bb, int zz, int rr, int vv, int hh) {
+        if (lane == 0) {
+            mbar_expect_tx(&bar_lz[warp], (unsigned)(R4::LZE * sizeof(C)));
+            r4_lines_box_load(lzone, &cmap, hh, rr, ((bb * pl.n3 + zz) * M) + (warp + vv * NW) * G, &bar_lz[warp]);
         }
     };
-    if (kplanes > 0) lines_prefetch(b, z, 0, 0);
+    // ... and from there into the registers: o0 = x = 4 n' + 2 h, o1 = x = 4 n' + 2 h + 1, n' = t + 8 q
+    auto box_read = [&](C (&o0)[1][8], C (&o1)[1][8]) {
+        mbar_wait(&bar_lz[warp], lz_par);
+        lz_par ^= 1u;
+        // 16-byte elements: half of the lanes take the odd element first, so that the 32-byte-strided 16-byte reads of a
+        // quarter warp fall into different bank groups (8-byte elements: a pair is one 16-byte access)
+        const bool sw = sizeof(C) == 16 && t >= 4;
+        const C *st = lzone + f * (2 * M);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int n = 2 * (t + 8 * q);
+            const C va = st[n + (sw ? 1 : 0)], vb = st[n + (sw ? 0 : 1)];
+            o0[0][q].x = sw ? vb.x : va.x; o0[0][q].y = sw ? vb.y : va.y;
+            o1[0][q].x = sw ? va.x : vb.x; o1[0][q].y = sw ? va.y : vb.y;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp(); // every lane has its values: the landing zone may be refilled
+    };
+    if (kplanes > 0) box_issue(b, z, 0, 0, 0);
 
 #pragma unroll 1
     for (int i = 0; i < kplanes; ++i) {
@@ -442,20 +488,19 @@ plane_r4_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
 #pragma unroll 1
             for (int v = 0; v < XT; ++v) {
                 const int yl = (warp + v * NW) * G + f;
-                const C *rowi = cub_in + (((long long)b * pl.n3 + z) * N + (4 * yl + r)) * N;
-                if (v + 1 < XT) lines_prefetch(b, z, r, v + 1);
-                else if (r < 3) lines_prefetch(b, z, r + 1, 0);
-                else if (more) lines_prefetch(bn, zn, 0, 0);
                 const ExSkew<T, P2, YP> ex{pbuf + yl, true}; // the line's slots are still unused: exchanged in them
                 C o0[1][8], o1[1][8], gq[8], fa[8], fb[8], fc;
-#pragma unroll
-                for (int q = 0; q < 8; ++q) ld_pair(rowi + 4 * (t + 8 * q), o0[0][q], o1[0][q]);
+                box_read(o0, o1);
+                box_issue(b, z, r, v, 1); // the other half of the same lines lands while e = 0, 1 are transformed
                 sub_fwd<F, T>(o0, gq, tws, ex, t);
                 r4_fold_fwd<0, 0, T>(gq, fa, fb, fc, wt[0]);
                 sub_fwd<F, T>(o1, gq, tws, ex, t);
                 r4_fold_fwd<1, 0, T>(gq, fa, fb, fc, wt[1]);
-#pragma unroll
-                for (int q = 0; q < 8; ++q) ld_pair(rowi + 4 * (t + 8 * q) + 2, o0[0][q], o1[0][q]);
+                box_read(o0, o1);
+                // the first half of this warp's next x task: same quarter, next quarter, or the next plane
+                if (v + 1 < XT) box_issue(b, z, r, v + 1, 0);
+                else if (r < 3) box_issue(b, z, r + 1, 0, 0);
+                else if (more) box_issue(bn, zn, 0, 0, 0);
                 sub_fwd<F, T>(o0, gq, tws, ex, t);
                 r4_fold_fwd<2, 0, T>(gq, fa, fb, fc, wt[2]);
                 sub_fwd<F, T>(o1, gq, tws, ex, t);
