@@ -216,6 +216,38 @@ template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
     using F = FastCfg<T, N, P1, P2>;
     return PlaneLaunch{1, {&launch_plane_fast<T, F, MODE_INV>, &launch_plane_fast<T, F, MODE_FWD>, &launch_plane_fast<T, F, MODE_VLOC>}};
 }
+// cuTensorMapEncodeTiled through the runtime (no link against libcuda); looked up once
+typedef CUresult (*tmap_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+tmap_encode_fn tmap_encoder()
+{
+    static const tmap_encode_fn fn = [] {
+        void *f = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            f = nullptr;
+        }
+        return (tmap_encode_fn)f;
+    }();
+    return fn;
+}
+// The cuboids of a call as a tensor of real numbers for the TMA engine (256 pattern, fftb_plane_r4.cuh): an (x, x+1) pair | half of a group
+// of four x | n' = x / 4 | y mod 4 | y / 4 over all planes and bands; a box = one half of the pairs of G = 4 lines four rows apart.
+template <typename T> int r4_cuboid_map(CUtensorMap *cmap, const DevPlan &pl, const void *cuboid, int nb)
+{
+    const tmap_encode_fn enc = tmap_encoder();
+    if (!enc) return FFTB_ECUDA;
+    constexpr cuuint64_t E = sizeof(cx<T>), PAIR = 2 * E / sizeof(T);
+    const cuuint64_t dims[5] = {PAIR, 2, 64, 4, (cuuint64_t)nb * pl.n3 * 64};
+    const cuuint64_t strides[4] = {2 * E, 4 * E, 256 * E, 4 * 256 * E};
+    const cuuint32_t box[5] = {(cuuint32_t)PAIR, 1, 64, 1, (cuuint32_t)PlaneR4<T, 8>::F::G};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    if (enc(cmap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void *>(cuboid), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return FFTB_ECUDA;
+    return 0;
+}
 // the 256 pattern parks per-thread values of the y tasks in tensor memory if every warp's y tasks fit its columns (fftb_plane_r4.cuh)
 template <typename T> bool r4_tasks_fit_tmem(const DevPlan &pl)
 {
@@ -232,7 +264,9 @@ int launch_plane_r4_inv_tm(const DevPlan &pl, const PlanTabs &tabs, const void *
     const int nplanes = pl.n3 * nb;
     int grid = pl.sms;
     if (grid > nplanes) grid = nplanes;
-    k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)Ain, (cx<T> *)cout, sin, nplanes);
+    CUtensorMap cmap;
+    if (int rc = r4_cuboid_map<T>(&cmap, pl, cout, nb)) return rc;
+    k<<<grid, NW * 32, smem, st>>>(pl, tabs.ct4, (const cx<T> *)Ain, (cx<T> *)cout, cmap, sin, nplanes);
     return launch_status();
 }
 // inverse plane kernel of the 256 pattern (fftb_plane_r4.cuh)
@@ -266,22 +300,6 @@ int launch_plane_r4_vloc(const DevPlan &pl, const PlanTabs &tabs, const void *Ai
                                     : launch_plane_r4_vloc_tm<T, false>(pl, tabs, Ain, Aout, v, sin, sout, nb, st);
 }
 
-// cuTensorMapEncodeTiled through the runtime (no link against libcuda); looked up once
-typedef CUresult (*tmap_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
-                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-tmap_encode_fn tmap_encoder()
-{
-    static const tmap_encode_fn fn = [] {
-        void *f = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess) {
-            cudaGetLastError();
-            f = nullptr;
-        }
-        return (tmap_encode_fn)f;
-    }();
-    return fn;
-}
 template <typename T, bool TM>
 int launch_plane_r4_fwd_tm(const DevPlan &pl, const PlanTabs &tabs, const void *cin, void *Aout, long long sout, int nb, cudaStream_t st)
 {
@@ -290,19 +308,8 @@ int launch_plane_r4_fwd_tm(const DevPlan &pl, const PlanTabs &tabs, const void *
     auto k = plane_r4_fwd_k<T, NW, TM>;
     const size_t smem = R4::smem_bytes_fwd;
     if (int rc = kernel_ready(k, NW * 32, smem, nullptr)) return rc;
-    // the cuboids of this call as a tensor of real numbers: an (x, x+1) pair | half of a group of four x | n' = x / 4 |
-    // y mod 4 | y / 4 over all planes and bands; a box = one half of the pairs of G = 4 lines four rows apart (fftb_plane_r4.cuh)
-    const tmap_encode_fn enc = tmap_encoder();
-    if (!enc) return FFTB_ECUDA;
-    constexpr cuuint64_t E = sizeof(cx<T>), PAIR = 2 * E / sizeof(T);
-    const cuuint64_t dims[5] = {PAIR, 2, 64, 4, (cuuint64_t)nb * pl.n3 * 64};
-    const cuuint64_t strides[4] = {2 * E, 4 * E, 256 * E, 4 * 256 * E};
-    const cuuint32_t box[5] = {(cuuint32_t)PAIR, 1, 64, 1, (cuuint32_t)R4::F::G};
-    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     CUtensorMap cmap;
-    if (enc(&cmap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void *>(cin), dims, strides, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return FFTB_ECUDA;
+    if (int rc = r4_cuboid_map<T>(&cmap, pl, cin, nb)) return rc;
     const int nplanes = pl.n3 * nb;
     int grid = pl.sms;
     if (grid > nplanes) grid = nplanes;

@@ -37,10 +37,10 @@ template <typename T, int NW> struct PlaneR4 {
     static constexpr int NCOL = 2 * M + 1, YP = F::YP;
     static constexpr int PB = NCOL * YP;          // one quarter plane
     static constexpr int ZCOL = 2 * M + 4;        // landing zone pitch per column (129 values + alignment slack, 16-byte multiple)
-    static constexpr int ZONE = F::G * ZCOL;      // per warp: the G columns of its next y task
+    static constexpr int ZONE = F::G * ZCOL;      // per warp: the G columns of its next y task (>= LZE: also a staging area, plane_r4_inv_k)
     static constexpr int NXT = M / F::G;          // x tasks per quarter (G lines each)
     static_assert(NXT % NW == 0, "x tasks must divide evenly over the warps");
-    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)PB + (size_t)NW * ZONE);
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)PB + (size_t)NW * ZONE) + 128; // + alignment slack of the zones
     // y tasks (G columns each) per quarter: at most ycol_tasks(NCOL), dealt round-robin over the warps
     static constexpr int MAXT = (((NCOL + 7) / 8 * 8 + F::G - 1) / F::G + NW - 1) / NW;
     // y tasks per warp whose partial sums fit the warp's share of tensor memory (two warps per lane quarter: 256 columns)
@@ -153,10 +153,27 @@ __device__ __forceinline__ void r4_fold_inv(const cx<T> (&a)[8], const cx<T> (&b
     }
 }
 
+// one half (h = 0: e = 0, 1; h = 1: e = 2, 3) of the (x, x+1) pairs of the G lines y = 4 (ylg mod 64 ..+G) + r of a plane:
+// coordinates of the cuboid tensor of plane_r4_fwd_k (built by the launcher): {0, h, 0, r, ylg}, ylg = (band n3 + z) 64 + y / 4
+__device__ __forceinline__ void r4_lines_box_load(void *sdst, const void *tmap, int half, int r, int ylg, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(smem_u32(sdst)),
+                 "l"(tmap), "r"(0), "r"(half), "r"(0), "r"(r), "r"(ylg), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// the same box the other way: shared memory -> cuboid (plane_r4_inv_k; completion by bulk async-group)
+__device__ __forceinline__ void r4_lines_box_store(const void *tmap, int half, int r, int ylg, const void *ssrc)
+{
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4, %5}], [%6];" ::"l"(tmap), "r"(0), "r"(half), "r"(0),
+                 "r"(r), "r"(ylg), "r"(smem_u32(ssrc))
+                 : "memory");
+}
+
 template <typename T, int NW, bool TM>
 __global__ void __launch_bounds__(NW * 32, 1)
 plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab4 ct, const cx<T> *__restrict__ Ain,
-               cx<T> *__restrict__ cub_out, long long a_in_stride, int nplanes)
+               cx<T> *__restrict__ cub_out, const __grid_constant__ CUtensorMap cmap, long long a_in_stride, int nplanes)
 {
     using C = cx<T>;
     using R4 = PlaneR4<T, NW>;
@@ -167,7 +184,11 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
     C *pbuf = reinterpret_cast<C *>(smem_raw); // [NCOL][YP]: column c = k1 - k1lo, line y' of the current quarter
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    C *zone = pbuf + R4::PB + warp * R4::ZONE;  // landing zone of this warp's next y task
+    // landing zone of this warp's next y task; TM: also the staging area of its x tasks (a tensor copy's shared-memory side
+    // must be 128-byte aligned)
+    unsigned char *z_raw = smem_raw + sizeof(C) * (size_t)R4::PB;
+    z_raw += (128u - (smem_u32(z_raw) & 127u)) & 127u;
+    C *zone = reinterpret_cast<C *>(z_raw) + warp * R4::ZONE;
     __shared__ __align__(8) unsigned long long bar_zone[NW];
     unsigned zone_par = 0;
     const C *tw = reinterpret_cast<const C *>(pl.tw1); // exp(+2 pi j i / 256)
@@ -253,8 +274,8 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
                     __syncwarp(); // every lane has its values: the landing zone may be refilled
                     if constexpr (TM) {
                         // the zone is used in quarter 0 only: the next task of this plane, or the first one of the next plane
+                        // (the first task of the next plane is requested when this plane's x tasks have left the zone)
                         if (k + 1 < ytasks_w) zone_issue(row, k + 1);
-                        else if (more) zone_issue(row_of(bn, zn), 0);
                         tmem_put16(tm_warp + (unsigned)(k * tmem_cols16<T>()), a, bq);
                         tmem_wait_st();
                     } else {
@@ -285,6 +306,28 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
         // ================================================== X_r: 64 lines y = 4 y' + r -> cuboid
         // (r is a run-time value: the x phase is most of the code and exists once -- with the four quarters
         // unrolled the kernel outgrows the instruction caches)
+        // TM: the zone is a landing zone in quarter 0's y phase only, so the x tasks stage their results there -- one half
+        // (e = 0, 1 or 2, 3) of the (x, x+1) pairs of the task's four lines, dense [line][n'][pair] -- and ONE tensor copy
+        // scatters them into the cuboid (the tensor of plane_r4_fwd_k): the stores do not hold registers and do not go
+        // through the 32 B/clk store port (0.598 -> 0.584 ms on config 5).  !TM: 32-byte stores from the registers.
+        auto stage_out = [&](const C (&o0)[1][8], const C (&o1)[1][8], int half, int r, int ylg) {
+            if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); // the previous box has left the zone
+            __syncwarp();
+            const bool sw = sizeof(C) == 16 && t >= 4; // see box_read of plane_r4_fwd_k
+            C *st = zone + f * (2 * M);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const int n = 2 * (t + 8 * q);
+                st[n + (sw ? 1 : 0)] = sw ? o1[0][q] : o0[0][q];
+                st[n + (sw ? 0 : 1)] = sw ? o0[0][q] : o1[0][q];
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) {
+                r4_lines_box_store(&cmap, half, r, ylg, zone);
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
+        };
         auto xphase = [&](int r) {
 #pragma unroll 1
             for (int v = 0; v < XT; ++v) {
@@ -299,20 +342,29 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
                 const int cc = M - k1lo;
                 const C cv = (t == 0 && (unsigned)cc < (unsigned)nx) ? pbuf[cc * YP + yl] : czero<T>();
                 C *rowo = cub_out + (((long long)b * pl.n3 + z) * N + (4 * yl + r)) * N;
+                const int ylg = ((b * pl.n3 + z) * M) + (warp + v * NW) * G; // the task's first line, in units of four rows
                 const ExSkew<T, P2, YP> ex{pbuf + yl, true}; // the line's slots are dead: exchanged in them
                 C u[8], o0[1][8], o1[1][8];
                 r4_fold_inv<0, 0, T>(a, bq, cv, u, wt[0]);
                 sub_inv<F, T>(u, o0, tws, ex, t);
                 r4_fold_inv<1, 0, T>(a, bq, cv, u, wt[1]);
                 sub_inv<F, T>(u, o1, tws, ex, t);
+                if constexpr (TM) {
+                    stage_out(o0, o1, 0, r, ylg);
+                } else {
 #pragma unroll
-                for (int q = 0; q < 8; ++q) st_pair(rowo + 4 * (t + 8 * q), o0[0][q], o1[0][q]);
+                    for (int q = 0; q < 8; ++q) st_pair(rowo + 4 * (t + 8 * q), o0[0][q], o1[0][q]);
+                }
                 r4_fold_inv<2, 0, T>(a, bq, cv, u, wt[2]);
                 sub_inv<F, T>(u, o0, tws, ex, t);
                 r4_fold_inv<3, 0, T>(a, bq, cv, u, wt[3]);
                 sub_inv<F, T>(u, o1, tws, ex, t);
+                if constexpr (TM) {
+                    stage_out(o0, o1, 1, r, ylg);
+                } else {
 #pragma unroll
-                for (int q = 0; q < 8; ++q) st_pair(rowo + 4 * (t + 8 * q) + 2, o0[0][q], o1[0][q]);
+                    for (int q = 0; q < 8; ++q) st_pair(rowo + 4 * (t + 8 * q) + 2, o0[0][q], o1[0][q]);
+                }
             }
         };
 #pragma unroll 1
@@ -327,21 +379,21 @@ plane_r4_inv_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTa
             xphase(r);
             __syncthreads();
         }
+        if constexpr (TM) {
+            // the last box of this plane has left the zone: it is a landing zone again
+            if (more && ytasks_w > 0) {
+                if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                __syncwarp();
+                zone_issue(row_of(bn, zn), 0);
+            }
+        }
         z = zn; b = bn;
     }
     if constexpr (TM) {
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); // the boxes have been written
         tmem_publish(); // every warp is done with its columns
         if (warp == 0) tmem_dealloc(tm_slot, 512);
     }
-}
-
-// one half (h = 0: e = 0, 1; h = 1: e = 2, 3) of the (x, x+1) pairs of the G lines y = 4 (ylg mod 64 ..+G) + r of a plane:
-// coordinates of the cuboid tensor of plane_r4_fwd_k (built by the launcher): {0, h, 0, r, ylg}, ylg = (band n3 + z) 64 + y / 4
-__device__ __forceinline__ void r4_lines_box_load(void *sdst, const void *tmap, int half, int r, int ylg, unsigned long long *bar)
-{
-    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(smem_u32(sdst)),
-                 "l"(tmap), "r"(0), "r"(half), "r"(0), "r"(r), "r"(ylg), "r"(smem_u32(bar))
-                 : "memory");
 }
 
 // adjoint of r4_fold_inv: accumulate F[k] = sum_e conj(W^{e k}) G_e[k mod 64] for k = s - 64 (fa), s (fb), +64 (fc)
