@@ -57,7 +57,9 @@ enum fftb_status {
                                unknown enum value, misaligned pointer */
     FFTB_EUNSUPPORTED = -2, /* a description outside the predefined patterns (see fftb_plan_create) */
     FFTB_ENOMEM = -3,       /* host allocation failed, or the bind block is too small */
-    FFTB_ECUDA = -4,        /* a CUDA call or launch failed; sticky until the plan is destroyed */
+    FFTB_ECUDA = -4,        /* a CUDA call or launch failed (this includes the driver's cuTensorMapEncodeTiled, which the
+                               N1 == N2 == 256 kernels and the fused launches need: CUDA 12 drivers have it); sticky until
+                               the plan is destroyed */
     FFTB_ESTATE = -5,       /* execute before fftb_plan_bind, or mismatched plans */
     FFTB_ETOOBIG = -6       /* fftb_inverse_static only: the plan's tables plus one band of its intermediate do not fit in
                                the library's static scratch array (FFTB_STATIC_SCRATCH_BYTES) */
