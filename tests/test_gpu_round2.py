@@ -118,6 +118,31 @@ def test_fused_launch_repeatable(fb):
     p.destroy()
 
 
+@pytest.mark.timeout(300)
+@pytest.mark.parametrize("n,a,dtype,nb", [((256, 256, 128), (64, 64, 32), "c128", 5), ((256, 256, 64), (40, 50, 16), "c64", 6)])
+def test_256_pattern_repeatable(fb, n, a, dtype, nb):
+    """The plane kernels of the 256 pattern park per-thread values in tensor memory, reuse one shared-memory zone as TMA landing
+    zone and staging area and move the cuboid by tensor copies: 12 back-to-back inverse + forward + fused apply calls on one
+    plan, every result bit-identical to the first (a zone refilled or a column of tensor memory rewritten too early would
+    show), and the round trip recovers the input."""
+    w = _w(n, a, batch=nb, dtype=dtype, number=5)
+    p = fb.Plan(w.n, w.cutoff, batch=nb, dtype=dtype).bind()
+    d_c = torch.from_numpy(wl.coefficients(w, *p.points())).cuda()
+    d_v = torch.from_numpy(wl.potential(w)).cuda()
+    psi0 = p.inverse(d_c).clone()
+    rt0 = p.forward(psi0).clone()
+    h0 = p.apply_vloc(d_c, d_v).clone()
+    torch.cuda.synchronize()
+    assert float((rt0 - d_c).abs().max() / d_c.abs().max()) <= (1e-12 if dtype == "c128" else 1e-5)
+    for _ in range(12):
+        psi = p.inverse(d_c)
+        rt = p.forward(psi)
+        h = p.apply_vloc(d_c, d_v)
+        torch.cuda.synchronize()
+        assert torch.equal(psi, psi0) and torch.equal(rt, rt0) and torch.equal(h, h0)
+    p.destroy()
+
+
 # ---------------------------------------------------------------------------------------------------------------
 # stage-level parity: the intermediate A read back through fftb_plan_info.workspace_offset / pitch
 # ---------------------------------------------------------------------------------------------------------------
