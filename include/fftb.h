@@ -93,8 +93,8 @@ typedef struct {
     int64_t n_sticks;     /* occupied (k1,k2) columns */
     int64_t n_xocc;       /* distinct k1 with at least one stick */
     int64_t device_bytes; /* smallest block fftb_plan_bind accepts (tables + workspace) */
-    int64_t device_bytes_host; /* block size that also holds the two staging areas of the *_host calls
-                                  (2 * batch * S elements more) */
+    int64_t device_bytes_host; /* block size that also holds the staging areas of the *_host calls (2 * batch * S
+                                  elements more; 4 * batch * S with FFTB_TUNE_HOST_DEFER) */
     int64_t chunk_bands;  /* bands per kernel group in fftb_inverse (the workspace holds this many) */
     int64_t min_bytes_per_band_dir; /* algorithmic bytes of one band, one direction: (S + C) * elem */
     int64_t workspace_offset; /* byte offset of the plane-major intermediate A inside the bind block */
@@ -120,7 +120,13 @@ enum fftb_tuning_flags {
     FFTB_TUNE_FUSED = 4u,         /* fftb_inverse / fftb_forward as ONE cooperative launch each (z tiles and planes of the whole
                                      batch, the intermediate in an L2-resident ring: 27% less DRAM traffic) where that launch
                                      exists (128^3 grids); measured slower than the separate launches, hence opt-in */
-    FFTB_TUNE_NO_L2_HINTS = 8u    /* fused launches without L2 eviction priorities (ring evict_last, streams evict_first) */
+    FFTB_TUNE_NO_L2_HINTS = 8u,   /* fused launches without L2 eviction priorities (ring evict_last, streams evict_first) */
+    FFTB_TUNE_HOST_DEFER = 16u    /* *_host calls: DEFERRED completion.  A call no longer makes `stream` wait for its own
+                                     device-to-host copies; fftb_host_flush does that for all calls so far.  The plan then
+                                     keeps two incoming and two outgoing staging areas (info.device_bytes_host counts
+                                     them) that successive calls take in turn, so the transforms of call i+1 run while
+                                     the results of call i are still leaving: a sequence of calls is bound by the link
+                                     (both directions busy), not by copies + kernels in a row */
 };
 typedef struct {
     int64_t workspace_bytes; /* budget for the intermediate A inside the bind block (the plan rounds it to whole bands,
@@ -226,11 +232,16 @@ int fftb_apply_vloc(fftb_plan p, const void *d_packed_in, void *d_packed_out, co
  * device-to-host copies of the previous call are still under way (both directions of the link at once).  Ordering:
  *   - a call's OUTPUT is complete in host memory when `stream` reaches the end of the call (work queued later sees it);
  *   - a call's host INPUT is read by copies that are ordered after the previous call's kernels, not after other work
- *     queued on `stream`: its contents must be final when the call is made. */
+ *     queued on `stream`: its contents must be final when the call is made;
+ *   - plans created with FFTB_TUNE_HOST_DEFER: the OUTPUT of a call is complete in host memory only once `stream` has
+ *     passed a later fftb_host_flush (the host array must not be read, reused or freed before that). */
 int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb, void *stream);
 int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb, void *stream);
 int fftb_apply_vloc_host(fftb_plan p, const void *h_packed_in, void *h_packed_out, const void *d_vloc, int nb,
                          void *stream);
+/* Makes `stream` wait for the device-to-host copies of every *_host call made on the plan so far (only enqueues the
+ * waits; a no-op for plans without FFTB_TUNE_HOST_DEFER, whose calls wait themselves).  FFTB_ESTATE before fftb_plan_bind. */
+int fftb_host_flush(fftb_plan p, void *stream);
 
 /* Comparison arm of BASELINE config 5 ("zero-pad the entire sphere ... the 3D
  * Fourier computation is applied on the entire cube"): scatter the packed sphere of `pruned` into the

@@ -18,7 +18,7 @@ FFTB_C64, FFTB_C128 = 0, 1
 FFTB_SCALE_NONE, FFTB_SCALE_FORWARD = 0, 1
 FFTB_FLAG_DENSE = 1
 FFTB_FLAG_BATCH_FASTEST = 2
-FFTB_TUNE_GENERIC_Z, FFTB_TUNE_GENERIC_PLANE, FFTB_TUNE_FUSED, FFTB_TUNE_NO_L2_HINTS = 1, 2, 4, 8
+FFTB_TUNE_GENERIC_Z, FFTB_TUNE_GENERIC_PLANE, FFTB_TUNE_FUSED, FFTB_TUNE_NO_L2_HINTS, FFTB_TUNE_HOST_DEFER = 1, 2, 4, 8, 16
 FFTB_OK, FFTB_EINVAL, FFTB_EUNSUPPORTED, FFTB_ENOMEM, FFTB_ECUDA, FFTB_ESTATE, FFTB_ETOOBIG = 0, -1, -2, -3, -4, -5, -6
 FFTB_STATIC_SCRATCH_BYTES = 16 * 1024 * 1024  # the library-held device array fftb_inverse_static works in
 
@@ -26,7 +26,7 @@ FFTB_STATIC_SCRATCH_BYTES = 16 * 1024 * 1024  # the library-held device array ff
 SYMBOLS = [
     "fftb_plan_create", "fftb_plan_create_tuned", "fftb_plan_create_explicit", "fftb_plan_create_explicit_tuned", "fftb_plan_info_get", "fftb_plan_get_map", "fftb_plan_bind",
     "fftb_inverse", "fftb_inverse_static", "fftb_forward", "fftb_apply_vloc",
-    "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host",
+    "fftb_inverse_host", "fftb_forward_host", "fftb_apply_vloc_host", "fftb_host_flush",
     "fftb_dense_embed", "fftb_dense_extract", "fftb_packed_transpose",
     "fftb_probe_fma", "fftb_probe_store_port", "fftb_plan_last_launches",
     "fftb_slab_plan_create", "fftb_slab_plan_info_get", "fftb_slab_plan_counts", "fftb_slab_plan_bind", "fftb_slab_plan_exchange_ptr",
@@ -83,6 +83,7 @@ def lib():
             getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
         for name in ("fftb_dense_embed", "fftb_dense_extract"):
             getattr(L, name).argtypes = [vp, vp, vp, vp, i32, vp]
+        L.fftb_host_flush.argtypes = [vp, vp]
         L.fftb_packed_transpose.argtypes = [vp, vp, vp, i32, i32, vp]
         L.fftb_probe_fma.argtypes = [i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
         L.fftb_probe_store_port.argtypes = [i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
@@ -289,6 +290,10 @@ class Plan:
                                           self._chk(vloc, (self.n[2], self.n[1], self.n[0]), dtype=self.torch_real),
                                           nb, _stream_ptr(stream)), "fftb_apply_vloc_host")
         return h_out
+
+    def host_flush(self, stream=None):
+        """FFTB_TUNE_HOST_DEFER plans: make the stream wait for the device-to-host copies of all *_host calls so far."""
+        _check(lib().fftb_host_flush(self._h, _stream_ptr(stream)), "fftb_host_flush")
 
     def dense_embed(self, dense_plan, packed, packed_dense=None, stream=None):
         import torch

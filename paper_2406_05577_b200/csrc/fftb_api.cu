@@ -697,7 +697,7 @@ struct fftb_plan_s {
     int ring_ntiles;
     CUtensorMap ring_map; // the ring as a 5-dimensional tensor (inverse plane items load a row out of every tile)
     // device block layout
-    size_t o_stick, o_col, o_perm, o_tw[3], o_sync, o_ws, o_stage, o_stage_out, bytes_min, bytes_stage;
+    size_t o_stick, o_col, o_perm, o_tw[3], o_sync, o_ws, o_stage[2], o_stage_out[2], bytes_min, bytes_stage;
     long long a_inv_stride, a_fwd_stride; // elements per band of the intermediate (a_fwd_stride: vloc and generic forward)
     int chunk;                            // bands per kernel group (vloc: both intermediates live)
     int chunk_inv, chunk_fwd;             // inverse / forward alone
@@ -707,8 +707,12 @@ struct fftb_plan_s {
     // *_host calls: the packed arrays cross PCIe in HOST_PIPE band chunks on two private copy streams, so
     // that a chunk's copy runs while its neighbours are transformed (created once in fftb_plan_bind)
     cudaStream_t cs_in, cs_out;
-    cudaEvent_t hev_in_free, hev_done, hev_in[8], hev_out[8];
-    bool in_free_recorded; // hev_in_free has been recorded at least once
+    cudaEvent_t hev_in_free[2], hev_done[2], hev_in[8], hev_out[8];
+    bool in_free_recorded[2], done_recorded[2]; // the event has been recorded at least once
+    // FFTB_TUNE_HOST_DEFER: two incoming and two outgoing staging areas, taken in turn by successive *_host calls, and no
+    // wait of the caller's stream for a call's device-to-host copies (fftb_host_flush does that)
+    bool host_defer;
+    unsigned host_in_calls, host_out_calls;
     bool pipe_ok;
     DevPlan dev;
     PlanTabs tabs; // the column table again, as a by-value kernel parameter of the fast plane kernels
@@ -766,7 +770,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
     if (!out || !desc) return FFTB_EINVAL;
     *out = nullptr;
     const uint32_t tflags = tune ? tune->flags : 0u;
-    if (tflags & ~(uint32_t)(FFTB_TUNE_GENERIC_Z | FFTB_TUNE_GENERIC_PLANE | FFTB_TUNE_FUSED | FFTB_TUNE_NO_L2_HINTS)) return FFTB_EINVAL;
+    if (tflags & ~(uint32_t)(FFTB_TUNE_GENERIC_Z | FFTB_TUNE_GENERIC_PLANE | FFTB_TUNE_FUSED | FFTB_TUNE_NO_L2_HINTS | FFTB_TUNE_HOST_DEFER)) return FFTB_EINVAL;
     if (tune && (tune->workspace_bytes < 0 || tune->ring_bands < 0 || tune->lead_bands < 0 || tune->z_ctas > 1024)) return FFTB_EINVAL;
     const bool dense = (desc->flags & FFTB_FLAG_DENSE) != 0;
     if (xm && (dense || xm->n < 1 || xm->n > (int64_t)1 << 24 || !xm->k1 || !xm->k2 || !xm->k3lo || !xm->len)) return FFTB_EINVAL;
@@ -855,6 +859,7 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         p->fused = fused;
         p->bf = bf;
         p->l2_hints = (tflags & FFTB_TUNE_NO_L2_HINTS) ? 0 : 1;
+        p->host_defer = (tflags & FFTB_TUNE_HOST_DEFER) != 0;
         p->z_ctas = tune ? (int)tune->z_ctas : 0;
         p->ry = plk.ry;
         const int n1 = desc->n[0], n2 = desc->n[1], n3 = desc->n[2];
@@ -1006,13 +1011,23 @@ static int plan_create_impl(fftb_plan *out, const fftb_plan_desc *desc, const Ex
         p->bytes_min = o;
         // two staging areas of the *_host calls: packed arrays arriving from the host and leaving for it (separate, so that
         // the next call's host-to-device copies run while this call's device-to-host copies are still under way)
-        p->o_stage = o; o = align_up(o + (size_t)desc->batch * (size_t)p->S * p->elem, 256);
-        p->o_stage_out = o; o = align_up(o + (size_t)desc->batch * (size_t)p->S * p->elem, 256);
+        // (FFTB_TUNE_HOST_DEFER: two of each, taken in turn, so that the next call's transforms run while this call's results leave)
+        const size_t area = (size_t)desc->batch * (size_t)p->S * p->elem;
+        p->o_stage[0] = o; o = align_up(o + area, 256);
+        p->o_stage_out[0] = o; o = align_up(o + area, 256);
+        p->o_stage[1] = p->o_stage[0];
+        p->o_stage_out[1] = p->o_stage_out[0];
+        if (p->host_defer) {
+            p->o_stage[1] = o; o = align_up(o + area, 256);
+            p->o_stage_out[1] = o; o = align_up(o + area, 256);
+        }
         p->bytes_stage = o;
         p->d_mem = nullptr;
         p->staging = false;
         p->pipe_ok = false;
-        p->in_free_recorded = false;
+        p->in_free_recorded[0] = p->in_free_recorded[1] = false;
+        p->done_recorded[0] = p->done_recorded[1] = false;
+        p->host_in_calls = p->host_out_calls = 0;
         p->sticky = 0;
         p->launches = 0;
         p->prof = false;
@@ -1114,8 +1129,10 @@ int fftb_plan_bind(fftb_plan p, void *d_mem, size_t bytes, void *stream)
     if (p->staging && !p->pipe_ok) {
         bool ok = cudaStreamCreateWithFlags(&p->cs_in, cudaStreamNonBlocking) == cudaSuccess &&
                   cudaStreamCreateWithFlags(&p->cs_out, cudaStreamNonBlocking) == cudaSuccess &&
-                  cudaEventCreateWithFlags(&p->hev_in_free, cudaEventDisableTiming) == cudaSuccess &&
-                  cudaEventCreateWithFlags(&p->hev_done, cudaEventDisableTiming) == cudaSuccess;
+                  cudaEventCreateWithFlags(&p->hev_in_free[0], cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&p->hev_in_free[1], cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&p->hev_done[0], cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&p->hev_done[1], cudaEventDisableTiming) == cudaSuccess;
         for (int i = 0; i < 8 && ok; ++i)
             ok = cudaEventCreateWithFlags(&p->hev_in[i], cudaEventDisableTiming) == cudaSuccess &&
                  cudaEventCreateWithFlags(&p->hev_out[i], cudaEventDisableTiming) == cudaSuccess;
@@ -1304,19 +1321,49 @@ static int host_chunk_start(fftb_plan p, int nb, int k, int K)
 }
 #define FFTB_CU(call) do { if ((call) != cudaSuccess) { p->sticky = FFTB_ECUDA; return FFTB_ECUDA; } } while (0)
 
-// The incoming staging area may be refilled once the kernels of the previous call that read it are done (not: once
+// The incoming staging area may be refilled once the kernels of the call that read it last are done (not: once
 // everything queued on the caller's stream is done -- that would put this call's host-to-device copies behind the
 // previous call's device-to-host copies, and PCIe would never carry both directions at once).
-static int host_in_begin(fftb_plan p)
+// FFTB_TUNE_HOST_DEFER: successive calls take the two incoming (and the two outgoing) areas in turn.
+static int host_in_area(fftb_plan p) { return p->host_defer ? (int)(p->host_in_calls++ & 1u) : 0; }
+static int host_out_area(fftb_plan p) { return p->host_defer ? (int)(p->host_out_calls++ & 1u) : 0; }
+static int host_in_begin(fftb_plan p, int a)
 {
-    if (p->in_free_recorded) FFTB_CU(cudaStreamWaitEvent(p->cs_in, p->hev_in_free, 0));
+    if (p->in_free_recorded[a]) FFTB_CU(cudaStreamWaitEvent(p->cs_in, p->hev_in_free[a], 0));
     return FFTB_OK;
 }
-static int host_in_end(fftb_plan p, cudaStream_t st)
+static int host_in_end(fftb_plan p, cudaStream_t st, int a)
 {
     if (!p->pipe_ok) return FFTB_OK;
-    FFTB_CU(cudaEventRecord(p->hev_in_free, st));
-    p->in_free_recorded = true;
+    FFTB_CU(cudaEventRecord(p->hev_in_free[a], st));
+    p->in_free_recorded[a] = true;
+    return FFTB_OK;
+}
+// An outgoing area may be rewritten once the device-to-host copies of the call that used it last are done.  Without
+// FFTB_TUNE_HOST_DEFER that is implied (every call ends by making the caller's stream wait for its copies).
+static int host_out_begin(fftb_plan p, cudaStream_t st, int a)
+{
+    if (p->host_defer && p->done_recorded[a]) FFTB_CU(cudaStreamWaitEvent(st, p->hev_done[a], 0));
+    return FFTB_OK;
+}
+// The call completes, in the caller's stream order, when its last chunk is in host memory (which also keeps the outgoing
+// area from being rewritten too early) -- unless completion is deferred to fftb_host_flush.
+static int host_out_end(fftb_plan p, cudaStream_t st, cudaStream_t copies, int a)
+{
+    FFTB_CU(cudaEventRecord(p->hev_done[a], copies));
+    p->done_recorded[a] = true;
+    if (!p->host_defer) FFTB_CU(cudaStreamWaitEvent(st, p->hev_done[a], 0));
+    return FFTB_OK;
+}
+
+int fftb_host_flush(fftb_plan p, void *stream)
+{
+    if (!p) return FFTB_EINVAL;
+    if (p->sticky) return p->sticky;
+    if (!p->d_mem) return FFTB_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int a = 0; a < 2; ++a)
+        if (p->pipe_ok && p->done_recorded[a]) FFTB_CU(cudaStreamWaitEvent(st, p->hev_done[a], 0));
     return FFTB_OK;
 }
 
@@ -1326,15 +1373,16 @@ int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb,
     if (rc) return rc;
     if (!h_packed || !d_cuboid) return FFTB_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned char *stg = p->d_mem + p->o_stage;
+    const int ai = host_in_area(p);
+    unsigned char *stg = p->d_mem + p->o_stage[ai];
     const int K = host_chunks(p, nb);
     const size_t band = (size_t)p->S * p->elem, cband = (size_t)p->C * p->elem;
     if (K == 1) {
         FFTB_CU(cudaMemcpyAsync(stg, h_packed, (size_t)nb * band, cudaMemcpyHostToDevice, st));
         rc = fftb_inverse(p, stg, d_cuboid, nb, stream);
-        return rc ? rc : host_in_end(p, st);
+        return rc ? rc : host_in_end(p, st, ai);
     }
-    if ((rc = host_in_begin(p))) return rc;
+    if ((rc = host_in_begin(p, ai))) return rc;
     int launches = 0;
     for (int k = 0; k < K; ++k) {
         const int b0 = host_chunk_start(p, nb, k, K), b1 = host_chunk_start(p, nb, k + 1, K);
@@ -1347,7 +1395,7 @@ int fftb_inverse_host(fftb_plan p, const void *h_packed, void *d_cuboid, int nb,
         launches += p->launches;
     }
     p->launches = launches;
-    return host_in_end(p, st);
+    return host_in_end(p, st, ai);
 }
 
 int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb, void *stream)
@@ -1356,14 +1404,23 @@ int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb,
     if (rc) return rc;
     if (!h_packed || !d_cuboid) return FFTB_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned char *stg = p->d_mem + p->o_stage_out;
+    const int ao = host_out_area(p);
+    unsigned char *stg = p->d_mem + p->o_stage_out[ao];
     const int K = host_chunks(p, nb);
     const size_t band = (size_t)p->S * p->elem, cband = (size_t)p->C * p->elem;
+    if ((rc = host_out_begin(p, st, ao))) return rc;
     if (K == 1) {
         rc = fftb_forward(p, d_cuboid, stg, nb, stream);
         if (rc) return rc;
-        FFTB_CU(cudaMemcpyAsync(h_packed, stg, (size_t)nb * band, cudaMemcpyDeviceToHost, st));
-        return FFTB_OK;
+        if (!p->host_defer || !p->pipe_ok) {
+            FFTB_CU(cudaMemcpyAsync(h_packed, stg, (size_t)nb * band, cudaMemcpyDeviceToHost, st));
+            return FFTB_OK;
+        }
+        // deferred completion: the copy leaves on the plan's own stream
+        FFTB_CU(cudaEventRecord(p->hev_out[0], st));
+        FFTB_CU(cudaStreamWaitEvent(p->cs_out, p->hev_out[0], 0));
+        FFTB_CU(cudaMemcpyAsync(h_packed, stg, (size_t)nb * band, cudaMemcpyDeviceToHost, p->cs_out));
+        return host_out_end(p, st, p->cs_out, ao);
     }
     int launches = 0;
     for (int k = 0; k < K; ++k) {
@@ -1376,12 +1433,8 @@ int fftb_forward_host(fftb_plan p, const void *d_cuboid, void *h_packed, int nb,
         FFTB_CU(cudaMemcpyAsync((unsigned char *)h_packed + b0 * band, stg + b0 * band, (size_t)(b1 - b0) * band,
                                 cudaMemcpyDeviceToHost, p->cs_out));
     }
-    // the call completes, in the caller's stream order, when the last chunk is in host memory (this also keeps the
-    // outgoing staging area from being rewritten too early)
-    FFTB_CU(cudaEventRecord(p->hev_done, p->cs_out));
-    FFTB_CU(cudaStreamWaitEvent(st, p->hev_done, 0));
     p->launches = launches;
-    return FFTB_OK;
+    return host_out_end(p, st, p->cs_out, ao);
 }
 
 int fftb_apply_vloc_host(fftb_plan p, const void *h_in, void *h_out, const void *d_vloc, int nb, void *stream)
@@ -1390,17 +1443,26 @@ int fftb_apply_vloc_host(fftb_plan p, const void *h_in, void *h_out, const void 
     if (rc) return rc;
     if (!h_in || !h_out) return FFTB_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned char *stg = p->d_mem + p->o_stage, *sto = p->d_mem + p->o_stage_out;
+    const int ai = host_in_area(p), ao = host_out_area(p);
+    unsigned char *stg = p->d_mem + p->o_stage[ai], *sto = p->d_mem + p->o_stage_out[ao];
     const int K = host_chunks(p, nb);
     const size_t band = (size_t)p->S * p->elem;
+    if ((rc = host_out_begin(p, st, ao))) return rc;
     if (K == 1) {
         FFTB_CU(cudaMemcpyAsync(stg, h_in, (size_t)nb * band, cudaMemcpyHostToDevice, st));
         rc = fftb_apply_vloc(p, stg, sto, d_vloc, nb, stream);
         if (rc) return rc;
-        FFTB_CU(cudaMemcpyAsync(h_out, sto, (size_t)nb * band, cudaMemcpyDeviceToHost, st));
-        return host_in_end(p, st);
+        if (!p->host_defer || !p->pipe_ok) {
+            FFTB_CU(cudaMemcpyAsync(h_out, sto, (size_t)nb * band, cudaMemcpyDeviceToHost, st));
+            return host_in_end(p, st, ai);
+        }
+        if ((rc = host_in_end(p, st, ai))) return rc;
+        FFTB_CU(cudaEventRecord(p->hev_out[0], st));
+        FFTB_CU(cudaStreamWaitEvent(p->cs_out, p->hev_out[0], 0));
+        FFTB_CU(cudaMemcpyAsync(h_out, sto, (size_t)nb * band, cudaMemcpyDeviceToHost, p->cs_out));
+        return host_out_end(p, st, p->cs_out, ao);
     }
-    if ((rc = host_in_begin(p))) return rc;
+    if ((rc = host_in_begin(p, ai))) return rc;
     int launches = 0;
     for (int k = 0; k < K; ++k) {
         const int b0 = host_chunk_start(p, nb, k, K), b1 = host_chunk_start(p, nb, k + 1, K);
@@ -1416,11 +1478,9 @@ int fftb_apply_vloc_host(fftb_plan p, const void *h_in, void *h_out, const void 
         FFTB_CU(cudaMemcpyAsync((unsigned char *)h_out + b0 * band, sto + b0 * band, (size_t)(b1 - b0) * band,
                                 cudaMemcpyDeviceToHost, p->cs_out));
     }
-    if ((rc = host_in_end(p, st))) return rc;
-    FFTB_CU(cudaEventRecord(p->hev_done, p->cs_out));
-    FFTB_CU(cudaStreamWaitEvent(st, p->hev_done, 0));
+    if ((rc = host_in_end(p, st, ai))) return rc;
     p->launches = launches;
-    return FFTB_OK;
+    return host_out_end(p, st, p->cs_out, ao);
 }
 
 static int dense_move(fftb_plan pruned, fftb_plan dense, const void *src, void *dst, int nb, void *stream, bool extract)
@@ -1523,8 +1583,7 @@ int fftb_plan_destroy(fftb_plan p)
     if (p->pipe_ok) {
         cudaStreamDestroy(p->cs_in);
         cudaStreamDestroy(p->cs_out);
-        cudaEventDestroy(p->hev_in_free);
-        cudaEventDestroy(p->hev_done);
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(p->hev_in_free[i]); cudaEventDestroy(p->hev_done[i]); }
         for (int i = 0; i < 8; ++i) { cudaEventDestroy(p->hev_in[i]); cudaEventDestroy(p->hev_out[i]); }
     }
     delete p;

@@ -118,6 +118,45 @@ def test_fused_launch_repeatable(fb):
     p.destroy()
 
 
+@pytest.mark.parametrize("dtype,nb", [("c128", 43), ("c64", 43), ("c128", 5)])
+def test_host_calls_with_deferred_completion(fb, oracle, dtype, nb):
+    """FFTB_TUNE_HOST_DEFER: the *_host calls do not make the stream wait for their device-to-host copies and take two
+    incoming / two outgoing staging areas in turn; fftb_host_flush closes them all.  Five calls in a row with DIFFERENT
+    inputs and outputs (more calls than staging areas: an area rewritten before its copies were done would show), then one
+    flush: every output equals what the same plan computes from device pointers, bit for bit, and the oracle within
+    tolerance.  43 bands cross PCIe in chunks, 5 bands in one piece."""
+    w = _w((64, 64, 64), (16, 16, 16), dtype=dtype, batch=nb, number=2)
+    p = fb.Plan(w.n, w.cutoff, batch=nb, dtype=dtype, tuning={"flags": fb.FFTB_TUNE_HOST_DEFER}).bind(host_staging=True)
+    plain = fb.Plan(w.n, w.cutoff, batch=nb, dtype=dtype)
+    assert p.info["device_bytes_host"] - p.info["device_bytes"] >= 2 * (plain.info["device_bytes_host"] - plain.info["device_bytes"]) - 4096
+    plain.destroy()
+    k = p.points()
+    base = wl.coefficients(w, *k)
+    v = wl.potential(w)
+    d_v = torch.from_numpy(v).cuda()
+    ins = [torch.from_numpy(np.ascontiguousarray(base * (1.0 + 0.25 * i))).pin_memory() for i in range(5)]
+    rts = [torch.zeros_like(ins[0]).pin_memory() for _ in range(5)]
+    outs = [torch.zeros_like(ins[0]).pin_memory() for _ in range(5)]
+    psis = [torch.empty(p.cuboid_shape(nb), dtype=p.torch_complex, device="cuda") for _ in range(5)]
+    for i in range(5):
+        p.inverse_host(ins[i], psis[i])
+        p.forward_host(psis[i], rts[i])
+        p.apply_vloc_host(ins[i], outs[i], d_v)
+    p.host_flush()
+    torch.cuda.current_stream().synchronize()
+    for i in range(5):
+        d_c = ins[i].cuda()
+        assert torch.equal(psis[i], p.inverse(d_c))
+        assert torch.equal(rts[i].cuda(), p.forward(psis[i]))
+        assert torch.equal(outs[i].cuda(), p.apply_vloc(d_c, d_v))
+        assert _rel(rts[i].numpy(), ins[i].numpy()) <= w.tol
+    ref = oracle.apply_vloc(w.n, k, ins[3].numpy()[[0, nb - 1]], v, 1.0 / float(np.prod(w.n)))
+    assert _rel(outs[3].numpy()[[0, nb - 1]], ref) <= w.tol
+    p.host_flush()  # a second flush with nothing new is harmless
+    torch.cuda.synchronize()
+    p.destroy()
+
+
 @pytest.mark.timeout(300)
 @pytest.mark.parametrize("n,a,dtype,nb", [((256, 256, 128), (64, 64, 32), "c128", 5), ((256, 256, 64), (40, 50, 16), "c64", 6)])
 def test_256_pattern_repeatable(fb, n, a, dtype, nb):
@@ -251,7 +290,7 @@ def test_generic_kernels_through_tuning_flags(fb, oracle, n, a, dtype, flags):
 
 def test_tuning_is_validated(fb):
     with pytest.raises(fb.FftbError) as e:
-        fb.Plan((64, 64, 64), (16, 16, 16), tuning={"flags": 16})
+        fb.Plan((64, 64, 64), (16, 16, 16), tuning={"flags": 32})  # an unknown flag
     assert e.value.code == fb.FFTB_EINVAL
     with pytest.raises(fb.FftbError) as e:
         fb.Plan((64, 64, 64), (16, 16, 16), tuning={"ring_bands": -1})
