@@ -382,6 +382,22 @@ template <typename T, int N, int P1, int P2> ZLaunch make_z_fast()
 }
 // z passes of the 256 pattern (fftb_plane_r4.cuh)
 constexpr int R4Z_NW = 4;
+// The intermediate of a z-pass launch as a tensor of real numbers for the TMA engine (fftb_zpass_pf.cuh): reals of a row of A | z mod 4 |
+// z / 4 | band; a box = the 128 bytes of SG sticks x 2 consecutive residues x all 64 n' of one band, written / read with the 128-byte swizzle.
+template <typename T> int zr4_a_map(CUtensorMap *amap, const DevPlan &pl, const void *A, long long stride, int nb)
+{
+    const tmap_encode_fn enc = tmap_encoder();
+    if (!enc) return FFTB_ECUDA;
+    constexpr cuuint64_t E = sizeof(cx<T>);
+    const cuuint64_t dims[4] = {(cuuint64_t)pl.pitch * (E / sizeof(T)), 4, 64, (cuuint64_t)nb};
+    const cuuint64_t strides[3] = {(cuuint64_t)pl.pitch * E, 4 * (cuuint64_t)pl.pitch * E, (cuuint64_t)stride * E};
+    const cuuint32_t box[4] = {(cuuint32_t)(128 / sizeof(T)), 2, 64, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    if (enc(amap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<void *>(A), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return FFTB_ECUDA;
+    return 0;
+}
 template <typename T> int launch_zr4_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, long long pk_pitch, cudaStream_t st)
 {
     if (pk_pitch) return FFTB_EUNSUPPORTED;
@@ -390,7 +406,9 @@ template <typename T> int launch_zr4_inv(const DevPlan &pl, const void *packed, 
     const int ntiles = (pl.nsticks + ZP::TS - 1) / ZP::TS, total = ntiles * nb;
     int grid = 0;
     if (int rc = zpers_launch_grid(kp, R4Z_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
-    kp<<<grid, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total);
+    CUtensorMap amap;
+    if (int rc = zr4_a_map<T>(&amap, pl, A, stride, nb)) return rc;
+    kp<<<grid, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, amap, ntiles, total);
     return launch_status();
 }
 template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, long long pk_pitch, cudaStream_t st)
@@ -402,7 +420,9 @@ template <typename T> int launch_zr4_fwd(const DevPlan &pl, const void *A, void 
         const int ntiles = (pl.nsticks + ZP::TS - 1) / ZP::TS, total = ntiles * nb;
         int grid = 0;
         if (int rc = zpers_launch_grid(kp, R4Z_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
-        kp<<<grid, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total);
+        CUtensorMap amap;
+        if (int rc = zr4_a_map<T>(&amap, pl, A, stride, nb)) return rc;
+        kp<<<grid, R4Z_NW * 32, ZP::smem_bytes, st>>>(pl, amap, (cx<T> *)packed, ntiles, total);
         return launch_status();
     }
     auto k = zpass_r4_fwd_k<T, R4Z_NW>;

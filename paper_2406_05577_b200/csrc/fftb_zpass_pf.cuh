@@ -16,6 +16,7 @@
 #pragma once
 #include "fftb_plane_pf.cuh"
 #include "fftb_plane_r4.cuh"
+#include <cuda.h>
 
 namespace fftb {
 
@@ -317,12 +318,43 @@ template <typename T, int NW> struct ZPersR4 {
     static constexpr int N = 256, M = 64, TS = Z::TS;
     static constexpr int EA = 16 / (int)sizeof(cx<T>);
     static constexpr int LZ = TS * (2 * M + 1) + 2 * (EA - 1);
-    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)Z::TILE + (size_t)NW * F::EXW + (size_t)LZ);
+    // The half tile as the TMA engine's 128-byte swizzle lays it out: 2 M rows (n', e & 1) of 128 bytes per group of SG
+    // sticks, the 16-byte piece q of row r at piece q ^ (r mod 8).  A half tile then leaves / arrives as ONE tensor copy per
+    // stick group instead of one bulk copy per row (the TMA unit takes a copy about every 19 cycles: 256 row copies per tile
+    // were most of the tile's time), and the transforms' column accesses -- rows two apart, one stick -- are 2-way instead of
+    // 8-way bank conflicts without any padding.  The tile must be 1024-byte aligned.
+    static constexpr int SG = 128 / (int)sizeof(cx<T>);      // sticks per 128-byte row: 8 (complex128), 16 (complex64)
+    static constexpr int NSG = TS / SG;                      // stick groups (tensor copies) per half tile
+    static_assert(TS % SG == 0, "tile rows must be whole 128-byte pieces");
+    static constexpr int HALF = 2 * M * SG;                  // elements of one stick group's half tile (16 KB)
+    static constexpr int TILE_SW = NSG * HALF;
+    __device__ static __forceinline__ int sw(int r, int sl)  // element index of (row r of the half, stick sl of the tile)
+    {
+        constexpr int PE = 16 / (int)sizeof(cx<T>);          // elements per 16-byte piece
+        const int g = sl / SG, s = sl % SG;
+        return g * HALF + r * SG + ((((s / PE) ^ (r & 7)) * PE) | (s % PE));
+    }
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)TILE_SW + (size_t)NW * F::EXW + (size_t)LZ) + 1024; // + alignment slack
 };
+
+// half tile <-> the rows z = 4 n' + e0, 4 n' + e0 + 1 of the sticks s0 + SG g .. of band `band` in A: coordinates of the tensor
+// the launcher builds over the intermediate (reals of SG sticks | z mod 4 | z / 4 | band), box = {128 bytes, 2, 64, 1}
+__device__ __forceinline__ void zr4_half_store(const void *tmap, int x0, int e0, int band, const void *ssrc)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4}], [%5];" ::"l"(tmap), "r"(x0), "r"(e0), "r"(0), "r"(band),
+                 "r"(smem_u32(ssrc))
+                 : "memory");
+}
+__device__ __forceinline__ void zr4_half_load(void *sdst, const void *tmap, int x0, int e0, int band, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(smem_u32(sdst)),
+                 "l"(tmap), "r"(x0), "r"(e0), "r"(0), "r"(band), "r"(smem_u32(bar))
+                 : "memory");
+}
 
 template <typename T, int NW>
 __global__ void __launch_bounds__(NW * 32, 2)
-zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride,
+zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, const __grid_constant__ CUtensorMap amap,
                     int ntiles, int total)
 {
     using C = cx<T>;
@@ -336,12 +368,13 @@ zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
     // elements from the 16-byte boundary pk at or below it
     const long long mis = (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
     const C *pk = packed - mis;
-    C *tile = reinterpret_cast<C *>(smem_raw);            // half tile: rows (n', e & 1)
-    C *land = tile + Z::TILE + NW * F::EXW;               // packed values of the tile's sticks
+    unsigned char *t_raw = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    C *tile = reinterpret_cast<C *>(t_raw);               // half tile: rows (n', e & 1), 128-byte swizzle (ZPersR4::sw)
+    C *land = tile + ZP::TILE_SW + NW * F::EXW;           // packed values of the tile's sticks
     __shared__ __align__(8) unsigned long long bar;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
+    const ExTile<T, P2> ex{tile + ZP::TILE_SW + warp * F::EXW + f * F::FS};
     const int sl = warp * G + f;
     const C *tw = reinterpret_cast<const C *>(pl.tw3);
     C tws[8], wt[4];
@@ -400,28 +433,29 @@ zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
         }
         const int ic = M - st.y;
         const C cv = (act && t == 0 && (unsigned)ic < (unsigned)st.z) ? fetch(ic) : czero<T>();
-        // the previous tile's second half must have left the tile
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        // the previous tile's second half must have left the tile (thread 0 issued the copies)
+        if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads(); // every thread holds its inputs: the landing zone may be refilled, the tile rewritten
         if (tid == 0 && w + (int)gridDim.x < total) issue(w + (int)gridDim.x);
-        C *dst = A + (long long)band * a_band_stride + s0;
-        const unsigned rbytes = (unsigned)((pl.pitch - s0 < TS ? pl.pitch - s0 : TS) * (int)sizeof(C));
-        // rows z = 4 n' + e0 + (r & 1), n' = r >> 1, of the half in the tile
+        // rows z = 4 n' + e0 + (r & 1), n' = r >> 1, of the half in the tile: one tensor copy per group of SG sticks
         auto send_half = [&](int e0) {
-            for (int r = tid; r < 2 * M; r += NT)
-                bulk_store(dst + (long long)(4 * (r >> 1) + e0 + (r & 1)) * pl.pitch, tile + Z::lin(r, 0), rbytes);
-            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            if (tid == 0) {
+#pragma unroll
+                for (int g = 0; g < ZP::NSG; ++g)
+                    zr4_half_store(&amap, (s0 + g * ZP::SG) * (int)(sizeof(C) / sizeof(T)), e0, band, tile + g * ZP::HALF);
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
         };
         C u[8], y[1][8], y2[1][8];
         r4_fold_inv<0, 0, T>(a, bq, cv, u, wt[0]);
         sub_inv<F, T>(u, y, tws, ex, t);
 #pragma unroll
-        for (int q = 0; q < 8; ++q) tile[Z::lin(2 * (t + 8 * q), sl)] = y[0][q];
+        for (int q = 0; q < 8; ++q) tile[ZP::sw(2 * (t + 8 * q), sl)] = y[0][q];
         r4_fold_inv<1, 0, T>(a, bq, cv, u, wt[1]);
         sub_inv<F, T>(u, y, tws, ex, t);
 #pragma unroll
-        for (int q = 0; q < 8; ++q) tile[Z::lin(2 * (t + 8 * q) + 1, sl)] = y[0][q];
+        for (int q = 0; q < 8; ++q) tile[ZP::sw(2 * (t + 8 * q) + 1, sl)] = y[0][q];
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         send_half(0);
@@ -429,25 +463,25 @@ zpass_r4_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
         sub_inv<F, T>(u, y, tws, ex, t);
         r4_fold_inv<3, 0, T>(a, bq, cv, u, wt[3]);
         sub_inv<F, T>(u, y2, tws, ex, t);
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         __syncthreads(); // the first half has left
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
-            tile[Z::lin(2 * (t + 8 * q), sl)] = y[0][q];
-            tile[Z::lin(2 * (t + 8 * q) + 1, sl)] = y2[0][q];
+            tile[ZP::sw(2 * (t + 8 * q), sl)] = y[0][q];
+            tile[ZP::sw(2 * (t + 8 * q) + 1, sl)] = y2[0][q];
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         send_half(2);
     }
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // forward z pass of the 256 pattern (one plane of A): the rows of the residues e = 0, 1 and e = 2, 3 arrive in the half
 // tile one after the other, each requested as soon as every thread holds the values of the half before it
 template <typename T, int NW>
 __global__ void __launch_bounds__(NW * 32, 2)
-zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride,
+zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ CUtensorMap amap, cx<T> *__restrict__ packed,
                     int ntiles, int total)
 {
     using C = cx<T>;
@@ -461,12 +495,13 @@ zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
     // elements from the 16-byte boundary pk at or below it
     const long long mis = (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
     C *pk = packed - mis;
-    C *tile = reinterpret_cast<C *>(smem_raw);            // half tile: rows (n', e & 1)
-    C *land = tile + Z::TILE + NW * F::EXW;               // results of the tile's sticks in packed order
+    unsigned char *t_raw = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    C *tile = reinterpret_cast<C *>(t_raw);               // half tile: rows (n', e & 1), 128-byte swizzle (ZPersR4::sw)
+    C *land = tile + ZP::TILE_SW + NW * F::EXW;           // results of the tile's sticks in packed order
     __shared__ __align__(8) unsigned long long bar;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
+    const ExTile<T, P2> ex{tile + ZP::TILE_SW + warp * F::EXW + f * F::FS};
     const int sl = warp * G + f;
     const C *tw = reinterpret_cast<const C *>(pl.tw3);
     C tws[8], wt[4];
@@ -477,15 +512,15 @@ zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
     for (int e = 0; e < 4; ++e) wt[e] = tw[e * t];
     const T scale = (T)pl.scale;
 
-    auto ncol_of = [&](int w) { const int s0 = (w % ntiles) * TS; return pl.pitch - s0 < TS ? pl.pitch - s0 : TS; };
-    // thread 0 announces the bytes of a half of tile w, then (after a CTA barrier) every thread asks for its rows
-    auto expect = [&](int w) { mbar_expect_tx(&bar, (unsigned)(2 * M * ncol_of(w) * (int)sizeof(C))); };
+    // thread 0 announces the bytes of a half of tile w and asks for it: one tensor copy per group of SG sticks
     auto issue_half = [&](int w, int e0) {
-        const int band = w / ntiles, s0 = (w % ntiles) * TS;
-        const C *src = A + (long long)band * a_band_stride + s0;
-        const unsigned bytes = (unsigned)(ncol_of(w) * (int)sizeof(C));
-        for (int r = tid; r < 2 * M; r += NT)
-            bulk_load(tile + Z::lin(r, 0), src + (long long)(4 * (r >> 1) + e0 + (r & 1)) * pl.pitch, bytes, &bar);
+        if (tid == 0) {
+            const int band = w / ntiles, s0 = (w % ntiles) * TS;
+            mbar_expect_tx(&bar, (unsigned)(ZP::TILE_SW * sizeof(C)));
+#pragma unroll
+            for (int g = 0; g < ZP::NSG; ++g)
+                zr4_half_load(tile + g * ZP::HALF, &amap, (s0 + g * ZP::SG) * (int)(sizeof(C) / sizeof(T)), e0, band, &bar);
+        }
     };
     if (tid == 0) {
         mbar_init(&bar, 1);
@@ -493,11 +528,7 @@ zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
     }
     __syncthreads();
     int w = blockIdx.x;
-    if (w < total) {
-        if (tid == 0) expect(w);
-        __syncthreads();
-        issue_half(w, 0);
-    }
+    if (w < total) issue_half(w, 0);
     unsigned par = 0;
 #pragma unroll 1
     for (; w < total; w += gridDim.x) {
@@ -514,10 +545,9 @@ zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
         par ^= 1u;
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
-            y[0][q] = tile[Z::lin(2 * (t + 8 * q), sl)];
-            y2[0][q] = tile[Z::lin(2 * (t + 8 * q) + 1, sl)];
+            y[0][q] = tile[ZP::sw(2 * (t + 8 * q), sl)];
+            y2[0][q] = tile[ZP::sw(2 * (t + 8 * q) + 1, sl)];
         }
-        if (tid == 0) expect(w);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads(); // every thread holds its values: the other half of the rows may land
         issue_half(w, 2);
@@ -530,14 +560,11 @@ zpass_r4_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict_
         par ^= 1u;
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
-            y[0][q] = tile[Z::lin(2 * (t + 8 * q), sl)];
-            y2[0][q] = tile[Z::lin(2 * (t + 8 * q) + 1, sl)];
+            y[0][q] = tile[ZP::sw(2 * (t + 8 * q), sl)];
+            y2[0][q] = tile[ZP::sw(2 * (t + 8 * q) + 1, sl)];
         }
         // the previous tile's packed store must have read the landing zone before it is rewritten
-        if (tid == 0) {
-            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-            if (more) expect(w + (int)gridDim.x);
-        }
+        if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         if (more) issue_half(w + (int)gridDim.x, 0);
