@@ -157,6 +157,22 @@ struct FusedLaunch {
                int lead, int nz, int hints, int *sync, cudaStream_t);
 };
 
+// cuTensorMapEncodeTiled through the runtime (no link against libcuda); looked up once
+typedef CUresult (*tmap_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+tmap_encode_fn tmap_encoder()
+{
+    static const tmap_encode_fn fn = [] {
+        void *f = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            f = nullptr;
+        }
+        return (tmap_encode_fn)f;
+    }();
+    return fn;
+}
 template <typename T, class AZ> int launch_zinv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, long long pk_pitch, cudaStream_t st)
 {
     if (pk_pitch) return FFTB_EUNSUPPORTED;
@@ -215,22 +231,6 @@ template <typename T, int N, int P1, int P2> PlaneLaunch make_plane_fast()
 {
     using F = FastCfg<T, N, P1, P2>;
     return PlaneLaunch{1, {&launch_plane_fast<T, F, MODE_INV>, &launch_plane_fast<T, F, MODE_FWD>, &launch_plane_fast<T, F, MODE_VLOC>}};
-}
-// cuTensorMapEncodeTiled through the runtime (no link against libcuda); looked up once
-typedef CUresult (*tmap_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
-                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-tmap_encode_fn tmap_encoder()
-{
-    static const tmap_encode_fn fn = [] {
-        void *f = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess) {
-            cudaGetLastError();
-            f = nullptr;
-        }
-        return (tmap_encode_fn)f;
-    }();
-    return fn;
 }
 // The cuboids of a call as a tensor of real numbers for the TMA engine (256 pattern, fftb_plane_r4.cuh): an (x, x+1) pair | half of a group
 // of four x | n' = x / 4 | y mod 4 | y / 4 over all planes and bands; a box = one half of the pairs of G = 4 lines four rows apart.
@@ -346,6 +346,22 @@ template <class K> int zpers_launch_grid(K kp, int threads, size_t smem, const D
     return 0;
 }
 
+// The intermediate of a z-pass launch as a tensor of real numbers for the TMA engine (fftb_zpass_pf.cuh): reals of a row of A | z | band; a box
+// = the 128 bytes of SG sticks x all N3 rows of one band, written / read with the 128-byte swizzle.
+template <typename T> int z_a_map(CUtensorMap *amap, const DevPlan &pl, const void *A, long long stride, int nb)
+{
+    const tmap_encode_fn enc = tmap_encoder();
+    if (!enc) return FFTB_ECUDA;
+    constexpr cuuint64_t E = sizeof(cx<T>);
+    const cuuint64_t dims[3] = {(cuuint64_t)pl.pitch * (E / sizeof(T)), (cuuint64_t)pl.n3, (cuuint64_t)nb};
+    const cuuint64_t strides[2] = {(cuuint64_t)pl.pitch * E, (cuuint64_t)(stride > 0 ? stride : (long long)pl.n3 * pl.pitch) * E};
+    const cuuint32_t box[3] = {(cuuint32_t)(128 / sizeof(T)), (cuuint32_t)pl.n3, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    if (enc(amap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void *>(A), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return FFTB_ECUDA;
+    return 0;
+}
 template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const void *packed, void *A, long long stride, int nb, long long pk_pitch, cudaStream_t st)
 {
     // persistent kernel, global memory moved by the TMA engine only (batch-fastest packed arrays: per-element cp.async)
@@ -354,7 +370,9 @@ template <typename T, class F> int launch_zfast_inv(const DevPlan &pl, const voi
     auto kp = pk_pitch ? zpass_pers_inv_k<T, F, FAST_NW, true> : zpass_pers_inv_k<T, F, FAST_NW, false>;
     int grid = 0;
     if (int rc = zpers_launch_grid(kp, FAST_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
-    kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, (cx<T> *)A, stride, ntiles, total, pk_pitch);
+    CUtensorMap amap;
+    if (int rc = z_a_map<T>(&amap, pl, A, stride, nb)) return rc;
+    kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)packed, amap, ntiles, total, pk_pitch);
     return launch_status();
 }
 template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const void *A, void *packed, long long stride, int nb, long long pk_pitch, cudaStream_t st)
@@ -365,7 +383,9 @@ template <typename T, class F> int launch_zfast_fwd(const DevPlan &pl, const voi
         auto kp = pk_pitch ? zpass_pers_fwd_k<T, F, FAST_NW, true> : zpass_pers_fwd_k<T, F, FAST_NW, false>;
         int grid = 0;
         if (int rc = zpers_launch_grid(kp, FAST_NW * 32, ZP::smem_bytes, pl, total, &grid)) return rc;
-        kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, (const cx<T> *)A, (cx<T> *)packed, stride, ntiles, total, pk_pitch);
+        CUtensorMap amap;
+        if (int rc = z_a_map<T>(&amap, pl, A, stride, nb)) return rc;
+        kp<<<grid, FAST_NW * 32, ZP::smem_bytes, st>>>(pl, amap, (cx<T> *)packed, ntiles, total, pk_pitch);
         return launch_status();
     }
     if (pk_pitch) return FFTB_EUNSUPPORTED;

@@ -24,9 +24,41 @@ template <typename T, class F, int NW> struct ZPers {
     using Z = ZFast<T, F, NW>;
     static constexpr int EA = 16 / (int)sizeof(cx<T>);      // elements per 16 bytes, the granularity of a bulk copy
     static constexpr int LZ = Z::TS * (F::M + 1) + 2 * (EA - 1); // landing zone: TS sticks of at most M + 1 values (+ alignment slack)
-    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)Z::TILE + (size_t)NW * F::EXW + (size_t)LZ);
+    // The tile as the TMA engine's 128-byte swizzle lays it out: per group of SG sticks, N rows (z) of 128 bytes, the 16-byte
+    // piece q of row z at piece q ^ (z mod 8).  A tile then leaves / arrives as ONE tensor copy per stick group instead of one
+    // bulk copy per z row (the TMA unit takes a copy about every 19 cycles; measured on the 256 pattern, where twice the
+    // copies cost 29% and this layout gained 16%), and the transforms' column accesses -- rows two apart, one stick -- stay at
+    // most 2-way bank conflicts without padding.  The tile must be 1024-byte aligned.
+    static constexpr int SG = 128 / (int)sizeof(cx<T>);      // sticks per 128-byte row: 8 (complex128), 16 (complex64)
+    static constexpr int NSG = Z::TS / SG;                   // stick groups (tensor copies) per tile
+    static_assert(Z::TS % SG == 0, "tile rows must be whole 128-byte pieces");
+    static constexpr int GROUP = F::N * SG;                  // elements of one stick group's part of the tile
+    static constexpr int TILE_SW = NSG * GROUP;
+    __device__ static __forceinline__ int sw(int z, int sl)  // element index of (row z, stick sl of the tile)
+    {
+        constexpr int PE = 16 / (int)sizeof(cx<T>);          // elements per 16-byte piece
+        const int g = sl / SG, s = sl % SG;
+        return g * GROUP + z * SG + ((((s / PE) ^ (z & 7)) * PE) | (s % PE));
+    }
+    static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)TILE_SW + (size_t)NW * F::EXW + (size_t)LZ) + 1024; // + alignment slack
     static constexpr int CTAS_PER_SM = F::P1 > 16 ? 2 : 3;
 };
+
+// tile <-> all N3 rows of the sticks x0 / 2 .. of band `band` in A: coordinates of the tensor the launcher builds over the
+// intermediate (reals of a row of A | z | band), box = {128 bytes, N3, 1}, 128-byte swizzle
+__device__ __forceinline__ void ztile_store(const void *tmap, int x0, int band, const void *ssrc)
+{
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tmap), "r"(x0), "r"(0), "r"(band),
+                 "r"((unsigned)__cvta_generic_to_shared(ssrc))
+                 : "memory");
+}
+__device__ __forceinline__ void ztile_load(void *sdst, const void *tmap, int x0, int band, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                     (unsigned)__cvta_generic_to_shared(sdst)),
+                 "l"(tmap), "r"(x0), "r"(0), "r"(band), "r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
 
 // Batch-fastest packed arrays (BF; Fig. 8 "b x y z": the band index is the fastest one, element
 // [point][band] with `pk_pitch` bands per point): the packed range of a tile is no contiguous run of memory any more but
@@ -52,11 +84,12 @@ __device__ __forceinline__ void cp_async_arrive(unsigned long long *bar)
 
 template <typename T, class F, int NW, bool BF>
 __global__ void __launch_bounds__(NW * 32, ZPers<T, F, NW>::CTAS_PER_SM)
-zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, cx<T> *__restrict__ A, long long a_band_stride,
+zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ packed, const __grid_constant__ CUtensorMap amap,
                  int ntiles, int total, long long pk_pitch)
 {
     using C = cx<T>;
     using Z = ZFast<T, F, NW>;
+    using ZP = ZPers<T, F, NW>;
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
     constexpr long long EA = BF ? 1 : ZPers<T, F, NW>::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -64,12 +97,13 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
     // elements from the 16-byte boundary pk at or below it
     const long long mis = BF ? 0 : (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
     const C *pk = packed - mis;
-    C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
-    C *land = tile + Z::TILE + NW * F::EXW;               // packed values of the tile's sticks
+    unsigned char *t_raw = smem_raw + ((1024u - ((unsigned)__cvta_generic_to_shared(smem_raw) & 1023u)) & 1023u);
+    C *tile = reinterpret_cast<C *>(t_raw);               // [stick group][N][SG], 128-byte swizzle (ZPers::sw)
+    C *land = tile + ZP::TILE_SW + NW * F::EXW;           // packed values of the tile's sticks
     __shared__ __align__(8) unsigned long long bar;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
+    const ExTile<T, P2> ex{tile + ZP::TILE_SW + warp * F::EXW + f * F::FS};
     const int sl = warp * G + f;
     const C *tw = reinterpret_cast<const C *>(pl.tw3);
     C tws[P1];
@@ -148,8 +182,8 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
         }
         const int idb = M / 2 - st.y;
         const C bv = (act && t == 0 && (unsigned)idb < (unsigned)st.z) ? fetch(idb) : czero<T>();
-        // the previous tile's bulk stores must have read the tile before it is overwritten
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        // the previous tile's tensor copies (thread 0's) must have read the tile before it is overwritten
+        if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads(); // every thread holds its inputs: the landing zone may be refilled, the tile rewritten
         if (more) issue(nxt);
@@ -161,23 +195,26 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
 #pragma unroll
         for (int bb = 0; bb < B2; ++bb)
 #pragma unroll
-            for (int q = 0; q < P2; ++q) tile[Z::lin(2 * ((t + P2 * bb) + P1 * q), sl)] = y[bb][q];
+            for (int q = 0; q < P2; ++q) tile[ZP::sw(2 * ((t + P2 * bb) + P1 * q), sl)] = y[bb][q];
         x[P1 / 2] = csub(x[P1 / 2], bv);
         pre_inv<F, 0, T>(x, g);
         sub_inv<F, T>(x, y, tws, ex, t);
 #pragma unroll
         for (int bb = 0; bb < B2; ++bb)
 #pragma unroll
-            for (int q = 0; q < P2; ++q) tile[Z::lin(2 * ((t + P2 * bb) + P1 * q) + 1, sl)] = y[bb][q];
+            for (int q = 0; q < P2; ++q) tile[ZP::sw(2 * ((t + P2 * bb) + P1 * q) + 1, sl)] = y[bb][q];
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
-        C *dst = A + (long long)band * a_band_stride + s0;
-        const int ncol = pl.pitch - s0 < TS ? pl.pitch - s0 : TS;
-        for (int z = tid; z < N; z += NT) bulk_store(dst + (long long)z * pl.pitch, tile + Z::lin(z, 0), (unsigned)(ncol * sizeof(C)));
-        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        // one tensor copy per group of SG sticks (groups beyond the row pitch do not exist)
+        if (tid == 0) {
+#pragma unroll
+            for (int gq = 0; gq < ZP::NSG; ++gq)
+                if (s0 + gq * ZP::SG < pl.pitch) ztile_store(&amap, (s0 + gq * ZP::SG) * (int)(sizeof(C) / sizeof(T)), band, tile + gq * ZP::GROUP);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
         cur = nxt;
     }
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // Forward (F5 z-DFT keeping the stick's k3, scale, F6 pack): the N rows A[z][s0 .. s0 + TS) of the next tile are
@@ -186,11 +223,12 @@ zpass_pers_inv_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ p
 // or (BF) as per-element stores into the batch-fastest array.  Only for one plane of A (ry == 1).
 template <typename T, class F, int NW, bool BF>
 __global__ void __launch_bounds__(NW * 32, ZPers<T, F, NW>::CTAS_PER_SM)
-zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A, cx<T> *__restrict__ packed, long long a_band_stride,
+zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const __grid_constant__ CUtensorMap amap, cx<T> *__restrict__ packed,
                  int ntiles, int total, long long pk_pitch)
 {
     using C = cx<T>;
     using Z = ZFast<T, F, NW>;
+    using ZP = ZPers<T, F, NW>;
     constexpr int N = F::N, M = F::M, P1 = F::P1, P2 = F::P2, B2 = F::B2, G = F::G, TS = Z::TS, NT = NW * 32;
     constexpr long long EA = BF ? 1 : ZPers<T, F, NW>::EA;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -198,12 +236,13 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
     // elements from the 16-byte boundary pk at or below it
     const long long mis = BF ? 0 : (long long)(((unsigned long long)packed / sizeof(C)) & (unsigned long long)(EA - 1));
     C *pk = packed - mis;
-    C *tile = reinterpret_cast<C *>(smem_raw);            // [N/2][RP], Z::lin
-    C *land = tile + Z::TILE + NW * F::EXW;               // results of the tile's sticks in packed order
+    unsigned char *t_raw = smem_raw + ((1024u - ((unsigned)__cvta_generic_to_shared(smem_raw) & 1023u)) & 1023u);
+    C *tile = reinterpret_cast<C *>(t_raw);               // [stick group][N][SG], 128-byte swizzle (ZPers::sw)
+    C *land = tile + ZP::TILE_SW + NW * F::EXW;           // results of the tile's sticks in packed order
     __shared__ __align__(8) unsigned long long bar;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int f = lane / P2, t = lane % P2;
-    const ExTile<T, P2> ex{tile + Z::TILE + warp * F::EXW + f * F::FS};
+    const ExTile<T, P2> ex{tile + ZP::TILE_SW + warp * F::EXW + f * F::FS};
     const int sl = warp * G + f;
     const C *tw = reinterpret_cast<const C *>(pl.tw3);
     C tws[P1];
@@ -216,14 +255,19 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
     auto band_of = [&](int w) { return BF ? w % nbands : w / ntiles; };
     auto s0_of = [&](int w) { return (BF ? w / nbands : w % ntiles) * TS; };
 
-    auto ncol_of = [&](int s0) { return pl.pitch - s0 < TS ? pl.pitch - s0 : TS; };
-    // thread 0 announces the bytes of tile w, then (after a CTA barrier) every thread asks for its rows
-    auto expect = [&](int w) { mbar_expect_tx(&bar, (unsigned)(N * ncol_of(s0_of(w)) * (int)sizeof(C))); };
+    // thread 0 announces the bytes of tile w and asks for it: one tensor copy per group of SG sticks (groups beyond the row
+    // pitch do not exist; their part of the tile is never looked at by an active stick)
     auto issue_rows = [&](int w) {
-        const int band = band_of(w), s0 = s0_of(w);
-        const C *src = A + (long long)band * a_band_stride + s0;
-        const unsigned bytes = (unsigned)(ncol_of(s0) * (int)sizeof(C));
-        for (int z = tid; z < N; z += NT) bulk_load(tile + Z::lin(z, 0), src + (long long)z * pl.pitch, bytes, &bar);
+        if (tid == 0) {
+            const int band = band_of(w), s0 = s0_of(w);
+            int ng = 0;
+#pragma unroll
+            for (int gq = 0; gq < ZP::NSG; ++gq) ng += (s0 + gq * ZP::SG < pl.pitch) ? 1 : 0;
+            mbar_expect_tx(&bar, (unsigned)(ng * ZP::GROUP * (int)sizeof(C)));
+#pragma unroll
+            for (int gq = 0; gq < ZP::NSG; ++gq)
+                if (s0 + gq * ZP::SG < pl.pitch) ztile_load(tile + gq * ZP::GROUP, &amap, (s0 + gq * ZP::SG) * (int)(sizeof(C) / sizeof(T)), band, &bar);
+        }
     };
     if (tid == 0) {
         mbar_init(&bar, 1);
@@ -231,11 +275,7 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
     }
     __syncthreads();
     int w = blockIdx.x;
-    if (w < total) {
-        if (tid == 0) expect(w);
-        __syncthreads();
-        issue_rows(w);
-    }
+    if (w < total) issue_rows(w);
     unsigned par = 0;
 #pragma unroll 1
     for (; w < total; w += gridDim.x) {
@@ -257,13 +297,12 @@ zpass_pers_fwd_k(const __grid_constant__ DevPlan pl, const cx<T> *__restrict__ A
         for (int bb = 0; bb < B2; ++bb)
 #pragma unroll
             for (int q = 0; q < P2; ++q) {
-                y[bb][q] = tile[Z::lin(2 * ((t + P2 * bb) + P1 * q), sl)];
-                y1[bb][q] = tile[Z::lin(2 * ((t + P2 * bb) + P1 * q) + 1, sl)];
+                y[bb][q] = tile[ZP::sw(2 * ((t + P2 * bb) + P1 * q), sl)];
+                y1[bb][q] = tile[ZP::sw(2 * ((t + P2 * bb) + P1 * q) + 1, sl)];
             }
         // the previous tile's packed store must have read the landing zone before it is rewritten
         if (tid == 0) {
             if constexpr (!BF) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-            if (more) expect(w + (int)gridDim.x);
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads(); // every thread holds its tile values: the next tile's rows may land
