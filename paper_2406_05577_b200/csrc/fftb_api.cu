@@ -346,18 +346,20 @@ template <class K> int zpers_launch_grid(K kp, int threads, size_t smem, const D
     return 0;
 }
 
-// The intermediate of a z-pass launch as a tensor of real numbers for the TMA engine (fftb_zpass_pf.cuh): reals of a row of A | z | band; a box
-// = the 128 bytes of SG sticks x all N3 rows of one band, written / read with the 128-byte swizzle.
+// The intermediate of a z-pass launch as a tensor of real numbers for the TMA engine (fftb_zpass_pf.cuh): reals of a row of A | (z / 2) mod 8 |
+// z / 16 | z mod 2 | band; a box = the 128 bytes of SG sticks x all N3 rows of one band (in that order), written / read with the 128-byte swizzle.
 template <typename T> int z_a_map(CUtensorMap *amap, const DevPlan &pl, const void *A, long long stride, int nb)
 {
     const tmap_encode_fn enc = tmap_encoder();
     if (!enc) return FFTB_ECUDA;
     constexpr cuuint64_t E = sizeof(cx<T>);
-    const cuuint64_t dims[3] = {(cuuint64_t)pl.pitch * (E / sizeof(T)), (cuuint64_t)pl.n3, (cuuint64_t)nb};
-    const cuuint64_t strides[2] = {(cuuint64_t)pl.pitch * E, (cuuint64_t)(stride > 0 ? stride : (long long)pl.n3 * pl.pitch) * E};
-    const cuuint32_t box[3] = {(cuuint32_t)(128 / sizeof(T)), (cuuint32_t)pl.n3, 1};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    if (enc(amap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void *>(A), dims, strides, box, estr,
+    const cuuint64_t row = (cuuint64_t)pl.pitch * E;
+    const cuuint64_t dims[5] = {(cuuint64_t)pl.pitch * (E / sizeof(T)), 8, (cuuint64_t)pl.n3 / 16, 2, (cuuint64_t)nb};
+    const cuuint64_t strides[4] = {2 * row, 16 * row, row, (cuuint64_t)(stride > 0 ? stride : (long long)pl.n3 * pl.pitch) * E};
+    const cuuint32_t box[5] = {(cuuint32_t)(128 / sizeof(T)), 8, (cuuint32_t)(pl.n3 / 16), 2, 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    if (pl.n3 % 16) return FFTB_EUNSUPPORTED;
+    if (enc(amap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void *>(A), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return FFTB_ECUDA;
     return 0;
@@ -402,18 +404,19 @@ template <typename T, int N, int P1, int P2> ZLaunch make_z_fast()
 }
 // z passes of the 256 pattern (fftb_plane_r4.cuh)
 constexpr int R4Z_NW = 4;
-// The intermediate of a z-pass launch as a tensor of real numbers for the TMA engine (fftb_zpass_pf.cuh): reals of a row of A | z mod 4 |
-// z / 4 | band; a box = the 128 bytes of SG sticks x 2 consecutive residues x all 64 n' of one band, written / read with the 128-byte swizzle.
+// The intermediate of a z-pass launch as a tensor of real numbers for the TMA engine (fftb_zpass_pf.cuh): reals of a row of A | n' mod 8 | n' / 8 |
+// z mod 4 | band (z = 4 n' + e); a box = the 128 bytes of SG sticks x all 64 n' x 2 consecutive residues of one band, written / read with the 128-byte swizzle.
 template <typename T> int zr4_a_map(CUtensorMap *amap, const DevPlan &pl, const void *A, long long stride, int nb)
 {
     const tmap_encode_fn enc = tmap_encoder();
     if (!enc) return FFTB_ECUDA;
     constexpr cuuint64_t E = sizeof(cx<T>);
-    const cuuint64_t dims[4] = {(cuuint64_t)pl.pitch * (E / sizeof(T)), 4, 64, (cuuint64_t)nb};
-    const cuuint64_t strides[3] = {(cuuint64_t)pl.pitch * E, 4 * (cuuint64_t)pl.pitch * E, (cuuint64_t)stride * E};
-    const cuuint32_t box[4] = {(cuuint32_t)(128 / sizeof(T)), 2, 64, 1};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    if (enc(amap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<void *>(A), dims, strides, box, estr,
+    const cuuint64_t row = (cuuint64_t)pl.pitch * E;
+    const cuuint64_t dims[5] = {(cuuint64_t)pl.pitch * (E / sizeof(T)), 8, 8, 4, (cuuint64_t)nb};
+    const cuuint64_t strides[4] = {4 * row, 32 * row, row, (cuuint64_t)(stride > 0 ? stride : (long long)pl.n3 * pl.pitch) * E};
+    const cuuint32_t box[5] = {(cuuint32_t)(128 / sizeof(T)), 8, 8, 2, 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    if (enc(amap, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void *>(A), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return FFTB_ECUDA;
     return 0;

@@ -34,29 +34,35 @@ template <typename T, class F, int NW> struct ZPers {
     static_assert(Z::TS % SG == 0, "tile rows must be whole 128-byte pieces");
     static constexpr int GROUP = F::N * SG;                  // elements of one stick group's part of the tile
     static constexpr int TILE_SW = NSG * GROUP;
+    // Row order inside a stick group: the transforms touch the rows z = 2 (t + P2 b + P1 q) + e of one stick with the lanes t
+    // of a group side by side, so the tensor the launcher describes splits z into (z / 2) mod 8 | z / 16 | z mod 2 and the
+    // box puts (z / 2) mod 8 FASTEST: the 8 (or 4) lanes then hit rows whose low three bits -- what the swizzle XORs into the
+    // piece index -- all differ: conflict-free column accesses.
+    static_assert(F::N % 16 == 0, "z axis must be a multiple of 16");
+    __device__ static __forceinline__ int row(int z) { return ((z & 1) * (F::N / 16) + (z >> 4)) * 8 + ((z >> 1) & 7); }
     __device__ static __forceinline__ int sw(int z, int sl)  // element index of (row z, stick sl of the tile)
     {
         constexpr int PE = 16 / (int)sizeof(cx<T>);          // elements per 16-byte piece
-        const int g = sl / SG, s = sl % SG;
-        return g * GROUP + z * SG + ((((s / PE) ^ (z & 7)) * PE) | (s % PE));
+        const int g = sl / SG, s = sl % SG, r = row(z);
+        return g * GROUP + r * SG + ((((s / PE) ^ (r & 7)) * PE) | (s % PE));
     }
     static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)TILE_SW + (size_t)NW * F::EXW + (size_t)LZ) + 1024; // + alignment slack
     static constexpr int CTAS_PER_SM = F::P1 > 16 ? 2 : 3;
 };
 
 // tile <-> all N3 rows of the sticks x0 / 2 .. of band `band` in A: coordinates of the tensor the launcher builds over the
-// intermediate (reals of a row of A | z | band), box = {128 bytes, N3, 1}, 128-byte swizzle
+// intermediate (reals of a row of A | (z / 2) mod 8 | z / 16 | z mod 2 | band), box = {128 bytes, 8, N3 / 16, 2, 1}, 128-byte swizzle
 __device__ __forceinline__ void ztile_store(const void *tmap, int x0, int band, const void *ssrc)
 {
-    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tmap), "r"(x0), "r"(0), "r"(band),
-                 "r"((unsigned)__cvta_generic_to_shared(ssrc))
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4, %5}], [%6];" ::"l"(tmap), "r"(x0), "r"(0), "r"(0), "r"(0),
+                 "r"(band), "r"((unsigned)__cvta_generic_to_shared(ssrc))
                  : "memory");
 }
 __device__ __forceinline__ void ztile_load(void *sdst, const void *tmap, int x0, int band, unsigned long long *bar)
 {
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(
                      (unsigned)__cvta_generic_to_shared(sdst)),
-                 "l"(tmap), "r"(x0), "r"(0), "r"(band), "r"((unsigned)__cvta_generic_to_shared(bar))
+                 "l"(tmap), "r"(x0), "r"(0), "r"(0), "r"(0), "r"(band), "r"((unsigned)__cvta_generic_to_shared(bar))
                  : "memory");
 }
 
@@ -367,27 +373,28 @@ template <typename T, int NW> struct ZPersR4 {
     static_assert(TS % SG == 0, "tile rows must be whole 128-byte pieces");
     static constexpr int HALF = 2 * M * SG;                  // elements of one stick group's half tile (16 KB)
     static constexpr int TILE_SW = NSG * HALF;
-    __device__ static __forceinline__ int sw(int r, int sl)  // element index of (row r of the half, stick sl of the tile)
+    // row r = 2 n' + (e & 1) of the half sits at ((e & 1) 8 + n' / 8) 8 + n' mod 8: n' mod 8 fastest, see ZPers::row
+    __device__ static __forceinline__ int sw(int rr, int sl) // element index of (row rr of the half, stick sl of the tile)
     {
         constexpr int PE = 16 / (int)sizeof(cx<T>);          // elements per 16-byte piece
-        const int g = sl / SG, s = sl % SG;
+        const int g = sl / SG, s = sl % SG, r = ((rr & 1) * 8 + (rr >> 4)) * 8 + ((rr >> 1) & 7);
         return g * HALF + r * SG + ((((s / PE) ^ (r & 7)) * PE) | (s % PE));
     }
     static constexpr size_t smem_bytes = sizeof(cx<T>) * ((size_t)TILE_SW + (size_t)NW * F::EXW + (size_t)LZ) + 1024; // + alignment slack
 };
 
 // half tile <-> the rows z = 4 n' + e0, 4 n' + e0 + 1 of the sticks s0 + SG g .. of band `band` in A: coordinates of the tensor
-// the launcher builds over the intermediate (reals of SG sticks | z mod 4 | z / 4 | band), box = {128 bytes, 2, 64, 1}
+// the launcher builds over the intermediate (reals of SG sticks | n' mod 8 | n' / 8 | z mod 4 | band), box = {128 bytes, 8, 8, 2, 1}
 __device__ __forceinline__ void zr4_half_store(const void *tmap, int x0, int e0, int band, const void *ssrc)
 {
-    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4}], [%5];" ::"l"(tmap), "r"(x0), "r"(e0), "r"(0), "r"(band),
-                 "r"(smem_u32(ssrc))
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4, %5}], [%6];" ::"l"(tmap), "r"(x0), "r"(0), "r"(0), "r"(e0),
+                 "r"(band), "r"(smem_u32(ssrc))
                  : "memory");
 }
 __device__ __forceinline__ void zr4_half_load(void *sdst, const void *tmap, int x0, int e0, int band, unsigned long long *bar)
 {
-    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(smem_u32(sdst)),
-                 "l"(tmap), "r"(x0), "r"(e0), "r"(0), "r"(band), "r"(smem_u32(bar))
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(smem_u32(sdst)),
+                 "l"(tmap), "r"(x0), "r"(0), "r"(0), "r"(e0), "r"(band), "r"(smem_u32(bar))
                  : "memory");
 }
 
