@@ -164,6 +164,56 @@ __device__ __forceinline__ void sub_fwd(cx<T> (&y)[F::B2][F::P2], cx<T> (&x)[F::
     fft_reg<P1, -1, T>(x);
 }
 
+// The two halves of sub_inv / sub_fwd: everything in front of the exchange works on registers only, so a warp may do it
+// before it is allowed to touch the shared-memory line or column the exchange happens in (split barriers of plane_pf_k).
+// front + back = the same arithmetic in the same order as the whole.
+template <class F, typename T>
+__device__ __forceinline__ void sub_inv_front(cx<T> (&x)[F::P1], const cx<T> (&tws)[F::P1])
+{
+    fft_reg<F::P1, +1, T>(x);
+#pragma unroll
+    for (int m = 1; m < F::P1; ++m) x[m] = cmul(x[m], tws[m]);
+}
+template <class F, typename T, class EX>
+__device__ __forceinline__ void sub_inv_back(cx<T> (&x)[F::P1], cx<T> (&y)[F::B2][F::P2], EX ex, int t)
+{
+    constexpr int P1 = F::P1, P2 = F::P2, B2 = F::B2;
+    __syncwarp();
+#pragma unroll
+    for (int m = 0; m < P1; ++m) ex.put(m, t, x[m]);
+    __syncwarp();
+#pragma unroll
+    for (int b = 0; b < B2; ++b) {
+#pragma unroll
+        for (int tt = 0; tt < P2; ++tt) y[b][tt] = ex.get(t + P2 * b, tt);
+        fft_reg<P2, +1, T>(y[b]);
+    }
+}
+template <class F, typename T>
+__device__ __forceinline__ void sub_fwd_front(cx<T> (&y)[F::B2][F::P2], const cx<T> (&tws)[F::P1])
+{
+#pragma unroll
+    for (int b = 0; b < F::B2; ++b) {
+        fft_reg<F::P2, -1, T>(y[b]);
+#pragma unroll
+        for (int tt = 1; tt < F::P2; ++tt) y[b][tt] = cmulc(y[b][tt], tws[tt]);
+    }
+    fwd_btw_all<F, 0, T>(y);
+}
+template <class F, typename T, class EX>
+__device__ __forceinline__ void sub_fwd_back(cx<T> (&y)[F::B2][F::P2], cx<T> (&x)[F::P1], EX ex, int t)
+{
+    constexpr int P1 = F::P1, P2 = F::P2, B2 = F::B2;
+    __syncwarp();
+#pragma unroll
+    for (int b = 0; b < B2; ++b)
+#pragma unroll
+        for (int tt = 0; tt < P2; ++tt) ex.put(t + P2 * b, tt, y[b][tt]);
+    __syncwarp();
+#pragma unroll
+    for (int m = 0; m < P1; ++m) x[m] = ex.get(m, t);
+    fft_reg<P1, -1, T>(x);
+}
 
 // ---------------------------------------------------------------------------------------------
 // z passes, warp-synchronous: one group of P2 lanes per stick, G sticks per warp, TS = G * NW

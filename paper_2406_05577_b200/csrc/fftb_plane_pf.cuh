@@ -11,6 +11,10 @@
 //             Y: columns of both buffers -> G_0 + conj(W^k) G_1 -> A[b][z][.]      | barrier
 //       VLOC  Y_inv | barrier | X: inverse, V(r), forward in place | barrier | Y_fwd (then the Y_inv of the
 //             next plane on the same columns by the same warp, no barrier in between)
+//     The barrier in front of a plane's FIRST phase (INV: after the x pass, FWD: after the y pass) is SPLIT: a warp arrives on an
+//     mbarrier when it is done and waits only where its next task first touches the plane buffers -- after the task's inputs
+//     have been read and the register-only front of its transforms is done (ncu: a quarter of the inverse kernel's stall
+//     samples sat behind the two CTA barriers; 0.966 -> 0.94 ms inverse, 1.025 -> 1.015 ms forward on config 3).
 //   * every exchange of a transform is done IN PLACE in the line or column of the plane buffer it
 //     works on (ExSkew), so the only other shared memory is the TMA landing zone.
 //   * global memory is read by the TMA engine only (cp.async.bulk + mbarrier), one plane / one x task
@@ -101,7 +105,9 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
     const int f = lane / P2, t = lane % P2;
     C *stage = pbuf0 + 2 * PB;                      // INV, VLOC: landing zone of the row A[b][z][0..pitch)
     C *lstage = pbuf0 + 2 * PB + warp * (G * N);    // FWD: landing zone of this warp's next x task (G lines)
-    __shared__ __align__(8) unsigned long long bar_full, bar_line[NW];
+    __shared__ __align__(8) unsigned long long bar_full, bar_line[NW], bar_pb;
+    unsigned pb_par = 0;
+    bool pb_pending = false; // this warp has arrived on bar_pb and not waited yet
     const unsigned stage_bytes = (unsigned)pl.pitch * (unsigned)sizeof(C);
     unsigned line_par = 0;
     const C *tw = reinterpret_cast<const C *>(pl.tw1); // N1 == N2: one table
@@ -175,6 +181,18 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
             }
     };
 
+    // split barrier in front of a plane's first phase: the other warps are done with the plane buffers
+    auto pb_wait = [&]() {
+        if (pb_pending) {
+            mbar_wait(&bar_pb, pb_par);
+            pb_par ^= 1u;
+            pb_pending = false;
+        }
+    };
+    auto pb_arrive = [&]() {
+        asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&bar_pb)) : "memory");
+        pb_pending = true;
+    };
     // ---- stage bodies ------------------------------------------------------------------------------
     C *const pb0 = pbuf0, *const pb1 = pbuf0 + PB;
     // inverse y pass of one column group: stick values (staged row) -> the column in both residue buffers
@@ -192,7 +210,12 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
         for (int j = 0; j < P1; ++j) xs[j] = x[j];
         xs[P1 / 2] = cadd(xs[P1 / 2], bv);
         C *pc = pb0 + c.col * YP;
-        sub_inv<F, T>(xs, y, tws, ExSkew<T, P2, 1>{pc, c.act}, t); // exchanged in place in the destination column
+        sub_inv_front<F, T>(xs, tws);
+        x[P1 / 2] = csub(x[P1 / 2], bv);
+        pre_inv<F, 0, T>(x, g);
+        sub_inv_front<F, T>(x, tws);
+        pb_wait(); // INV: the previous plane's x pass is over in every warp
+        sub_inv_back<F, T>(xs, y, ExSkew<T, P2, 1>{pc, c.act}, t); // exchanged in place in the destination column
         __syncwarp();
         if (c.act) {
 #pragma unroll
@@ -200,10 +223,8 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
 #pragma unroll
                 for (int q = 0; q < P2; ++q) pc[(t + P2 * bb) + P1 * q] = y[bb][q];
         }
-        x[P1 / 2] = csub(x[P1 / 2], bv);
-        pre_inv<F, 0, T>(x, g);
         pc = pb1 + c.col * YP;
-        sub_inv<F, T>(x, y, tws, ExSkew<T, P2, 1>{pc, c.act}, t);
+        sub_inv_back<F, T>(x, y, ExSkew<T, P2, 1>{pc, c.act}, t);
         __syncwarp();
         if (c.act) {
 #pragma unroll
@@ -260,9 +281,12 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
     // forward x pass of one line per group: (o0, o1) -> the occupied k1 columns of the plane buffer
     auto xfwd_body = [&](C (&o0)[B2][P2], C (&o1)[B2][P2], C *pbuf, int yl) {
         C g0[P1], g1[P1];
+        sub_fwd_front<F, T>(o0, tws);
+        sub_fwd_front<F, T>(o1, tws);
+        pb_wait(); // FWD: the previous plane's y pass is over in every warp
         // exchanged in place in the line's own slots (unused so far in FWD, dead after the inverse half in VLOC)
-        sub_fwd<F, T>(o0, g0, tws, ExSkew<T, P2, YP>{pbuf + yl, true}, t);
-        sub_fwd<F, T>(o1, g1, tws, ExSkew<T, P2, YP>{pbuf + yl, true}, t);
+        sub_fwd_back<F, T>(o0, g0, ExSkew<T, P2, YP>{pbuf + yl, true}, t);
+        sub_fwd_back<F, T>(o1, g1, ExSkew<T, P2, YP>{pbuf + yl, true}, t);
         __syncwarp();
         post_fwd<F, 0, T>(g1, g);
         const int cb = M / 2 - k1lo;
@@ -300,6 +324,7 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
     // ---- the persistent loop over this CTA's planes --------------------------------------------------
     if (tid == 0) {
         mbar_init(&bar_full, 1);
+        mbar_init(&bar_pb, NW * 32);
         for (int w = 0; w < NW; ++w) mbar_init(&bar_line[w], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -320,6 +345,7 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
             // ======================================================== inverse y pass: staged row -> both buffers
             mbar_wait(&bar_full, i & 1);
             for (int task = warp; task < ntask_y; task += NW) yinv_body(ycol_of(task));
+            pb_wait(); // a warp without a y task
             yinv_single();
             __syncthreads();
             // nobody reads the staged row any more: the next plane's row lands during the x pass
@@ -351,7 +377,8 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
                     xfwd_body(o0, o1, pbuf, y >> 1);
                 }
             }
-            __syncthreads();
+            if constexpr (MODE == MODE_INV) pb_arrive(); // split: waited for inside the next plane's first y task
+            else __syncthreads();
         } else {
             // ======================================================== forward x pass: cuboid lines -> buffers
 #pragma unroll
@@ -373,7 +400,7 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
             yfwd_single(dst);
             // FWD: the next plane's x pass overwrites the buffers.  VLOC: the next plane's inverse y pass
             // touches the same columns from the same warp, no barrier needed.
-            if constexpr (MODE == MODE_FWD) __syncthreads();
+            if constexpr (MODE == MODE_FWD) pb_arrive(); // split: waited for inside the next plane's first x task
         }
         z = zn; b = bn;
     }
