@@ -299,11 +299,24 @@ plane_pf_k(const __grid_constant__ DevPlan pl, const __grid_constant__ ColTab ct
     };
     // single-stick columns, one warp per column.  Inverse: closed form x W^{k2 y}; forward: dot product.
     auto yinv_single = [&]() {
-        for (int i = warp; i < n_one; i += NW) {
-            const int col = ct.perm[pl.n_multi + i];
-            const int4 co = ct.col[col];
-            const C v = stage[co.x];
-            for (int y = lane; y < N; y += 32) (y & 1 ? pb1 : pb0)[col * YP + (y >> 1)] = cmul(v, tw[modn<N>(co.z * y)]);
+        if constexpr (MODE == MODE_INV) {
+            // the (column, y) pairs are dealt over ALL threads of the CTA: a warp per column would leave the other warps waiting
+            // at the barrier behind this phase (two such columns for a sphere: about 350 cycles per plane on two of eight warps)
+            for (int it = tid; it < n_one * N; it += NW * 32) {
+                const int i = it / N, y = it % N;
+                const int col = ct.perm[pl.n_multi + i];
+                const int4 co = ct.col[col];
+                (y & 1 ? pb1 : pb0)[col * YP + (y >> 1)] = cmul(stage[co.x], tw[modn<N>(co.z * y)]);
+            }
+        } else {
+            // VLOC: a column belongs to ONE warp from the forward y pass of a plane through the inverse y pass of the next
+            // (there is no barrier in between)
+            for (int i = warp; i < n_one; i += NW) {
+                const int col = ct.perm[pl.n_multi + i];
+                const int4 co = ct.col[col];
+                const C v = stage[co.x];
+                for (int y = lane; y < N; y += 32) (y & 1 ? pb1 : pb0)[col * YP + (y >> 1)] = cmul(v, tw[modn<N>(co.z * y)]);
+            }
         }
     };
     auto yfwd_single = [&](C *dst) {
